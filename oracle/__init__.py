@@ -1,0 +1,187 @@
+"""CPU FP64 oracle for SABLE's batched NR power flow + adjoint -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may import
+this package.  It never imports `paper_2606_07099_b200` and shares no code with the CUDA path.
+The arithmetic lives in `sable_oracle.c` (plain C, FP64, each function citing the PAPER.md passage it
+follows); this file only compiles it with gcc and marshals numpy arrays through ctypes.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): 2-bus closed form, hand-derived 3-bus example
+(tests/golden/), Jacobian vs central finite differences and vs the complex-matrix identities,
+power balance vs branch losses, adjoint vs finite-difference sensitivities, dense vs sparse vs scipy
+solves, permutation / batch-composition invariance.  No function of this oracle is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sable_oracle.c")
+_LIB = os.path.join(_HERE, "libsable_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp -shared; rebuilt when the source is newer than the library."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp", "-Wall", "-o", tmp,
+                               _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.oracle_mismatch.restype = C.c_double
+    return _lib
+
+
+def _p(a, t):
+    return None if a is None else a.ctypes.data_as(C.POINTER(t))
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _u8(a):
+    return np.ascontiguousarray(a, dtype=np.uint8)
+
+
+def ybus(n_bus, f, t, r, x, b):
+    """Y_bus CSR from a pi-model branch list.  Returns (row_ptr, col, G, B)."""
+    f, t, r, x, b = _i32(f), _i32(t), _f64(r), _f64(x), _f64(b)
+    L = lib()
+    nnz = L.oracle_ybus(int(n_bus), int(f.shape[0]), _p(f, C.c_int), _p(t, C.c_int), _p(r, C.c_double),
+                        _p(x, C.c_double), _p(b, C.c_double), None, None, None, None)
+    row_ptr = np.zeros(n_bus + 1, dtype=np.int32)
+    col = np.zeros(nnz, dtype=np.int32)
+    g = np.zeros(nnz)
+    bb = np.zeros(nnz)
+    L.oracle_ybus(int(n_bus), int(f.shape[0]), _p(f, C.c_int), _p(t, C.c_int), _p(r, C.c_double),
+                  _p(x, C.c_double), _p(b, C.c_double), _p(row_ptr, C.c_int), _p(col, C.c_int),
+                  _p(g, C.c_double), _p(bb, C.c_double))
+    return row_ptr, col, g, bb
+
+
+def index_maps(bus_type):
+    bus_type = _u8(bus_type)
+    nb = bus_type.shape[0]
+    th = np.zeros(nb, dtype=np.int32)
+    vmx = np.zeros(nb, dtype=np.int32)
+    n = lib().oracle_index_maps(nb, _p(bus_type, C.c_uint8), _p(th, C.c_int), _p(vmx, C.c_int))
+    return n, th, vmx
+
+
+def injections(Y, vm, va):
+    row_ptr, col, g, bb = Y
+    vm, va = _f64(vm), _f64(va)
+    nb = vm.shape[0]
+    P = np.zeros(nb)
+    Q = np.zeros(nb)
+    lib().oracle_injections(nb, _p(row_ptr, C.c_int), _p(col, C.c_int), _p(g, C.c_double), _p(bb, C.c_double),
+                            _p(vm, C.c_double), _p(va, C.c_double), _p(P, C.c_double), _p(Q, C.c_double))
+    return P, Q
+
+
+def mismatch(Y, bus_type, p_spec, q_spec, vm, va):
+    """One scenario.  Returns (F [n] in oracle order, inf-norm, P, Q)."""
+    row_ptr, col, g, bb = Y
+    bus_type = _u8(bus_type)
+    p_spec, q_spec, vm, va = _f64(p_spec), _f64(q_spec), _f64(vm), _f64(va)
+    nb = vm.shape[0]
+    n, th, vmx = index_maps(bus_type)
+    F = np.zeros(max(n, 1))
+    P = np.zeros(nb)
+    Q = np.zeros(nb)
+    r = lib().oracle_mismatch(nb, _p(row_ptr, C.c_int), _p(col, C.c_int), _p(g, C.c_double), _p(bb, C.c_double),
+                              _p(bus_type, C.c_uint8), _p(p_spec, C.c_double), _p(q_spec, C.c_double),
+                              _p(vm, C.c_double), _p(va, C.c_double), _p(th, C.c_int), _p(vmx, C.c_int),
+                              _p(F, C.c_double), _p(P, C.c_double), _p(Q, C.c_double))
+    return F[:n], r, P, Q
+
+
+def jacobian(Y, bus_type, vm, va):
+    """One scenario.  Returns (n, rows, cols, vals) of J1 in COO, oracle order."""
+    row_ptr, col, g, bb = Y
+    bus_type = _u8(bus_type)
+    vm, va = _f64(vm), _f64(va)
+    nb = vm.shape[0]
+    n, th, vmx = index_maps(bus_type)
+    P, Q = injections(Y, vm, va)
+    cap = 4 * int(row_ptr[nb]) + 4 * nb
+    jr = np.zeros(cap, dtype=np.int32)
+    jc = np.zeros(cap, dtype=np.int32)
+    jv = np.zeros(cap)
+    m = lib().oracle_jacobian_coo(nb, _p(row_ptr, C.c_int), _p(col, C.c_int), _p(g, C.c_double),
+                                  _p(bb, C.c_double), _p(vm, C.c_double), _p(va, C.c_double), _p(P, C.c_double),
+                                  _p(Q, C.c_double), _p(th, C.c_int), _p(vmx, C.c_int), _p(jr, C.c_int),
+                                  _p(jc, C.c_int), _p(jv, C.c_double))
+    return n, jr[:m].copy(), jc[:m].copy(), jv[:m].copy()
+
+
+def jacobian_dense(Y, bus_type, vm, va):
+    n, jr, jc, jv = jacobian(Y, bus_type, vm, va)
+    J = np.zeros((n, n))
+    np.add.at(J, (jr, jc), jv)
+    return J
+
+
+def linear_solve(n, jr, jc, jv, rhs, method=0, transpose=False, mixed=False):
+    jr, jc, jv = _i32(jr), _i32(jc), _f64(jv)
+    x = np.array(rhs, dtype=np.float64, copy=True)
+    rc = lib().oracle_linear_solve(int(n), int(jv.shape[0]), _p(jr, C.c_int), _p(jc, C.c_int), _p(jv, C.c_double),
+                                   _p(x, C.c_double), int(method), int(bool(transpose)), int(bool(mixed)))
+    if rc:
+        raise np.linalg.LinAlgError("oracle: singular matrix")
+    return x
+
+
+def nr_batch(Y, bus_type, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, method=1,
+             mixed=False, n_threads=0, want_hist=False):
+    """Batched Newton-Raphson.  Returns dict(vm, va, iterations, converged, final_norm, threads[, hist])."""
+    row_ptr, col, g, bb = Y
+    bus_type = _u8(bus_type)
+    p_spec, q_spec, v_set = _f64(p_spec), _f64(q_spec), _f64(v_set)
+    vm0, va0 = _f64(vm0), _f64(va0)
+    batch, nb = p_spec.shape
+    vm = np.zeros((batch, nb))
+    va = np.zeros((batch, nb))
+    it = np.zeros(batch, dtype=np.int32)
+    conv = np.zeros(batch, dtype=np.uint8)
+    fn = np.zeros(batch)
+    hist = np.zeros((batch, max_it + 1)) if want_hist else None
+    used = lib().oracle_nr_batch(nb, _p(row_ptr, C.c_int), _p(col, C.c_int), _p(g, C.c_double), _p(bb, C.c_double),
+                                 _p(bus_type, C.c_uint8), batch, _p(p_spec, C.c_double), _p(q_spec, C.c_double),
+                                 _p(v_set, C.c_double), _p(vm0, C.c_double), _p(va0, C.c_double),
+                                 C.c_double(tol), int(max_it), int(method), int(bool(mixed)), int(n_threads),
+                                 _p(vm, C.c_double), _p(va, C.c_double), _p(it, C.c_int), _p(conv, C.c_uint8),
+                                 _p(fn, C.c_double), _p(hist, C.c_double))
+    out = dict(vm=vm, va=va, iterations=it, converged=conv, final_norm=fn, threads=used)
+    if want_hist:
+        out["hist"] = hist
+    return out
+
+
+def adjoint_batch(Y, bus_type, vm, va, g_va, g_vm, method=1, mixed=False, n_threads=0):
+    """J1(V)^T lambda = g per scenario.  Returns (lam_p, lam_q, threads)."""
+    row_ptr, col, g, bb = Y
+    bus_type = _u8(bus_type)
+    vm, va, g_va, g_vm = _f64(vm), _f64(va), _f64(g_va), _f64(g_vm)
+    batch, nb = vm.shape
+    lp = np.zeros((batch, nb))
+    lq = np.zeros((batch, nb))
+    used = lib().oracle_adjoint_batch(nb, _p(row_ptr, C.c_int), _p(col, C.c_int), _p(g, C.c_double),
+                                      _p(bb, C.c_double), _p(bus_type, C.c_uint8), batch, _p(vm, C.c_double),
+                                      _p(va, C.c_double), _p(g_va, C.c_double), _p(g_vm, C.c_double), int(method),
+                                      int(bool(mixed)), int(n_threads), _p(lp, C.c_double), _p(lq, C.c_double))
+    return lp, lq, used
