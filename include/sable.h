@@ -1,0 +1,173 @@
+/*
+ * sable.h -- C ABI of the B200-native batched Newton-Raphson AC power-flow library
+ * (hot path of SABLE, arxiv/paper_2606_07099; PAPER.md = text of the paper).
+ *
+ * What the library computes (per scenario b of a batch sharing one network):
+ *   Step-1 equations  F1(z1) = [P_i(V) - P_spec,i  (i not slack);  Q_i(V) - Q_spec,i  (i PQ)] = 0     (eq. 6)
+ *   with S = V o conj(Y_bus V), V_i = Vm_i e^{j theta_i}, unknowns z1 = [theta (non-slack); Vm (PQ)]  (eq. 4)
+ *   Newton step       J1(z1_t) dz = -F1(z1_t),  z1_{t+1} = z1_t + dz                                  (eq. 7-8)
+ *   adjoint           J1(z1*)^T lambda = g                                                            (eq. 14)
+ * Sign convention: F = S_calc - S_spec (BASELINE.json north_star); the paper writes spec - calc
+ * (PAPER.md:55): the Newton step is identical, lambda here = -lambda_paper = d(g^T z1)/dS_spec.
+ *
+ * Units: per-unit and radians.  One slack bus.  No Q-limits, taps or shunts beyond what Y_bus carries.
+ * Threading: a context may be used by one host thread at a time.  Errors never abort or throw;
+ * every call returns a sable_status and leaves a message retrievable with sable_last_error().
+ */
+#ifndef SABLE_H
+#define SABLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sable_ctx sable_ctx;          /* opaque; owned by the library */
+
+typedef enum {
+    SABLE_OK = 0,
+    SABLE_ERR_INVALID_ARG = 1,               /* null pointer, negative size, batch > max_batch, bad option */
+    SABLE_ERR_STRUCTURE = 2,                 /* malformed CSR, bus_type/slack inconsistent, bus not connected to the slack */
+    SABLE_ERR_ALLOC = 3,                     /* host or device allocation failed */
+    SABLE_ERR_CUDA = 4,                      /* CUDA runtime error (launch, copy, no device) */
+    SABLE_ERR_STATE = 5                      /* e.g. sable_adjoint before a sable_solve that kept factors */
+} sable_status;
+
+enum { SABLE_BUS_PQ = 0, SABLE_BUS_PV = 1, SABLE_BUS_SLACK = 2 };
+enum { SABLE_FP64 = 0, SABLE_MIXED = 1 };    /* MIXED: FP64 mismatch / state, FP32 Jacobian factors and solves (Table I) */
+enum { SABLE_MODE_FUSED = 0, SABLE_MODE_STAGED = 1 };
+
+typedef struct {
+    int32_t max_batch;      /* scenarios per sable_solve call; all device buffers are sized for it at create time */
+    int32_t precision;      /* SABLE_FP64 or SABLE_MIXED */
+    int32_t keep_factors;   /* 1: after the NR loop, J1 is re-factored at the final iterate and the factors are kept
+                               for sable_adjoint (reading 16) */
+    int32_t mode;           /* SABLE_MODE_FUSED: one persistent kernel runs the whole NR loop of a scenario on chip;
+                               SABLE_MODE_STAGED: one kernel per stage (mismatch / fill / refactor / solve), state in HBM
+                               between stages -- used for per-stage profiling */
+    int32_t device;         /* CUDA device ordinal; -1 = host-only context (symbolic phase only: sable_get_info and the
+                               sable_debug_* pattern queries work, solve / adjoint return SABLE_ERR_STATE) */
+    int32_t threads;        /* threads per CTA for the NR kernels; 0 = library default for the grid size */
+} sable_options;
+
+typedef struct {
+    int32_t n_bus, n_pq, n_pv;
+    int32_t n;              /* scalar unknowns n_pv + 2 n_pq */
+    int32_t nnz_y;          /* stored Y_bus entries after canonicalisation */
+    int32_t nnz_j;          /* scalar nonzeros of J1 */
+    int32_t nnz_lu;         /* scalar nonzeros of L+U on the static fill pattern (unit diagonal of L not counted) */
+    int32_t n_node;         /* bus-level nodes = n_bus - 1 */
+    int32_t n_pair;         /* bus-level off-diagonal block pairs {U(m,j), L(j,m)} in the filled pattern */
+    int32_t n_pair_j;       /* of which structurally present in J1 (the rest is fill) */
+    int32_t n_level;        /* elimination levels */
+    int64_t n_term;         /* block multiply-subtract terms per refactorisation (pair targets) */
+    int64_t n_term_diag;    /* ... (diagonal targets) */
+    int64_t lu_flops;       /* scalar FP multiply-adds x2 per refactorisation on the unpadded pattern */
+    int64_t factor_bytes;   /* bytes of one scenario's stored factors (padded 2x2 blocks, in factor precision) */
+    int64_t bytes_iter_m0;  /* SURVEY.md §8(d) model M0: algorithmic HBM bytes per scenario per NR iteration */
+    int64_t bytes_adjoint_m0; /* same for one adjoint solve */
+    int32_t smem_bytes;     /* dynamic shared memory per CTA of the NR kernel */
+    int32_t placement;      /* 0: factors, V and rhs in shared memory; 1: factors + V in HBM/L2, rhs in shared memory;
+                               2: everything in HBM/L2 */
+    int32_t threads;        /* threads per CTA */
+    int32_t ctas_per_sm;    /* occupancy the NR kernel was sized for */
+} sable_info;
+
+/* Build the shared fixed-pattern template for one network (host symbolic phase, run once; PAPER.md:185-197:
+ * "symbolic setup only once for a shared topology"): canonical Y_bus CSR, PV/PQ/slack index maps, minimum-degree
+ * ordering of the bus graph, static block L+U fill pattern, elimination levels, multiply-subtract term lists and
+ * Jacobian fill metadata; uploads it and allocates every device buffer for opt->max_batch scenarios.
+ *   n_bus            number of buses (>= 2)
+ *   row_ptr[n_bus+1], col_idx[nnz], y_re[nnz], y_im[nnz]   HOST.  Y_bus = G + jB in CSR; columns may be unsorted,
+ *                    duplicates are summed, a missing diagonal or transpose entry is added with value 0.
+ *   bus_type[n_bus]  HOST.  SABLE_BUS_PQ / PV / SLACK; exactly one slack, and it must equal `slack`.
+ *   opt              may be NULL (defaults: max_batch 1, FP64, keep_factors 1, fused, device 0).
+ *   out              receives the context.  The input arrays are not referenced after the call returns.
+ * Errors: INVALID_ARG, STRUCTURE, ALLOC, CUDA.  On error *out = NULL (message via sable_last_error(NULL)). */
+sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx,
+                          const double* y_re, const double* y_im, const uint8_t* bus_type, int32_t slack,
+                          const sable_options* opt, sable_ctx** out);
+
+/* Batched Newton-Raphson (eq. 6-8; loop convention DESIGN.md):
+ *   it = 0; loop { r = ||F1(V)||_inf; if r <= tol: converged; if it == max_it or r not finite: stop; solve; update; ++it }
+ * All arrays are DEVICE pointers, row-major [batch][n_bus], owned by the caller, not kept after the call.
+ *   p_spec, q_spec   net injections P_spec = p_g - p_d, Q_spec = q_g - q_d.  p_spec is ignored at the
+ *                    slack, q_spec is used at PQ buses only.
+ *   v_set            |V| at PV and slack buses (the decision block x of eq. 3); ignored at PQ buses.
+ *   vm0, va0         initial |V| (PQ buses) and angle (non-slack), or both NULL for the flat start (PAPER.md:287:
+ *                    Vm = 1, theta = 0; PV/slack magnitudes at their setpoints, slack angle 0).
+ *   vm, va           out: final |V| and angle (rad).  May not alias the inputs.
+ *   iterations       out [batch] int32: Newton updates applied if converged, max_it otherwise.
+ *   converged        out [batch] uint8.  Non-convergence is not an error.
+ *   final_norm       out [batch] double or NULL: ||F1||_inf at the returned V.
+ *   cuda_stream      cudaStream_t; the call only enqueues work (no host synchronisation in fused mode).
+ * Converged scenarios stop consuming bandwidth (per-scenario masking).  Errors: INVALID_ARG, STATE, CUDA. */
+sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                         const double* v_set, const double* vm0, const double* va0, double tol, int32_t max_it,
+                         double* vm, double* va, int32_t* iterations, uint8_t* converged, double* final_norm,
+                         void* cuda_stream);
+
+/* Adjoint J1^T lambda = g (eq. 14) on the factors kept by the last sable_solve (keep_factors = 1),
+ * i.e. J1 at that call's final iterates; only transposed triangular solves run.
+ *   g_va [batch][n_bus]  dl/dtheta_i (slack entry ignored);   g_vm [batch][n_bus]  dl/dVm_i (PQ entries used)
+ *   lam_p, lam_q [batch][n_bus]  out: multipliers of the P_i / Q_i equations; 0 at the slack / off PQ buses.
+ * All DEVICE pointers.  batch must equal the batch of the last solve.  Errors: INVALID_ARG, STATE, CUDA. */
+sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm,
+                           double* lam_p, double* lam_q, void* cuda_stream);
+
+/* Host-buffer convenience wrappers: same semantics with HOST pointers; they copy in, run on the context's
+ * device and copy out (synchronous).  Used for the end-to-end measurement. */
+sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                              const double* v_set, const double* vm0, const double* va0, double tol,
+                              int32_t max_it, double* vm, double* va, int32_t* iterations, uint8_t* converged,
+                              double* final_norm);
+sable_status sable_adjoint_host(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm,
+                                double* lam_p, double* lam_q);
+
+sable_status sable_get_info(const sable_ctx* ctx, sable_info* info);
+const char*  sable_last_error(const sable_ctx* ctx);   /* ctx may be NULL: message of the last failed sable_create */
+void         sable_destroy(sable_ctx* ctx);
+
+/* Number of kernel launches the library has enqueued on this context since creation (for bench accounting). */
+int64_t      sable_launch_count(const sable_ctx* ctx);
+
+/* ---- debug / parity exports (used by tests; not part of the public surface) -------------------------------- */
+
+/* Template queries (HOST out arrays; pass NULL to skip one).  Sizes come from sable_get_info.
+ *   node_bus[n_node]      bus index of node p (nodes are in elimination order, grouped by level)
+ *   node_level[n_node]
+ *   pair_ptr[n_node+1]    pairs owned by node m are [pair_ptr[m], pair_ptr[m+1]); pair p = {U(m,j), L(j,m)}
+ *   pair_col[n_pair]      node j of pair p (j > m)
+ *   pair_in_j[n_pair]     1 if the pair is structurally present in J1, 0 if pure fill
+ *   term_ptr[n_pair+1], term_a[n_term], term_b[n_term]   pair target p = (m,j) subtracts, for each term t,
+ *                         L(m,k) U(k,j) and L(j,k) U(k,m) with term_a[t] = pair (k,m), term_b[t] = pair (k,j)
+ *   dterm_ptr[n_node+1], dterm[n_pair]   diagonal target m subtracts L(m,k) U(k,m) for each pair dterm[t] = (k,m) */
+sable_status sable_debug_pattern(const sable_ctx* ctx, int32_t* node_bus, int32_t* node_level, int32_t* pair_ptr,
+                                 int32_t* pair_col, uint8_t* pair_in_j, int32_t* term_ptr, int32_t* term_a,
+                                 int32_t* term_b, int32_t* dterm_ptr, int32_t* dterm);
+
+/* Mismatch at a given state (DEVICE pointers, [batch][n_bus]): f_p[i] = P_i - P_spec,i (0 at slack),
+ * f_q[i] = Q_i - Q_spec,i (0 off PQ), norm[b] = ||F1||_inf. */
+sable_status sable_debug_mismatch(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                  const double* vm, const double* va, double* f_p, double* f_q, double* norm,
+                                  void* cuda_stream);
+
+/* Jacobian blocks at a given state, written by the library's fill code in its padded block layout
+ * (DEVICE out, doubles): diag[batch][n_node][4] = [dP/dth, dP/dVm, dQ/dth, dQ/dVm] of node m w.r.t. itself;
+ * pairs[batch][n_pair][8] = block J1(m,j) (4 values, same order) followed by block J1(j,m).
+ * Padded entries (V-column / Q-row of a PV node) are 0, except dQ/dVm = 1 on a PV diagonal. */
+sable_status sable_debug_jacobian(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                  double* diag, double* pairs, void* cuda_stream);
+
+/* One linear solve with the library's refactor + triangular solves at a given state:
+ * transpose = 0: J1(V) x = rhs;  1: J1(V)^T x = rhs.  rhs_p/rhs_q and x_p/x_q are [batch][n_bus] DEVICE arrays
+ * holding the theta/P component and the Vm/Q component per bus. */
+sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                      const double* rhs_p, const double* rhs_q, int32_t transpose,
+                                      double* x_p, double* x_q, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SABLE_H */
