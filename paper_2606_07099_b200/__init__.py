@@ -1,0 +1,250 @@
+"""Thin Python binding of the SABLE B200 C-ABI library (include/sable.h) -- argument marshalling only.
+
+Every step of the path (mismatch, Jacobian fill, LU refactor, triangular solves, masking) runs in the CUDA
+kernels of `csrc/`; PyTorch is used by callers for device memory and streams only.  There is no CPU fallback:
+if `libsable.so` is missing, `lib()` raises.  Build it with `python -m paper_2606_07099_b200.build` (nvcc,
+sm_100a) or `__graft_entry__.build()`.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsable.so")
+_lib = None
+
+PQ, PV, SLACK = 0, 1, 2
+FP64, MIXED = 0, 1
+FUSED, STAGED = 0, 1
+STATUS = {0: "OK", 1: "INVALID_ARG", 2: "STRUCTURE", 3: "ALLOC", 4: "CUDA", 5: "STATE"}
+
+
+class SableError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"sable: {STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class Options(C.Structure):
+    _fields_ = [("max_batch", C.c_int32), ("precision", C.c_int32), ("keep_factors", C.c_int32),
+                ("mode", C.c_int32), ("device", C.c_int32), ("threads", C.c_int32)]
+
+
+class Info(C.Structure):
+    _fields_ = [("n_bus", C.c_int32), ("n_pq", C.c_int32), ("n_pv", C.c_int32), ("n", C.c_int32),
+                ("nnz_y", C.c_int32), ("nnz_j", C.c_int32), ("nnz_lu", C.c_int32), ("n_node", C.c_int32),
+                ("n_pair", C.c_int32), ("n_pair_j", C.c_int32), ("n_level", C.c_int32),
+                ("n_term", C.c_int64), ("n_term_diag", C.c_int64), ("lu_flops", C.c_int64),
+                ("factor_bytes", C.c_int64), ("bytes_iter_m0", C.c_int64), ("bytes_adjoint_m0", C.c_int64),
+                ("smem_bytes", C.c_int32), ("placement", C.c_int32), ("threads", C.c_int32),
+                ("ctas_per_sm", C.c_int32)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_solve_host", "sable_adjoint_host",
+           "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
+           "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve"]
+
+
+def lib():
+    """Load libsable.so; raises (no fallback) if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2606_07099_b200.build` (needs nvcc)")
+        L = C.CDLL(LIB_PATH)
+        L.sable_last_error.restype = C.c_char_p
+        L.sable_last_error.argtypes = [C.c_void_p]
+        L.sable_launch_count.restype = C.c_int64
+        L.sable_launch_count.argtypes = [C.c_void_p]
+        L.sable_destroy.restype = None
+        L.sable_destroy.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _hp(a, dtype):
+    """host numpy array -> pointer (keeps a reference alive through the returned tuple)."""
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, a.ctypes.data_as(C.c_void_p)
+
+
+def _dp(t):
+    """torch CUDA tensor (or None) -> device pointer."""
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_cuda and t.is_contiguous(), "device arrays must be contiguous CUDA tensors"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Context:
+    """Owns one `sable_ctx*`.  Method names follow the C calls (sable_solve -> .solve, ...)."""
+
+    def __init__(self, n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, max_batch=1, precision=FP64,
+                 keep_factors=True, mode=FUSED, device=0, threads=0):
+        L = lib()
+        keep = []
+        ptrs = []
+        for a, dt in ((row_ptr, np.int32), (col_idx, np.int32), (y_re, np.float64), (y_im, np.float64),
+                      (bus_type, np.uint8)):
+            arr, p = _hp(a, dt)
+            keep.append(arr)
+            ptrs.append(p)
+        opt = Options(int(max_batch), int(precision), int(bool(keep_factors)), int(mode), int(device), int(threads))
+        self._h = C.c_void_p(0)
+        st = L.sable_create(C.c_int32(int(n_bus)), *ptrs, C.c_int32(int(slack)), C.byref(opt), C.byref(self._h))
+        if st != 0:
+            raise SableError(st, (L.sable_last_error(None) or b"").decode())
+        self.n_bus = int(n_bus)
+        self.max_batch = int(max_batch)
+        self.device = int(device)
+        self.info = self.get_info()
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def _check(self, st):
+        if st != 0:
+            raise SableError(st, (lib().sable_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().sable_destroy(self._h)
+            self._h = C.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def get_info(self) -> dict:
+        info = Info()
+        self._check(lib().sable_get_info(self._h, C.byref(info)))
+        return info.as_dict()
+
+    def launch_count(self) -> int:
+        return int(lib().sable_launch_count(self._h))
+
+    # -- device-pointer calls (torch CUDA tensors, float64 [batch][n_bus]) ------------------------------
+    def solve(self, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, out=None):
+        """sable_solve.  Returns dict(vm, va, iterations, converged, final_norm) of torch CUDA tensors.
+        Asynchronous on torch's current stream."""
+        import torch
+        batch = int(p_spec.shape[0])
+        dev = p_spec.device
+        if out is None:
+            out = dict(vm=torch.empty((batch, self.n_bus), dtype=torch.float64, device=dev),
+                       va=torch.empty((batch, self.n_bus), dtype=torch.float64, device=dev),
+                       iterations=torch.empty(batch, dtype=torch.int32, device=dev),
+                       converged=torch.empty(batch, dtype=torch.uint8, device=dev),
+                       final_norm=torch.empty(batch, dtype=torch.float64, device=dev))
+        self._check(lib().sable_solve(self._h, C.c_int32(batch), _dp(p_spec), _dp(q_spec), _dp(v_set), _dp(vm0),
+                                      _dp(va0), C.c_double(tol), C.c_int32(int(max_it)), _dp(out["vm"]),
+                                      _dp(out["va"]), _dp(out["iterations"]), _dp(out["converged"]),
+                                      _dp(out["final_norm"]), _stream()))
+        return out
+
+    def adjoint(self, g_va, g_vm, out=None):
+        """sable_adjoint.  Returns (lam_p, lam_q)."""
+        import torch
+        batch = int(g_va.shape[0])
+        if out is None:
+            out = (torch.empty_like(g_va), torch.empty_like(g_vm))
+        self._check(lib().sable_adjoint(self._h, C.c_int32(batch), _dp(g_va), _dp(g_vm), _dp(out[0]), _dp(out[1]),
+                                        _stream()))
+        return out
+
+    # -- host-buffer calls (numpy) ----------------------------------------------------------------------
+    def solve_host(self, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, out=None):
+        batch = int(p_spec.shape[0])
+        if out is None:
+            out = dict(vm=np.empty((batch, self.n_bus)), va=np.empty((batch, self.n_bus)),
+                       iterations=np.empty(batch, dtype=np.int32), converged=np.empty(batch, dtype=np.uint8),
+                       final_norm=np.empty(batch))
+        hp = lambda a: C.c_void_p(0) if a is None else C.c_void_p(a.ctypes.data)
+        for a in (p_spec, q_spec, v_set, vm0, va0):
+            assert a is None or (a.dtype == np.float64 and a.flags.c_contiguous)
+        self._check(lib().sable_solve_host(self._h, C.c_int32(batch), hp(p_spec), hp(q_spec), hp(v_set), hp(vm0),
+                                           hp(va0), C.c_double(tol), C.c_int32(int(max_it)), hp(out["vm"]),
+                                           hp(out["va"]), hp(out["iterations"]), hp(out["converged"]),
+                                           hp(out["final_norm"])))
+        return out
+
+    def adjoint_host(self, g_va, g_vm, out=None):
+        batch = int(g_va.shape[0])
+        if out is None:
+            out = (np.empty_like(g_va), np.empty_like(g_vm))
+        for a in (g_va, g_vm):
+            assert a.dtype == np.float64 and a.flags.c_contiguous
+        self._check(lib().sable_adjoint_host(self._h, C.c_int32(batch), C.c_void_p(g_va.ctypes.data),
+                                             C.c_void_p(g_vm.ctypes.data), C.c_void_p(out[0].ctypes.data),
+                                             C.c_void_p(out[1].ctypes.data)))
+        return out
+
+    # -- debug exports ------------------------------------------------------------------------------------
+    def debug_pattern(self) -> dict:
+        I = self.info
+        nn, npair, nt = I["n_node"], I["n_pair"], I["n_term"]
+        a = dict(node_bus=np.zeros(nn, np.int32), node_level=np.zeros(nn, np.int32), pair_ptr=np.zeros(nn + 1, np.int32),
+                 pair_col=np.zeros(npair, np.int32), pair_in_j=np.zeros(npair, np.uint8),
+                 term_ptr=np.zeros(npair + 1, np.int32), term_a=np.zeros(nt, np.int32), term_b=np.zeros(nt, np.int32),
+                 dterm_ptr=np.zeros(nn + 1, np.int32), dterm=np.zeros(npair, np.int32))
+        order = ["node_bus", "node_level", "pair_ptr", "pair_col", "pair_in_j", "term_ptr", "term_a", "term_b",
+                 "dterm_ptr", "dterm"]
+        self._check(lib().sable_debug_pattern(self._h, *[C.c_void_p(a[k].ctypes.data) for k in order]))
+        return a
+
+    def debug_mismatch(self, p_spec, q_spec, vm, va):
+        import torch
+        batch = int(vm.shape[0])
+        f_p, f_q = torch.empty_like(vm), torch.empty_like(vm)
+        norm = torch.empty(batch, dtype=torch.float64, device=vm.device)
+        self._check(lib().sable_debug_mismatch(self._h, C.c_int32(batch), _dp(p_spec), _dp(q_spec), _dp(vm), _dp(va),
+                                               _dp(f_p), _dp(f_q), _dp(norm), _stream()))
+        return f_p, f_q, norm
+
+    def debug_jacobian(self, vm, va):
+        import torch
+        batch = int(vm.shape[0])
+        diag = torch.empty((batch, self.info["n_node"], 4), dtype=torch.float64, device=vm.device)
+        pairs = torch.empty((batch, self.info["n_pair"], 8), dtype=torch.float64, device=vm.device)
+        self._check(lib().sable_debug_jacobian(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(diag), _dp(pairs),
+                                               _stream()))
+        return diag, pairs
+
+    def debug_linear_solve(self, vm, va, rhs_p, rhs_q, transpose=False):
+        import torch
+        batch = int(vm.shape[0])
+        x_p, x_q = torch.empty_like(vm), torch.empty_like(vm)
+        self._check(lib().sable_debug_linear_solve(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(rhs_p), _dp(rhs_q),
+                                                   C.c_int32(int(bool(transpose))), _dp(x_p), _dp(x_q), _stream()))
+        return x_p, x_q
+
+
+def sable_create(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt) -> Context:
+    return Context(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt)
+
+
+def ybus_from_branches(n_bus, f, t, r, x, b):
+    """Harness-side Y_bus CSR (pi-model; the paper takes Y_bus as given) -- unsorted triplets with
+    duplicates, which sable_create canonicalises.  Returns (row_ptr, col, G, B)."""
+    f = np.asarray(f, np.int64); t = np.asarray(t, np.int64)
+    y = 1.0 / (np.asarray(r, float) + 1j * np.asarray(x, float))
+    sh = 0.5j * np.asarray(b, float)
+    rows = np.concatenate([f, t, f, t]); cols = np.concatenate([f, t, t, f])
+    vals = np.concatenate([y + sh, y + sh, -y, -y])
+    order = np.argsort(rows, kind="stable")
+    rows, cols, vals = rows[order], cols[order], vals[order]
+    row_ptr = np.zeros(n_bus + 1, np.int64)
+    np.add.at(row_ptr, rows + 1, 1)
+    row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    return row_ptr, cols.astype(np.int32), np.ascontiguousarray(vals.real), np.ascontiguousarray(vals.imag)

@@ -1,0 +1,353 @@
+// C ABI of the SABLE B200 library (include/sable.h): context, device upload of the template, launches.
+#include "../../include/sable.h"
+#include "sable_symbolic.hpp"
+#include "sable_kernels2.cuh"
+
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace sable;
+
+struct sable_ctx {
+    Template T;
+    sable_options opt{};
+    sable_info info{};
+    DevTemplate d{};
+    std::vector<void*> dev_allocs;
+    void* factors = nullptr;  double* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
+    int64_t fac_stride = 0, work_stride = 0;
+    int threads = 0, grid = 0, placement = 0, smem = 0;
+    int last_batch = -1;  bool have_factors = false;
+    int64_t launches = 0;
+    std::string err;
+    // host wrapper staging (device)
+    double* hbuf = nullptr; int32_t* hbuf_it = nullptr; uint8_t* hbuf_cv = nullptr;
+};
+
+static std::string g_create_err;
+
+static sable_status fail(sable_ctx* c, sable_status s, const std::string& m) { if (c) c->err = m; else g_create_err = m; return s; }
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, e_ == cudaErrorMemoryAllocation ? SABLE_ERR_ALLOC : SABLE_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+
+template <typename V>
+static cudaError_t upload(sable_ctx* c, const std::vector<V>& h, const V** out) {
+    void* p = nullptr;
+    size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(V);
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) return e;
+    c->dev_allocs.push_back(p);
+    if (!h.empty()) e = cudaMemcpy(p, h.data(), h.size() * sizeof(V), cudaMemcpyHostToDevice);
+    *out = reinterpret_cast<const V*>(p);
+    return e;
+}
+
+static void fill_info(sable_ctx* c) {
+    const Template& T = c->T;
+    sable_info& I = c->info;
+    const int64_t w = c->opt.precision == SABLE_MIXED ? 4 : 8;
+    I.n_bus = T.n_bus; I.n_pq = T.n_pq; I.n_pv = T.n_pv; I.n = T.n_pv + 2 * T.n_pq;
+    I.nnz_y = (int32_t)T.nnz_y; I.nnz_j = (int32_t)T.nnz_j; I.nnz_lu = (int32_t)T.nnz_lu;
+    I.n_node = T.n_node; I.n_pair = (int32_t)T.pair_col.size(); I.n_pair_j = (int32_t)T.n_pair_j;
+    I.n_level = T.n_level; I.n_term = (int64_t)T.term_a.size(); I.n_term_diag = (int64_t)T.dterm.size();
+    I.lu_flops = T.lu_flops;
+    I.factor_bytes = fac_elems(T.n_node, I.n_pair) * w;
+    // SURVEY.md §8(d) model M0: 8 nnzJ (a2 write) + w nnzJ (a4 read) + 2 w nnzLU (a4 write, a5 read) + 8 (10 nB + 4 n)
+    I.bytes_iter_m0 = 8 * T.nnz_j + w * T.nnz_j + 2 * w * T.nnz_lu + 8 * (10 * (int64_t)T.n_bus + 4 * (int64_t)I.n);
+    I.bytes_adjoint_m0 = w * T.nnz_lu + 16 * (int64_t)I.n;
+    I.smem_bytes = c->smem; I.placement = c->placement; I.threads = c->threads;
+    I.ctas_per_sm = c->grid > 0 ? std::max(1, c->grid / 148) : 0;
+}
+
+template <typename T> static const void* fused_fn() { return (const void*)k_nr_fused<T>; }
+
+// placement / launch shape: the smallest placement number that still allows >= 2 CTAs per SM, else the smallest that fits
+static sable_status choose_launch(sable_ctx* ctx) {
+    const int nn = ctx->T.n_node, np = (int)ctx->T.pair_col.size();
+    const bool mixed = ctx->opt.precision == SABLE_MIXED;
+    int dev = 0; CU(cudaGetDevice(&dev));
+    int max_optin = 0, n_sm = 0, smem_sm = 0;
+    CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    auto need = [&](int pl) { return mixed ? smem_need<float>(pl, nn, np) : smem_need<double>(pl, nn, np); };
+    int pl = 3;
+    const char* env = getenv("SABLE_PLACEMENT");
+    if (env) pl = atoi(env);
+    else {
+        for (int cand = 0; cand <= 3; ++cand) if (need(cand) + 1024 <= smem_sm / 2) { pl = cand; break; }
+        if (pl == 3) for (int cand = 0; cand <= 3; ++cand) if (need(cand) <= max_optin) { pl = cand; break; }
+    }
+    if (pl < 0 || pl > 3 || need(pl) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
+    int th = ctx->opt.threads;
+    if (th <= 0) { th = nn <= 64 ? 64 : nn <= 160 ? 128 : nn <= 1200 ? 256 : 512; }
+    if (const char* e2 = getenv("SABLE_THREADS")) th = atoi(e2);
+    th = std::min(1024, std::max(32, (th + 31) / 32 * 32));
+    const void* fn = mixed ? fused_fn<float>() : fused_fn<double>();
+    CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need(pl)));
+    int occ = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)need(pl)));
+    if (occ < 1) return fail(ctx, SABLE_ERR_CUDA, "NR kernel does not fit on an SM");
+    ctx->placement = pl; ctx->threads = th; ctx->smem = (int)need(pl); ctx->grid = occ * n_sm;
+    return SABLE_OK;
+}
+
+extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx, const double* y_re,
+                                     const double* y_im, const uint8_t* bus_type, int32_t slack,
+                                     const sable_options* opt, sable_ctx** out) {
+    sable_ctx* ctx = nullptr;      // CU() reports into g_create_err while ctx is null
+    if (!out) return fail(nullptr, SABLE_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    sable_options o{1, SABLE_FP64, 1, SABLE_MODE_FUSED, 0, 0};
+    if (opt) o = *opt;
+    if (o.max_batch < 1 || (o.precision != SABLE_FP64 && o.precision != SABLE_MIXED) ||
+        (o.mode != SABLE_MODE_FUSED && o.mode != SABLE_MODE_STAGED) || o.device < -1 || o.threads < 0)
+        return fail(nullptr, SABLE_ERR_INVALID_ARG, "bad option value");
+    sable_ctx* c = new (std::nothrow) sable_ctx;
+    if (!c) return fail(nullptr, SABLE_ERR_ALLOC, "host allocation failed");
+    c->opt = o;
+    std::string err;
+    int rc = build_template(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, c->T, err);
+    if (rc) { delete c; return fail(nullptr, (sable_status)rc, err); }
+    if (o.device < 0) { fill_info(c); *out = c; return SABLE_OK; }
+
+    const Template& T = c->T;
+    const int nn = T.n_node, np = (int)T.pair_col.size();
+    auto bail = [&](sable_status s) { std::string m = c->err; sable_destroy(c); g_create_err = m; return s; };
+    cudaError_t e = cudaSetDevice(o.device);
+    if (e != cudaSuccess) { c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(e); return bail(SABLE_ERR_CUDA); }
+    // packed device arrays
+    std::vector<int32_t> node_bus(T.node_bus); node_bus.push_back(T.slack);
+    std::vector<double2> ygb(T.ycol.size()), ydg(nn);
+    for (size_t k = 0; k < T.ycol.size(); ++k) ygb[k] = make_double2(T.yg[k], T.yb[k]);
+    for (int m = 0; m < nn; ++m) ydg[m] = make_double2(T.yg[T.ydiag[m]], T.yb[T.ydiag[m]]);
+    std::vector<double4> py(np);
+    for (int p = 0; p < np; ++p) {
+        const int su = T.pair_yu[p], sl = T.pair_yl[p];
+        py[p] = make_double4(su >= 0 ? T.yg[su] : 0.0, su >= 0 ? T.yb[su] : 0.0, sl >= 0 ? T.yg[sl] : 0.0, sl >= 0 ? T.yb[sl] : 0.0);
+    }
+    std::vector<int2> tab(T.term_a.size());
+    for (size_t q = 0; q < tab.size(); ++q) tab[q] = make_int2(T.term_a[q], T.term_b[q]);
+    DevTemplate& d = c->d;
+    d.n_bus = T.n_bus; d.n_node = nn; d.n_pair = np; d.n_level = T.n_level; d.slack = T.slack;
+    bool ok = true;
+    auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
+    up(T.level_ptr, &d.level_ptr); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
+    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(T.pair_ptr, &d.pair_ptr); up(T.pair_row, &d.pair_row);
+    up(T.pair_col, &d.pair_col); up(py, &d.pair_y); up(T.term_ptr, &d.term_ptr); up(tab, &d.term_ab);
+    up(T.dterm_ptr, &d.dterm_ptr); up(T.dterm, &d.dterm);
+    if (!ok) return bail(SABLE_ERR_ALLOC);
+    ctx = c;
+    sable_status st = choose_launch(c);
+    if (st != SABLE_OK) return bail(st);
+    const size_t w = o.precision == SABLE_MIXED ? 4 : 8;
+    c->fac_stride = fac_elems(nn, np); c->work_stride = work_doubles(nn);
+    auto dmalloc = [&](void** p, size_t bytes) {
+        if (cudaMalloc(p, bytes) != cudaSuccess) { c->err = "device allocation failed (" + std::to_string(bytes) + " bytes)"; return false; }
+        c->dev_allocs.push_back(*p); return true;
+    };
+    const size_t mb = (size_t)o.max_batch, nb = (size_t)T.n_bus;
+    if (!dmalloc(&c->factors, mb * c->fac_stride * w) || !dmalloc((void**)&c->work, mb * c->work_stride * 8) ||
+        !dmalloc((void**)&c->ints, (2 * mb + 4) * 4) || !dmalloc((void**)&c->hbuf, 9 * mb * nb * 8 + mb * 8) ||
+        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb))
+        return bail(SABLE_ERR_ALLOC);
+    const void* lin = o.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
+    if (2 * (size_t)nn * 8 > 48 * 1024) cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * nn * 8);
+    fill_info(c);
+    *out = c;
+    return SABLE_OK;
+}
+
+extern "C" void sable_destroy(sable_ctx* c) {
+    if (!c) return;
+    for (void* p : c->dev_allocs) cudaFree(p);
+    delete c;
+}
+extern "C" const char* sable_last_error(const sable_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+extern "C" int64_t sable_launch_count(const sable_ctx* c) { return c ? c->launches : 0; }
+extern "C" sable_status sable_get_info(const sable_ctx* c, sable_info* info) {
+    if (!c || !info) return SABLE_ERR_INVALID_ARG;
+    *info = c->info; return SABLE_OK;
+}
+
+// ---- solve -------------------------------------------------------------------------------------------------------
+template <typename T>
+static cudaError_t launch_solve(sable_ctx* c, const SolveArgs& A, cudaStream_t s) {
+    if (c->opt.mode == SABLE_MODE_FUSED) {
+        cudaError_t e = cudaMemsetAsync(A.queue, 0, 4, s);
+        if (e != cudaSuccess) return e;
+        const int grid = std::min(A.batch, c->grid);
+        k_nr_fused<T><<<grid, c->threads, c->smem, s>>>(A);
+        c->launches += 1;
+    } else {
+        k_st_init<T><<<A.batch, c->threads, 0, s>>>(A);
+        for (int i = 0; i <= A.max_it; ++i) {
+            k_st_mismatch_fill<T><<<A.batch, c->threads, 0, s>>>(A);
+            if (i < A.max_it) k_st_factor_solve<T><<<A.batch, c->threads, 0, s>>>(A);
+        }
+        c->launches += 2 + 2 * (int64_t)A.max_it;
+    }
+    return cudaGetLastError();
+}
+
+extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                    const double* v_set, const double* vm0, const double* va0, double tol, int32_t max_it,
+                                    double* vm, double* va, int32_t* iterations, uint8_t* converged, double* final_norm,
+                                    void* cuda_stream) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
+    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
+        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
+    if (max_it < 0 || !(tol >= 0.0)) return fail(ctx, SABLE_ERR_INVALID_ARG, "max_it < 0 or tol < 0");
+    ctx->have_factors = false; ctx->last_batch = batch;
+    if (batch == 0) return SABLE_OK;
+    CU(cudaSetDevice(ctx->opt.device));
+    SolveArgs A{};
+    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.placement = ctx->placement; A.tol = tol;
+    A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
+    A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
+    A.factors = ctx->factors; A.work = ctx->work; A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride;
+    A.queue = ctx->ints; A.status = ctx->ints + 4; A.it = ctx->ints + 4 + ctx->opt.max_batch;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    CU(ctx->opt.precision == SABLE_MIXED ? launch_solve<float>(ctx, A, s) : launch_solve<double>(ctx, A, s));
+    ctx->have_factors = ctx->opt.keep_factors != 0;
+    return SABLE_OK;
+}
+
+// ---- adjoint / linear solves on kept factors ---------------------------------------------------------------------
+static sable_status launch_lin(sable_ctx* ctx, int batch, const double* rp, const double* rq, int transposed, double* xp,
+                               double* xq, cudaStream_t s) {
+    LinArgs L{};
+    L.t = ctx->d; L.batch = batch; L.transposed = transposed; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
+    L.factors = ctx->factors; L.fac_stride = ctx->fac_stride;
+    const size_t sm = 2 * (size_t)ctx->T.n_node * 8;
+    int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
+    const int use_smem = sm <= (size_t)max_optin;
+    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<batch, ctx->threads, use_smem ? sm : 0, s>>>(L, ctx->work, ctx->work_stride, use_smem);
+    else k_linsolve<double><<<batch, ctx->threads, use_smem ? sm : 0, s>>>(L, ctx->work, ctx->work_stride, use_smem);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return SABLE_OK;
+}
+
+extern "C" sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm, double* lam_p,
+                                      double* lam_q, void* cuda_stream) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (!ctx->have_factors) return fail(ctx, SABLE_ERR_STATE, "no kept factors: call sable_solve with keep_factors = 1 first");
+    if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
+    if (!g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    if (batch == 0) return SABLE_OK;
+    CU(cudaSetDevice(ctx->opt.device));
+    return launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, (cudaStream_t)cuda_stream);
+}
+
+// ---- host-buffer wrappers (end-to-end path: H2D, solve, D2H; synchronous) ------------------------------------------
+extern "C" sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                         const double* v_set, const double* vm0, const double* va0, double tol,
+                                         int32_t max_it, double* vm, double* va, int32_t* iterations, uint8_t* converged,
+                                         double* final_norm) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
+    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
+        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    if (batch == 0) { ctx->have_factors = false; ctx->last_batch = 0; return SABLE_OK; }
+    CU(cudaSetDevice(ctx->opt.device));
+    const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
+    double* d = ctx->hbuf;       // slots: 0 p, 1 q, 2 vset, 3 vm0, 4 va0, 5 vm, 6 va, (7, 8 adjoint), then norm
+    double* dn = ctx->hbuf + 9 * (size_t)ctx->opt.max_batch * ctx->T.n_bus;
+    CU(cudaMemcpyAsync(d, p_spec, bytes, cudaMemcpyHostToDevice, 0));
+    CU(cudaMemcpyAsync(d + n, q_spec, bytes, cudaMemcpyHostToDevice, 0));
+    CU(cudaMemcpyAsync(d + 2 * n, v_set, bytes, cudaMemcpyHostToDevice, 0));
+    if (vm0) { CU(cudaMemcpyAsync(d + 3 * n, vm0, bytes, cudaMemcpyHostToDevice, 0)); CU(cudaMemcpyAsync(d + 4 * n, va0, bytes, cudaMemcpyHostToDevice, 0)); }
+    sable_status st = sable_solve(ctx, batch, d, d + n, d + 2 * n, vm0 ? d + 3 * n : nullptr, vm0 ? d + 4 * n : nullptr, tol, max_it,
+                                  d + 5 * n, d + 6 * n, ctx->hbuf_it, ctx->hbuf_cv, dn, nullptr);
+    if (st != SABLE_OK) return st;
+    CU(cudaMemcpyAsync(vm, d + 5 * n, bytes, cudaMemcpyDeviceToHost, 0));
+    CU(cudaMemcpyAsync(va, d + 6 * n, bytes, cudaMemcpyDeviceToHost, 0));
+    CU(cudaMemcpyAsync(iterations, ctx->hbuf_it, (size_t)batch * 4, cudaMemcpyDeviceToHost, 0));
+    CU(cudaMemcpyAsync(converged, ctx->hbuf_cv, (size_t)batch, cudaMemcpyDeviceToHost, 0));
+    if (final_norm) CU(cudaMemcpyAsync(final_norm, dn, (size_t)batch * 8, cudaMemcpyDeviceToHost, 0));
+    CU(cudaStreamSynchronize(0));
+    return SABLE_OK;
+}
+
+extern "C" sable_status sable_adjoint_host(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm,
+                                           double* lam_p, double* lam_q) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 0 || batch > ctx->opt.max_batch || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "bad argument");
+    if (batch == 0) return SABLE_OK;
+    CU(cudaSetDevice(ctx->opt.device));
+    const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
+    double* d = ctx->hbuf;
+    CU(cudaMemcpyAsync(d, g_va, bytes, cudaMemcpyHostToDevice, 0));
+    CU(cudaMemcpyAsync(d + n, g_vm, bytes, cudaMemcpyHostToDevice, 0));
+    sable_status st = sable_adjoint(ctx, batch, d, d + n, d + 7 * n, d + 8 * n, nullptr);
+    if (st != SABLE_OK) return st;
+    CU(cudaMemcpyAsync(lam_p, d + 7 * n, bytes, cudaMemcpyDeviceToHost, 0));
+    CU(cudaMemcpyAsync(lam_q, d + 8 * n, bytes, cudaMemcpyDeviceToHost, 0));
+    CU(cudaStreamSynchronize(0));
+    return SABLE_OK;
+}
+
+// ---- debug exports -----------------------------------------------------------------------------------------------
+extern "C" sable_status sable_debug_pattern(const sable_ctx* c, int32_t* node_bus, int32_t* node_level, int32_t* pair_ptr,
+                                            int32_t* pair_col, uint8_t* pair_in_j, int32_t* term_ptr, int32_t* term_a,
+                                            int32_t* term_b, int32_t* dterm_ptr, int32_t* dterm) {
+    if (!c) return SABLE_ERR_INVALID_ARG;
+    const Template& T = c->T;
+    auto cp = [](auto* dst, const auto& v) { if (dst && !v.empty()) memcpy(dst, v.data(), v.size() * sizeof(v[0])); };
+    cp(node_bus, T.node_bus); cp(node_level, T.node_level); cp(pair_ptr, T.pair_ptr); cp(pair_col, T.pair_col);
+    cp(term_ptr, T.term_ptr); cp(term_a, T.term_a); cp(term_b, T.term_b); cp(dterm_ptr, T.dterm_ptr); cp(dterm, T.dterm);
+    if (pair_in_j) for (size_t p = 0; p < T.pair_yu.size(); ++p) pair_in_j[p] = T.pair_yu[p] >= 0;
+    return SABLE_OK;
+}
+
+static sable_status launch_debug(sable_ctx* ctx, DebugArgs& D, cudaStream_t s) {
+    D.t = ctx->d; D.factors = ctx->factors; D.work = ctx->work; D.fac_stride = ctx->fac_stride; D.work_stride = ctx->work_stride;
+    if (ctx->opt.precision == SABLE_MIXED) k_debug<float><<<D.batch, ctx->threads, 0, s>>>(D);
+    else k_debug<double><<<D.batch, ctx->threads, 0, s>>>(D);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return SABLE_OK;
+}
+static sable_status debug_check(sable_ctx* ctx, int batch) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 1 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
+    ctx->have_factors = false;
+    CU(cudaSetDevice(ctx->opt.device));
+    return SABLE_OK;
+}
+
+extern "C" sable_status sable_debug_mismatch(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                             const double* vm, const double* va, double* f_p, double* f_q, double* norm,
+                                             void* cuda_stream) {
+    sable_status st = debug_check(ctx, batch); if (st) return st;
+    if (!p_spec || !q_spec || !vm || !va || !f_p || !f_q || !norm) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    DebugArgs D{}; D.batch = batch; D.what = 0; D.p_spec = p_spec; D.q_spec = q_spec; D.vm = vm; D.va = va; D.f_p = f_p; D.f_q = f_q; D.norm = norm;
+    return launch_debug(ctx, D, (cudaStream_t)cuda_stream);
+}
+
+extern "C" sable_status sable_debug_jacobian(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* diag,
+                                             double* pairs, void* cuda_stream) {
+    sable_status st = debug_check(ctx, batch); if (st) return st;
+    if (!vm || !va || !diag || !pairs) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    DebugArgs D{}; D.batch = batch; D.what = 1; D.vm = vm; D.va = va; D.diag = diag; D.pairs = pairs;
+    return launch_debug(ctx, D, (cudaStream_t)cuda_stream);
+}
+
+extern "C" sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                                 const double* rhs_p, const double* rhs_q, int32_t transpose, double* x_p,
+                                                 double* x_q, void* cuda_stream) {
+    sable_status st = debug_check(ctx, batch); if (st) return st;
+    if (!vm || !va || !rhs_p || !rhs_q || !x_p || !x_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    DebugArgs D{}; D.batch = batch; D.what = 2; D.vm = vm; D.va = va;
+    st = launch_debug(ctx, D, (cudaStream_t)cuda_stream); if (st) return st;
+    return launch_lin(ctx, batch, rhs_p, rhs_q, transpose ? 1 : 0, x_p, x_q, (cudaStream_t)cuda_stream);
+}
