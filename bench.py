@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py -- converged power-flow solves/s of the batched Newton-Raphson hot path on B200 (one JSON line).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--no-sweep]
+
+A "step" is one pass of the whole hot path over one batch of synthetic scenarios of a BASELINE.json config:
+sable_solve (mismatch + norm, masking, Jacobian fill, LU refactor, triangular solves, update -- until every scenario
+converged or stopped) and, for configs that ask for it, sable_adjoint on the kept factors.  Default workload:
+BASELINE.json configs[1] (118 buses, 1024 scenarios); `--config k` picks configs[k-1]; unless --no-sweep the line also
+carries a short measurement of all five configs under "per_config" (HBM-roofline fractions are meaningful for
+configs 3-5 only: configs 1-2 are L2-resident).
+
+Timing: W >= 3 warm-up steps, then K steps each bracketed by CUDA events on the launching stream (torch's current
+stream, which is the stream handed to the library); L2 is flushed (256 MiB memset) between steps, outside the timed
+region; barrier + synchronize on both sides; max over ranks.  N > 1: scenarios shard with no collective (weak
+scaling: every rank solves its own batch of the config with its own scenario seed).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import sable_synth as S  # noqa: E402
+
+WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward",
+            2: "BASELINE.json configs[1]: 118 buses x 1024 scenarios, FP64 forward",
+            3: "BASELINE.json configs[2]: 300 buses x 8192 scenarios, FP64 forward + adjoint",
+            4: "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
+            5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
+METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
+UNIT = "solves/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.stop, self.index = [], threading.Event(), index
+        self.th = threading.Thread(target=self.run, daemon=True)
+
+    def run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def __enter__(self):
+        self.th.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.th.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if len(r) == 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) == 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) == 6 and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def make_inputs(cfg_id, seed_offset=0):
+    net = S.make_network(cfg_id)
+    ps, qs, vs = S.make_scenarios(net, seed=10_000 + net.extra["s_net"] + 1000 * seed_offset)
+    gva = gvm = None
+    if net.cfg.adjoint:
+        gva, gvm = S.make_adjoint_rhs(net)
+    return net, ps, qs, vs, gva, gvm
+
+
+def algorithmic_bytes(info, iterations, batch, keep, w):
+    """SURVEY §8(d) M0 bytes per scenario-iteration x Newton updates actually executed, plus
+    (keep_factors) one more fill + refactor at the final iterate, plus the boundary arrays (3 in, 2 out)."""
+    per_it = info["bytes_iter_m0"]
+    b = per_it * int(iterations.sum()) + 5 * 8 * info["n_bus"] * batch
+    if keep:
+        b += (8 * info["nnz_j"] + w * info["nnz_j"] + w * info["nnz_lu"]) * batch
+    return b
+
+
+def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True):
+    import torch
+    import paper_2606_07099_b200 as sb
+    import torch.distributed as dist
+    from paper_2606_07099_b200.sharding import reduce_job
+    net, ps, qs, vs, gva, gvm = make_inputs(cfg_id, seed_offset=rank)
+    c = net.cfg
+    B = c.batch
+    Yh = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+    t0 = time.perf_counter()
+    ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=B, precision=c.precision,
+                     keep_factors=c.adjoint, mode=sb.FUSED, device=torch.cuda.current_device())
+    create_s = time.perf_counter() - t0
+    info = ctx.info
+    dev = torch.device("cuda", torch.cuda.current_device())
+    d = lambda a: None if a is None else torch.from_numpy(a).to(dev)
+    dps, dqs, dvs, dga, dgm = d(ps), d(qs), d(vs), d(gva), d(gvm)
+    out = dict(vm=torch.empty((B, net.n_bus), dtype=torch.float64, device=dev), va=torch.empty((B, net.n_bus), dtype=torch.float64, device=dev),
+               iterations=torch.empty(B, dtype=torch.int32, device=dev), converged=torch.empty(B, dtype=torch.uint8, device=dev),
+               final_norm=torch.empty(B, dtype=torch.float64, device=dev))
+    lam = (torch.empty_like(out["vm"]), torch.empty_like(out["vm"])) if c.adjoint else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        ctx.solve(dps, dqs, dvs, tol=c.tol, max_it=c.max_it, out=out)
+        if c.adjoint:
+            ctx.adjoint(dga, dgm, out=lam)
+
+    for _ in range(max(warmup, 3)):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(steps)]
+    l0 = ctx.launch_count()
+    sampler = ClockSampler(torch.cuda.current_device()) if clocks else None
+    if sampler:
+        sampler.__enter__()
+    torch.cuda.synchronize()
+    for a, m, b in ev:
+        flush.zero_()
+        a.record()
+        ctx.solve(dps, dqs, dvs, tol=c.tol, max_it=c.max_it, out=out)
+        m.record()
+        if c.adjoint:
+            ctx.adjoint(dga, dgm, out=lam)
+        b.record()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.__exit__()
+    launches = ctx.launch_count() - l0
+    if world > 1:
+        dist.barrier()
+    step_ms = [a.elapsed_time(b) for a, m, b in ev]
+    solve_ms = [a.elapsed_time(m) for a, m, b in ev]
+    its = out["iterations"].cpu().numpy()
+    conv = int(out["converged"].sum().item())
+    secs, conv_all, solves_all = reduce_job(sum(step_ms) / 1e3, conv * steps, B * steps, device=dev)
+    w = 4 if c.precision == 1 else 8
+    alg = algorithmic_bytes(info, its, B, c.adjoint, w)
+    peak, peak_src = peaks()
+    kern_s = float(np.mean(solve_ms)) / 1e3
+    res = {"value": conv_all / secs, "ms_per_step": 1e3 * secs / steps, "converged": conv, "batch": B,
+           "iterations_hist": np.bincount(its).tolist(), "solve_ms": float(np.mean(solve_ms)),
+           "adjoint_ms": float(np.mean(step_ms) - np.mean(solve_ms)) if c.adjoint else None,
+           "roofline": {"bound": "hbm", "kernel": "k_nr_fused (one launch = the whole NR loop of the batch)",
+                        "achieved": alg / kern_s / 1e9, "peak": peak, "unit": "GB/s", "frac": alg / kern_s / 1e9 / peak,
+                        "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
+                        "note": "achieved = model-M0 bytes / kernel time; the fused kernel keeps factors on chip, so its "
+                                "DRAM traffic is far below M0 (profiles/)"},
+           "launches": launches, "create_s": create_s, "info": {k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level",
+                                                                                   "placement", "threads", "smem_bytes", "bytes_iter_m0")},
+           "clocks": sampler.summary() if sampler else None}
+    if e2e:
+        pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory().numpy()
+        hps, hqs, hvs, hga, hgm = pin(ps), pin(qs), pin(vs), pin(gva), pin(gvm)
+        hout = dict(vm=pin(np.empty((B, net.n_bus))), va=pin(np.empty((B, net.n_bus))), iterations=pin(np.empty(B, np.int32)),
+                    converged=pin(np.empty(B, np.uint8)), final_norm=pin(np.empty(B)))
+        hlam = (pin(np.empty((B, net.n_bus))), pin(np.empty((B, net.n_bus)))) if c.adjoint else None
+
+        def estep():
+            ctx.solve_host(hps, hqs, hvs, tol=c.tol, max_it=c.max_it, out=hout)
+            if c.adjoint:
+                ctx.adjoint_host(hga, hgm, out=hlam)
+        for _ in range(3):
+            estep()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            estep()
+        torch.cuda.synchronize()
+        es = time.perf_counter() - t0
+        econv = int(hout["converged"].sum())
+        es, econv_all, _ = reduce_job(es, econv * steps, B * steps, device=dev)
+        nb8 = B * net.n_bus * 8
+        res["e2e"] = {"value": econv_all / es, "unit": UNIT, "h2d_bytes_per_step": (3 + (2 if c.adjoint else 0)) * nb8,
+                      "d2h_bytes_per_step": (2 + (2 if c.adjoint else 0)) * nb8 + B * 13}
+    ctx.close()
+    return res, (net, ps, qs, vs, gva, gvm)
+
+
+def run_oracle(cfg_id, inputs=None, budget_s=15.0):
+    """The oracle as it stands on the host cores, on a bounded sample of the workload (first `m` scenarios)."""
+    import oracle
+    net, ps, qs, vs, gva, gvm = inputs or make_inputs(cfg_id)
+    c = net.cfg
+    Y = oracle.ybus(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+    cores = os.cpu_count() or 1
+    probe = min(c.batch, cores)
+    t0 = time.perf_counter()
+    oracle.nr_batch(Y, net.bus_type, ps[:probe], qs[:probe], vs[:probe], tol=c.tol, max_it=c.max_it, method=1)
+    per_wave = max(time.perf_counter() - t0, 1e-4)
+    m = int(min(c.batch, max(probe, cores * int(budget_s / per_wave))))
+    t0 = time.perf_counter()
+    r = oracle.nr_batch(Y, net.bus_type, ps[:m], qs[:m], vs[:m], tol=c.tol, max_it=c.max_it, method=1)
+    if c.adjoint:
+        oracle.adjoint_batch(Y, net.bus_type, r["vm"], r["va"], gva[:m], gvm[:m], method=1)
+    dt = time.perf_counter() - t0
+    return {"value": float(r["converged"].sum()) / dt, "unit": UNIT, "cores": int(r["threads"]), "kind": "oracle",
+            "sample": f"first {m} of {c.batch} scenarios of the same workload, FP64 sparse-LU oracle, {dt:.2f} s"}, dt, m
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true")
+    a = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = S.CONFIGS[a.config]
+    config = {"workload": WORKLOAD[a.config], "name": cfg.name, "batch_per_gpu": cfg.batch, "tol": cfg.tol,
+              "max_it": cfg.max_it, "precision": "fp64 mismatch + fp32 LU" if cfg.precision else "fp64",
+              "adjoint": cfg.adjoint, "network_seed": cfg.s_net, "load_scale_kappa": cfg.kappa,
+              "parallelism": f"scenario sharding x{world}, no collective", "cache": "L2 flushed between steps (256 MiB memset)"}
+
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        t0 = time.perf_counter()
+        vals, m = [], 0
+        inputs = make_inputs(a.config)
+        for i in range(a.warmup + a.steps):
+            cb, dt, m = run_oracle(a.config, inputs, budget_s=max(0.5, 60.0 / (a.warmup + a.steps)))
+            if i >= a.warmup:
+                vals.append((cb["value"], dt))
+        v = float(np.mean([x[0] for x in vals]))
+        cb["value"] = v
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+                          "warmup": a.warmup, "ms_per_step": 1e3 * float(np.mean([x[1] for x in vals])),
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                          "data": "synthetic", "config": config, "cpu_baseline": cb,
+                          "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0, "wall_s": time.perf_counter() - t0}))
+        return
+
+    import torch
+    assert torch.cuda.is_available(), "bench.py (impl ours) needs a CUDA device: there is no CPU fallback"
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    res, inputs = run_ours(a.config, a.steps, a.warmup, rank, world)
+    line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+            "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if not cfg.precision else "f64+f32", "data": "synthetic", "config": config,
+            "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["launches"], "roofline": res["roofline"],
+            "converged": res["converged"], "iterations_hist": res["iterations_hist"], "solve_ms": res["solve_ms"],
+            "adjoint_ms": res["adjoint_ms"], "create_s": res["create_s"], "info": res["info"]}
+    if rank == 0 and world == 1:
+        line["cpu_baseline"], _, _ = run_oracle(a.config, inputs)
+        if not a.no_sweep:
+            per = {}
+            for k in (1, 2, 3, 4, 5):
+                r, _ = run_ours(k, 5, 3, 0, 1, e2e=False, clocks=False)
+                per[S.CONFIGS[k].name] = {"solves_per_s": r["value"], "ms_per_step": r["ms_per_step"], "solve_ms": r["solve_ms"],
+                                          "adjoint_ms": r["adjoint_ms"], "converged": r["converged"], "batch": r["batch"],
+                                          "iterations_hist": r["iterations_hist"], "roofline_frac": r["roofline"]["frac"],
+                                          "achieved_gbs": r["roofline"]["achieved"], "info": r["info"]}
+            line["per_config"] = per
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -199,11 +199,11 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
     if (!ctx) return SABLE_ERR_INVALID_ARG;
     if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
     if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
-    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
-        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
     if (max_it < 0 || !(tol >= 0.0)) return fail(ctx, SABLE_ERR_INVALID_ARG, "max_it < 0 or tol < 0");
     ctx->have_factors = false; ctx->last_batch = batch;
-    if (batch == 0) return SABLE_OK;
+    if (batch == 0) return SABLE_OK;                       /* empty batch: nothing is read or written */
+    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
+        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
     CU(cudaSetDevice(ctx->opt.device));
     SolveArgs A{};
     A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.placement = ctx->placement; A.tol = tol;

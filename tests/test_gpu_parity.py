@@ -1,0 +1,365 @@
+"""GPU parity: the CUDA path (through the C ABI, include/sable.h) against the CPU oracle on the same seeded
+inputs.  Tolerances are BASELINE.json's (north_star) where it states them, DESIGN.md "Tolerances" otherwise:
+  * bus voltages: |dVm| <= 1e-9 p.u., |dtheta| <= 1e-9 rad on converged scenarios (FP64 mode)
+  * final ||F1||inf <= 1e-8 (= tol) wherever converged = 1, identical converged flags, iterations within +-1
+  * mixed precision: same flags, final mismatch <= 1e-8, iterations within +-1, voltages within 1e-7
+    (the accepted iterate of a different Newton sequence: both satisfy ||F|| <= 1e-8)
+  * adjoint: ||lam_gpu - lam_oracle||inf <= 1e-8 max(1, ||lam_oracle||inf) per scenario (SURVEY §8(c) reading 19)
+  * per-kernel: F and J entries within 1e-13 x (sum_j |Y_ij| Vm_i Vm_j), the rounding scale of the row sum.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import sable_synth as S
+from util import dev, gpu_jacobian_dense, make_ctx, oracle_Y, random_state
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+import paper_2606_07099_b200 as sb  # noqa: E402
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    sb.lib()   # raises if libsable.so is missing: no fallback
+
+
+_NETS = {}
+
+
+def get_net(cfg):
+    if cfg not in _NETS:
+        net = S.make_network(cfg)
+        _NETS[cfg] = (net, oracle_Y(net))
+    return _NETS[cfg]
+
+
+def row_scale(Y, vm):
+    """sum_j |Y_ij| Vm_i Vm_j per bus: magnitude of the terms whose sum is P_i, Q_i (rounding scale)."""
+    row_ptr, col, g, bb = Y
+    a = np.hypot(g, bb)
+    out = np.zeros_like(vm)
+    for i in range(vm.shape[1]):
+        sl = slice(row_ptr[i], row_ptr[i + 1])
+        out[:, i] = vm[:, i] * (vm[:, col[sl]] * a[sl][None, :]).sum(axis=1)
+    return out
+
+
+# ---- a1: mismatch + norm --------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,batch,flat", [(1, 64, True), (1, 7, False), (2, 33, False), (3, 9, False), (4, 5, False),
+                                            (5, 3, False)])
+def test_mismatch_kernel(cfg, batch, flat):
+    net, Y = get_net(cfg)
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    if flat:
+        vm, va = vs.copy(), np.zeros_like(vs)
+    else:
+        vm, va = random_state(net, batch, 77 + cfg)
+    ctx = make_ctx(net, max_batch=batch)
+    f_p, f_q, nrm = ctx.debug_mismatch(dev(ps), dev(qs), dev(vm), dev(va))
+    f_p, f_q, nrm = f_p.cpu().numpy(), f_q.cpu().numpy(), nrm.cpu().numpy()
+    n, th, vmx = oracle.index_maps(net.bus_type)
+    sc = row_scale(Y, vm)
+    for b in range(batch):
+        F, r, P, Q = oracle.mismatch(Y, net.bus_type, ps[b], qs[b], vm[b], va[b])
+        for i in range(net.n_bus):
+            tol = 1e-13 * max(sc[b, i], 1.0)
+            if th[i] >= 0:
+                assert abs(f_p[b, i] - F[th[i]]) <= tol, (b, i)
+            else:
+                assert f_p[b, i] == 0.0
+            if vmx[i] >= 0:
+                assert abs(f_q[b, i] - F[vmx[i]]) <= tol, (b, i)
+            else:
+                assert f_q[b, i] == 0.0
+        assert abs(nrm[b] - r) <= 1e-13 * max(sc[b].max(), 1.0)
+    ctx.close()
+
+
+def test_mismatch_nan_propagates():
+    net, Y = get_net(1)
+    ps, qs, vs = S.make_scenarios(net, batch=2)
+    vm, va = random_state(net, 2, 5)
+    va[1, 3] = np.nan
+    ctx = make_ctx(net, max_batch=2)
+    _, _, nrm = ctx.debug_mismatch(dev(ps), dev(qs), dev(vm), dev(va))
+    nrm = nrm.cpu().numpy()
+    assert np.isfinite(nrm[0]) and np.isnan(nrm[1])
+    ctx.close()
+
+
+# ---- a2: Jacobian fill --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg,batch", [(1, 5), (2, 4), (3, 3), (4, 2)])
+def test_jacobian_fill_kernel(cfg, batch):
+    net, Y = get_net(cfg)
+    vm, va = random_state(net, batch, 177 + cfg)
+    ctx = make_ctx(net, max_batch=batch)
+    diag, pairs = ctx.debug_jacobian(dev(vm), dev(va))
+    diag, pairs = diag.cpu().numpy(), pairs.cpu().numpy()
+    sc = row_scale(Y, vm)
+    n, th, vmx = oracle.index_maps(net.bus_type)
+    rs = np.zeros((batch, n))
+    for i in range(net.n_bus):
+        if th[i] >= 0:
+            rs[:, th[i]] = sc[:, i]
+        if vmx[i] >= 0:
+            rs[:, vmx[i]] = sc[:, i]
+    for b in range(batch):
+        Jg, seen, pad_ok = gpu_jacobian_dense(ctx, net, diag[b], pairs[b])
+        Jo = oracle.jacobian_dense(Y, net.bus_type, vm[b], va[b])
+        assert pad_ok
+        _, jr, jc, _ = oracle.jacobian(Y, net.bus_type, vm[b], va[b])
+        assert seen[jr, jc].all(), "a structural J1 entry has no slot in the template"
+        err = np.abs(Jg - Jo)
+        assert (err <= 1e-13 * np.maximum(rs[b][:, None], 1.0) / 0.9).all(), err.max()
+    ctx.close()
+
+
+# ---- a4 + a5 (+ transposed, a7): one linear solve on the static pattern ---------------------------------------------
+@pytest.mark.parametrize("cfg,batch,precision", [(1, 4, sb.FP64), (2, 3, sb.FP64), (3, 3, sb.FP64), (4, 2, sb.FP64),
+                                                 (5, 2, sb.FP64), (2, 3, sb.MIXED), (4, 2, sb.MIXED)])
+@pytest.mark.parametrize("transpose", [False, True])
+def test_refactor_and_triangular_solves(cfg, batch, precision, transpose):
+    net, Y = get_net(cfg)
+    vm, va = random_state(net, batch, 277 + cfg, spread=0.05)
+    rng = np.random.Generator(np.random.PCG64(5))
+    rp = rng.standard_normal((batch, net.n_bus))
+    rq = rng.standard_normal((batch, net.n_bus))
+    ctx = make_ctx(net, max_batch=batch, precision=precision)
+    xp, xq = ctx.debug_linear_solve(dev(vm), dev(va), dev(rp), dev(rq), transpose=transpose)
+    xp, xq = xp.cpu().numpy(), xq.cpu().numpy()
+    n, th, vmx = oracle.index_maps(net.bus_type)
+    rel = 1e-9 if precision == sb.FP64 else 2e-3
+    for b in range(batch):
+        nn, jr, jc, jv = oracle.jacobian(Y, net.bus_type, vm[b], va[b])
+        rhs = np.zeros(n)
+        for i in range(net.n_bus):
+            if th[i] >= 0:
+                rhs[th[i]] = rp[b, i]
+            if vmx[i] >= 0:
+                rhs[vmx[i]] = rq[b, i]
+        x = oracle.linear_solve(n, jr, jc, jv, rhs, method=1, transpose=transpose)
+        xg = np.zeros(n)
+        for i in range(net.n_bus):
+            if th[i] >= 0:
+                xg[th[i]] = xp[b, i]
+            else:
+                assert xp[b, i] == 0.0
+            if vmx[i] >= 0:
+                xg[vmx[i]] = xq[b, i]
+            else:
+                assert xq[b, i] == 0.0
+        assert np.abs(xg - x).max() <= rel * max(1.0, np.abs(x).max()), np.abs(xg - x).max()
+    ctx.close()
+
+
+# ---- whole path: NR loop with masking, both launch modes ------------------------------------------------------------
+def check_solution(res, ref, tol, v_tol, conv_only=True):
+    it, cv = res["iterations"], res["converged"]
+    assert np.array_equal(cv, ref["converged"]), "converged flags differ"
+    assert (np.abs(it.astype(int) - ref["iterations"].astype(int)) <= 1).all()
+    ok = cv == 1
+    assert (res["final_norm"][ok] <= tol).all()
+    same = ok & (it == ref["iterations"])
+    dvm = np.abs(res["vm"] - ref["vm"]).max(axis=1)
+    dva = np.abs(res["va"] - ref["va"]).max(axis=1)
+    assert (dvm[same] <= v_tol).all() and (dva[same] <= v_tol).all(), (dvm[same].max(), dva[same].max())
+    # a scenario whose mismatch lands within rounding of tol may take one more / one fewer update (DESIGN.md reading
+    # 22): both iterates satisfy ||F|| <= tol; they differ by the size of that last step
+    edge = ok & ~same
+    if edge.any():
+        assert (dvm[edge] <= 1e-7).all() and (dva[edge] <= 1e-7).all()
+    return int(same.sum()), int(edge.sum())
+
+
+def to_np(out):
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+@pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 1024), (3, 1024), (4, 96), (5, 8)])
+@pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
+def test_nr_parity_fp64(cfg, batch, mode):
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    ctx = make_ctx(net, max_batch=batch, mode=mode, keep_factors=False)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    same, edge = check_solution(res, ref, c.tol, 1e-9)
+    assert same >= 0.9 * batch
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,batch", [(2, 256), (4, 128)])
+@pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
+def test_nr_parity_mixed_precision(cfg, batch, mode):
+    """FP64 mismatch / state, FP32 factors and solves (Table I); acceptance is against the FP64 oracle."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    ctx = make_ctx(net, max_batch=batch, mode=mode, precision=sb.MIXED, keep_factors=False)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    assert np.array_equal(res["converged"], ref["converged"])
+    assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+    ok = res["converged"] == 1
+    assert (res["final_norm"][ok] <= c.tol).all()
+    assert np.abs(res["vm"] - ref["vm"])[ok].max() <= 1e-7 and np.abs(res["va"] - ref["va"])[ok].max() <= 1e-7
+    # the reported norm is the FP64 mismatch at the returned state: re-evaluate it with the oracle
+    for b in range(0, batch, max(1, batch // 8)):
+        _, r, _, _ = oracle.mismatch(Y, net.bus_type, ps[b], qs[b], res["vm"][b], res["va"][b])
+        assert r <= c.tol * (1 + 1e-6) + 1e-12
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,batch", [(1, 64), (3, 512), (5, 6)])
+@pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
+def test_adjoint_parity(cfg, batch, mode):
+    """a7: J1(z*)^T lambda = g on the kept factors (eq. 14; reading 16)."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, mode=mode, keep_factors=True)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    check_solution(res, ref, c.tol, 1e-9)
+    # the oracle forms J1 at the GPU's returned state, so the comparison isolates the adjoint solve
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    assert (np.abs(lp - rp).max(axis=1) <= 1e-8 * scale).all()
+    assert (np.abs(lq - rq).max(axis=1) <= 1e-8 * scale).all()
+    assert (lp[:, net.slack] == 0).all() and (lq[:, net.bus_type != S.PQ] == 0).all()
+    ctx.close()
+
+
+# ---- masking, conventions, edge cases --------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
+def test_conventions_and_masking(mode):
+    net, Y = get_net(2)
+    c = net.cfg
+    batch = 48
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ps[5] *= 40.0      # infeasible: diverges or stalls -> converged = 0, iterations = max_it
+    qs[5] *= 40.0
+    ps[9, 3] = np.nan  # non-finite input: frozen at once
+    ctx = make_ctx(net, max_batch=64, mode=mode, keep_factors=False)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=12, method=1)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
+    assert res["converged"][5] == 0 and res["iterations"][5] == 12
+    assert res["converged"][9] == 0 and res["iterations"][9] == 12 and np.isnan(res["final_norm"][9])
+    check_solution(res, ref, c.tol, 1e-9)
+    # warm start at the solution: zero updates
+    res2 = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), vm0=dev(ref["vm"]), va0=dev(ref["va"]), tol=1e-7, max_it=12))
+    good = ref["converged"] == 1
+    assert (res2["iterations"][good] == 0).all() and (res2["converged"][good] == 1).all()
+    assert np.array_equal(res2["vm"][good], ref["vm"][good])
+    # max_it = 0: nothing converges from the flat start, state is the flat start
+    res3 = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=0))
+    assert (res3["converged"] == 0).all() and (res3["iterations"] == 0).all()
+    assert np.array_equal(res3["vm"][0], vs[0]) and (res3["va"] == 0).all()
+    # batch composition / order invariance (scenarios are independent blocks)
+    perm = np.random.Generator(np.random.PCG64(3)).permutation(batch)
+    res4 = to_np(ctx.solve(dev(ps[perm]), dev(qs[perm]), dev(vs[perm]), tol=c.tol, max_it=12))
+    assert np.array_equal(res4["vm"][good[perm]], res["vm"][perm][good[perm]])
+    assert np.array_equal(res4["iterations"], res["iterations"][perm])
+    ctx.close()
+
+
+def test_errors_and_empty_batch():
+    net, _ = get_net(1)
+    ctx = make_ctx(net, max_batch=4)
+    ps, qs, vs = S.make_scenarios(net, batch=8)
+    with pytest.raises(sb.SableError) as e:
+        ctx.solve(dev(ps), dev(qs), dev(vs))
+    assert e.value.status == 1
+    with pytest.raises(sb.SableError) as e:
+        ctx.adjoint(dev(ps[:4]), dev(qs[:4]))
+    assert e.value.status == 5
+    out = ctx.solve(dev(ps[:0]), dev(qs[:0]), dev(vs[:0]))
+    assert out["vm"].shape[0] == 0
+    ctx.close()
+
+
+@pytest.mark.parametrize("n_pv", [0, 9])
+def test_all_pq_and_all_pv_networks(n_pv):
+    net = S.tiny_network(10, 4, n_pv, seed=4)
+    Y = oracle_Y(net)
+    ps, qs, vs = S.make_scenarios(net, batch=8)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=1e-8, max_it=20, method=0)
+    ctx = make_ctx(net, max_batch=8)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=1e-8, max_it=20))
+    check_solution(res, ref, 1e-8, 1e-9)
+    ctx.close()
+
+
+def test_two_bus_closed_form_on_gpu():
+    """The library against the closed form directly (SURVEY §8(c) pins), not through the oracle."""
+    E, r, x, P, Q = 1.03, 0.02, 0.09, 0.8, 0.3
+    y = 1.0 / complex(r, x)
+    row_ptr = np.array([0, 2, 4], np.int32)
+    col = np.array([0, 1, 0, 1], np.int32)
+    vals = np.array([y, -y, -y, y])
+    ctx = sb.Context(2, row_ptr, col, vals.real.copy(), vals.imag.copy(), np.array([2, 0], np.uint8), 0, max_batch=1)
+    ps = np.array([[0.0, -P]])
+    qs = np.array([[0.0, -Q]])
+    vs = np.array([[E, 1.0]])
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=1e-12, max_it=20))
+    a = E * E - 2 * (r * P + x * Q)
+    v = 0.5 * (a + np.sqrt(a * a - 4 * (r * r + x * x) * (P * P + Q * Q)))
+    assert res["converged"][0] == 1
+    assert abs(res["vm"][0, 1] - np.sqrt(v)) < 1e-12
+    assert abs(res["va"][0, 1] + np.arctan2(x * P - r * Q, v + r * P + x * Q)) < 1e-12
+    ctx.close()
+
+
+# ---- full BASELINE.json sizes, in the launch configuration bench.py times (fused, max_batch = batch) -----------------
+@pytest.mark.parametrize("cfg,sample", [(2, 1024), (3, 2048), (4, 256), (5, 24)])
+def test_full_size_sampled_parity(cfg, sample):
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net)
+    ctx = make_ctx(net, max_batch=c.batch, precision=c.precision, keep_factors=c.adjoint)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    rng = np.random.Generator(np.random.PCG64(99))
+    idx = np.unique(np.concatenate([[0, c.batch - 1], rng.choice(c.batch, size=min(sample, c.batch), replace=False)]))
+    ref = oracle.nr_batch(Y, net.bus_type, ps[idx], qs[idx], vs[idx], tol=c.tol, max_it=c.max_it, method=1)
+    sub = {k: v[idx] for k, v in res.items()}
+    if c.precision == sb.FP64:
+        check_solution(sub, ref, c.tol, 1e-9)
+    else:
+        assert np.array_equal(sub["converged"], ref["converged"])
+        assert (np.abs(sub["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+        assert np.abs(sub["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(sub["va"] - ref["va"]).max() <= 1e-7
+    # properties that hold at any size: every converged scenario satisfies the tolerance; masking froze nothing early
+    assert (res["final_norm"][res["converged"] == 1] <= c.tol).all()
+    assert res["converged"].mean() >= 0.99
+    if c.adjoint:
+        gva, gvm = S.make_adjoint_rhs(net)
+        lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+        lp, lq = lp.cpu().numpy()[idx], lq.cpu().numpy()[idx]
+        rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, sub["vm"], sub["va"], gva[idx], gvm[idx], method=1)
+        scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+        assert (np.abs(lp - rp).max(axis=1) <= 1e-8 * scale).all()
+        assert (np.abs(lq - rq).max(axis=1) <= 1e-8 * scale).all()
+    ctx.close()
+
+
+def test_host_buffer_calls_match_device_calls():
+    net, Y = get_net(2)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=64)
+    gva, gvm = S.make_adjoint_rhs(net, batch=64)
+    ctx = make_ctx(net, max_batch=64)
+    a = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    la = [t.cpu().numpy() for t in ctx.adjoint(dev(gva), dev(gvm))]
+    b = ctx.solve_host(ps, qs, vs, tol=c.tol, max_it=c.max_it)
+    lb = ctx.adjoint_host(gva, gvm)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(la[0], lb[0]) and np.array_equal(la[1], lb[1])
+    ctx.close()
