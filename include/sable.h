@@ -43,7 +43,7 @@ typedef struct {
     int32_t precision;      /* SABLE_FP64 or SABLE_MIXED */
     int32_t keep_factors;   /* 1: after the NR loop, J1 is re-factored at the final iterate and the factors are kept
                                for sable_adjoint (reading 16) */
-    int32_t mode;           /* SABLE_MODE_FUSED: one persistent kernel runs the whole NR loop of a scenario on chip;
+    int32_t mode;           /* SABLE_MODE_FUSED: one persistent kernel runs the whole NR loops of the batch on chip;
                                SABLE_MODE_STAGED: one kernel per stage (mismatch / fill / refactor / solve), state in HBM
                                between stages -- used for per-stage profiling */
     int32_t device;         /* CUDA device ordinal; -1 = host-only context (symbolic phase only: sable_get_info and the
@@ -68,10 +68,12 @@ typedef struct {
     int64_t bytes_iter_m0;  /* SURVEY.md §8(d) model M0: algorithmic HBM bytes per scenario per NR iteration */
     int64_t bytes_adjoint_m0; /* same for one adjoint solve */
     int32_t smem_bytes;     /* dynamic shared memory per CTA of the NR kernel */
-    int32_t placement;      /* 0: factors, V and rhs in shared memory; 1: factors + V in HBM/L2, rhs in shared memory;
-                               2: everything in HBM/L2 */
+    int32_t placement;      /* 0: factors, V and rhs of every slot in shared memory; 1: elimination levels >= cut_level
+                               in shared memory, the wide early levels in the scenario's HBM workspace slice */
     int32_t threads;        /* threads per CTA */
     int32_t ctas_per_sm;    /* occupancy the NR kernel was sized for */
+    int32_t slots_per_cta;  /* scenarios a CTA of the NR kernel advances in lockstep */
+    int32_t cut_level;      /* placement 1: first elimination level kept in shared memory */
 } sable_info;
 
 /* Build the shared fixed-pattern template for one network (host symbolic phase, run once; PAPER.md:185-197:

@@ -40,7 +40,7 @@ class Info(C.Structure):
                 ("n_term", C.c_int64), ("n_term_diag", C.c_int64), ("lu_flops", C.c_int64),
                 ("factor_bytes", C.c_int64), ("bytes_iter_m0", C.c_int64), ("bytes_adjoint_m0", C.c_int64),
                 ("smem_bytes", C.c_int32), ("placement", C.c_int32), ("threads", C.c_int32),
-                ("ctas_per_sm", C.c_int32)]
+                ("ctas_per_sm", C.c_int32), ("slots_per_cta", C.c_int32), ("cut_level", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

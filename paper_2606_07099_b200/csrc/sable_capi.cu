@@ -17,9 +17,14 @@ struct sable_ctx {
     sable_info info{};
     DevTemplate d{};
     std::vector<void*> dev_allocs;
-    void* factors = nullptr;  double* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
-    int64_t fac_stride = 0, work_stride = 0;
-    int threads = 0, grid = 0, placement = 0, smem = 0;
+    char* factors = nullptr;  char* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
+    double* zeros = nullptr;
+    int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
+    // launch plan of the fused kernel (choose_launch) and of the one-scenario-per-CTA kernels
+    int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1;
+    int dg_cut = 0, pr_cut = 0, st_cut = 0, cut_level = 0;
+    int threads1 = 0;                                        // staged / adjoint / debug kernels
+    const LevelDesc* level_fused = nullptr; const LevelDesc* level_one = nullptr;
     int last_batch = -1;  bool have_factors = false;
     int64_t launches = 0;
     std::string err;
@@ -53,44 +58,100 @@ static void fill_info(sable_ctx* c) {
     I.n_node = T.n_node; I.n_pair = (int32_t)T.pair_col.size(); I.n_pair_j = (int32_t)T.n_pair_j;
     I.n_level = T.n_level; I.n_term = (int64_t)T.term_a.size(); I.n_term_diag = (int64_t)T.dterm.size();
     I.lu_flops = T.lu_flops;
-    I.factor_bytes = fac_elems(T.n_node, I.n_pair) * w;
+    I.factor_bytes = (int64_t)(T.n_node + 2 * (int64_t)I.n_pair) * 4 * w;
     // SURVEY.md §8(d) model M0: 8 nnzJ (a2 write) + w nnzJ (a4 read) + 2 w nnzLU (a4 write, a5 read) + 8 (10 nB + 4 n)
     I.bytes_iter_m0 = 8 * T.nnz_j + w * T.nnz_j + 2 * w * T.nnz_lu + 8 * (10 * (int64_t)T.n_bus + 4 * (int64_t)I.n);
     I.bytes_adjoint_m0 = w * T.nnz_lu + 16 * (int64_t)I.n;
     I.smem_bytes = c->smem; I.placement = c->placement; I.threads = c->threads;
-    I.ctas_per_sm = c->grid > 0 ? std::max(1, c->grid / 148) : 0;
+    I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->cut_level;
 }
 
-template <typename T> static const void* fused_fn() { return (const void*)k_nr_fused<T>; }
+static const void* fused_fn(bool mixed, bool all_smem) {
+    if (mixed) return all_smem ? (const void*)k_nr_fused<float, true> : (const void*)k_nr_fused<float, false>;
+    return all_smem ? (const void*)k_nr_fused<double, true> : (const void*)k_nr_fused<double, false>;
+}
 
-// placement / launch shape: the smallest placement number that still allows >= 2 CTAs per SM, else the smallest that fits
+static int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
+
+// lanes per target (log2) for a level with n targets whose longest list has max_len entries: as many as keep every
+// thread busy at most once, never more than a warp's share per slot
+static uint8_t pick_split(int n, int max_len, int threads, int gsh) {
+    int s = 0;
+    while ((2 << s) <= (32 >> gsh) && (int64_t)n * (2 << s) <= (threads >> gsh) && (2 << s) <= std::max(1, max_len)) ++s;
+    return (uint8_t)s;
+}
+
+static std::vector<LevelDesc> build_levels(const Template& T, int threads, int gsh) {
+    std::vector<LevelDesc> lv(T.n_level);
+    for (int l = 0; l < T.n_level; ++l) {
+        LevelDesc d{};
+        d.m0 = T.level_ptr[l]; d.m1 = T.level_ptr[l + 1]; d.p0 = T.pair_ptr[d.m0]; d.p1 = T.pair_ptr[d.m1];
+        int maxd = 0, maxt = 0, maxb = 0;
+        for (int m = d.m0; m < d.m1; ++m) {
+            maxd = std::max(maxd, T.dterm_ptr[m + 1] - T.dterm_ptr[m]);
+            maxb = std::max(maxb, T.pair_ptr[m + 1] - T.pair_ptr[m]);
+        }
+        for (int p = d.p0; p < d.p1; ++p) maxt = std::max(maxt, T.term_ptr[p + 1] - T.term_ptr[p]);
+        d.sd = pick_split(d.m1 - d.m0, maxd, threads, gsh);
+        d.sp = pick_split(d.p1 - d.p0, maxt, threads, gsh);
+        d.sb = pick_split(d.m1 - d.m0, maxb, threads, gsh);
+        lv[l] = d;
+    }
+    return lv;
+}
+
+// Launch plan of the fused kernel: as many scenario slots per CTA as fit entirely in shared
+// memory (G = 8, 4, 2, 1); if not even one fits, one slot per CTA with the top of the elimination tree (levels >=
+// cut_level) on chip and the wide early levels in the scenario's HBM slice.
 static sable_status choose_launch(sable_ctx* ctx) {
-    const int nn = ctx->T.n_node, np = (int)ctx->T.pair_col.size();
+    const Template& T = ctx->T;
+    const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
     const bool mixed = ctx->opt.precision == SABLE_MIXED;
     int dev = 0; CU(cudaGetDevice(&dev));
     int max_optin = 0, n_sm = 0, smem_sm = 0;
     CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
-    auto need = [&](int pl) { return mixed ? smem_need<float>(pl, nn, np) : smem_need<double>(pl, nn, np); };
-    int pl = 3;
-    const char* env = getenv("SABLE_PLACEMENT");
-    if (env) pl = atoi(env);
-    else {
-        for (int cand = 0; cand <= 3; ++cand) if (need(cand) + 1024 <= smem_sm / 2) { pl = cand; break; }
-        if (pl == 3) for (int cand = 0; cand <= 3; ++cand) if (need(cand) <= max_optin) { pl = cand; break; }
-    }
-    if (pl < 0 || pl > 3 || need(pl) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
+    auto need = [&](int gsh, int dgc, int prc, int stc) {
+        return mixed ? smem_need<float>(nn, np, nl, gsh, dgc, prc, stc) : smem_need<double>(nn, np, nl, gsh, dgc, prc, stc);
+    };
     int th = ctx->opt.threads;
-    if (th <= 0) { th = nn <= 64 ? 64 : nn <= 160 ? 128 : nn <= 1200 ? 256 : 512; }
-    if (const char* e2 = getenv("SABLE_THREADS")) th = atoi(e2);
-    th = std::min(1024, std::max(32, (th + 31) / 32 * 32));
-    const void* fn = mixed ? fused_fn<float>() : fused_fn<double>();
-    CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need(pl)));
+    if (th <= 0) th = nn <= 64 ? 64 : nn <= 1200 ? 256 : 512;
+    th = env_int("SABLE_THREADS", th);
+    th = std::min(512, std::max(32, (th + 31) / 32 * 32));
+    const int mb = ctx->opt.max_batch;
+    int gsh = -1, want_ctas = 1;
+    const int g_env = env_int("SABLE_G", 0);
+    for (int cand = 3; cand >= 0; --cand) {
+        if (g_env > 0 && (1 << cand) != g_env) continue;
+        if (need(cand, 0, 0, 0) > max_optin) continue;
+        // do not group more scenarios per CTA than leaves every SM a CTA (small batches stay spread out)
+        if (g_env <= 0 && cand > 0 && (int64_t)n_sm * (1 << cand) > (int64_t)mb) continue;
+        gsh = cand; break;
+    }
+    if (gsh >= 0) {
+        ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
+    } else {
+        // split placement: the smallest cut level whose top fits the per-CTA budget for `want_ctas` CTAs per SM
+        want_ctas = env_int("SABLE_CTAS", mb > n_sm ? 2 : 1);
+        const int64_t budget = std::min<int64_t>(max_optin, smem_sm / want_ctas - 1024);
+        int cl = env_int("SABLE_CUT", -1);
+        if (cl < 0) { cl = 0; while (cl < nl && need(0, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
+        cl = std::min(cl, nl);
+        const int nc = cl < nl ? T.level_ptr[cl] : nn;
+        ctx->placement = 1; ctx->gsh = 0; ctx->dg_cut = nc; ctx->st_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->cut_level = cl;
+        if (need(0, ctx->dg_cut, ctx->pr_cut, ctx->st_cut) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
+    }
+    ctx->threads = th;
+    ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
+    const void* fn = fused_fn(mixed, ctx->placement == 0);
+    CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem));
     int occ = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)need(pl)));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)ctx->smem));
     if (occ < 1) return fail(ctx, SABLE_ERR_CUDA, "NR kernel does not fit on an SM");
-    ctx->placement = pl; ctx->threads = th; ctx->smem = (int)need(pl); ctx->grid = occ * n_sm;
+    occ = std::min(occ, env_int("SABLE_CTAS", occ));
+    ctx->ctas_per_sm = occ; ctx->grid = occ * n_sm;
+    ctx->threads1 = env_int("SABLE_THREADS1", nn <= 64 ? 64 : nn <= 1200 ? 128 : 256);
     return SABLE_OK;
 }
 
@@ -124,37 +185,49 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     for (size_t k = 0; k < T.ycol.size(); ++k) ygb[k] = make_double2(T.yg[k], T.yb[k]);
     for (int m = 0; m < nn; ++m) ydg[m] = make_double2(T.yg[T.ydiag[m]], T.yb[T.ydiag[m]]);
     std::vector<double4> py(np);
+    std::vector<int2> pmj(np);
     for (int p = 0; p < np; ++p) {
         const int su = T.pair_yu[p], sl = T.pair_yl[p];
         py[p] = make_double4(su >= 0 ? T.yg[su] : 0.0, su >= 0 ? T.yb[su] : 0.0, sl >= 0 ? T.yg[sl] : 0.0, sl >= 0 ? T.yb[sl] : 0.0);
+        const int m = T.pair_row[p], j = T.pair_col[p];
+        pmj[p] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
     }
-    std::vector<int2> tab(T.term_a.size());
+    std::vector<int2> tab(T.term_a.size()), dak(T.dterm.size());
     for (size_t q = 0; q < tab.size(); ++q) tab[q] = make_int2(T.term_a[q], T.term_b[q]);
+    for (size_t q = 0; q < dak.size(); ++q) dak[q] = make_int2(T.dterm[q], T.pair_row[T.dterm[q]]);
     DevTemplate& d = c->d;
     d.n_bus = T.n_bus; d.n_node = nn; d.n_pair = np; d.n_level = T.n_level; d.slack = T.slack;
     bool ok = true;
     auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
-    up(T.level_ptr, &d.level_ptr); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
-    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(T.pair_ptr, &d.pair_ptr); up(T.pair_row, &d.pair_row);
-    up(T.pair_col, &d.pair_col); up(py, &d.pair_y); up(T.term_ptr, &d.term_ptr); up(tab, &d.term_ab);
-    up(T.dterm_ptr, &d.dterm_ptr); up(T.dterm, &d.dterm);
+    up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
+    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(T.pair_ptr, &d.pair_ptr); up(pmj, &d.pair_mj);
+    up(py, &d.pair_y); up(T.term_ptr, &d.term_ptr); up(tab, &d.term_ab);
+    up(T.dterm_ptr, &d.dterm_ptr); up(dak, &d.dterm_ak);
     if (!ok) return bail(SABLE_ERR_ALLOC);
     ctx = c;
     sable_status st = choose_launch(c);
     if (st != SABLE_OK) return bail(st);
-    const size_t w = o.precision == SABLE_MIXED ? 4 : 8;
-    c->fac_stride = fac_elems(nn, np); c->work_stride = work_doubles(nn);
+    {
+        std::vector<LevelDesc> lf = build_levels(T, c->threads, c->gsh), l1 = build_levels(T, c->threads1, 0);
+        up(lf, &c->level_fused); up(l1, &c->level_one);
+        if (!ok) return bail(SABLE_ERR_ALLOC);
+    }
+    const bool mixed = o.precision == SABLE_MIXED;
+    c->fac_stride = align16(mixed ? fac_bytes<float>(nn, np) : fac_bytes<double>(nn, np));
+    c->work_stride = work_bytes(nn);
     auto dmalloc = [&](void** p, size_t bytes) {
         if (cudaMalloc(p, bytes) != cudaSuccess) { c->err = "device allocation failed (" + std::to_string(bytes) + " bytes)"; return false; }
         c->dev_allocs.push_back(*p); return true;
     };
     const size_t mb = (size_t)o.max_batch, nb = (size_t)T.n_bus;
-    if (!dmalloc(&c->factors, mb * c->fac_stride * w) || !dmalloc((void**)&c->work, mb * c->work_stride * 8) ||
+    if (!dmalloc((void**)&c->factors, (mb + 1) * c->fac_stride) || !dmalloc((void**)&c->work, (mb + 1) * c->work_stride) ||
         !dmalloc((void**)&c->ints, (2 * mb + 4) * 4) || !dmalloc((void**)&c->hbuf, 9 * mb * nb * 8 + mb * 8) ||
-        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb))
+        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb) || !dmalloc((void**)&c->zeros, nb * 8))
         return bail(SABLE_ERR_ALLOC);
-    const void* lin = o.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
-    if (2 * (size_t)nn * 8 > 48 * 1024) cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * nn * 8);
+    if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work + mb * c->work_stride, 0, c->work_stride) != cudaSuccess ||
+        cudaMemset(c->factors + mb * c->fac_stride, 0, c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
+    const void* lin = mixed ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
+    if ((size_t)nn * 16 > 48 * 1024) cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, nn * 16);
     fill_info(c);
     *out = c;
     return SABLE_OK;
@@ -174,18 +247,23 @@ extern "C" sable_status sable_get_info(const sable_ctx* c, sable_info* info) {
 
 // ---- solve -------------------------------------------------------------------------------------------------------
 template <typename T>
-static cudaError_t launch_solve(sable_ctx* c, const SolveArgs& A, cudaStream_t s) {
+static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
     if (c->opt.mode == SABLE_MODE_FUSED) {
         cudaError_t e = cudaMemsetAsync(A.queue, 0, 4, s);
         if (e != cudaSuccess) return e;
-        const int grid = std::min(A.batch, c->grid);
-        k_nr_fused<T><<<grid, c->threads, c->smem, s>>>(A);
+        A.t.level = c->level_fused;
+        A.gsh = c->gsh; A.dg_cut = c->dg_cut; A.pr_cut = c->pr_cut; A.st_cut = c->st_cut;
+        const int G = 1 << c->gsh;
+        const int grid = std::min((A.batch + G - 1) / G, c->grid);
+        if (c->placement == 0) k_nr_fused<T, true><<<grid, c->threads, c->smem, s>>>(A);
+        else k_nr_fused<T, false><<<grid, c->threads, c->smem, s>>>(A);
         c->launches += 1;
     } else {
-        k_st_init<T><<<A.batch, c->threads, 0, s>>>(A);
+        A.t.level = c->level_one;
+        k_st_init<T><<<A.batch, c->threads1, 0, s>>>(A);
         for (int i = 0; i <= A.max_it; ++i) {
-            k_st_mismatch_fill<T><<<A.batch, c->threads, 0, s>>>(A);
-            if (i < A.max_it) k_st_factor_solve<T><<<A.batch, c->threads, 0, s>>>(A);
+            k_st_mismatch_fill<T><<<A.batch, c->threads1, 0, s>>>(A);
+            if (i < A.max_it) k_st_factor_solve<T><<<A.batch, c->threads1, 0, s>>>(A);
         }
         c->launches += 2 + 2 * (int64_t)A.max_it;
     }
@@ -206,7 +284,7 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
         return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
     CU(cudaSetDevice(ctx->opt.device));
     SolveArgs A{};
-    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.placement = ctx->placement; A.tol = tol;
+    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.trash = ctx->opt.max_batch; A.tol = tol;
     A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
     A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
     A.factors = ctx->factors; A.work = ctx->work; A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride;
@@ -221,13 +299,14 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
 static sable_status launch_lin(sable_ctx* ctx, int batch, const double* rp, const double* rq, int transposed, double* xp,
                                double* xq, cudaStream_t s) {
     LinArgs L{};
-    L.t = ctx->d; L.batch = batch; L.transposed = transposed; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
-    L.factors = ctx->factors; L.fac_stride = ctx->fac_stride;
-    const size_t sm = 2 * (size_t)ctx->T.n_node * 8;
+    L.t = ctx->d; L.t.level = ctx->level_one;
+    L.batch = batch; L.transposed = transposed; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
+    L.factors = ctx->factors; L.fac_stride = ctx->fac_stride; L.work = ctx->work; L.work_stride = ctx->work_stride;
+    const size_t sm = (size_t)ctx->T.n_node * 16;
     int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
-    const int use_smem = sm <= (size_t)max_optin;
-    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<batch, ctx->threads, use_smem ? sm : 0, s>>>(L, ctx->work, ctx->work_stride, use_smem);
-    else k_linsolve<double><<<batch, ctx->threads, use_smem ? sm : 0, s>>>(L, ctx->work, ctx->work_stride, use_smem);
+    L.rhs_in_smem = sm <= (size_t)max_optin;
+    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<batch, ctx->threads1, L.rhs_in_smem ? sm : 0, s>>>(L);
+    else k_linsolve<double><<<batch, ctx->threads1, L.rhs_in_smem ? sm : 0, s>>>(L);
     ctx->launches += 1;
     CU(cudaGetLastError());
     return SABLE_OK;
@@ -309,9 +388,10 @@ extern "C" sable_status sable_debug_pattern(const sable_ctx* c, int32_t* node_bu
 }
 
 static sable_status launch_debug(sable_ctx* ctx, DebugArgs& D, cudaStream_t s) {
-    D.t = ctx->d; D.factors = ctx->factors; D.work = ctx->work; D.fac_stride = ctx->fac_stride; D.work_stride = ctx->work_stride;
-    if (ctx->opt.precision == SABLE_MIXED) k_debug<float><<<D.batch, ctx->threads, 0, s>>>(D);
-    else k_debug<double><<<D.batch, ctx->threads, 0, s>>>(D);
+    D.t = ctx->d; D.t.level = ctx->level_one; D.zeros = ctx->zeros;
+    D.factors = ctx->factors; D.work = ctx->work; D.fac_stride = ctx->fac_stride; D.work_stride = ctx->work_stride;
+    if (ctx->opt.precision == SABLE_MIXED) k_debug<float><<<D.batch, ctx->threads1, 0, s>>>(D);
+    else k_debug<double><<<D.batch, ctx->threads1, 0, s>>>(D);
     ctx->launches += 1;
     CU(cudaGetLastError());
     return SABLE_OK;

@@ -1,22 +1,35 @@
-// Device-side view of the shared fixed-pattern template and the per-scenario stage routines of the batched
-// Newton-Raphson power flow (eq. 6-8, eq. 14).  One CTA works on one scenario; every routine below is
-// a CTA-wide cooperative step that ends WITHOUT a barrier unless stated.  The same routines serve the fused
-// persistent kernel and the staged per-stage kernels (sable_kernels.cu).
+// Device-side view of the shared fixed-pattern template and of one scenario slot's storage.
 //
 // Block conventions.  Every non-slack bus is a node with a 2x2 block: rows (P_m, Q_m), columns (theta_m, Vm_m),
-// stored row-major [dP/dth, dP/dVm, dQ/dth, dQ/dVm].  A PV node keeps the block with the Q row and Vm column
-// padded (0 off the diagonal, 1 on it).  Per scenario the factor storage is
-//   dg[4*n_node]   : J(m,m), then after refactor the INVERSE of the pivot block D_m
-//   pr[8*n_pair]   : pair p = (m,j), m < j:  pr[8p..8p+3] = J(m,j) -> U(m,j);  pr[8p+4..8p+7] = J(j,m) -> L(j,m)
+// stored row-major [dP/dth, dP/dVm, dQ/dth, dQ/dVm].  A PV node keeps the block with the Q row and Vm column padded
+// (0 off the diagonal, 1 on it).  Per scenario the factor storage is, in units of one block (4 values of T):
+//   dg[n_node]     : J(m,m), then after refactor the INVERSE of the pivot block D_m
+//   pr[2*n_pair]   : pair p = (m,j), m < j:  pr[2p] = J(m,j) -> U(m,j);  pr[2p+1] = J(j,m) -> L(j,m)
+// and the state, three 16-byte records per node (index n_node = slack):
+//   vv = (V_re, V_im)   ma = (|V|, theta)   rh = (rhs_P/theta, rhs_Q/Vm): -F, then y, then dz (g, w, lambda: adjoint)
+//
+// Placement.  A CTA works on G = 2^gsh scenarios in lockstep ("slots"; thread tid serves slot g = tid % G).  The late
+// part of every array (nodes >= cut, pairs >= cut: the top of the elimination tree, where levels are narrow and
+// latency decides) lives in shared memory, interleaved over the slots in 16-byte vectors:
+//   address = base + ((index_in_vectors << gsh) + g) * 16
+// so that the G lanes serving one target read consecutive 16-byte words (conflict-free LDS.128).  The early part
+// (wide levels: throughput decides) lives in the scenario's own contiguous slice of the HBM workspace, which is also
+// where kept factors are handed to sable_adjoint.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
 
 namespace sable {
 
+struct LevelDesc {            // one elimination level: node range, pair range, log2 of the lane split per target
+    int32_t m0, m1, p0, p1;
+    uint8_t sd, sp, sb, pad;  // diag-target, pair-target and backward-target splits (lanes per target = 1 << s)
+    int32_t pad2;
+};
+
 struct DevTemplate {
     int32_t n_bus, n_node, n_pair, n_level, slack;
-    const int32_t* level_ptr;   // [n_level+1]
+    const LevelDesc* level;     // [n_level]
     const int32_t* node_bus;    // [n_node+1]  (entry n_node = slack bus)
     const uint8_t* node_pq;     // [n_node]
     const int32_t* yptr;        // [n_node+1]  Y rows of the non-slack buses in node order
@@ -24,33 +37,17 @@ struct DevTemplate {
     const double2* ygb;         // (G, B) per stored Y entry
     const double2* ydiag_gb;    // [n_node] (G_mm, B_mm)
     const int32_t* pair_ptr;    // [n_node+1]
-    const int32_t* pair_row;    // [n_pair]
-    const int32_t* pair_col;    // [n_pair]
+    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)
     const double4* pair_y;      // [n_pair] (G_mj, B_mj, G_jm, B_jm); zeros for a fill pair
     const int32_t* term_ptr;    // [n_pair+1]
     const int2*    term_ab;     // [n_term] (pair (k,m), pair (k,j))
     const int32_t* dterm_ptr;   // [n_node+1]
-    const int32_t* dterm;       // [n_pair]
+    const int2*    dterm_ak;    // [n_pair] (pair (k,m), node k)
 };
+constexpr int kIdxMask = 0x3fffffff;
 
 template <typename T> struct Blk { T a, b, c, d; };   // [[a b][c d]]
 
-template <typename T> __device__ __forceinline__ Blk<T> ld_blk(const T* p);
-template <> __device__ __forceinline__ Blk<double> ld_blk<double>(const double* p) {
-    double2 x = *reinterpret_cast<const double2*>(p), y = *reinterpret_cast<const double2*>(p + 2);
-    return {x.x, x.y, y.x, y.y};
-}
-template <> __device__ __forceinline__ Blk<float> ld_blk<float>(const float* p) {
-    float4 x = *reinterpret_cast<const float4*>(p);
-    return {x.x, x.y, x.z, x.w};
-}
-__device__ __forceinline__ void st_blk(double* p, const Blk<double>& v) {
-    *reinterpret_cast<double2*>(p) = make_double2(v.a, v.b);
-    *reinterpret_cast<double2*>(p + 2) = make_double2(v.c, v.d);
-}
-__device__ __forceinline__ void st_blk(float* p, const Blk<float>& v) {
-    *reinterpret_cast<float4*>(p) = make_float4(v.a, v.b, v.c, v.d);
-}
 // acc -= x * y  (2x2)
 template <typename T> __device__ __forceinline__ void mulsub(Blk<T>& acc, const Blk<T>& x, const Blk<T>& y) {
     acc.a -= x.a * y.a + x.b * y.c;  acc.b -= x.a * y.b + x.b * y.d;
@@ -63,19 +60,74 @@ template <typename T> __device__ __forceinline__ Blk<T> inv(const Blk<T>& x) {
     T det = x.a * x.d - x.b * x.c, r = T(1) / det;
     return {x.d * r, -x.b * r, -x.c * r, x.a * r};
 }
+template <typename T> __device__ __forceinline__ T shx(T v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
+template <typename T> __device__ __forceinline__ void blk_add_shx(Blk<T>& v, int o) {
+    v.a += shx(v.a, o); v.b += shx(v.b, o); v.c += shx(v.c, o); v.d += shx(v.d, o);
+}
 
-// CTA-wide max of a non-negative value; NaN-propagating (a NaN anywhere gives NaN, like the paper's ||F||inf on a
-// diverged iterate, reading 18).  `red` is a shared array of >= 32 doubles.  Contains barriers.
-__device__ __forceinline__ double cta_max_nan(double v, double* red) {
-    auto mx = [](double x, double y) { return (x != x || y != y) ? __longlong_as_double(0x7ff8000000000000LL) : fmax(x, y); };
-    for (int o = 16; o > 0; o >>= 1) v = mx(v, __shfl_xor_sync(0xffffffffu, v, o));
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
+// 16-byte vector access to one block of T at p; the second vector of an FP64 block is `vs` bytes further
+__device__ __forceinline__ Blk<double> ld_blk(const double* p, int vs) {
+    const double2 x = *reinterpret_cast<const double2*>(p);
+    const double2 y = *reinterpret_cast<const double2*>(reinterpret_cast<const char*>(p) + vs);
+    return {x.x, x.y, y.x, y.y};
+}
+__device__ __forceinline__ Blk<float> ld_blk(const float* p, int) {
+    const float4 x = *reinterpret_cast<const float4*>(p);
+    return {x.x, x.y, x.z, x.w};
+}
+__device__ __forceinline__ void st_blk(double* p, int vs, const Blk<double>& v) {
+    *reinterpret_cast<double2*>(p) = make_double2(v.a, v.b);
+    *reinterpret_cast<double2*>(reinterpret_cast<char*>(p) + vs) = make_double2(v.c, v.d);
+}
+__device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
+    *reinterpret_cast<float4*>(p) = make_float4(v.a, v.b, v.c, v.d);
+}
+
+// One thread's view of the slot it serves.  kSmem = true: everything is in shared memory (cuts are 0, no branches).
+template <typename T, bool kSmem> struct Slot {
+    static constexpr int VPB = (int)(4 * sizeof(T) / 16);      // 16-byte vectors per block: 2 (FP64) or 1 (FP32)
+    char *s_dg, *s_pr, *s_vv, *s_ma, *s_rh;                   // shared bases, already offset by g * 16
+    char *g_dg, *g_pr, *g_vv, *g_ma, *g_rh;                   // this scenario's slices of the HBM workspace
+    int dg_cut, pr_cut, st_cut, gsh;                          // node cut of dg, pair cut of pr, node cut of vv/ma/rh
+
+    __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
+        if (kSmem || idx >= cut_blocks) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
+        vs = 16; return reinterpret_cast<T*>(gb + (size_t)idx * (VPB * 16));
+    }
+    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); return ld_blk(p, vs); }
+    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); st_blk(p, vs, v); }
+    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(s_pr, g_pr, 2 * p, 2 * pr_cut, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(s_pr, g_pr, 2 * p + 1, 2 * pr_cut, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr, g_pr, 2 * p, 2 * pr_cut, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr, g_pr, 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
+
+    __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
+        if (kSmem || m >= st_cut) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
+        return reinterpret_cast<double2*>(gb + (size_t)m * 16);
+    }
+    __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv, g_vv, m); }
+    __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma, g_ma, m); }
+    __device__ __forceinline__ double2 rh(int m) const { return *st_ptr(s_rh, g_rh, m); }
+    __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(s_vv, g_vv, m) = v; }
+    __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(s_ma, g_ma, m) = v; }
+    __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(s_rh, g_rh, m) = v; }
+};
+
+__device__ __forceinline__ double nan_max(double x, double y) {   // NaN-propagating max of non-negative values
+    return (x != x || y != y) ? __longlong_as_double(0x7ff8000000000000LL) : fmax(x, y);
+}
+
+// Per-slot CTA-wide max (a NaN anywhere in slot g gives NaN for g, reading 18).  `red` holds
+// (blockDim.x / 32) * 8 doubles.  Every thread returns the max over the threads that serve its slot.  Two barriers.
+__device__ __forceinline__ double slot_max_nan(double v, double* red, int gsh) {
+    for (int o = 16; o >= (1 << gsh); o >>= 1) v = nan_max(v, __shfl_xor_sync(0xffffffffu, v, o));
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5, g = threadIdx.x & ((1 << gsh) - 1);
     __syncthreads();
-    if (l == 0) red[w] = v;
+    if (l < (1 << gsh)) red[w * 8 + l] = v;
     __syncthreads();
-    v = l < nw ? red[l] : 0.0;
-    for (int o = 16; o > 0; o >>= 1) v = mx(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
+    double r = red[g];
+    for (int i = 1; i < nw; ++i) r = nan_max(r, red[i * 8 + g]);
+    return r;
 }
 
 }  // namespace sable

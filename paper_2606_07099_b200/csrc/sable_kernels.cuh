@@ -1,6 +1,6 @@
-// Kernels of the batched NR power flow: the fused persistent kernel (whole NR loop of a scenario on one CTA,
-// scenarios pulled from an atomic queue = convergence masking by construction), the staged per-stage kernels
-// (profiling mode), the adjoint kernel and the debug kernels.  Launched from sable_capi.cu.
+// The fused persistent Newton-Raphson kernel: a CTA serves G scenario slots in lockstep and runs their whole NR loops
+// on chip; a slot whose scenario converged (or stopped) is refilled from an atomic queue at once, which is the
+// per-scenario convergence masking (a converged scenario costs nothing further).  Launched from sable_capi.cu.
 #pragma once
 #include "sable_stages.cuh"
 
@@ -8,128 +8,185 @@ namespace sable {
 
 struct SolveArgs {
     DevTemplate t;
-    int32_t batch, max_it, keep, placement;
+    int32_t batch, max_it, keep, trash;                   // trash = index of the spare workspace slice (empty slots)
     double tol;
-    const double *p_spec, *q_spec, *v_set, *vm0, *va0;     // [batch][n_bus]
+    const double *p_spec, *q_spec, *v_set, *vm0, *va0;    // [batch][n_bus]
     double *vm, *va, *final_norm;
     int32_t* iterations;
     uint8_t* converged;
-    void* factors;            // [max_batch][fac_stride] of T
-    double* work;             // [max_batch][work_stride]
+    char* factors;            // [max_batch + 1][fac_stride] bytes
+    char* work;               // [max_batch + 1][work_stride] bytes
     int64_t fac_stride, work_stride;
+    int32_t gsh, dg_cut, pr_cut, st_cut;                   // slots per CTA = 1 << gsh; placement cuts (nodes, pairs, nodes)
     int32_t* queue;           // persistent-kernel scenario counter
     int32_t* status;          // staged mode: [batch] 0 = active, 1 = converged, 2 = stopped
     int32_t* it;              // staged mode: [batch]
 };
 
-__host__ __device__ inline int state_len(int n_node) { return (n_node + 2) & ~1; }          // padded array length
-__host__ __device__ inline int64_t work_doubles(int n_node) { return 8 * (int64_t)state_len(n_node); }
-__host__ __device__ inline int64_t fac_elems(int n_node, int n_pair) { return 4 * (int64_t)n_node + 8 * (int64_t)n_pair; }
-// dynamic shared memory (bytes) a placement needs, incl. 32 doubles of reduction scratch
-template <typename T> __host__ __device__ inline int64_t smem_need(int placement, int n_node, int n_pair) {
-    const int64_t na = state_len(n_node);
-    int64_t b = 32 * 8;
-    if (placement <= 1) b += 8 * na * 8;
-    else if (placement == 2) b += 2 * na * 8;              // rhs only
-    if (placement == 0) b += fac_elems(n_node, n_pair) * (int64_t)sizeof(T);
+constexpr int kSmemHeader = 2048 + 64;                     // reduction scratch + slot bookkeeping
+__host__ __device__ inline int64_t align16(int64_t x) { return (x + 15) & ~int64_t(15); }
+template <typename T> __host__ __device__ inline int64_t fac_bytes(int n_node, int n_pair) { return (int64_t)(n_node + 2 * (int64_t)n_pair) * 4 * sizeof(T); }
+__host__ __device__ inline int64_t work_bytes(int n_node) { return 3 * (int64_t)(n_node + 1) * 16; }
+// dynamic shared memory of a kernel that keeps nodes >= st_cut / dg_cut and pairs >= pr_cut on chip for 2^gsh slots
+template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, int n_pair, int n_level, int gsh, int dg_cut, int pr_cut, int st_cut) {
+    int64_t b = kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc));
+    b += (3 * (int64_t)(n_node + 1 - st_cut) * 16) << gsh;
+    b += ((int64_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh;
+    b += (2 * (int64_t)(n_pair - pr_cut) * 4 * sizeof(T)) << gsh;
     return b;
 }
 
-// placement 0: all in smem; 1: factors in HBM, state + rhs in smem; 2: rhs in smem, rest in HBM/L2; 3: all in HBM/L2
-template <typename T>
-__device__ __forceinline__ Scen<T> carve(unsigned char* smem, int placement, int n_node, int n_pair, double* work_b, T* fac_b) {
-    const int na = state_len(n_node);
-    double* sm = reinterpret_cast<double*>(smem) + 32;
-    Scen<T> s;
-    double* st = (placement <= 1) ? sm : work_b;
-    s.vre = st; s.vim = st + na; s.vmag = st + 2 * na; s.ang = st + 3 * na; s.psp = st + 4 * na; s.qsp = st + 5 * na;
-    s.rhs = (placement <= 1) ? sm + 6 * na : (placement == 2 ? sm : work_b + 6 * na);
-    T* f = (placement == 0) ? reinterpret_cast<T*>(sm + 8 * na) : fac_b;
-    s.dg = f; s.pr = f + 4 * n_node;
+// shared-memory part of a slot view (fixed for the lifetime of the CTA)
+template <typename T, bool kSmem>
+__device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
+    Slot<T, kSmem> s;
+    char* p = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc)) + g * 16;
+    const size_t ns = ((size_t)(n_node + 1 - st_cut) * 16) << gsh;
+    s.s_vv = p; s.s_ma = p + ns; s.s_rh = p + 2 * ns;
+    s.s_dg = p + 3 * ns;
+    s.s_pr = s.s_dg + (((size_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh);
+    s.g_dg = s.g_pr = s.g_vv = s.g_ma = s.g_rh = nullptr;
+    s.dg_cut = dg_cut; s.pr_cut = pr_cut; s.st_cut = st_cut; s.gsh = gsh;
     return s;
 }
+// HBM part: scenario b's slices
+template <typename T, bool kSmem>
+__device__ __forceinline__ void bind(Slot<T, kSmem>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
+    s.g_dg = factors + (size_t)b * fac_stride;
+    s.g_pr = s.g_dg + (size_t)n_node * 4 * sizeof(T);
+    s.g_vv = work + (size_t)b * work_stride;
+    s.g_ma = s.g_vv + (size_t)(n_node + 1) * 16;
+    s.g_rh = s.g_ma + (size_t)(n_node + 1) * 16;
+}
 
-template <typename T>
-__device__ __forceinline__ void scen_init(const SolveArgs& A, const Scen<T>& s, int b) {
+template <typename T, bool kSmem>
+__device__ __forceinline__ void scen_init(const SolveArgs& A, const Slot<T, kSmem>& s, int b, int tsub, int nsub) {
     const DevTemplate& t = A.t;
     const size_t o = (size_t)b * t.n_bus;
-    for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {       // PAPER.md:287 flat start unless vm0/va0 given
+    for (int m = tsub; m <= t.n_node; m += nsub) {       // PAPER.md:287 flat start unless vm0/va0 given
         const int bus = t.node_bus[m];
         const bool pq = m < t.n_node && t.node_pq[m];
         const double vm = pq ? (A.vm0 ? A.vm0[o + bus] : 1.0) : A.v_set[o + bus];
         const double th = A.va0 ? A.va0[o + bus] : 0.0;
         double sn, cs; sincos(th, &sn, &cs);
-        s.vmag[m] = vm; s.ang[m] = th; s.vre[m] = vm * cs; s.vim[m] = vm * sn;
-        if (m < t.n_node) { s.psp[m] = A.p_spec[o + bus]; s.qsp[m] = pq ? A.q_spec[o + bus] : 0.0; }
+        s.set_ma(m, make_double2(vm, th));
+        s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
 }
 
-template <typename T>
-__device__ __forceinline__ void scen_update(const DevTemplate& t, const Scen<T>& s) {   // PAPER.md:90, FP64 accumulate
-    for (int m = threadIdx.x; m < t.n_node; m += blockDim.x) {
-        const double th = s.ang[m] + s.rhs[2 * m];
-        const double vm = t.node_pq[m] ? s.vmag[m] + s.rhs[2 * m + 1] : s.vmag[m];
-        double sn, cs; sincos(th, &sn, &cs);
-        s.ang[m] = th; s.vmag[m] = vm; s.vre[m] = vm * cs; s.vim[m] = vm * sn;
-    }
-}
-
-template <typename T>
-__device__ __forceinline__ void scen_finish(const SolveArgs& A, const Scen<T>& s, int b, int it, bool conv, double r,
-                                            T* fac_b) {
+template <typename T, bool kSmem>
+__device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kSmem>& s, int b, int it, bool conv, double r, int tsub, int nsub) {
     const DevTemplate& t = A.t;
     const size_t o = (size_t)b * t.n_bus;
-    for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
+    for (int m = tsub; m <= t.n_node; m += nsub) {
         const int bus = t.node_bus[m];
-        A.vm[o + bus] = s.vmag[m]; A.va[o + bus] = s.ang[m];
+        const double2 a = s.ma(m);
+        A.vm[o + bus] = a.x; A.va[o + bus] = a.y;
     }
-    if (threadIdx.x == 0) {
+    if (tsub == 0) {
         A.iterations[b] = conv ? it : A.max_it;
         A.converged[b] = conv ? 1 : 0;
         if (A.final_norm) A.final_norm[b] = r;
     }
-    if (A.keep) {        // factors of J1 at the final iterate for the adjoint (reading 16)
-        stage_fill_pairs<T>(t, s);
-        __syncthreads();
-        stage_factor_forward<T, true, false, false>(t, s);
-        if (s.dg != fac_b) {
-            const int64_t n4 = fac_elems(t.n_node, t.n_pair) / 4;
-            for (int64_t i = threadIdx.x; i < n4; i += blockDim.x) st_blk(fac_b + 4 * i, ld_blk<T>(s.dg + 4 * i));
-        }
-    }
 }
 
-// Fused persistent kernel: loop of DESIGN.md "NR loop convention", all state on chip / in L2.
-template <typename T>
-__global__ void __launch_bounds__(1024) k_nr_fused(const SolveArgs A) {
+// kept factors (reading 16): the on-chip part of the factors of J1 at the final
+// iterate goes to the scenario's HBM slice, next to the part that already lives there
+template <typename T, bool kSmem>
+__device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
+    constexpr int VPB = Slot<T, kSmem>::VPB;
+    const int n_dg = (t.n_node - s.dg_cut) * VPB, n_pr = 2 * (t.n_pair - s.pr_cut) * VPB;
+    int4* gd = reinterpret_cast<int4*>(s.g_dg) + (size_t)s.dg_cut * VPB;
+    int4* gp = reinterpret_cast<int4*>(s.g_pr) + (size_t)2 * s.pr_cut * VPB;
+    for (int i = tsub; i < n_dg; i += nsub) gd[i] = *reinterpret_cast<const int4*>(s.s_dg + ((size_t)i << (s.gsh + 4)));
+    for (int i = tsub; i < n_pr; i += nsub) gp[i] = *reinterpret_cast<const int4*>(s.s_pr + ((size_t)i << (s.gsh + 4)));
+}
+
+__device__ __forceinline__ int pop_scenario(const SolveArgs& A) {
+    const int v = atomicAdd(A.queue, 1);
+    return v < A.batch ? v : -1;
+}
+
+// Loop convention, per slot:
+//   it = 0; loop { r = ||F1||inf; if r <= tol: converged; if it == max_it or r not finite: stop; solve; update; ++it }
+template <typename T, bool kSmem>
+__global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ int s_b;
-    double* red = reinterpret_cast<double*>(smem);
     const DevTemplate& t = A.t;
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
+    double* red = reinterpret_cast<double*>(smem);
+    int* s_b = reinterpret_cast<int*>(smem + 2048);
+    int* s_fresh = s_b + 8;
+    LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
+    for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
+    Slot<T, kSmem> s = carve<T, kSmem>(smem, t.n_node, t.n_pair, t.n_level, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    const double kInf = __longlong_as_double(0x7ff0000000000000LL);
+    int b = -1, it = 0;
+    bool fin = false;
     for (;;) {
         __syncthreads();
-        if (threadIdx.x == 0) s_b = atomicAdd(A.queue, 1);
+        if (threadIdx.x < G) s_b[threadIdx.x] = b < 0 ? pop_scenario(A) : b;
         __syncthreads();
-        const int b = s_b;
-        if (b >= A.batch) return;
-        T* fac_b = reinterpret_cast<T*>(A.factors) + (size_t)b * A.fac_stride;
-        const Scen<T> s = carve<T>(smem, A.placement, t.n_node, t.n_pair, A.work + (size_t)b * A.work_stride, fac_b);
-        scen_init<T>(A, s, b);
-        __syncthreads();
-        int it = 0; bool conv = false; double r;
-        for (;;) {
-            r = cta_max_nan(stage_mismatch<T>(t, s, true), red);
-            if (r <= A.tol) { conv = true; break; }
-            if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) break;
-            stage_fill_pairs<T>(t, s);
-            __syncthreads();
-            stage_factor_forward<T, true, true, false>(t, s);
-            stage_backward<T, false>(t, s);
-            scen_update<T>(t, s);
-            __syncthreads();
-            ++it;
+        bool need;
+        {
+            const int nb = s_b[g];
+            const bool fresh = b < 0 && nb >= 0;
+            b = nb;
+            bool any = false;
+            for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
+            if (!any) return;
+            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, b >= 0 ? b : A.trash);
+            if (fresh) { it = 0; scen_init<T, kSmem>(A, s, b, tsub, nsub); }
+            need = b >= 0;
         }
-        scen_finish<T>(A, s, b, it, conv, r, fac_b);
+        __syncthreads();
+        for (;;) {
+            const double loc = need ? stage_mismatch<T, kSmem>(t, s, A.p_spec + (size_t)b * t.n_bus, A.q_spec + (size_t)b * t.n_bus, tsub, nsub) : 0.0;
+            const double r = slot_max_nan(loc, red, gsh);
+            if (need) {
+                bool done = false, conv = false;
+                if (r <= A.tol) { done = true; conv = true; }
+                else if (it == A.max_it || !(fabs(r) < kInf)) done = true;
+                if (done) {
+                    scen_output<T, kSmem>(A, s, b, it, conv, r, tsub, nsub);
+                    if (A.keep) fin = true; else b = -1;
+                }
+            }
+            need = false;
+            if (A.keep) break;
+            __syncthreads();
+            if (threadIdx.x < G) {
+                int nb = b, fr = 0;
+                if (b < 0) { nb = pop_scenario(A); fr = nb >= 0; }
+                s_b[threadIdx.x] = nb; s_fresh[threadIdx.x] = fr;
+            }
+            __syncthreads();
+            bool anyfresh = false;
+            for (int x = 0; x < G; ++x) anyfresh |= s_fresh[x] != 0;
+            if (s_fresh[g]) {
+                b = s_b[g]; it = 0; need = true;
+                bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, b);
+                scen_init<T, kSmem>(A, s, b, tsub, nsub);
+            }
+            if (!anyfresh) break;
+            __syncthreads();
+        }
+        __syncthreads();
+        if (threadIdx.x < G) s_b[threadIdx.x] = b;
+        __syncthreads();
+        {
+            bool any = false;
+            for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
+            if (!any) return;
+            if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, A.trash);
+        }
+        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv);
+        stage_backward<T, kSmem, false, true>(t, s, lv);
+        if (b >= 0 && !fin) ++it;
+        if (fin) {
+            store_top_factors<T, kSmem>(t, s, tsub, nsub);
+            b = -1; fin = false;
+        }
     }
 }
 

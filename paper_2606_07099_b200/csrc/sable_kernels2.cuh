@@ -1,47 +1,48 @@
-// Staged (one kernel per stage, state in HBM/L2 between stages), adjoint and debug kernels.
+// Staged kernels (one kernel per stage, state in HBM between stages -- the per-stage profiling mode), the adjoint /
+// linear-solve kernel on kept factors, and the debug kernels.  All of them serve one scenario per CTA (gsh = 0).
 #pragma once
 #include "sable_kernels.cuh"
 
 namespace sable {
 
-// ---- staged mode: grid = batch, CTA b = scenario b, all arrays in the HBM workspace (placement 3 layout) -------
+// everything in the scenario's HBM slices
+template <typename T>
+__device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b) {
+    Slot<T, false> s;
+    s.s_dg = s.s_pr = s.s_vv = s.s_ma = s.s_rh = nullptr;
+    s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = 0;
+    bind<T, false>(s, factors, fac_stride, work, work_stride, t.n_node, b);
+    return s;
+}
+
 template <typename T>
 __global__ void k_st_init(const SolveArgs A) {
     const int b = blockIdx.x;
-    T* fac_b = reinterpret_cast<T*>(A.factors) + (size_t)b * A.fac_stride;
-    const Scen<T> s = carve<T>(nullptr, 3, A.t.n_node, A.t.n_pair, A.work + (size_t)b * A.work_stride, fac_b);
-    scen_init<T>(A, s, b);
+    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    scen_init<T, false>(A, s, b, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) { A.status[b] = 0; A.it[b] = 0; }
 }
 
-// a1 + a6 + a2: mismatch, norm, convergence decision, Jacobian fill for the scenarios that go on
+// a1 + a6 + a2: mismatch, norm, convergence decision, Jacobian fill (in place, into the factor value array) for the
+// scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here
 template <typename T>
 __global__ void k_st_mismatch_fill(const SolveArgs A) {
-    __shared__ double red[32];
+    __shared__ double red[32 * 8];
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
-    T* fac_b = reinterpret_cast<T*>(A.factors) + (size_t)b * A.fac_stride;
-    const Scen<T> s = carve<T>(nullptr, 3, A.t.n_node, A.t.n_pair, A.work + (size_t)b * A.work_stride, fac_b);
-    const double r = cta_max_nan(stage_mismatch<T>(A.t, s, true), red);
+    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    const double r = slot_max_nan(stage_mismatch<T, false>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus,
+                                                           threadIdx.x, blockDim.x), red, 0);
     const int it = A.it[b];
     int st = 0;
     if (r <= A.tol) st = 1;
     else if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) st = 2;
-    if (st == 0 || A.keep) stage_fill_pairs<T>(A.t, s);
+    if (st == 0 || A.keep) stage_fill_pairs<T, false>(A.t, s, threadIdx.x, blockDim.x);
     if (st != 0) {
+        scen_output<T, false>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
         __syncthreads();
-        if (threadIdx.x == 0) {
-            A.status[b] = st;
-            A.iterations[b] = st == 1 ? it : A.max_it;
-            A.converged[b] = st == 1;
-            if (A.final_norm) A.final_norm[b] = r;
-        }
-        const size_t o = (size_t)b * A.t.n_bus;
-        for (int m = threadIdx.x; m <= A.t.n_node; m += blockDim.x) {
-            const int bus = A.t.node_bus[m];
-            A.vm[o + bus] = s.vmag[m]; A.va[o + bus] = s.ang[m];
-        }
-        if (A.keep) { __syncthreads(); stage_factor_forward<T, true, false, false>(A.t, s); }
+        if (threadIdx.x == 0) A.status[b] = st;
+        if (A.keep) stage_factor_forward<T, false, true, false, false, false>(A.t, s, A.t.level);
     }
 }
 
@@ -50,47 +51,43 @@ template <typename T>
 __global__ void k_st_factor_solve(const SolveArgs A) {
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;
-    T* fac_b = reinterpret_cast<T*>(A.factors) + (size_t)b * A.fac_stride;
-    const Scen<T> s = carve<T>(nullptr, 3, A.t.n_node, A.t.n_pair, A.work + (size_t)b * A.work_stride, fac_b);
-    stage_factor_forward<T, true, true, false>(A.t, s);
-    stage_backward<T, false>(A.t, s);
-    scen_update<T>(A.t, s);
+    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    stage_factor_forward<T, false, true, true, false, false>(A.t, s, A.t.level);
+    stage_backward<T, false, false, true>(A.t, s, A.t.level);
     if (threadIdx.x == 0) A.it[b] += 1;
 }
 
 // ---- adjoint / generic linear solve on stored factors ---------------------------------------------------------
 struct LinArgs {
     DevTemplate t;
-    int32_t batch, transposed;
+    int32_t batch, transposed, rhs_in_smem;
     const double *rhs_p, *rhs_q;      // [batch][n_bus]: theta/P component and Vm/Q component per bus
     double *x_p, *x_q;
-    const void* factors; int64_t fac_stride;
+    char* factors; char* work; int64_t fac_stride, work_stride;
 };
 
 // a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, L^T lambda = w descending.
-// rhs lives in shared memory when it fits (use_smem), else in the caller's x_p/x_q is not usable -> work buffer.
+// Factors stream from the scenario's HBM slice; the right-hand side lives in shared memory when it fits.
 template <typename T>
-__global__ void k_linsolve(const LinArgs A, double* work, int64_t work_stride, int use_smem) {
+__global__ void k_linsolve(const LinArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int b = blockIdx.x;
-    Scen<T> s{};
-    s.rhs = use_smem ? reinterpret_cast<double*>(smem) : work + (size_t)b * work_stride;
-    T* f = const_cast<T*>(reinterpret_cast<const T*>(A.factors)) + (size_t)b * A.fac_stride;
-    s.dg = f; s.pr = f + 4 * t.n_node;
+    Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    if (A.rhs_in_smem) { s.st_cut = 0; s.s_rh = reinterpret_cast<char*>(smem); }
     const size_t o = (size_t)b * t.n_bus;
     for (int m = threadIdx.x; m < t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
-        s.rhs[2 * m] = A.rhs_p[o + bus];
-        s.rhs[2 * m + 1] = t.node_pq[m] ? A.rhs_q[o + bus] : 0.0;
+        s.set_rh(m, make_double2(A.rhs_p[o + bus], t.node_pq[m] ? A.rhs_q[o + bus] : 0.0));
     }
     __syncthreads();
-    if (A.transposed) { stage_factor_forward<T, false, true, true>(t, s); stage_backward<T, true>(t, s); }
-    else              { stage_factor_forward<T, false, true, false>(t, s); stage_backward<T, false>(t, s); }
+    if (A.transposed) { stage_factor_forward<T, false, false, true, true, false>(t, s, t.level); stage_backward<T, false, true, false>(t, s, t.level); }
+    else              { stage_factor_forward<T, false, false, true, false, false>(t, s, t.level); stage_backward<T, false, false, false>(t, s, t.level); }
     for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
-        A.x_p[o + bus] = m < t.n_node ? s.rhs[2 * m] : 0.0;
-        A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? s.rhs[2 * m + 1] : 0.0;
+        const double2 x = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
+        A.x_p[o + bus] = x.x;
+        A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? x.y : 0.0;
     }
 }
 
@@ -100,43 +97,47 @@ struct DebugArgs {
     int32_t batch, what;              // what: 0 mismatch, 1 jacobian, 2 refactor only (factors kept for k_linsolve)
     const double *p_spec, *q_spec, *vm, *va;
     double *f_p, *f_q, *norm, *diag, *pairs;
-    void* factors; double* work; int64_t fac_stride, work_stride;
+    char* factors; char* work; int64_t fac_stride, work_stride;
+    const double* zeros;              // [n_bus] zeros: stands in for absent p_spec / q_spec
 };
 
 template <typename T>
 __global__ void k_debug(const DebugArgs A) {
-    __shared__ double red[32];
+    __shared__ double red[32 * 8];
     const DevTemplate& t = A.t;
     const int b = blockIdx.x;
-    T* fac_b = reinterpret_cast<T*>(A.factors) + (size_t)b * A.fac_stride;
-    const Scen<T> s = carve<T>(nullptr, 3, t.n_node, t.n_pair, A.work + (size_t)b * A.work_stride, fac_b);
+    const Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
     const size_t o = (size_t)b * t.n_bus;
     for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
         const double vm = A.vm[o + bus], th = A.va[o + bus];
         double sn, cs; sincos(th, &sn, &cs);
-        s.vmag[m] = vm; s.ang[m] = th; s.vre[m] = vm * cs; s.vim[m] = vm * sn;
-        if (m < t.n_node) { s.psp[m] = A.p_spec ? A.p_spec[o + bus] : 0.0; s.qsp[m] = A.q_spec ? A.q_spec[o + bus] : 0.0; }
+        s.set_ma(m, make_double2(vm, th));
+        s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = cta_max_nan(stage_mismatch<T>(t, s, true), red);
+    const double r = slot_max_nan(stage_mismatch<T, false>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros,
+                                                           threadIdx.x, blockDim.x), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];
-            A.f_p[o + bus] = m < t.n_node ? -s.rhs[2 * m] : 0.0;
-            A.f_q[o + bus] = m < t.n_node ? -s.rhs[2 * m + 1] : 0.0;
+            const double2 f = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
+            A.f_p[o + bus] = m < t.n_node ? -f.x : 0.0;
+            A.f_q[o + bus] = m < t.n_node ? -f.y : 0.0;
         }
         if (threadIdx.x == 0) A.norm[b] = r;
         return;
     }
-    stage_fill_pairs<T>(t, s);
+    stage_fill_pairs<T, false>(t, s, threadIdx.x, blockDim.x);
     __syncthreads();
     if (A.what == 1) {
-        for (int i = threadIdx.x; i < 4 * t.n_node; i += blockDim.x) A.diag[(size_t)b * 4 * t.n_node + i] = double(s.dg[i]);
-        for (int i = threadIdx.x; i < 8 * t.n_pair; i += blockDim.x) A.pairs[(size_t)b * 8 * t.n_pair + i] = double(s.pr[i]);
+        const T* dg = reinterpret_cast<const T*>(s.g_dg);
+        const T* pr = reinterpret_cast<const T*>(s.g_pr);
+        for (int i = threadIdx.x; i < 4 * t.n_node; i += blockDim.x) A.diag[(size_t)b * 4 * t.n_node + i] = double(dg[i]);
+        for (int i = threadIdx.x; i < 8 * t.n_pair; i += blockDim.x) A.pairs[(size_t)b * 8 * t.n_pair + i] = double(pr[i]);
         return;
     }
-    stage_factor_forward<T, true, false, false>(t, s);
+    stage_factor_forward<T, false, true, false, false, false>(t, s, t.level);
 }
 
 }  // namespace sable

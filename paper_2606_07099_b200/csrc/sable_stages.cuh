@@ -1,52 +1,44 @@
-// Per-scenario stage routines (one CTA = one scenario).  See sable_device.cuh for the block conventions.
+// CTA-wide stage routines of the batched Newton-Raphson power flow (eq. 6-8, eq. 14).  A CTA serves G
+// scenario slots in lockstep: thread tid serves slot g = tid % G.  Targets of one elimination level are spread over
+// the warps; a target whose multiply-subtract list is long is served by S = 2^s consecutive lane groups that each
+// take every S-th term and combine by warp shuffles (lane = (target_in_warp, part, slot), slot fastest).
 #pragma once
 #include "sable_device.cuh"
 
 namespace sable {
 
-// Per-scenario working set.  Pointers are generic: they point into shared memory or into the scenario's slice of
-// the HBM workspace, depending on the placement chosen at sable_create (sable_info.placement).
-template <typename T> struct Scen {
-    double *vre, *vim, *vmag, *ang;   // [n_node+1] node order, entry n_node = slack
-    double *psp, *qsp;                // [n_node]   specified injections in node order
-    double *rhs;                      // [2*n_node] -F, then y, then dz (or g, w, lambda for the adjoint)
-    T *dg, *pr;                       // factors
-};
-
-// a1 (+ diagonal part of a2): S = V o conj(Ybus V), F1 rows (eq. 6), real form of
-// PAPER.md:201-207; writes rhs = -F1, the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated
-// P_i, Q_i -- PAPER.md:193, :215) and returns this thread's max |F1| (NaN-propagating).  Reads vre/vim/vmag.
-template <typename T>
-__device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Scen<T>& s, bool write_diag) {
+// a1 (+ diagonal case of a2): S = V o conj(Ybus V), F1 rows (eq. 6), real form of
+// PAPER.md:201-207; writes rh = -F1 and the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated
+// P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
+template <typename T, bool kSmem>
+__device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kSmem>& s, const double* p_row,
+                                                 const double* q_row, int tsub, int nsub) {
     double loc = 0.0;
-    for (int m = threadIdx.x; m < t.n_node; m += blockDim.x) {
+    for (int m = tsub; m < t.n_node; m += nsub) {
         double ire = 0.0, iim = 0.0;
         const int k1 = t.yptr[m + 1];
         for (int k = t.yptr[m]; k < k1; ++k) {
             const int c = t.ycol[k];
             const double2 y = t.ygb[k];
-            const double xr = s.vre[c], xi = s.vim[c];
-            ire += y.x * xr - y.y * xi;
-            iim += y.y * xr + y.x * xi;
+            const double2 x = s.vv(c);
+            ire += y.x * x.x - y.y * x.y;
+            iim += y.y * x.x + y.x * x.y;
         }
-        const double vr = s.vre[m], vi = s.vim[m], vm = s.vmag[m];
-        const double P = vr * ire + vi * iim, Q = vi * ire - vr * iim;
+        const double2 v = s.vv(m);
+        const double vm = s.ma(m).x;
+        const double P = v.x * ire + v.y * iim, Q = v.y * ire - v.x * iim;
         const bool pq = t.node_pq[m];
-        const double fp = P - s.psp[m], fq = pq ? Q - s.qsp[m] : 0.0;
-        s.rhs[2 * m] = -fp;
-        s.rhs[2 * m + 1] = -fq;
-        const double ap = fabs(fp), aq = fabs(fq);
-        if (!(ap <= loc)) loc = (ap != ap || loc != loc) ? ap + loc : ap;
-        if (!(aq <= loc)) loc = (aq != aq || loc != loc) ? aq + loc : aq;
-        if (write_diag) {
-            const double2 yd = t.ydiag_gb[m];
-            const double v2 = vm * vm;
-            Blk<T> d;
-            d.a = T(-Q - yd.y * v2);
-            if (pq) { d.b = T(P / vm + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q / vm - yd.y * vm); }
-            else    { d.b = T(0); d.c = T(0); d.d = T(1); }
-            st_blk(s.dg + 4 * m, d);
-        }
+        const int bus = t.node_bus[m];
+        const double fp = P - p_row[bus], fq = pq ? Q - q_row[bus] : 0.0;
+        s.set_rh(m, make_double2(-fp, -fq));
+        loc = nan_max(loc, nan_max(fabs(fp), fabs(fq)));
+        const double2 yd = t.ydiag_gb[m];
+        const double v2 = vm * vm;
+        Blk<T> d;
+        d.a = T(-Q - yd.y * v2);
+        if (pq) { d.b = T(P / vm + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q / vm - yd.y * vm); }
+        else    { d.b = T(0); d.c = T(0); d.d = T(1); }
+        s.stD(m, d);
     }
     return loc;
 }
@@ -54,23 +46,28 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Sce
 // a2, off-diagonal case of Alg. 1 (body reconstructed, reading 4) with
 // theta_mj = theta_m - theta_j:  a = Vm_m Vm_j cos theta_mj,  b = Vm_m Vm_j sin theta_mj
 //   dP_m/dth_j = G b - B a     dP_m/dVm_j = (G a + B b)/Vm_j     dQ_m/dth_j = -(G a + B b)     dQ_m/dVm_j = (G b - B a)/Vm_j
-// Every pair slot of the filled pattern is written (fill pairs get zeros) so refactor starts from a ready array.
-template <typename T>
-__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Scen<T>& s) {
-    for (int p = threadIdx.x; p < t.n_pair; p += blockDim.x) {
-        const int m = t.pair_row[p], j = t.pair_col[p];
-        const double4 y = t.pair_y[p];
-        const double mr = s.vre[m], mi = s.vim[m], jr = s.vre[j], ji = s.vim[j];
-        const double a = mr * jr + mi * ji, b = mi * jr - mr * ji;
-        const bool mpq = t.node_pq[m], jpq = t.node_pq[j];
-        const double ivm = mpq ? 1.0 / s.vmag[m] : 0.0, ivj = jpq ? 1.0 / s.vmag[j] : 0.0;
-        const double u1 = y.x * b - y.y * a, u2 = y.x * a + y.y * b;        // block (m,j), Y_mj
-        const double l1 = -y.z * b - y.w * a, l2 = y.z * a - y.w * b;       // block (j,m), Y_jm, theta_jm = -theta_mj
+// evaluated in FP64 and rounded to T (Table I: value update DP, solver copy SP).  Fill pairs get zeros.
+template <typename T, bool kSmem>
+__device__ __forceinline__ void fill_pair(const DevTemplate& t, const Slot<T, kSmem>& s, int p, int2 mj, Blk<T>& U, Blk<T>& L) {
+    const int m = mj.x & kIdxMask, j = mj.y & kIdxMask;
+    const bool mpq = mj.x >> 30, jpq = mj.y >> 30;
+    const double4 y = t.pair_y[p];
+    const double2 vm_ = s.vv(m), vj = s.vv(j);
+    const double a = vm_.x * vj.x + vm_.y * vj.y, b = vm_.y * vj.x - vm_.x * vj.y;
+    const double ivm = mpq ? 1.0 / s.ma(m).x : 0.0, ivj = jpq ? 1.0 / s.ma(j).x : 0.0;
+    const double u1 = y.x * b - y.y * a, u2 = y.x * a + y.y * b;        // block (m,j), Y_mj
+    const double l1 = -y.z * b - y.w * a, l2 = y.z * a - y.w * b;       // block (j,m), Y_jm, theta_jm = -theta_mj
+    U.a = T(u1);  U.b = T(u2 * ivj);  U.c = mpq ? T(-u2) : T(0);  U.d = mpq ? T(u1 * ivj) : T(0);
+    L.a = T(l1);  L.b = T(l2 * ivm);  L.c = jpq ? T(-l2) : T(0);  L.d = jpq ? T(l1 * ivm) : T(0);
+}
+
+// separate a2 pass (staged mode and debug export): every pair slot of the filled pattern is written
+template <typename T, bool kSmem>
+__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
+    for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
-        U.a = T(u1);  U.b = T(u2 * ivj);  U.c = mpq ? T(-u2) : T(0);  U.d = mpq ? T(u1 * ivj) : T(0);
-        L.a = T(l1);  L.b = T(l2 * ivm);  L.c = jpq ? T(-l2) : T(0);  L.d = jpq ? T(l1 * ivm) : T(0);
-        st_blk(s.pr + 8 * p, U);
-        st_blk(s.pr + 8 * p + 4, L);
+        fill_pair<T, kSmem>(t, s, p, t.pair_mj[p], U, L);
+        s.stU(p, U); s.stL(p, L);
     }
 }
 
@@ -78,47 +75,81 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Sce
 // inverted), fused with the forward substitution L y = rhs which walks the same lists.  Contains barriers.
 //   diag target m :  D_m = J(m,m) - sum_k L(m,k) U(k,m);   y_m = rhs_m - sum_k L(m,k) y_k      (k: pairs (k,m))
 //   pair target p :  U(m,j) = J(m,j) - sum_k L(m,k) U(k,j);  L(j,m) = (J(j,m) - sum_k L(j,k) U(k,m)) D_m^-1
-// transposed = true runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
-template <typename T, bool kFactor, bool kSolve, bool kTransposed>
-__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Scen<T>& s) {
+// kInlineFill: J(m,j), J(j,m) are evaluated here (a2 fused into a4, the value array is written once, final).
+// kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
+template <typename T, bool kSmem, bool kFactor, bool kSolve, bool kTransposed, bool kInlineFill>
+__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     for (int l = 0; l < t.n_level; ++l) {
-        const int m0 = t.level_ptr[l], m1 = t.level_ptr[l + 1];
-        for (int m = m0 + threadIdx.x; m < m1; m += blockDim.x) {
-            const int t0 = t.dterm_ptr[m], t1 = t.dterm_ptr[m + 1];
-            Blk<T> D = ld_blk<T>(s.dg + 4 * m);
-            T y0 = T(s.rhs[2 * m]), y1 = T(s.rhs[2 * m + 1]);
-            for (int q = t0; q < t1; ++q) {
-                const int a = t.dterm[q];
-                const int k = t.pair_row[a];
-                const Blk<T> U = ld_blk<T>(s.pr + 8 * a), L = ld_blk<T>(s.pr + 8 * a + 4);
-                if (kFactor) mulsub(D, L, U);
-                if (kSolve) {
-                    const T x0 = T(s.rhs[2 * k]), x1 = T(s.rhs[2 * k + 1]);
-                    if (!kTransposed) { y0 -= L.a * x0 + L.b * x1;  y1 -= L.c * x0 + L.d * x1; }
-                    else              { y0 -= U.a * x0 + U.c * x1;  y1 -= U.b * x0 + U.d * x1; }
+        const LevelDesc d = lv[l];
+        {
+            const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
+            const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
+            for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
+                const bool valid = base + tl < d.m1;
+                const int m = valid ? base + tl : d.m1 - 1;
+                const bool lead = valid && part == 0;
+                const int t0 = t.dterm_ptr[m], t1 = valid ? t.dterm_ptr[m + 1] : t0;
+                Blk<T> D = {T(0), T(0), T(0), T(0)};
+                T y0 = T(0), y1 = T(0);
+                if (lead) {
+                    if (kFactor) D = s.ldD(m);
+                    if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
                 }
-            }
-            if (kFactor) { D = inv(D); st_blk(s.dg + 4 * m, D); }
-            if (kSolve) {
-                if (kTransposed) { const T z0 = D.a * y0 + D.c * y1, z1 = D.b * y0 + D.d * y1; y0 = z0; y1 = z1; }
-                s.rhs[2 * m] = double(y0);
-                s.rhs[2 * m + 1] = double(y1);
+                for (int q = t0 + part; q < t1; q += S) {
+                    const int2 ak = t.dterm_ak[q];
+                    if (kFactor || kTransposed) {
+                        const Blk<T> U = s.ldU(ak.x);
+                        if (kFactor) mulsub(D, s.ldL(ak.x), U);
+                        if (kSolve && kTransposed) { const double2 x = s.rh(ak.y); y0 -= U.a * T(x.x) + U.c * T(x.y);  y1 -= U.b * T(x.x) + U.d * T(x.y); }
+                    }
+                    if (kSolve && !kTransposed) {
+                        const Blk<T> L = s.ldL(ak.x);
+                        const double2 x = s.rh(ak.y);
+                        y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y);
+                    }
+                }
+                for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) {
+                    if (kFactor) blk_add_shx(D, o);
+                    if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
+                }
+                if (lead) {
+                    if (kFactor) { D = inv(D); s.stD(m, D); }
+                    if (kSolve) {
+                        if (kTransposed) {
+                            if (!kFactor) D = s.ldD(m);
+                            const T z0 = D.a * y0 + D.c * y1, z1 = D.b * y0 + D.d * y1; y0 = z0; y1 = z1;
+                        }
+                        s.set_rh(m, make_double2(double(y0), double(y1)));
+                    }
+                }
             }
         }
         if (kFactor) {
             __syncthreads();
-            const int p0 = t.pair_ptr[m0], p1 = t.pair_ptr[m1];
-            for (int p = p0 + threadIdx.x; p < p1; p += blockDim.x) {
-                Blk<T> U = ld_blk<T>(s.pr + 8 * p), L = ld_blk<T>(s.pr + 8 * p + 4);
-                const int q1 = t.term_ptr[p + 1];
-                for (int q = t.term_ptr[p]; q < q1; ++q) {
-                    const int2 ab = t.term_ab[q];
-                    mulsub(U, ld_blk<T>(s.pr + 8 * ab.x + 4), ld_blk<T>(s.pr + 8 * ab.y));
-                    mulsub(L, ld_blk<T>(s.pr + 8 * ab.y + 4), ld_blk<T>(s.pr + 8 * ab.x));
+            const int ssh = d.sp, tsh = 5 - gsh - ssh, S = 1 << ssh;
+            const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
+            for (int base = d.p0 + (warp << tsh); base < d.p1; base += nwarps << tsh) {
+                const bool valid = base + tl < d.p1;
+                const int p = valid ? base + tl : d.p1 - 1;
+                const bool lead = valid && part == 0;
+                const int t0 = t.term_ptr[p], t1 = valid ? t.term_ptr[p + 1] : t0;
+                const int2 mj = t.pair_mj[p];
+                Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
+                if (lead) {
+                    if (kInlineFill) fill_pair<T, kSmem>(t, s, p, mj, U, L);
+                    else { U = s.ldU(p); L = s.ldL(p); }
                 }
-                L = mul(L, ld_blk<T>(s.dg + 4 * t.pair_row[p]));
-                st_blk(s.pr + 8 * p, U);
-                st_blk(s.pr + 8 * p + 4, L);
+                for (int q = t0 + part; q < t1; q += S) {
+                    const int2 ab = t.term_ab[q];
+                    mulsub(U, s.ldL(ab.x), s.ldU(ab.y));
+                    mulsub(L, s.ldL(ab.y), s.ldU(ab.x));
+                }
+                for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
+                if (lead) {
+                    L = mul(L, s.ldD(mj.x & kIdxMask));
+                    s.stU(p, U); s.stL(p, L);
+                }
             }
         }
         __syncthreads();
@@ -126,26 +157,44 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
 }
 
 // backward half of a5: U x = y, i.e. x_m = D_m^-1 (y_m - sum_j U(m,j) x_j) over the pairs owned by m, levels
-// descending.  transposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
-template <typename T, bool kTransposed>
-__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Scen<T>& s) {
+// descending; kUpdate applies the Newton update of PAPER.md:90 to node m in the same pass, accumulated in FP64
+// (PAPER.md:255).  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
+template <typename T, bool kSmem, bool kTransposed, bool kUpdate>
+__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     for (int l = t.n_level - 1; l >= 0; --l) {
-        const int m0 = t.level_ptr[l], m1 = t.level_ptr[l + 1];
-        for (int m = m0 + threadIdx.x; m < m1; m += blockDim.x) {
-            T y0 = T(s.rhs[2 * m]), y1 = T(s.rhs[2 * m + 1]);
-            const int p1 = t.pair_ptr[m + 1];
-            for (int p = t.pair_ptr[m]; p < p1; ++p) {
-                const int j = t.pair_col[p];
-                const T x0 = T(s.rhs[2 * j]), x1 = T(s.rhs[2 * j + 1]);
-                if (!kTransposed) { const Blk<T> U = ld_blk<T>(s.pr + 8 * p); y0 -= U.a * x0 + U.b * x1; y1 -= U.c * x0 + U.d * x1; }
-                else { const Blk<T> L = ld_blk<T>(s.pr + 8 * p + 4); y0 -= L.a * x0 + L.c * x1; y1 -= L.b * x0 + L.d * x1; }
+        const LevelDesc d = lv[l];
+        const int ssh = d.sb, tsh = 5 - gsh - ssh, S = 1 << ssh;
+        const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
+        for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
+            const bool valid = base + tl < d.m1;
+            const int m = valid ? base + tl : d.m1 - 1;
+            const bool lead = valid && part == 0;
+            const int p0 = t.pair_ptr[m], p1 = valid ? t.pair_ptr[m + 1] : p0;
+            T y0 = T(0), y1 = T(0);
+            if (lead) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
+            for (int p = p0 + part; p < p1; p += S) {
+                const int j = t.pair_mj[p].y & kIdxMask;
+                const double2 x = s.rh(j);
+                if (!kTransposed) { const Blk<T> U = s.ldU(p); y0 -= U.a * T(x.x) + U.b * T(x.y); y1 -= U.c * T(x.x) + U.d * T(x.y); }
+                else              { const Blk<T> L = s.ldL(p); y0 -= L.a * T(x.x) + L.c * T(x.y); y1 -= L.b * T(x.x) + L.d * T(x.y); }
             }
-            if (!kTransposed) {
-                const Blk<T> D = ld_blk<T>(s.dg + 4 * m);
-                const T z0 = D.a * y0 + D.b * y1, z1 = D.c * y0 + D.d * y1; y0 = z0; y1 = z1;
+            for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { y0 += shx(y0, o); y1 += shx(y1, o); }
+            if (lead) {
+                if (!kTransposed) {
+                    const Blk<T> D = s.ldD(m);
+                    const T z0 = D.a * y0 + D.b * y1, z1 = D.c * y0 + D.d * y1; y0 = z0; y1 = z1;
+                }
+                s.set_rh(m, make_double2(double(y0), double(y1)));
+                if (kUpdate) {
+                    const double2 a = s.ma(m);
+                    const double th = a.y + double(y0);
+                    const double vm = t.node_pq[m] ? a.x + double(y1) : a.x;
+                    double sn, cs; sincos(th, &sn, &cs);
+                    s.set_ma(m, make_double2(vm, th));
+                    s.set_vv(m, make_double2(vm * cs, vm * sn));
+                }
             }
-            s.rhs[2 * m] = double(y0);
-            s.rhs[2 * m + 1] = double(y1);
         }
         __syncthreads();
     }
