@@ -169,6 +169,13 @@ sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, const doubl
                                       const double* rhs_p, const double* rhs_q, int32_t transpose,
                                       double* x_p, double* x_q, void* cuda_stream);
 
+/* Per-phase cycle counters of CTA 0 of the fused kernel, accumulated since the last call (then reset).  Only when
+ * the context was created with SABLE_TIMING=1 in the environment (else SABLE_ERR_STATE).  out[4 l + 0 / 1 / 2] = cycles
+ * in the diagonal-target / pair-target / backward phase of elimination level l; out[4 L] = cycles in decision +
+ * output; out[4 L + 1] = loop trips; out[4 L + 2] = refill + init; out[4 L + 3] = mismatch + norm; L = n_level;
+ * n = entries wanted, at most 4 L + 4 (HOST out). */
+sable_status sable_debug_timing(sable_ctx* ctx, uint64_t* out, int32_t n);
+
 #ifdef __cplusplus
 }
 #endif

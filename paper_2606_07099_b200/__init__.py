@@ -48,7 +48,7 @@ class Info(C.Structure):
 
 EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
-           "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve"]
+           "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing"]
 
 
 def lib():
@@ -202,6 +202,16 @@ class Context:
                  "dterm_ptr", "dterm"]
         self._check(lib().sable_debug_pattern(self._h, *[C.c_void_p(a[k].ctypes.data) for k in order]))
         return a
+
+    def debug_timing(self):
+        """Per-phase cycle counters of CTA 0 (needs SABLE_TIMING=1 at create).
+        Returns (per_level [L][3], dict(decide_output, trips, refill_init, mismatch_norm))."""
+        L = self.info["n_level"]
+        buf = np.zeros(4 * L + 4, np.uint64)
+        self._check(lib().sable_debug_timing(self._h, C.c_void_p(buf.ctypes.data), C.c_int32(buf.size)))
+        return (buf[:4 * L].reshape(L, 4)[:, :3].astype(np.int64),
+                dict(decide_output=int(buf[4 * L]), trips=int(buf[4 * L + 1]), refill_init=int(buf[4 * L + 2]),
+                     mismatch_norm=int(buf[4 * L + 3])))
 
     def debug_mismatch(self, p_spec, q_spec, vm, va):
         import torch

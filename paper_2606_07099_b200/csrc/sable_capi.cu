@@ -19,12 +19,16 @@ struct sable_ctx {
     std::vector<void*> dev_allocs;
     char* factors = nullptr;  char* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
     double* zeros = nullptr;
+    unsigned long long* tim = nullptr;                       // SABLE_TIMING=1: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
     // launch plan of the fused kernel (choose_launch) and of the one-scenario-per-CTA kernels
     int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1;
     int dg_cut = 0, pr_cut = 0, st_cut = 0, cut_level = 0;
     int threads1 = 0;                                        // staged / adjoint / debug kernels
     const LevelDesc* level_fused = nullptr; const LevelDesc* level_one = nullptr;
+    std::vector<LevelDesc> lv_host;                          // blob offsets per level (splits filled per kernel family)
+    std::vector<char> blob_host;
+    int ring_r = 0, ring_slot = 0, first_staged = 0;
     int last_batch = -1;  bool have_factors = false;
     int64_t launches = 0;
     std::string err;
@@ -81,11 +85,50 @@ static uint8_t pick_split(int n, int max_len, int threads, int gsh) {
     return (uint8_t)s;
 }
 
-static std::vector<LevelDesc> build_levels(const Template& T, int threads, int gsh) {
-    std::vector<LevelDesc> lv(T.n_level);
+// level slices of the index program (layout: LevelDesc in sable_device.cuh)
+static void build_blobs(const Template& T, std::vector<LevelDesc>& lv, std::vector<char>& blob) {
+    lv.assign(T.n_level, LevelDesc{});
+    blob.clear();
+    auto al = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
     for (int l = 0; l < T.n_level; ++l) {
-        LevelDesc d{};
+        LevelDesc& d = lv[l];
         d.m0 = T.level_ptr[l]; d.m1 = T.level_ptr[l + 1]; d.p0 = T.pair_ptr[d.m0]; d.p1 = T.pair_ptr[d.m1];
+        const int nm = d.m1 - d.m0, np = d.p1 - d.p0;
+        const int nd = T.dterm_ptr[d.m1] - T.dterm_ptr[d.m0], nt = T.term_ptr[d.p1] - T.term_ptr[d.p0];
+        size_t o = 0;
+        o += (size_t)(nm + 1) * 4; d.o_tptr = (int32_t)o;
+        o += (size_t)(np + 1) * 4; d.o_pptr = (int32_t)o;
+        o += (size_t)(nm + 1) * 4; o = al(o, 8); d.o_dak = (int32_t)o;
+        o += (size_t)nd * 8; d.o_pmj = (int32_t)o;
+        o += (size_t)np * 8; d.o_tab = (int32_t)o;
+        o += (size_t)nt * 8; o = al(o, 32); d.o_py = (int32_t)o;
+        o += (size_t)np * 32; o = al(o, 128);
+        d.blob_off = (int32_t)blob.size(); d.blob_bytes = (int32_t)o;
+        blob.resize(blob.size() + o, 0);
+        char* base = blob.data() + d.blob_off;
+        int32_t* dptr = (int32_t*)base; int32_t* tptr = (int32_t*)(base + d.o_tptr); int32_t* pptr = (int32_t*)(base + d.o_pptr);
+        int2* dak = (int2*)(base + d.o_dak); int2* pmj = (int2*)(base + d.o_pmj); int2* tab = (int2*)(base + d.o_tab);
+        double4* py = (double4*)(base + d.o_py);
+        for (int i = 0; i <= nm; ++i) {
+            dptr[i] = T.dterm_ptr[d.m0 + i] - T.dterm_ptr[d.m0];
+            pptr[i] = (T.pair_ptr[d.m0 + i] - d.p0) | ((i < nm && T.node_pq[d.m0 + i]) ? 1 << 30 : 0);
+        }
+        for (int i = 0; i <= np; ++i) tptr[i] = T.term_ptr[d.p0 + i] - T.term_ptr[d.p0];
+        for (int q = 0; q < nd; ++q) { const int a = T.dterm[T.dterm_ptr[d.m0] + q]; dak[q] = make_int2(a, T.pair_row[a]); }
+        for (int q = 0; q < nt; ++q) tab[q] = make_int2(T.term_a[T.term_ptr[d.p0] + q], T.term_b[T.term_ptr[d.p0] + q]);
+        for (int i = 0; i < np; ++i) {
+            const int p = d.p0 + i, m = T.pair_row[p], j = T.pair_col[p], su = T.pair_yu[p], sl = T.pair_yl[p];
+            pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
+            py[i] = make_double4(su >= 0 ? T.yg[su] : 0.0, su >= 0 ? T.yb[su] : 0.0, sl >= 0 ? T.yg[sl] : 0.0, sl >= 0 ? T.yb[sl] : 0.0);
+        }
+    }
+}
+
+// lane splits for a kernel family (threads per CTA, slots per CTA) and the streamed-level flag
+static std::vector<LevelDesc> build_levels(const Template& T, const std::vector<LevelDesc>& base, int threads, int gsh, int first_staged) {
+    std::vector<LevelDesc> lv(base);
+    for (int l = 0; l < T.n_level; ++l) {
+        LevelDesc& d = lv[l];
         int maxd = 0, maxt = 0, maxb = 0;
         for (int m = d.m0; m < d.m1; ++m) {
             maxd = std::max(maxd, T.dterm_ptr[m + 1] - T.dterm_ptr[m]);
@@ -95,7 +138,7 @@ static std::vector<LevelDesc> build_levels(const Template& T, int threads, int g
         d.sd = pick_split(d.m1 - d.m0, maxd, threads, gsh);
         d.sp = pick_split(d.p1 - d.p0, maxt, threads, gsh);
         d.sb = pick_split(d.m1 - d.m0, maxb, threads, gsh);
-        lv[l] = d;
+        d.staged = l >= first_staged;
     }
     return lv;
 }
@@ -112,35 +155,53 @@ static sable_status choose_launch(sable_ctx* ctx) {
     CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    int ring_bytes = 0;
     auto need = [&](int gsh, int dgc, int prc, int stc) {
-        return mixed ? smem_need<float>(nn, np, nl, gsh, dgc, prc, stc) : smem_need<double>(nn, np, nl, gsh, dgc, prc, stc);
+        return mixed ? smem_need<float>(nn, np, nl, ring_bytes, gsh, dgc, prc, stc) : smem_need<double>(nn, np, nl, ring_bytes, gsh, dgc, prc, stc);
+    };
+    // ring candidates (slots, slot capacity): the streamed levels are the trailing run of levels whose blobs fit a slot
+    struct RingOpt { int r, cap; };
+    const int r_env = env_int("SABLE_RING_R", -1), cap_env = env_int("SABLE_RING_SLOT", -1);
+    std::vector<RingOpt> ropts = {{3, 16384}, {3, 8192}, {2, 8192}, {3, 4096}, {2, 4096}, {2, 2048}, {0, 0}};
+    if (r_env >= 0 || cap_env >= 0) ropts = {{r_env >= 0 ? r_env : 3, cap_env >= 0 ? cap_env : 8192}, {0, 0}};
+    auto set_ring = [&](const RingOpt& o) {
+        int first = nl, slot = 0;
+        if (o.r > 0) while (first > 0 && ctx->lv_host[first - 1].blob_bytes <= o.cap) { --first; slot = std::max(slot, ctx->lv_host[first].blob_bytes); }
+        if (first == nl) { ctx->ring_r = 0; ctx->ring_slot = 0; ctx->first_staged = nl; ring_bytes = 0; return; }
+        ctx->ring_r = o.r; ctx->ring_slot = slot; ctx->first_staged = first; ring_bytes = o.r * slot;
     };
     int th = ctx->opt.threads;
-    if (th <= 0) th = nn <= 64 ? 64 : nn <= 1200 ? 256 : 512;
+    if (th <= 0) th = nn <= 64 ? 64 : nn <= 200 ? 256 : (nn > 1200 && mixed) ? 256 : 512;   // measured: profiles/r01_v2_sweeps.md
     th = env_int("SABLE_THREADS", th);
     th = std::min(512, std::max(32, (th + 31) / 32 * 32));
     const int mb = ctx->opt.max_batch;
     int gsh = -1, want_ctas = 1;
     const int g_env = env_int("SABLE_G", 0);
-    for (int cand = 3; cand >= 0; --cand) {
+    for (int cand = 3; cand >= 0 && gsh < 0; --cand) {
         if (g_env > 0 && (1 << cand) != g_env) continue;
-        if (need(cand, 0, 0, 0) > max_optin) continue;
         // do not group more scenarios per CTA than leaves every SM a CTA (small batches stay spread out)
         if (g_env <= 0 && cand > 0 && (int64_t)n_sm * (1 << cand) > (int64_t)mb) continue;
-        gsh = cand; break;
+        for (const RingOpt& o : ropts) {
+            set_ring(o);
+            if (need(cand, 0, 0, 0) <= max_optin) { gsh = cand; break; }
+        }
     }
-    if (gsh >= 0) {
+    const int cut_env = env_int("SABLE_CUT", -1);
+    if (gsh >= 0 && cut_env < 0) {
         ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
     } else {
         // split placement: the smallest cut level whose top fits the per-CTA budget for `want_ctas` CTAs per SM
         want_ctas = env_int("SABLE_CTAS", mb > n_sm ? 2 : 1);
+        set_ring(ropts[0]);
         const int64_t budget = std::min<int64_t>(max_optin, smem_sm / want_ctas - 1024);
-        int cl = env_int("SABLE_CUT", -1);
-        if (cl < 0) { cl = 0; while (cl < nl && need(0, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
+        int cl = cut_env;
+        int sg = 0;
+        while ((2 << sg) <= std::max(1, g_env)) ++sg;          // slots per CTA in split placement: SABLE_G (default 1)
+        if (cl < 0) { cl = 0; while (cl < nl && need(sg, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
         cl = std::min(cl, nl);
         const int nc = cl < nl ? T.level_ptr[cl] : nn;
-        ctx->placement = 1; ctx->gsh = 0; ctx->dg_cut = nc; ctx->st_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->cut_level = cl;
-        if (need(0, ctx->dg_cut, ctx->pr_cut, ctx->st_cut) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
+        ctx->placement = 1; ctx->gsh = sg; ctx->dg_cut = nc; ctx->st_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->cut_level = cl;
+        if (need(sg, ctx->dg_cut, ctx->pr_cut, ctx->st_cut) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
     }
     ctx->threads = th;
     ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
@@ -192,24 +253,41 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         const int m = T.pair_row[p], j = T.pair_col[p];
         pmj[p] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
     }
-    std::vector<int2> tab(T.term_a.size()), dak(T.dterm.size());
-    for (size_t q = 0; q < tab.size(); ++q) tab[q] = make_int2(T.term_a[q], T.term_b[q]);
-    for (size_t q = 0; q < dak.size(); ++q) dak[q] = make_int2(T.dterm[q], T.pair_row[T.dterm[q]]);
     DevTemplate& d = c->d;
     d.n_bus = T.n_bus; d.n_node = nn; d.n_pair = np; d.n_level = T.n_level; d.slack = T.slack;
+    // mismatch pass: nodes by descending Y-row length; a row of up to 12 << s entries is served by 1 << s lanes
+    std::vector<int32_t> mm_order(nn);
+    std::vector<int4> mm_row(nn);
+    {
+        for (int m = 0; m < nn; ++m) mm_order[m] = m;
+        auto deg = [&](int m) { return T.yptr[m + 1] - T.yptr[m]; };
+        std::stable_sort(mm_order.begin(), mm_order.end(), [&](int a, int b) { return deg(a) > deg(b); });
+        auto cls = [&](int m) { int sft = 0; while (sft < 5 && deg(m) > (12 << sft)) ++sft; return sft; };
+        d.n_class = 0;
+        for (int i = 0; i < nn;) {
+            int j = i; const int sft = cls(mm_order[i]);
+            while (j < nn && cls(mm_order[j]) == sft) ++j;
+            d.mm_class[d.n_class++] = RowClass{i, j, sft};
+            i = j;
+        }
+        for (int i = 0; i < nn; ++i) {
+            const int m = mm_order[i];
+            mm_row[i] = make_int4(m, T.yptr[m], T.yptr[m + 1], T.node_bus[m] | (T.node_pq[m] ? 1 << 30 : 0));
+        }
+    }
     bool ok = true;
     auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
-    up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
-    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(T.pair_ptr, &d.pair_ptr); up(pmj, &d.pair_mj);
-    up(py, &d.pair_y); up(T.term_ptr, &d.term_ptr); up(tab, &d.term_ab);
-    up(T.dterm_ptr, &d.dterm_ptr); up(dak, &d.dterm_ak);
+    up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
+    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(pmj, &d.pair_mj); up(py, &d.pair_y);
     if (!ok) return bail(SABLE_ERR_ALLOC);
     ctx = c;
+    build_blobs(T, c->lv_host, c->blob_host);
     sable_status st = choose_launch(c);
     if (st != SABLE_OK) return bail(st);
     {
-        std::vector<LevelDesc> lf = build_levels(T, c->threads, c->gsh), l1 = build_levels(T, c->threads1, 0);
-        up(lf, &c->level_fused); up(l1, &c->level_one);
+        std::vector<LevelDesc> lf = build_levels(T, c->lv_host, c->threads, c->gsh, c->first_staged);
+        std::vector<LevelDesc> l1 = build_levels(T, c->lv_host, c->threads1, 0, T.n_level);
+        up(lf, &c->level_fused); up(l1, &c->level_one); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
     }
     const bool mixed = o.precision == SABLE_MIXED;
@@ -226,6 +304,11 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         return bail(SABLE_ERR_ALLOC);
     if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work + mb * c->work_stride, 0, c->work_stride) != cudaSuccess ||
         cudaMemset(c->factors + mb * c->fac_stride, 0, c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
+    if (env_int("SABLE_TIMING", 0)) {
+        const size_t tb = (4 * (size_t)T.n_level + 4) * 8;
+        if (!dmalloc((void**)&c->tim, tb)) return bail(SABLE_ERR_ALLOC);
+        cudaMemset(c->tim, 0, tb);
+    }
     const void* lin = mixed ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
     if ((size_t)nn * 16 > 48 * 1024) cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, nn * 16);
     fill_info(c);
@@ -253,6 +336,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         if (e != cudaSuccess) return e;
         A.t.level = c->level_fused;
         A.gsh = c->gsh; A.dg_cut = c->dg_cut; A.pr_cut = c->pr_cut; A.st_cut = c->st_cut;
+        A.ring_r = c->ring_r; A.ring_slot = c->ring_slot; A.first_staged = c->first_staged;
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
         if (c->placement == 0) k_nr_fused<T, true><<<grid, c->threads, c->smem, s>>>(A);
@@ -288,6 +372,7 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
     A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
     A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
     A.factors = ctx->factors; A.work = ctx->work; A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride;
+    A.tim = ctx->tim;
     A.queue = ctx->ints; A.status = ctx->ints + 4; A.it = ctx->ints + 4 + ctx->opt.max_batch;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     CU(ctx->opt.precision == SABLE_MIXED ? launch_solve<float>(ctx, A, s) : launch_solve<double>(ctx, A, s));
@@ -371,6 +456,15 @@ extern "C" sable_status sable_adjoint_host(sable_ctx* ctx, int32_t batch, const 
     CU(cudaMemcpyAsync(lam_p, d + 7 * n, bytes, cudaMemcpyDeviceToHost, 0));
     CU(cudaMemcpyAsync(lam_q, d + 8 * n, bytes, cudaMemcpyDeviceToHost, 0));
     CU(cudaStreamSynchronize(0));
+    return SABLE_OK;
+}
+
+extern "C" sable_status sable_debug_timing(sable_ctx* ctx, uint64_t* out, int32_t n) {
+    if (!ctx || !out) return SABLE_ERR_INVALID_ARG;
+    if (!ctx->tim) return fail(ctx, SABLE_ERR_STATE, "timing counters are off (create the context with SABLE_TIMING=1 in the environment)");
+    const int have = 4 * ctx->T.n_level + 4;
+    CU(cudaMemcpy(out, ctx->tim, (size_t)std::min(n, have) * 8, cudaMemcpyDeviceToHost));
+    CU(cudaMemset(ctx->tim, 0, (size_t)have * 8));
     return SABLE_OK;
 }
 

@@ -21,28 +21,44 @@
 
 namespace sable {
 
-struct LevelDesc {            // one elimination level: node range, pair range, log2 of the lane split per target
+// One elimination level: node range [m0, m1), the pairs those nodes own [p0, p1), the lane split per target, and the
+// level's slice of the index program ("blob": everything the factor / forward / backward phases of this level read
+// besides values).  Blob layout (byte offsets from the blob start; counts nm = m1 - m0, np = p1 - p0):
+//   int32 dptr[nm+1]   diag target i subtracts the terms dak[dptr[i] .. dptr[i+1])
+//   int32 tptr[np+1]   pair target i subtracts the terms tab[tptr[i] .. tptr[i+1])
+//   int32 pptr[nm+1]   node i owns the pairs p0 + [pptr[i] & kIdxMask, pptr[i+1] & kIdxMask); bit 30 of pptr[i] = PQ node
+//   int2  dak[]        (pair (k,m), node k)                                  at o_dak
+//   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                      at o_pmj
+//   int2  tab[]        (pair (k,m), pair (k,j))                              at o_tab
+//   double4 py[np]     (G_mj, B_mj, G_jm, B_jm), zeros for a fill pair       at o_py
+// Narrow levels (staged = 1) are streamed through a shared-memory ring by cp.async.bulk one or two levels ahead of
+// use, so that no index load of the latency-critical top of the elimination tree goes to L2; wide levels are read
+// in place (their latency hides behind the many targets in flight).
+struct LevelDesc {
     int32_t m0, m1, p0, p1;
-    uint8_t sd, sp, sb, pad;  // diag-target, pair-target and backward-target splits (lanes per target = 1 << s)
-    int32_t pad2;
+    uint8_t sd, sp, sb, staged;   // diag / pair / backward lane splits (lanes per target = 1 << s)
+    int32_t blob_off, blob_bytes; // slice of DevTemplate::blob (16-byte aligned, size a multiple of 16)
+    int32_t o_tptr, o_pptr, o_dak, o_pmj, o_tab, o_py;
+    int32_t pad;
 };
+
+struct RowClass { int32_t i0, i1, ssh; };   // rows mm_order[i0 .. i1) of the mismatch pass are served by 1 << ssh lanes each
 
 struct DevTemplate {
     int32_t n_bus, n_node, n_pair, n_level, slack;
+    int32_t n_class;            // mismatch pass: nodes sorted by Y-row length, long rows split over lanes
+    RowClass mm_class[6];
+    const int4* mm_row;         // [n_node] (node m, first Y slot, end Y slot, bus | pq << 30), longest rows first
     const LevelDesc* level;     // [n_level]
+    const char* blob;           // level slices of the index program
     const int32_t* node_bus;    // [n_node+1]  (entry n_node = slack bus)
     const uint8_t* node_pq;     // [n_node]
     const int32_t* yptr;        // [n_node+1]  Y rows of the non-slack buses in node order
     const int32_t* ycol;        // node positions (slack = n_node)
     const double2* ygb;         // (G, B) per stored Y entry
     const double2* ydiag_gb;    // [n_node] (G_mm, B_mm)
-    const int32_t* pair_ptr;    // [n_node+1]
-    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)
-    const double4* pair_y;      // [n_pair] (G_mj, B_mj, G_jm, B_jm); zeros for a fill pair
-    const int32_t* term_ptr;    // [n_pair+1]
-    const int2*    term_ab;     // [n_term] (pair (k,m), pair (k,j))
-    const int32_t* dterm_ptr;   // [n_node+1]
-    const int2*    dterm_ak;    // [n_pair] (pair (k,m), node k)
+    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)   (separate fill pass only)
+    const double4* pair_y;      // [n_pair]                                     (separate fill pass only)
 };
 constexpr int kIdxMask = 0x3fffffff;
 
@@ -111,6 +127,71 @@ template <typename T, bool kSmem> struct Slot {
     __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(s_vv, g_vv, m) = v; }
     __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(s_ma, g_ma, m) = v; }
     __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(s_rh, g_rh, m) = v; }
+};
+
+// ---- level-blob ring: cp.async.bulk (TMA 1-D bulk copy) + mbarrier ------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* b) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity) {
+    asm volatile("{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
+                 ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+
+// The staged levels [first, n_level) are visited forward then backward, once per sweep pair; entry e of that endless
+// sequence lives in ring slot e % R.  Thread 0 is the producer; every thread consumes and tracks `use` itself.
+struct BlobRing {
+    char* slots; unsigned long long* mbar;
+    const char* gblob; const LevelDesc* lv;
+    int R, slot_bytes, first, n_level;
+    unsigned use;
+    unsigned long long* tim;   // optional per-phase cycle counters of CTA 0 (sable_debug_timing); nullptr = off
+    __device__ __forceinline__ void tick(int slot, long long& t0) const {   // thread 0 of CTA 0, right after a barrier
+        if (tim && threadIdx.x == 0) { const long long t1 = clock64(); tim[slot] += (unsigned long long)(t1 - t0); t0 = t1; }
+    }
+    __device__ __forceinline__ int level_of(unsigned e) const {
+        const int ns = n_level - first, r = (int)(e % (unsigned)(2 * ns));
+        return r < ns ? first + r : n_level - 1 - (r - ns);
+    }
+    __device__ __forceinline__ void issue(unsigned e) const {          // producer thread only
+        const LevelDesc& d = lv[level_of(e)];
+        const int sl = (int)(e % (unsigned)R);
+        mbar_expect_tx(mbar + sl, (uint32_t)d.blob_bytes);
+        bulk_g2s(slots + (size_t)sl * slot_bytes, gblob + d.blob_off, (uint32_t)d.blob_bytes, mbar + sl);
+    }
+    __device__ __forceinline__ void start() {                          // all threads, once; contains a barrier
+        use = 0;
+        if (first < n_level && threadIdx.x == 0) {
+            for (int i = 0; i < R; ++i) mbar_init(mbar + i, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        if (first < n_level && threadIdx.x == 0) for (int i = 0; i < R; ++i) issue((unsigned)i);
+    }
+    __device__ __forceinline__ const char* acquire(int l, const LevelDesc& d) const {
+        if (l < first) return gblob + d.blob_off;
+        const int sl = (int)(use % (unsigned)R);
+        mbar_wait(mbar + sl, (use / (unsigned)R) & 1u);
+        return slots + (size_t)sl * slot_bytes;
+    }
+    // after a CTA barrier that follows the last read of level l's blob
+    __device__ __forceinline__ void release(int l) {
+        if (l < first) return;
+        if (threadIdx.x == 0) issue(use + (unsigned)R);
+        ++use;
+    }
+    __device__ __forceinline__ void drain() const {                    // before the CTA exits: no copy may be in flight
+        if (first < n_level && threadIdx.x == 0)
+            for (unsigned e = use; e < use + (unsigned)R; ++e) mbar_wait(mbar + (e % (unsigned)R), (e / (unsigned)R) & 1u);
+    }
 };
 
 __device__ __forceinline__ double nan_max(double x, double y) {   // NaN-propagating max of non-negative values

@@ -18,18 +18,23 @@ struct SolveArgs {
     char* work;               // [max_batch + 1][work_stride] bytes
     int64_t fac_stride, work_stride;
     int32_t gsh, dg_cut, pr_cut, st_cut;                   // slots per CTA = 1 << gsh; placement cuts (nodes, pairs, nodes)
+    int32_t ring_r, ring_slot, first_staged;               // level-blob ring: slots, bytes per slot, first streamed level
+    unsigned long long* tim;  // optional cycle counters (sable_debug_timing), else nullptr
     int32_t* queue;           // persistent-kernel scenario counter
     int32_t* status;          // staged mode: [batch] 0 = active, 1 = converged, 2 = stopped
     int32_t* it;              // staged mode: [batch]
 };
 
-constexpr int kSmemHeader = 2048 + 64;                     // reduction scratch + slot bookkeeping
+constexpr int kSmemHeader = 2048 + 64 + 64;                // reduction scratch + slot bookkeeping + ring mbarriers
 __host__ __device__ inline int64_t align16(int64_t x) { return (x + 15) & ~int64_t(15); }
 template <typename T> __host__ __device__ inline int64_t fac_bytes(int n_node, int n_pair) { return (int64_t)(n_node + 2 * (int64_t)n_pair) * 4 * sizeof(T); }
 __host__ __device__ inline int64_t work_bytes(int n_node) { return 3 * (int64_t)(n_node + 1) * 16; }
 // dynamic shared memory of a kernel that keeps nodes >= st_cut / dg_cut and pairs >= pr_cut on chip for 2^gsh slots
-template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, int n_pair, int n_level, int gsh, int dg_cut, int pr_cut, int st_cut) {
-    int64_t b = kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc));
+__host__ __device__ inline int64_t smem_fixed(int n_level, int ring_bytes) {
+    return kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc)) + align16(ring_bytes);
+}
+template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut) {
+    int64_t b = smem_fixed(n_level, ring_bytes);
     b += (3 * (int64_t)(n_node + 1 - st_cut) * 16) << gsh;
     b += ((int64_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh;
     b += (2 * (int64_t)(n_pair - pr_cut) * 4 * sizeof(T)) << gsh;
@@ -38,9 +43,9 @@ template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, i
 
 // shared-memory part of a slot view (fixed for the lifetime of the CTA)
 template <typename T, bool kSmem>
-__device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
+__device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
     Slot<T, kSmem> s;
-    char* p = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc)) + g * 16;
+    char* p = reinterpret_cast<char*>(smem) + smem_fixed(n_level, ring_bytes) + g * 16;
     const size_t ns = ((size_t)(n_node + 1 - st_cut) * 16) << gsh;
     s.s_vv = p; s.s_ma = p + ns; s.s_rh = p + 2 * ns;
     s.s_dg = p + 3 * ns;
@@ -119,7 +124,16 @@ __global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
     int* s_fresh = s_b + 8;
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
     for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
-    Slot<T, kSmem> s = carve<T, kSmem>(smem, t.n_node, t.n_pair, t.n_level, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    Slot<T, kSmem> s = carve<T, kSmem>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    BlobRing ring;
+    ring.slots = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)t.n_level * (int64_t)sizeof(LevelDesc));
+    ring.mbar = reinterpret_cast<unsigned long long*>(smem + 2048 + 64);
+    ring.gblob = t.blob; ring.lv = lv; ring.R = A.ring_r; ring.slot_bytes = A.ring_slot;
+    ring.first = A.first_staged; ring.n_level = t.n_level;
+    ring.tim = blockIdx.x == 0 ? A.tim : nullptr;
+    long long tk = clock64();
+    __syncthreads();                                       // lv[] complete before the producer reads it
+    ring.start();
     const double kInf = __longlong_as_double(0x7ff0000000000000LL);
     int b = -1, it = 0;
     bool fin = false;
@@ -134,15 +148,18 @@ __global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
             b = nb;
             bool any = false;
             for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
-            if (!any) return;
+            if (!any) { ring.drain(); return; }
             bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, b >= 0 ? b : A.trash);
             if (fresh) { it = 0; scen_init<T, kSmem>(A, s, b, tsub, nsub); }
             need = b >= 0;
         }
         __syncthreads();
+        ring.tick(4 * t.n_level + 2, tk);                  // refill + init
         for (;;) {
-            const double loc = need ? stage_mismatch<T, kSmem>(t, s, A.p_spec + (size_t)b * t.n_bus, A.q_spec + (size_t)b * t.n_bus, tsub, nsub) : 0.0;
+            const size_t row = (size_t)(need ? b : 0) * t.n_bus;
+            const double loc = stage_mismatch<T, kSmem>(t, s, A.p_spec + row, A.q_spec + row, need);
             const double r = slot_max_nan(loc, red, gsh);
+            ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
             if (need) {
                 bool done = false, conv = false;
                 if (r <= A.tol) { done = true; conv = true; }
@@ -177,11 +194,14 @@ __global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
         {
             bool any = false;
             for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
-            if (!any) return;
+            if (!any) { ring.drain(); return; }
             if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, A.trash);
         }
-        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv);
-        stage_backward<T, kSmem, false, true>(t, s, lv);
+        ring.tick(4 * t.n_level, tk);                      // refill + init + mismatch + norm + decision + output
+        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv, ring);
+        stage_backward<T, kSmem, false>(t, s, lv, ring);
+        stage_update<T, kSmem>(t, s, tsub, nsub);
+        if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
         if (b >= 0 && !fin) ++it;
         if (fin) {
             store_top_factors<T, kSmem>(t, s, tsub, nsub);

@@ -15,6 +15,14 @@ __device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* f
     return s;
 }
 
+// index program read in place (no shared-memory ring)
+__device__ __forceinline__ BlobRing no_ring(const DevTemplate& t) {
+    BlobRing r;
+    r.slots = nullptr; r.mbar = nullptr; r.gblob = t.blob; r.lv = t.level; r.R = 0; r.slot_bytes = 0;
+    r.first = t.n_level; r.n_level = t.n_level; r.use = 0; r.tim = nullptr;
+    return r;
+}
+
 template <typename T>
 __global__ void k_st_init(const SolveArgs A) {
     const int b = blockIdx.x;
@@ -31,8 +39,7 @@ __global__ void k_st_mismatch_fill(const SolveArgs A) {
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
     const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    const double r = slot_max_nan(stage_mismatch<T, false>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus,
-                                                           threadIdx.x, blockDim.x), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, false>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true), red, 0);
     const int it = A.it[b];
     int st = 0;
     if (r <= A.tol) st = 1;
@@ -42,7 +49,7 @@ __global__ void k_st_mismatch_fill(const SolveArgs A) {
         scen_output<T, false>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
         __syncthreads();
         if (threadIdx.x == 0) A.status[b] = st;
-        if (A.keep) stage_factor_forward<T, false, true, false, false, false>(A.t, s, A.t.level);
+        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, false, true, false, false, false>(A.t, s, A.t.level, ring); }
     }
 }
 
@@ -52,8 +59,10 @@ __global__ void k_st_factor_solve(const SolveArgs A) {
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;
     const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    stage_factor_forward<T, false, true, true, false, false>(A.t, s, A.t.level);
-    stage_backward<T, false, false, true>(A.t, s, A.t.level);
+    BlobRing ring = no_ring(A.t);
+    stage_factor_forward<T, false, true, true, false, false>(A.t, s, A.t.level, ring);
+    stage_backward<T, false, false>(A.t, s, A.t.level, ring);
+    stage_update<T, false>(A.t, s, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) A.it[b] += 1;
 }
 
@@ -81,8 +90,9 @@ __global__ void k_linsolve(const LinArgs A) {
         s.set_rh(m, make_double2(A.rhs_p[o + bus], t.node_pq[m] ? A.rhs_q[o + bus] : 0.0));
     }
     __syncthreads();
-    if (A.transposed) { stage_factor_forward<T, false, false, true, true, false>(t, s, t.level); stage_backward<T, false, true, false>(t, s, t.level); }
-    else              { stage_factor_forward<T, false, false, true, false, false>(t, s, t.level); stage_backward<T, false, false, false>(t, s, t.level); }
+    BlobRing ring = no_ring(t);
+    if (A.transposed) { stage_factor_forward<T, false, false, true, true, false>(t, s, t.level, ring); stage_backward<T, false, true>(t, s, t.level, ring); }
+    else              { stage_factor_forward<T, false, false, true, false, false>(t, s, t.level, ring); stage_backward<T, false, false>(t, s, t.level, ring); }
     for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
         const double2 x = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
@@ -116,8 +126,7 @@ __global__ void k_debug(const DebugArgs A) {
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = slot_max_nan(stage_mismatch<T, false>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros,
-                                                           threadIdx.x, blockDim.x), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, false>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];
@@ -137,7 +146,8 @@ __global__ void k_debug(const DebugArgs A) {
         for (int i = threadIdx.x; i < 8 * t.n_pair; i += blockDim.x) A.pairs[(size_t)b * 8 * t.n_pair + i] = double(pr[i]);
         return;
     }
-    stage_factor_forward<T, false, true, false, false, false>(t, s, t.level);
+    BlobRing ring = no_ring(t);
+    stage_factor_forward<T, false, true, false, false, false>(t, s, t.level, ring);
 }
 
 }  // namespace sable

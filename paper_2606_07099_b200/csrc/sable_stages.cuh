@@ -12,33 +12,48 @@ namespace sable {
 // P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
 template <typename T, bool kSmem>
 __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kSmem>& s, const double* p_row,
-                                                 const double* q_row, int tsub, int nsub) {
+                                                 const double* q_row, bool act) {
+    // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
+    // the evaluation (act = false) takes part in the shuffles and writes nothing
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     double loc = 0.0;
-    for (int m = tsub; m < t.n_node; m += nsub) {
-        double ire = 0.0, iim = 0.0;
-        const int k1 = t.yptr[m + 1];
-        for (int k = t.yptr[m]; k < k1; ++k) {
-            const int c = t.ycol[k];
-            const double2 y = t.ygb[k];
-            const double2 x = s.vv(c);
-            ire += y.x * x.x - y.y * x.y;
-            iim += y.y * x.x + y.x * x.y;
+    for (int c = 0; c < t.n_class; ++c) {
+        const RowClass rc = t.mm_class[c];
+        const int ssh = min(rc.ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
+        const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
+        for (int base = rc.i0 + (warp << tsh); base < rc.i1; base += nwarps << tsh) {
+            const bool valid = base + tl < rc.i1;
+            const int4 row = t.mm_row[valid ? base + tl : rc.i1 - 1];
+            const int m = row.x;
+            const bool lead = valid && part == 0 && act;
+            double ire = 0.0, iim = 0.0;
+            const int k1 = valid ? row.z : 0;
+            for (int k = row.y + part; k < k1; k += S) {
+                const int col = t.ycol[k];
+                const double2 y = t.ygb[k];
+                const double2 x = s.vv(col);
+                ire += y.x * x.x - y.y * x.y;
+                iim += y.y * x.x + y.x * x.y;
+            }
+            for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { ire += shx(ire, o); iim += shx(iim, o); }
+            if (lead) {
+                const double2 v = s.vv(m);
+                const double vm = s.ma(m).x;
+                const double P = v.x * ire + v.y * iim, Q = v.y * ire - v.x * iim;
+                const bool pq = row.w >> 30;
+                const int bus = row.w & kIdxMask;
+                const double fp = P - p_row[bus], fq = pq ? Q - q_row[bus] : 0.0;
+                s.set_rh(m, make_double2(-fp, -fq));
+                loc = nan_max(loc, nan_max(fabs(fp), fabs(fq)));
+                const double2 yd = t.ydiag_gb[m];
+                const double v2 = vm * vm, iv = 1.0 / vm;
+                Blk<T> d;
+                d.a = T(-Q - yd.y * v2);
+                if (pq) { d.b = T(P * iv + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q * iv - yd.y * vm); }
+                else    { d.b = T(0); d.c = T(0); d.d = T(1); }
+                s.stD(m, d);
+            }
         }
-        const double2 v = s.vv(m);
-        const double vm = s.ma(m).x;
-        const double P = v.x * ire + v.y * iim, Q = v.y * ire - v.x * iim;
-        const bool pq = t.node_pq[m];
-        const int bus = t.node_bus[m];
-        const double fp = P - p_row[bus], fq = pq ? Q - q_row[bus] : 0.0;
-        s.set_rh(m, make_double2(-fp, -fq));
-        loc = nan_max(loc, nan_max(fabs(fp), fabs(fq)));
-        const double2 yd = t.ydiag_gb[m];
-        const double v2 = vm * vm;
-        Blk<T> d;
-        d.a = T(-Q - yd.y * v2);
-        if (pq) { d.b = T(P / vm + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q / vm - yd.y * vm); }
-        else    { d.b = T(0); d.c = T(0); d.d = T(1); }
-        s.stD(m, d);
     }
     return loc;
 }
@@ -48,10 +63,9 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
 //   dP_m/dth_j = G b - B a     dP_m/dVm_j = (G a + B b)/Vm_j     dQ_m/dth_j = -(G a + B b)     dQ_m/dVm_j = (G b - B a)/Vm_j
 // evaluated in FP64 and rounded to T (Table I: value update DP, solver copy SP).  Fill pairs get zeros.
 template <typename T, bool kSmem>
-__device__ __forceinline__ void fill_pair(const DevTemplate& t, const Slot<T, kSmem>& s, int p, int2 mj, Blk<T>& U, Blk<T>& L) {
+__device__ __forceinline__ void fill_pair(const Slot<T, kSmem>& s, int2 mj, double4 y, Blk<T>& U, Blk<T>& L) {
     const int m = mj.x & kIdxMask, j = mj.y & kIdxMask;
     const bool mpq = mj.x >> 30, jpq = mj.y >> 30;
-    const double4 y = t.pair_y[p];
     const double2 vm_ = s.vv(m), vj = s.vv(j);
     const double a = vm_.x * vj.x + vm_.y * vj.y, b = vm_.y * vj.x - vm_.x * vj.y;
     const double ivm = mpq ? 1.0 / s.ma(m).x : 0.0, ivj = jpq ? 1.0 / s.ma(j).x : 0.0;
@@ -66,7 +80,7 @@ template <typename T, bool kSmem>
 __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
     for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
-        fill_pair<T, kSmem>(t, s, p, t.pair_mj[p], U, L);
+        fill_pair<T, kSmem>(s, t.pair_mj[p], t.pair_y[p], U, L);
         s.stU(p, U); s.stL(p, L);
     }
 }
@@ -78,10 +92,18 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slo
 // kInlineFill: J(m,j), J(j,m) are evaluated here (a2 fused into a4, the value array is written once, final).
 // kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
 template <typename T, bool kSmem, bool kFactor, bool kSolve, bool kTransposed, bool kInlineFill>
-__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv) {
+__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv, BlobRing& ring) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
+    long long tk = clock64();
     for (int l = 0; l < t.n_level; ++l) {
         const LevelDesc d = lv[l];
+        const char* lb = ring.acquire(l, d);
+        const int* dptr = reinterpret_cast<const int*>(lb);
+        const int* tptr = reinterpret_cast<const int*>(lb + d.o_tptr);
+        const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
+        const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
+        const int2* tab = reinterpret_cast<const int2*>(lb + d.o_tab);
+        const double4* py = reinterpret_cast<const double4*>(lb + d.o_py);
         {
             const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
             const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
@@ -89,7 +111,7 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
                 const bool valid = base + tl < d.m1;
                 const int m = valid ? base + tl : d.m1 - 1;
                 const bool lead = valid && part == 0;
-                const int t0 = t.dterm_ptr[m], t1 = valid ? t.dterm_ptr[m + 1] : t0;
+                const int t0 = dptr[m - d.m0], t1 = valid ? dptr[m - d.m0 + 1] : t0;
                 Blk<T> D = {T(0), T(0), T(0), T(0)};
                 T y0 = T(0), y1 = T(0);
                 if (lead) {
@@ -97,7 +119,7 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
                     if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
                 }
                 for (int q = t0 + part; q < t1; q += S) {
-                    const int2 ak = t.dterm_ak[q];
+                    const int2 ak = dak[q];
                     if (kFactor || kTransposed) {
                         const Blk<T> U = s.ldU(ak.x);
                         if (kFactor) mulsub(D, s.ldL(ak.x), U);
@@ -126,55 +148,66 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
             }
         }
         if (kFactor) {
-            __syncthreads();
+            // pair targets accumulate J - sum(terms) concurrently with the diagonal targets (they only need factors of
+            // earlier levels); warps are taken from the other end so that a narrow level spreads over distinct warps
             const int ssh = d.sp, tsh = 5 - gsh - ssh, S = 1 << ssh;
             const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-            for (int base = d.p0 + (warp << tsh); base < d.p1; base += nwarps << tsh) {
+            for (int base = d.p0 + ((nwarps - 1 - warp) << tsh); base < d.p1; base += nwarps << tsh) {
                 const bool valid = base + tl < d.p1;
                 const int p = valid ? base + tl : d.p1 - 1;
                 const bool lead = valid && part == 0;
-                const int t0 = t.term_ptr[p], t1 = valid ? t.term_ptr[p + 1] : t0;
-                const int2 mj = t.pair_mj[p];
+                const int t0 = tptr[p - d.p0], t1 = valid ? tptr[p - d.p0 + 1] : t0;
+                const int2 mj = pmj[p - d.p0];
                 Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
                 if (lead) {
-                    if (kInlineFill) fill_pair<T, kSmem>(t, s, p, mj, U, L);
+                    if (kInlineFill) fill_pair<T, kSmem>(s, mj, py[p - d.p0], U, L);
                     else { U = s.ldU(p); L = s.ldL(p); }
                 }
                 for (int q = t0 + part; q < t1; q += S) {
-                    const int2 ab = t.term_ab[q];
+                    const int2 ab = tab[q];
                     mulsub(U, s.ldL(ab.x), s.ldU(ab.y));
                     mulsub(L, s.ldL(ab.y), s.ldU(ab.x));
                 }
                 for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
-                if (lead) {
-                    L = mul(L, s.ldD(mj.x & kIdxMask));
-                    s.stU(p, U); s.stL(p, L);
-                }
+                if (lead) { s.stU(p, U); s.stL(p, L); }
+            }
+            __syncthreads();
+            ring.tick(4 * l, tk);
+            // scale: L(j,m) = L'(j,m) D_m^-1 with the pivot inverses of this level
+            const int np = d.p1 - d.p0;
+            for (int i = threadIdx.x >> gsh; i < np; i += blockDim.x >> gsh) {
+                const int p = d.p0 + i;
+                s.stL(p, mul(s.ldL(p), s.ldD(pmj[i].x & kIdxMask)));
             }
         }
         __syncthreads();
+        ring.tick(4 * l + 1, tk);
+        ring.release(l);
     }
 }
 
 // backward half of a5: U x = y, i.e. x_m = D_m^-1 (y_m - sum_j U(m,j) x_j) over the pairs owned by m, levels
-// descending; kUpdate applies the Newton update of PAPER.md:90 to node m in the same pass, accumulated in FP64
-// (PAPER.md:255).  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
-template <typename T, bool kSmem, bool kTransposed, bool kUpdate>
-__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv) {
+// descending.  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
+template <typename T, bool kSmem, bool kTransposed>
+__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv, BlobRing& ring) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
+    long long tk = clock64();
     for (int l = t.n_level - 1; l >= 0; --l) {
         const LevelDesc d = lv[l];
+        const char* lb = ring.acquire(l, d);
+        const int* pptr = reinterpret_cast<const int*>(lb + d.o_pptr);
+        const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
         const int ssh = d.sb, tsh = 5 - gsh - ssh, S = 1 << ssh;
         const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
         for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
             const bool valid = base + tl < d.m1;
             const int m = valid ? base + tl : d.m1 - 1;
             const bool lead = valid && part == 0;
-            const int p0 = t.pair_ptr[m], p1 = valid ? t.pair_ptr[m + 1] : p0;
+            const int p0 = pptr[m - d.m0] & kIdxMask, p1 = valid ? pptr[m - d.m0 + 1] & kIdxMask : p0;
             T y0 = T(0), y1 = T(0);
             if (lead) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
-            for (int p = p0 + part; p < p1; p += S) {
-                const int j = t.pair_mj[p].y & kIdxMask;
+            for (int pi = p0 + part; pi < p1; pi += S) {
+                const int j = pmj[pi].y & kIdxMask, p = d.p0 + pi;
                 const double2 x = s.rh(j);
                 if (!kTransposed) { const Blk<T> U = s.ldU(p); y0 -= U.a * T(x.x) + U.b * T(x.y); y1 -= U.c * T(x.x) + U.d * T(x.y); }
                 else              { const Blk<T> L = s.ldL(p); y0 -= L.a * T(x.x) + L.c * T(x.y); y1 -= L.b * T(x.x) + L.d * T(x.y); }
@@ -186,17 +219,25 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
                     const T z0 = D.a * y0 + D.b * y1, z1 = D.c * y0 + D.d * y1; y0 = z0; y1 = z1;
                 }
                 s.set_rh(m, make_double2(double(y0), double(y1)));
-                if (kUpdate) {
-                    const double2 a = s.ma(m);
-                    const double th = a.y + double(y0);
-                    const double vm = t.node_pq[m] ? a.x + double(y1) : a.x;
-                    double sn, cs; sincos(th, &sn, &cs);
-                    s.set_ma(m, make_double2(vm, th));
-                    s.set_vv(m, make_double2(vm * cs, vm * sn));
-                }
             }
         }
         __syncthreads();
+        ring.tick(4 * l + 2, tk);
+        ring.release(l);
+    }
+}
+
+// Newton update of PAPER.md:90 for every node, accumulated in FP64; one wide pass (the sincos is kept
+// off the level-by-level critical path of the backward sweep).  No barrier.
+template <typename T, bool kSmem>
+__device__ __forceinline__ void stage_update(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
+    for (int m = tsub; m < t.n_node; m += nsub) {
+        const double2 a = s.ma(m), x = s.rh(m);
+        const double th = a.y + x.x;
+        const double vm = t.node_pq[m] ? a.x + x.y : a.x;
+        double sn, cs; sincos(th, &sn, &cs);
+        s.set_ma(m, make_double2(vm, th));
+        s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
 }
 

@@ -15,7 +15,7 @@ import sable_synth as S
 from util import dev, gpu_jacobian_dense, make_ctx, oracle_Y, random_state
 
 torch = pytest.importorskip("torch")
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.timeout(240)]
 
 import paper_2606_07099_b200 as sb  # noqa: E402
 
