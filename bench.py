@@ -110,7 +110,7 @@ def algorithmic_bytes(info, iterations, batch, keep, w):
     return b
 
 
-def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True):
+def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
     import torch
     import paper_2606_07099_b200 as sb
     import torch.distributed as dist
@@ -121,7 +121,7 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True):
     Yh = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
     t0 = time.perf_counter()
     ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=B, precision=c.precision,
-                     keep_factors=c.adjoint, mode=sb.FUSED, device=torch.cuda.current_device())
+                     keep_factors=c.adjoint, mode=mode, device=torch.cuda.current_device())
     create_s = time.perf_counter() - t0
     info = ctx.info
     dev = torch.device("cuda", torch.cuda.current_device())
@@ -177,7 +177,7 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True):
     res = {"value": conv_all / secs, "ms_per_step": 1e3 * secs / steps, "converged": conv, "batch": B,
            "iterations_hist": np.bincount(its).tolist(), "solve_ms": float(np.mean(solve_ms)),
            "adjoint_ms": float(np.mean(step_ms) - np.mean(solve_ms)) if c.adjoint else None,
-           "roofline": {"bound": "hbm", "kernel": "k_nr_fused (one launch = the whole NR loop of the batch)",
+           "roofline": {"bound": "hbm", "kernel": "k_nr_fused (one launch = the whole NR loop of the batch)" if mode == 0 else "staged: k_st_mismatch_fill + k_st_factor_solve per iteration (time = whole sable_solve)",
                         "achieved": alg / kern_s / 1e9, "peak": peak, "unit": "GB/s", "frac": alg / kern_s / 1e9 / peak,
                         "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                         "note": "achieved = model-M0 bytes / kernel time; the fused kernel keeps factors on chip, so its "
@@ -251,6 +251,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--mode", default="fused", choices=["fused", "staged"],
+                    help="staged = one kernel per stage (mismatch+fill / refactor+solve), state in HBM between: per-stage profiling")
     a = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -259,7 +261,7 @@ def main():
     config = {"workload": WORKLOAD[a.config], "name": cfg.name, "batch_per_gpu": cfg.batch, "tol": cfg.tol,
               "max_it": cfg.max_it, "precision": "fp64 mismatch + fp32 LU" if cfg.precision else "fp64",
               "adjoint": cfg.adjoint, "network_seed": cfg.s_net, "load_scale_kappa": cfg.kappa,
-              "parallelism": f"scenario sharding x{world}, no collective", "cache": "L2 flushed between steps (256 MiB memset)"}
+              "parallelism": f"scenario sharding x{world}, no collective", "launch_mode": a.mode, "cache": "L2 flushed between steps (256 MiB memset)"}
 
     if a.impl == "reference":
         if rank != 0:
@@ -287,7 +289,7 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    res, inputs = run_ours(a.config, a.steps, a.warmup, rank, world)
+    res, inputs = run_ours(a.config, a.steps, a.warmup, rank, world, mode=1 if a.mode == "staged" else 0)
     line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
             "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if not cfg.precision else "f64+f32", "data": "synthetic", "config": config,

@@ -162,7 +162,7 @@ static sable_status choose_launch(sable_ctx* ctx) {
     // ring candidates (slots, slot capacity): the streamed levels are the trailing run of levels whose blobs fit a slot
     struct RingOpt { int r, cap; };
     const int r_env = env_int("SABLE_RING_R", -1), cap_env = env_int("SABLE_RING_SLOT", -1);
-    std::vector<RingOpt> ropts = {{3, 16384}, {3, 8192}, {2, 8192}, {3, 4096}, {2, 4096}, {2, 2048}, {0, 0}};
+    std::vector<RingOpt> ropts = {{3, 8192}, {2, 8192}, {3, 4096}, {2, 4096}, {2, 2048}, {0, 0}};
     if (r_env >= 0 || cap_env >= 0) ropts = {{r_env >= 0 ? r_env : 3, cap_env >= 0 ? cap_env : 8192}, {0, 0}};
     auto set_ring = [&](const RingOpt& o) {
         int first = nl, slot = 0;
@@ -171,7 +171,7 @@ static sable_status choose_launch(sable_ctx* ctx) {
         ctx->ring_r = o.r; ctx->ring_slot = slot; ctx->first_staged = first; ring_bytes = o.r * slot;
     };
     int th = ctx->opt.threads;
-    if (th <= 0) th = nn <= 64 ? 64 : nn <= 200 ? 256 : (nn > 1200 && mixed) ? 256 : 512;   // measured: profiles/r01_v2_sweeps.md
+    if (th <= 0) th = nn <= 64 ? 64 : nn <= 200 ? 256 : (nn > 1200 && nn <= 4000) ? 256 : 512;   // measured: profiles/r01_v2_sweeps.md
     th = env_int("SABLE_THREADS", th);
     th = std::min(512, std::max(32, (th + 31) / 32 * 32));
     const int mb = ctx->opt.max_batch;
@@ -190,10 +190,14 @@ static sable_status choose_launch(sable_ctx* ctx) {
     if (gsh >= 0 && cut_env < 0) {
         ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
     } else {
-        // split placement: the smallest cut level whose top fits the per-CTA budget for `want_ctas` CTAs per SM
-        want_ctas = env_int("SABLE_CTAS", mb > n_sm ? 2 : 1);
-        set_ring(ropts[0]);
-        const int64_t budget = std::min<int64_t>(max_optin, smem_sm / want_ctas - 1024);
+        // split placement.  Measured (profiles/r01_v2_sweeps.md): for grids whose factors do not fit on chip, resident
+        // warps and a large L1 (which then holds the shared index program and Y_bus) buy more than shared-memory
+        // residency of a part of the factors: keep only a small top of the elimination tree on chip (<= 24 KB per
+        // CTA), read the level blobs in place (no ring), and let the register file set the CTA count (the split
+        // kernel is built for 64 registers: 1024 threads per SM).
+        want_ctas = env_int("SABLE_CTAS", std::max(1, 1024 / th));
+        set_ring(r_env >= 0 ? ropts[0] : RingOpt{0, 0});
+        const int64_t budget = std::min<int64_t>({(int64_t)max_optin, (int64_t)smem_sm / want_ctas - 2048, (int64_t)env_int("SABLE_SPLIT_SMEM", 24576)});
         int cl = cut_env;
         int sg = 0;
         while ((2 << sg) <= std::max(1, g_env)) ++sg;          // slots per CTA in split placement: SABLE_G (default 1)
@@ -212,7 +216,7 @@ static sable_status choose_launch(sable_ctx* ctx) {
     if (occ < 1) return fail(ctx, SABLE_ERR_CUDA, "NR kernel does not fit on an SM");
     occ = std::min(occ, env_int("SABLE_CTAS", occ));
     ctx->ctas_per_sm = occ; ctx->grid = occ * n_sm;
-    ctx->threads1 = env_int("SABLE_THREADS1", nn <= 64 ? 64 : nn <= 1200 ? 128 : 256);
+    ctx->threads1 = env_int("SABLE_THREADS1", nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512);
     return SABLE_OK;
 }
 

@@ -115,7 +115,7 @@ __device__ __forceinline__ int pop_scenario(const SolveArgs& A) {
 // Loop convention, per slot:
 //   it = 0; loop { r = ||F1||inf; if r <= tol: converged; if it == max_it or r not finite: stop; solve; update; ++it }
 template <typename T, bool kSmem>
-__global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
+__global__ void __launch_bounds__(512, kSmem ? 1 : 2) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
@@ -197,8 +197,11 @@ __global__ void __launch_bounds__(512) k_nr_fused(const SolveArgs A) {
             if (!any) { ring.drain(); return; }
             if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, A.trash);
         }
-        ring.tick(4 * t.n_level, tk);                      // refill + init + mismatch + norm + decision + output
-        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv, ring);
+        // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
+        stage_fill_pairs<T, kSmem>(t, s, tsub, nsub);
+        __syncthreads();
+        ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
+        stage_factor_forward<T, kSmem, true, true, false, false>(t, s, lv, ring);
         stage_backward<T, kSmem, false>(t, s, lv, ring);
         stage_update<T, kSmem>(t, s, tsub, nsub);
         if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
