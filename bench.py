@@ -34,6 +34,9 @@ WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward"
             3: "BASELINE.json configs[2]: 300 buses x 8192 scenarios, FP64 forward + adjoint",
             4: "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
             5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
+# captures (profiles/r01_v2_README.md); None where no capture exists
+NCU_TRAFFIC = {3: 59.070976e6 + 283.826944e6, 5: 10.338136e9 + 5.761298e9}
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 
@@ -179,7 +182,7 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
            "adjoint_ms": float(np.mean(step_ms) - np.mean(solve_ms)) if c.adjoint else None,
            "roofline": {"bound": "hbm", "kernel": "k_nr_fused (one launch = the whole NR loop of the batch)" if mode == 0 else "staged: k_st_mismatch_fill + k_st_factor_solve per iteration (time = whole sable_solve)",
                         "achieved": alg / kern_s / 1e9, "peak": peak, "unit": "GB/s", "frac": alg / kern_s / 1e9 / peak,
-                        "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
+                        "traffic": NCU_TRAFFIC.get(cfg_id) if mode == 0 else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                         "note": "achieved = model-M0 bytes / kernel time; the fused kernel keeps factors on chip, so its "
                                 "DRAM traffic is far below M0 (profiles/)"},
            "launches": launches, "create_s": create_s, "info": {k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level",
