@@ -25,7 +25,9 @@ struct sable_ctx {
     int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1;
     int dg_cut = 0, pr_cut = 0, st_cut = 0, cut_level = 0;
     int threads1 = 0;                                        // staged / adjoint / debug kernels
-    const LevelDesc* level_fused = nullptr; const LevelDesc* level_one = nullptr;
+    int factor_gsh = 0;                                      // group layout of the factors currently in the workspace
+    const LevelDesc* level_fused = nullptr; const LevelDesc* level_one = nullptr; const LevelDesc* level_lin = nullptr;
+    int threads_lin = 0;                                     // adjoint kernel on group-interleaved factors
     std::vector<LevelDesc> lv_host;                          // blob offsets per level (splits filled per kernel family)
     std::vector<char> blob_host;
     int ring_r = 0, ring_slot = 0, first_staged = 0;
@@ -187,7 +189,14 @@ static sable_status choose_launch(sable_ctx* ctx) {
         }
     }
     const int cut_env = env_int("SABLE_CUT", -1);
-    if (gsh >= 0 && cut_env < 0) {
+    // all on chip only while the SMs can hold a good part of the batch at once; a batch of many waves runs faster from
+    // the group-interleaved HBM workspace with many small CTAs (cfg 3: 3.5 ms vs 4.4 ms, profiles/r01_v2_sweeps.md)
+    bool on_chip = gsh >= 0 && cut_env < 0;
+    if (on_chip && g_env <= 0 && env_int("SABLE_THREADS", 0) <= 0) {
+        const int64_t slots_sm = (int64_t)std::max<int64_t>(1, smem_sm / (need(gsh, 0, 0, 0) + 1024)) << gsh;
+        if (slots_sm * n_sm * 2 < (int64_t)mb) on_chip = false;
+    }
+    if (on_chip) {
         ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
     } else {
         // split placement.  Measured (profiles/r01_v2_sweeps.md): for grids whose factors do not fit on chip, resident
@@ -195,12 +204,15 @@ static sable_status choose_launch(sable_ctx* ctx) {
         // residency of a part of the factors: keep only a small top of the elimination tree on chip (<= 24 KB per
         // CTA), read the level blobs in place (no ring), and let the register file set the CTA count (the split
         // kernel is built for 64 registers: 1024 threads per SM).
+        if (ctx->opt.threads <= 0 && env_int("SABLE_THREADS", 0) <= 0) th = nn <= 1200 ? 128 : nn <= 4000 ? 256 : 512;
         want_ctas = env_int("SABLE_CTAS", std::max(1, 1024 / th));
         set_ring(r_env >= 0 ? ropts[0] : RingOpt{0, 0});
         const int64_t budget = std::min<int64_t>({(int64_t)max_optin, (int64_t)smem_sm / want_ctas - 2048, (int64_t)env_int("SABLE_SPLIT_SMEM", 24576)});
         int cl = cut_env;
+        // slots per CTA (= scenarios whose HBM slices are interleaved): 4 / 2 / 1 by grid size, or SABLE_G
         int sg = 0;
-        while ((2 << sg) <= std::max(1, g_env)) ++sg;          // slots per CTA in split placement: SABLE_G (default 1)
+        const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : nn <= 4000 ? 2 : 1);
+        while ((2 << sg) <= g_want && ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1)) ++sg;
         if (cl < 0) { cl = 0; while (cl < nl && need(sg, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
         cl = std::min(cl, nl);
         const int nc = cl < nl ? T.level_ptr[cl] : nn;
@@ -291,7 +303,9 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     {
         std::vector<LevelDesc> lf = build_levels(T, c->lv_host, c->threads, c->gsh, c->first_staged);
         std::vector<LevelDesc> l1 = build_levels(T, c->lv_host, c->threads1, 0, T.n_level);
-        up(lf, &c->level_fused); up(l1, &c->level_one); up(c->blob_host, &d.blob);
+        c->threads_lin = env_int("SABLE_THREADS_LIN", std::min(512, std::max(c->threads1 << c->gsh, 32)));
+        std::vector<LevelDesc> ll = build_levels(T, c->lv_host, c->threads_lin, c->gsh, T.n_level);
+        up(lf, &c->level_fused); up(l1, &c->level_one); up(ll, &c->level_lin); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
     }
     const bool mixed = o.precision == SABLE_MIXED;
@@ -302,19 +316,19 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         c->dev_allocs.push_back(*p); return true;
     };
     const size_t mb = (size_t)o.max_batch, nb = (size_t)T.n_bus;
-    if (!dmalloc((void**)&c->factors, (mb + 1) * c->fac_stride) || !dmalloc((void**)&c->work, (mb + 1) * c->work_stride) ||
+    // workspace for whole groups of 1 << gsh scenarios (fused mode interleaves a group's slices; staged mode: gsh 0)
+    const size_t G = (size_t)1 << c->gsh, mb_alloc = (mb + G - 1) / G * G + G;
+    if (!dmalloc((void**)&c->factors, mb_alloc * c->fac_stride) || !dmalloc((void**)&c->work, mb_alloc * c->work_stride) ||
         !dmalloc((void**)&c->ints, (2 * mb + 4) * 4) || !dmalloc((void**)&c->hbuf, 9 * mb * nb * 8 + mb * 8) ||
         !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb) || !dmalloc((void**)&c->zeros, nb * 8))
         return bail(SABLE_ERR_ALLOC);
-    if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work + mb * c->work_stride, 0, c->work_stride) != cudaSuccess ||
-        cudaMemset(c->factors + mb * c->fac_stride, 0, c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
+    if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work, 0, mb_alloc * c->work_stride) != cudaSuccess ||
+        cudaMemset(c->factors, 0, mb_alloc * c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
     if (env_int("SABLE_TIMING", 0)) {
         const size_t tb = (4 * (size_t)T.n_level + 4) * 8;
         if (!dmalloc((void**)&c->tim, tb)) return bail(SABLE_ERR_ALLOC);
         cudaMemset(c->tim, 0, tb);
     }
-    const void* lin = mixed ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
-    if ((size_t)nn * 16 > 48 * 1024) cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, nn * 16);
     fill_info(c);
     *out = c;
     return SABLE_OK;
@@ -341,13 +355,16 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         A.t.level = c->level_fused;
         A.gsh = c->gsh; A.dg_cut = c->dg_cut; A.pr_cut = c->pr_cut; A.st_cut = c->st_cut;
         A.ring_r = c->ring_r; A.ring_slot = c->ring_slot; A.first_staged = c->first_staged;
+        A.trash_grp = (c->opt.max_batch + (1 << c->gsh) - 1) >> c->gsh;
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
+        c->factor_gsh = c->gsh;
         if (c->placement == 0) k_nr_fused<T, true><<<grid, c->threads, c->smem, s>>>(A);
         else k_nr_fused<T, false><<<grid, c->threads, c->smem, s>>>(A);
         c->launches += 1;
     } else {
         A.t.level = c->level_one;
+        A.gsh = 0; c->factor_gsh = 0;
         k_st_init<T><<<A.batch, c->threads1, 0, s>>>(A);
         for (int i = 0; i <= A.max_it; ++i) {
             k_st_mismatch_fill<T><<<A.batch, c->threads1, 0, s>>>(A);
@@ -372,7 +389,7 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
         return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
     CU(cudaSetDevice(ctx->opt.device));
     SolveArgs A{};
-    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.trash = ctx->opt.max_batch; A.tol = tol;
+    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.tol = tol;
     A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
     A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
     A.factors = ctx->factors; A.work = ctx->work; A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride;
@@ -388,14 +405,19 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
 static sable_status launch_lin(sable_ctx* ctx, int batch, const double* rp, const double* rq, int transposed, double* xp,
                                double* xq, cudaStream_t s) {
     LinArgs L{};
-    L.t = ctx->d; L.t.level = ctx->level_one;
-    L.batch = batch; L.transposed = transposed; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
+    const int gsh = ctx->factor_gsh, G = 1 << gsh;
+    L.t = ctx->d;
+    L.t.level = gsh == 0 ? ctx->level_one : ctx->level_lin;
+    L.batch = batch; L.transposed = transposed; L.gsh = gsh; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
     L.factors = ctx->factors; L.fac_stride = ctx->fac_stride; L.work = ctx->work; L.work_stride = ctx->work_stride;
-    const size_t sm = (size_t)ctx->T.n_node * 16;
+    const size_t sm = ((size_t)ctx->T.n_node * 16) << gsh;
     int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
-    L.rhs_in_smem = sm <= (size_t)max_optin;
-    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<batch, ctx->threads1, L.rhs_in_smem ? sm : 0, s>>>(L);
-    else k_linsolve<double><<<batch, ctx->threads1, L.rhs_in_smem ? sm : 0, s>>>(L);
+    L.rhs_in_smem = sm <= std::min<size_t>((size_t)max_optin, 64 * 1024);
+    const void* lin = ctx->opt.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
+    if (L.rhs_in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int th = gsh == 0 ? ctx->threads1 : ctx->threads_lin, grid = (batch + G - 1) / G;
+    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<grid, th, L.rhs_in_smem ? sm : 0, s>>>(L);
+    else k_linsolve<double><<<grid, th, L.rhs_in_smem ? sm : 0, s>>>(L);
     ctx->launches += 1;
     CU(cudaGetLastError());
     return SABLE_OK;
@@ -486,7 +508,7 @@ extern "C" sable_status sable_debug_pattern(const sable_ctx* c, int32_t* node_bu
 }
 
 static sable_status launch_debug(sable_ctx* ctx, DebugArgs& D, cudaStream_t s) {
-    D.t = ctx->d; D.t.level = ctx->level_one; D.zeros = ctx->zeros;
+    D.t = ctx->d; D.t.level = ctx->level_one; D.zeros = ctx->zeros; ctx->factor_gsh = 0;
     D.factors = ctx->factors; D.work = ctx->work; D.fac_stride = ctx->fac_stride; D.work_stride = ctx->work_stride;
     if (ctx->opt.precision == SABLE_MIXED) k_debug<float><<<D.batch, ctx->threads1, 0, s>>>(D);
     else k_debug<double><<<D.batch, ctx->threads1, 0, s>>>(D);

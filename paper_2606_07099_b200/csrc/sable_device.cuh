@@ -12,9 +12,12 @@
 // part of every array (nodes >= cut, pairs >= cut: the top of the elimination tree, where levels are narrow and
 // latency decides) lives in shared memory, interleaved over the slots in 16-byte vectors:
 //   address = base + ((index_in_vectors << gsh) + g) * 16
-// so that the G lanes serving one target read consecutive 16-byte words (conflict-free LDS.128).  The early part
-// (wide levels: throughput decides) lives in the scenario's own contiguous slice of the HBM workspace, which is also
-// where kept factors are handed to sable_adjoint.
+// so that the G lanes serving one target read consecutive 16-byte words (conflict-free LDS.128).  The early part lives
+// in the HBM workspace of the scenario's GROUP (scenarios b with equal b >> gsh), interleaved over the group in the same
+// way -- a warp then touches 16 G contiguous bytes per target instead of 32 scattered sectors (coalesced LDG.128; the
+// L1 wavefront count, which bounded the scenario-major layout at 65 % of its peak, drops by up to G) -- and that is also
+// where kept factors are handed to sable_adjoint.  With gsh = 0 (staged / debug kernels) this is a plain contiguous
+// slice per scenario.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -103,12 +106,12 @@ __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
 template <typename T, bool kSmem> struct Slot {
     static constexpr int VPB = (int)(4 * sizeof(T) / 16);      // 16-byte vectors per block: 2 (FP64) or 1 (FP32)
     char *s_dg, *s_pr, *s_vv, *s_ma, *s_rh;                   // shared bases, already offset by g * 16
-    char *g_dg, *g_pr, *g_vv, *g_ma, *g_rh;                   // this scenario's slices of the HBM workspace
+    char *g_dg, *g_pr, *g_vv, *g_ma, *g_rh;                   // HBM workspace of this scenario's group, offset by g * 16
     int dg_cut, pr_cut, st_cut, gsh;                          // node cut of dg, pair cut of pr, node cut of vv/ma/rh
 
     __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
         if (kSmem || idx >= cut_blocks) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
-        vs = 16; return reinterpret_cast<T*>(gb + (size_t)idx * (VPB * 16));
+        vs = 16 << gsh; return reinterpret_cast<T*>(gb + (((size_t)idx * VPB) << (gsh + 4)));
     }
     __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); return ld_blk(p, vs); }
     __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); st_blk(p, vs, v); }
@@ -119,7 +122,7 @@ template <typename T, bool kSmem> struct Slot {
 
     __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
         if (kSmem || m >= st_cut) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
-        return reinterpret_cast<double2*>(gb + (size_t)m * 16);
+        return reinterpret_cast<double2*>(gb + ((size_t)m << (gsh + 4)));
     }
     __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv, g_vv, m); }
     __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma, g_ma, m); }
@@ -199,15 +202,15 @@ __device__ __forceinline__ double nan_max(double x, double y) {   // NaN-propaga
 }
 
 // Per-slot CTA-wide max (a NaN anywhere in slot g gives NaN for g, reading 18).  `red` holds
-// (blockDim.x / 32) * 8 doubles.  Every thread returns the max over the threads that serve its slot.  Two barriers.
+// (blockDim.x / 32) * 32 doubles.  Every thread returns the max over the threads that serve its slot.  Two barriers.
 __device__ __forceinline__ double slot_max_nan(double v, double* red, int gsh) {
     for (int o = 16; o >= (1 << gsh); o >>= 1) v = nan_max(v, __shfl_xor_sync(0xffffffffu, v, o));
     const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5, g = threadIdx.x & ((1 << gsh) - 1);
     __syncthreads();
-    if (l < (1 << gsh)) red[w * 8 + l] = v;
+    if (l < (1 << gsh)) red[w * 32 + l] = v;
     __syncthreads();
     double r = red[g];
-    for (int i = 1; i < nw; ++i) r = nan_max(r, red[i * 8 + g]);
+    for (int i = 1; i < nw; ++i) r = nan_max(r, red[i * 32 + g]);
     return r;
 }
 

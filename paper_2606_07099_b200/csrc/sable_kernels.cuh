@@ -8,7 +8,7 @@ namespace sable {
 
 struct SolveArgs {
     DevTemplate t;
-    int32_t batch, max_it, keep, trash;                   // trash = index of the spare workspace slice (empty slots)
+    int32_t batch, max_it, keep, trash_grp;               // trash_grp: spare group of the workspace (finished slots run along on it)
     double tol;
     const double *p_spec, *q_spec, *v_set, *vm0, *va0;    // [batch][n_bus]
     double *vm, *va, *final_norm;
@@ -25,7 +25,8 @@ struct SolveArgs {
     int32_t* it;              // staged mode: [batch]
 };
 
-constexpr int kSmemHeader = 2048 + 64 + 64;                // reduction scratch + slot bookkeeping + ring mbarriers
+constexpr int kRedBytes = 16 * 32 * 8;                      // per-slot norm reduction scratch: 16 warps x 32 slots
+constexpr int kSmemHeader = kRedBytes + 128 + 64;           // + slot bookkeeping + ring mbarriers
 __host__ __device__ inline int64_t align16(int64_t x) { return (x + 15) & ~int64_t(15); }
 template <typename T> __host__ __device__ inline int64_t fac_bytes(int n_node, int n_pair) { return (int64_t)(n_node + 2 * (int64_t)n_pair) * 4 * sizeof(T); }
 __host__ __device__ inline int64_t work_bytes(int n_node) { return 3 * (int64_t)(n_node + 1) * 16; }
@@ -54,14 +55,16 @@ __device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node,
     s.dg_cut = dg_cut; s.pr_cut = pr_cut; s.st_cut = st_cut; s.gsh = gsh;
     return s;
 }
-// HBM part: scenario b's slices
+// HBM part: the slices of scenario b's group (b >> gsh), offset to lane b & (G - 1); strides are per scenario
 template <typename T, bool kSmem>
 __device__ __forceinline__ void bind(Slot<T, kSmem>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
-    s.g_dg = factors + (size_t)b * fac_stride;
-    s.g_pr = s.g_dg + (size_t)n_node * 4 * sizeof(T);
-    s.g_vv = work + (size_t)b * work_stride;
-    s.g_ma = s.g_vv + (size_t)(n_node + 1) * 16;
-    s.g_rh = s.g_ma + (size_t)(n_node + 1) * 16;
+    const int gsh = s.gsh;
+    const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
+    s.g_dg = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
+    s.g_pr = s.g_dg + (((size_t)n_node * 4 * sizeof(T)) << gsh);
+    s.g_vv = work + ((grp * (size_t)work_stride) << gsh) + lane16;
+    s.g_ma = s.g_vv + (((size_t)(n_node + 1) * 16) << gsh);
+    s.g_rh = s.g_ma + (((size_t)(n_node + 1) * 16) << gsh);
 }
 
 template <typename T, bool kSmem>
@@ -101,33 +104,35 @@ template <typename T, bool kSmem>
 __device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
     constexpr int VPB = Slot<T, kSmem>::VPB;
     const int n_dg = (t.n_node - s.dg_cut) * VPB, n_pr = 2 * (t.n_pair - s.pr_cut) * VPB;
-    int4* gd = reinterpret_cast<int4*>(s.g_dg) + (size_t)s.dg_cut * VPB;
-    int4* gp = reinterpret_cast<int4*>(s.g_pr) + (size_t)2 * s.pr_cut * VPB;
-    for (int i = tsub; i < n_dg; i += nsub) gd[i] = *reinterpret_cast<const int4*>(s.s_dg + ((size_t)i << (s.gsh + 4)));
-    for (int i = tsub; i < n_pr; i += nsub) gp[i] = *reinterpret_cast<const int4*>(s.s_pr + ((size_t)i << (s.gsh + 4)));
+    char* gd = s.g_dg + (((size_t)s.dg_cut * VPB) << (s.gsh + 4));
+    char* gp = s.g_pr + (((size_t)2 * s.pr_cut * VPB) << (s.gsh + 4));
+    for (int i = tsub; i < n_dg; i += nsub) *reinterpret_cast<int4*>(gd + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_dg + ((size_t)i << (s.gsh + 4)));
+    for (int i = tsub; i < n_pr; i += nsub) *reinterpret_cast<int4*>(gp + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_pr + ((size_t)i << (s.gsh + 4)));
 }
 
-__device__ __forceinline__ int pop_scenario(const SolveArgs& A) {
+__device__ __forceinline__ int pop_group(const SolveArgs& A) {
     const int v = atomicAdd(A.queue, 1);
-    return v < A.batch ? v : -1;
+    return v < ((A.batch + (1 << A.gsh) - 1) >> A.gsh) ? v : -1;
 }
 
 // Loop convention, per slot:
 //   it = 0; loop { r = ||F1||inf; if r <= tol: converged; if it == max_it or r not finite: stop; solve; update; ++it }
+// A CTA takes one GROUP of G consecutive scenarios at a time from the atomic queue (slot g serves scenario
+// group * G + g, whose HBM slices are interleaved with the rest of its group) and advances its slots in lockstep; a slot
+// that has finished stops being evaluated (its lanes run along and write nothing that is read) until the group is done.
 template <typename T, bool kSmem>
 __global__ void __launch_bounds__(512, kSmem ? 1 : 2) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
     double* red = reinterpret_cast<double*>(smem);
-    int* s_b = reinterpret_cast<int*>(smem + 2048);
-    int* s_fresh = s_b + 8;
+    int* s_b = reinterpret_cast<int*>(smem + kRedBytes);
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
     for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
     Slot<T, kSmem> s = carve<T, kSmem>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
     BlobRing ring;
     ring.slots = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)t.n_level * (int64_t)sizeof(LevelDesc));
-    ring.mbar = reinterpret_cast<unsigned long long*>(smem + 2048 + 64);
+    ring.mbar = reinterpret_cast<unsigned long long*>(smem + kRedBytes + 128);
     ring.gblob = t.blob; ring.lv = lv; ring.R = A.ring_r; ring.slot_bytes = A.ring_slot;
     ring.first = A.first_staged; ring.n_level = t.n_level;
     ring.tim = blockIdx.x == 0 ? A.tim : nullptr;
@@ -137,66 +142,47 @@ __global__ void __launch_bounds__(512, kSmem ? 1 : 2) k_nr_fused(const SolveArgs
     const double kInf = __longlong_as_double(0x7ff0000000000000LL);
     int b = -1, it = 0;
     bool fin = false;
+    auto any_slot = [&](bool mine) {                       // CTA-uniform OR over the slots; two barriers
+        __syncthreads();
+        if (threadIdx.x < G) s_b[threadIdx.x] = mine ? 1 : 0;
+        __syncthreads();
+        bool any = false;
+        for (int x = 0; x < G; ++x) any |= s_b[x] != 0;
+        return any;
+    };
     for (;;) {
-        __syncthreads();
-        if (threadIdx.x < G) s_b[threadIdx.x] = b < 0 ? pop_scenario(A) : b;
-        __syncthreads();
-        bool need;
-        {
-            const int nb = s_b[g];
-            const bool fresh = b < 0 && nb >= 0;
-            b = nb;
-            bool any = false;
-            for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
-            if (!any) { ring.drain(); return; }
-            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, b >= 0 ? b : A.trash);
-            if (fresh) { it = 0; scen_init<T, kSmem>(A, s, b, tsub, nsub); }
-            need = b >= 0;
+        if (!any_slot(b >= 0)) {                           // group done: take the next one
+            __syncthreads();
+            if (threadIdx.x == 0) s_b[0] = pop_group(A);
+            __syncthreads();
+            const int grp = s_b[0];
+            if (grp < 0) { ring.drain(); return; }
+            const int bb = (grp << gsh) + g;
+            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, bb);
+            b = bb < A.batch ? bb : -1;
+            it = 0; fin = false;
+            if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
+            if (b >= 0) scen_init<T, kSmem>(A, s, b, tsub, nsub);
+            __syncthreads();
         }
-        __syncthreads();
-        ring.tick(4 * t.n_level + 2, tk);                  // refill + init
-        for (;;) {
-            const size_t row = (size_t)(need ? b : 0) * t.n_bus;
-            const double loc = stage_mismatch<T, kSmem>(t, s, A.p_spec + row, A.q_spec + row, need);
+        ring.tick(4 * t.n_level + 2, tk);                  // group bookkeeping + init
+        {
+            const size_t row = (size_t)(b >= 0 ? b : 0) * t.n_bus;
+            const double loc = stage_mismatch<T, kSmem>(t, s, A.p_spec + row, A.q_spec + row, b >= 0);
             const double r = slot_max_nan(loc, red, gsh);
             ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
-            if (need) {
+            if (b >= 0) {
                 bool done = false, conv = false;
                 if (r <= A.tol) { done = true; conv = true; }
                 else if (it == A.max_it || !(fabs(r) < kInf)) done = true;
                 if (done) {
                     scen_output<T, kSmem>(A, s, b, it, conv, r, tsub, nsub);
-                    if (A.keep) fin = true; else b = -1;
+                    if (A.keep) fin = true;
+                    else { b = -1; bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g); }
                 }
             }
-            need = false;
-            if (A.keep) break;
-            __syncthreads();
-            if (threadIdx.x < G) {
-                int nb = b, fr = 0;
-                if (b < 0) { nb = pop_scenario(A); fr = nb >= 0; }
-                s_b[threadIdx.x] = nb; s_fresh[threadIdx.x] = fr;
-            }
-            __syncthreads();
-            bool anyfresh = false;
-            for (int x = 0; x < G; ++x) anyfresh |= s_fresh[x] != 0;
-            if (s_fresh[g]) {
-                b = s_b[g]; it = 0; need = true;
-                bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, b);
-                scen_init<T, kSmem>(A, s, b, tsub, nsub);
-            }
-            if (!anyfresh) break;
-            __syncthreads();
         }
-        __syncthreads();
-        if (threadIdx.x < G) s_b[threadIdx.x] = b;
-        __syncthreads();
-        {
-            bool any = false;
-            for (int x = 0; x < G; ++x) any |= s_b[x] >= 0;
-            if (!any) { ring.drain(); return; }
-            if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, A.trash);
-        }
+        if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
         stage_fill_pairs<T, kSmem>(t, s, tsub, nsub);
         __syncthreads();
@@ -208,7 +194,8 @@ __global__ void __launch_bounds__(512, kSmem ? 1 : 2) k_nr_fused(const SolveArgs
         if (b >= 0 && !fin) ++it;
         if (fin) {
             store_top_factors<T, kSmem>(t, s, tsub, nsub);
-            b = -1; fin = false;
+            b = -1; fin = false;                           // the kept factors stay untouched: run along on the spare group
+            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
         }
     }
 }

@@ -7,10 +7,10 @@ namespace sable {
 
 // everything in the scenario's HBM slices
 template <typename T>
-__device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b) {
+__device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
     Slot<T, false> s;
     s.s_dg = s.s_pr = s.s_vv = s.s_ma = s.s_rh = nullptr;
-    s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = 0;
+    s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = gsh;
     bind<T, false>(s, factors, fac_stride, work, work_stride, t.n_node, b);
     return s;
 }
@@ -35,7 +35,7 @@ __global__ void k_st_init(const SolveArgs A) {
 // scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here
 template <typename T>
 __global__ void k_st_mismatch_fill(const SolveArgs A) {
-    __shared__ double red[32 * 8];
+    __shared__ double red[32 * 32];
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
     const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
@@ -69,36 +69,40 @@ __global__ void k_st_factor_solve(const SolveArgs A) {
 // ---- adjoint / generic linear solve on stored factors ---------------------------------------------------------
 struct LinArgs {
     DevTemplate t;
-    int32_t batch, transposed, rhs_in_smem;
+    int32_t batch, transposed, rhs_in_smem, gsh;   // gsh: group size (log2) of the factor layout = that of the kernel that wrote them
     const double *rhs_p, *rhs_q;      // [batch][n_bus]: theta/P component and Vm/Q component per bus
     double *x_p, *x_q;
     char* factors; char* work; int64_t fac_stride, work_stride;
 };
 
 // a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, L^T lambda = w descending.
-// Factors stream from the scenario's HBM slice; the right-hand side lives in shared memory when it fits.
+// One CTA per group of G scenarios in lockstep (lane layout as in the NR kernel): factors stream from the group's
+// interleaved HBM slices (coalesced), the right-hand sides live in shared memory when they fit.
 template <typename T>
 __global__ void k_linsolve(const LinArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
-    const int b = blockIdx.x;
-    Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    if (A.rhs_in_smem) { s.st_cut = 0; s.s_rh = reinterpret_cast<char*>(smem); }
-    const size_t o = (size_t)b * t.n_bus;
-    for (int m = threadIdx.x; m < t.n_node; m += blockDim.x) {
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
+    const int bb = (blockIdx.x << gsh) + g;
+    const bool act = bb < A.batch;
+    Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
+    if (A.rhs_in_smem) { s.st_cut = 0; s.s_rh = reinterpret_cast<char*>(smem) + g * 16; }
+    const size_t o = (size_t)(act ? bb : 0) * t.n_bus;
+    for (int m = tsub; m < t.n_node; m += nsub) {
         const int bus = t.node_bus[m];
-        s.set_rh(m, make_double2(A.rhs_p[o + bus], t.node_pq[m] ? A.rhs_q[o + bus] : 0.0));
+        s.set_rh(m, act ? make_double2(A.rhs_p[o + bus], t.node_pq[m] ? A.rhs_q[o + bus] : 0.0) : make_double2(0.0, 0.0));
     }
     __syncthreads();
     BlobRing ring = no_ring(t);
     if (A.transposed) { stage_factor_forward<T, false, false, true, true, false>(t, s, t.level, ring); stage_backward<T, false, true>(t, s, t.level, ring); }
     else              { stage_factor_forward<T, false, false, true, false, false>(t, s, t.level, ring); stage_backward<T, false, false>(t, s, t.level, ring); }
-    for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
-        const int bus = t.node_bus[m];
-        const double2 x = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
-        A.x_p[o + bus] = x.x;
-        A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? x.y : 0.0;
-    }
+    if (act)
+        for (int m = tsub; m <= t.n_node; m += nsub) {
+            const int bus = t.node_bus[m];
+            const double2 x = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
+            A.x_p[o + bus] = x.x;
+            A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? x.y : 0.0;
+        }
 }
 
 // ---- debug: state from caller's (vm, va), mismatch / Jacobian / refactor at that state ---------------------------
@@ -113,7 +117,7 @@ struct DebugArgs {
 
 template <typename T>
 __global__ void k_debug(const DebugArgs A) {
-    __shared__ double red[32 * 8];
+    __shared__ double red[32 * 32];
     const DevTemplate& t = A.t;
     const int b = blockIdx.x;
     const Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);

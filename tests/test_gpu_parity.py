@@ -363,3 +363,36 @@ def test_host_buffer_calls_match_device_calls():
         assert np.array_equal(a[k], b[k]), k
     assert np.array_equal(la[0], lb[0]) and np.array_equal(la[1], lb[1])
     ctx.close()
+
+
+# ---- every placement / slot-group layout of the fused kernel gives the same answers -----------------------------------
+@pytest.mark.parametrize("env", [dict(SABLE_G="1"), dict(SABLE_G="8"), dict(SABLE_G="4", SABLE_CUT="3"),
+                                 dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="64"),
+                                 dict(SABLE_G="32", SABLE_CUT="99", SABLE_THREADS="128"),
+                                 dict(SABLE_G="2", SABLE_CUT="2", SABLE_RING_R="2", SABLE_RING_SLOT="4096"),
+                                 dict(SABLE_RING_R="0")])
+def test_placements_and_group_layouts(env, monkeypatch):
+    for k in ("SABLE_G", "SABLE_CUT", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT"):
+        monkeypatch.delenv(k, raising=False)
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    net, Y = get_net(2)
+    c = net.cfg
+    batch = 203                                    # ragged: the last group is partly empty
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ps[7] *= 30.0                                  # one scenario that does not converge: its group mates go on
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=12, method=1)
+    for keep in (False, True):
+        ctx = make_ctx(net, max_batch=256, keep_factors=keep)
+        res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
+        check_solution(res, ref, c.tol, 1e-9)
+        if keep:
+            lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+            lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+            rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+            ok = res["converged"] == 1
+            scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+            assert (np.abs(lp - rp).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
+            assert (np.abs(lq - rq).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
+        ctx.close()
