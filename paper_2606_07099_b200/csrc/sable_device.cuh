@@ -105,31 +105,44 @@ __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
 // One thread's view of the slot it serves.  kSmem = true: everything is in shared memory (cuts are 0, no branches).
 template <typename T, bool kSmem> struct Slot {
     static constexpr int VPB = (int)(4 * sizeof(T) / 16);      // 16-byte vectors per block: 2 (FP64) or 1 (FP32)
-    char *s_dg, *s_pr, *s_vv, *s_ma, *s_rh;                   // shared bases, already offset by g * 16
-    char *g_dg, *g_pr, *g_vv, *g_ma, *g_rh;                   // HBM workspace of this scenario's group, offset by g * 16
+    // Three per-thread pointers (shared base, factor slice and state slice of the group, each offset by g * 16) plus
+    // CTA-uniform byte offsets of the arrays behind them (uniform registers / constant bank: keeps the register count
+    // of the persistent kernel down).  Shared order: vv | ma | rh | dg | pr.  HBM: factors = dg | pr, state = vv | ma | rh.
+    char *sb, *gf, *gw;
+    unsigned so_ma, so_rh, so_dg, so_pr, go_pr, go_ma, go_rh;
     int dg_cut, pr_cut, st_cut, gsh;                          // node cut of dg, pair cut of pr, node cut of vv/ma/rh
+    __device__ __forceinline__ char* s_vv() const { return sb; }
+    __device__ __forceinline__ char* s_ma() const { return sb + so_ma; }
+    __device__ __forceinline__ char* s_rh() const { return sb + so_rh; }
+    __device__ __forceinline__ char* s_dg() const { return sb + so_dg; }
+    __device__ __forceinline__ char* s_pr() const { return sb + so_pr; }
+    __device__ __forceinline__ char* g_dg() const { return gf; }
+    __device__ __forceinline__ char* g_pr() const { return gf + go_pr; }
+    __device__ __forceinline__ char* g_vv() const { return gw; }
+    __device__ __forceinline__ char* g_ma() const { return gw + go_ma; }
+    __device__ __forceinline__ char* g_rh() const { return gw + go_rh; }
 
     __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
         if (kSmem || idx >= cut_blocks) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
         vs = 16 << gsh; return reinterpret_cast<T*>(gb + (((size_t)idx * VPB) << (gsh + 4)));
     }
-    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); return ld_blk(p, vs); }
-    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg, g_dg, m, dg_cut, vs); st_blk(p, vs, v); }
-    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(s_pr, g_pr, 2 * p, 2 * pr_cut, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(s_pr, g_pr, 2 * p + 1, 2 * pr_cut, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr, g_pr, 2 * p, 2 * pr_cut, vs); st_blk(q, vs, v); }
-    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr, g_pr, 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); return ld_blk(p, vs); }
+    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); st_blk(p, vs, v); }
+    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(s_pr(), g_pr(), 2 * p, 2 * pr_cut, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p, 2 * pr_cut, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
 
     __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
         if (kSmem || m >= st_cut) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
         return reinterpret_cast<double2*>(gb + ((size_t)m << (gsh + 4)));
     }
-    __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv, g_vv, m); }
-    __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma, g_ma, m); }
-    __device__ __forceinline__ double2 rh(int m) const { return *st_ptr(s_rh, g_rh, m); }
-    __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(s_vv, g_vv, m) = v; }
-    __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(s_ma, g_ma, m) = v; }
-    __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(s_rh, g_rh, m) = v; }
+    __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv(), g_vv(), m); }
+    __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma(), g_ma(), m); }
+    __device__ __forceinline__ double2 rh(int m) const { return *st_ptr(s_rh(), g_rh(), m); }
+    __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(s_vv(), g_vv(), m) = v; }
+    __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(s_ma(), g_ma(), m) = v; }
+    __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(s_rh(), g_rh(), m) = v; }
 };
 
 // ---- level-blob ring: cp.async.bulk (TMA 1-D bulk copy) + mbarrier ------------------------------------------------

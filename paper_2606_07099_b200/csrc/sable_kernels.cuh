@@ -47,11 +47,12 @@ template <typename T, bool kSmem>
 __device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
     Slot<T, kSmem> s;
     char* p = reinterpret_cast<char*>(smem) + smem_fixed(n_level, ring_bytes) + g * 16;
-    const size_t ns = ((size_t)(n_node + 1 - st_cut) * 16) << gsh;
-    s.s_vv = p; s.s_ma = p + ns; s.s_rh = p + 2 * ns;
-    s.s_dg = p + 3 * ns;
-    s.s_pr = s.s_dg + (((size_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh);
-    s.g_dg = s.g_pr = s.g_vv = s.g_ma = s.g_rh = nullptr;
+    const unsigned ns = (unsigned)(((size_t)(n_node + 1 - st_cut) * 16) << gsh);
+    s.sb = p; s.so_ma = ns; s.so_rh = 2 * ns; s.so_dg = 3 * ns;
+    s.so_pr = s.so_dg + (unsigned)(((size_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh);
+    s.gf = s.gw = nullptr;
+    s.go_pr = (unsigned)(((size_t)n_node * 4 * sizeof(T)) << gsh);
+    s.go_ma = (unsigned)(((size_t)(n_node + 1) * 16) << gsh); s.go_rh = 2 * s.go_ma;
     s.dg_cut = dg_cut; s.pr_cut = pr_cut; s.st_cut = st_cut; s.gsh = gsh;
     return s;
 }
@@ -60,11 +61,8 @@ template <typename T, bool kSmem>
 __device__ __forceinline__ void bind(Slot<T, kSmem>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
     const int gsh = s.gsh;
     const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
-    s.g_dg = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
-    s.g_pr = s.g_dg + (((size_t)n_node * 4 * sizeof(T)) << gsh);
-    s.g_vv = work + ((grp * (size_t)work_stride) << gsh) + lane16;
-    s.g_ma = s.g_vv + (((size_t)(n_node + 1) * 16) << gsh);
-    s.g_rh = s.g_ma + (((size_t)(n_node + 1) * 16) << gsh);
+    s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
+    s.gw = work + ((grp * (size_t)work_stride) << gsh) + lane16;
 }
 
 template <typename T, bool kSmem>
@@ -104,10 +102,10 @@ template <typename T, bool kSmem>
 __device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
     constexpr int VPB = Slot<T, kSmem>::VPB;
     const int n_dg = (t.n_node - s.dg_cut) * VPB, n_pr = 2 * (t.n_pair - s.pr_cut) * VPB;
-    char* gd = s.g_dg + (((size_t)s.dg_cut * VPB) << (s.gsh + 4));
-    char* gp = s.g_pr + (((size_t)2 * s.pr_cut * VPB) << (s.gsh + 4));
-    for (int i = tsub; i < n_dg; i += nsub) *reinterpret_cast<int4*>(gd + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_dg + ((size_t)i << (s.gsh + 4)));
-    for (int i = tsub; i < n_pr; i += nsub) *reinterpret_cast<int4*>(gp + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_pr + ((size_t)i << (s.gsh + 4)));
+    char* gd = s.g_dg() + (((size_t)s.dg_cut * VPB) << (s.gsh + 4));
+    char* gp = s.g_pr() + (((size_t)2 * s.pr_cut * VPB) << (s.gsh + 4));
+    for (int i = tsub; i < n_dg; i += nsub) *reinterpret_cast<int4*>(gd + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_dg() + ((size_t)i << (s.gsh + 4)));
+    for (int i = tsub; i < n_pr; i += nsub) *reinterpret_cast<int4*>(gp + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_pr() + ((size_t)i << (s.gsh + 4)));
 }
 
 __device__ __forceinline__ int pop_group(const SolveArgs& A) {

@@ -9,7 +9,9 @@ namespace sable {
 template <typename T>
 __device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
     Slot<T, false> s;
-    s.s_dg = s.s_pr = s.s_vv = s.s_ma = s.s_rh = nullptr;
+    s.sb = nullptr; s.so_ma = s.so_rh = s.so_dg = s.so_pr = 0;
+    s.go_pr = (unsigned)(((size_t)t.n_node * 4 * sizeof(T)) << gsh);
+    s.go_ma = (unsigned)(((size_t)(t.n_node + 1) * 16) << gsh); s.go_rh = 2 * s.go_ma;
     s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = gsh;
     bind<T, false>(s, factors, fac_stride, work, work_stride, t.n_node, b);
     return s;
@@ -34,7 +36,7 @@ __global__ void k_st_init(const SolveArgs A) {
 // a1 + a6 + a2: mismatch, norm, convergence decision, Jacobian fill (in place, into the factor value array) for the
 // scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here
 template <typename T>
-__global__ void k_st_mismatch_fill(const SolveArgs A) {
+__global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) {
     __shared__ double red[32 * 32];
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
@@ -55,7 +57,7 @@ __global__ void k_st_mismatch_fill(const SolveArgs A) {
 
 // a4 + a5: refactor, forward/backward substitution, FP64 state update
 template <typename T>
-__global__ void k_st_factor_solve(const SolveArgs A) {
+__global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;
     const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
@@ -86,7 +88,7 @@ __global__ void k_linsolve(const LinArgs A) {
     const int bb = (blockIdx.x << gsh) + g;
     const bool act = bb < A.batch;
     Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
-    if (A.rhs_in_smem) { s.st_cut = 0; s.s_rh = reinterpret_cast<char*>(smem) + g * 16; }
+    if (A.rhs_in_smem) { s.st_cut = 0; s.sb = reinterpret_cast<char*>(smem) + g * 16; s.so_rh = 0; }   // only rh is touched
     const size_t o = (size_t)(act ? bb : 0) * t.n_bus;
     for (int m = tsub; m < t.n_node; m += nsub) {
         const int bus = t.node_bus[m];
@@ -144,8 +146,8 @@ __global__ void k_debug(const DebugArgs A) {
     stage_fill_pairs<T, false>(t, s, threadIdx.x, blockDim.x);
     __syncthreads();
     if (A.what == 1) {
-        const T* dg = reinterpret_cast<const T*>(s.g_dg);
-        const T* pr = reinterpret_cast<const T*>(s.g_pr);
+        const T* dg = reinterpret_cast<const T*>(s.g_dg());
+        const T* pr = reinterpret_cast<const T*>(s.g_pr());
         for (int i = threadIdx.x; i < 4 * t.n_node; i += blockDim.x) A.diag[(size_t)b * 4 * t.n_node + i] = double(dg[i]);
         for (int i = threadIdx.x; i < 8 * t.n_pair; i += blockDim.x) A.pairs[(size_t)b * 8 * t.n_pair + i] = double(pr[i]);
         return;
