@@ -35,8 +35,8 @@ WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward"
             4: "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
             5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
-# captures (profiles/r01_v2_README.md); None where no capture exists
-NCU_TRAFFIC = {3: 59.070976e6 + 283.826944e6, 5: 10.338136e9 + 5.761298e9}
+# captures (profiles/r01_v3_README.md); None where no capture exists
+NCU_TRAFFIC = {2: 2.989056e6, 3: 4.315116e9 + 4.499813e9, 4: 6.467309e9 + 4.686739e9, 5: 10.355699e9 + 5.722466e9}
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 
