@@ -17,7 +17,7 @@ def build(force=False, verbose=False):
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = OUT + f".{os.getpid()}.tmp"
-    subprocess.check_call([nvcc] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC)
+    subprocess.check_call([nvcc] + FLAGS + os.environ.get("SABLE_NVCC_FLAGS", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC)
     os.replace(tmp, OUT)
     return OUT
 

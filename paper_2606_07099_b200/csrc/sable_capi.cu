@@ -72,9 +72,10 @@ static void fill_info(sable_ctx* c) {
     I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->cut_level;
 }
 
-static const void* fused_fn(bool mixed, bool all_smem) {
-    if (mixed) return all_smem ? (const void*)k_nr_fused<float, true> : (const void*)k_nr_fused<float, false>;
-    return all_smem ? (const void*)k_nr_fused<double, true> : (const void*)k_nr_fused<double, false>;
+static const void* fused_fn(bool mixed, bool all_smem, bool small) {
+    if (all_smem) return mixed ? (const void*)k_nr_fused<float, true, false> : (const void*)k_nr_fused<double, true, false>;
+    if (small) return mixed ? (const void*)k_nr_fused<float, false, true> : (const void*)k_nr_fused<double, false, true>;
+    return mixed ? (const void*)k_nr_fused<float, false, false> : (const void*)k_nr_fused<double, false, false>;
 }
 
 static int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
@@ -221,7 +222,7 @@ static sable_status choose_launch(sable_ctx* ctx) {
     }
     ctx->threads = th;
     ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
-    const void* fn = fused_fn(mixed, ctx->placement == 0);
+    const void* fn = fused_fn(mixed, ctx->placement == 0, th <= 128);
     CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)ctx->smem));
@@ -359,8 +360,9 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
         c->factor_gsh = c->gsh;
-        if (c->placement == 0) k_nr_fused<T, true><<<grid, c->threads, c->smem, s>>>(A);
-        else k_nr_fused<T, false><<<grid, c->threads, c->smem, s>>>(A);
+        if (c->placement == 0) k_nr_fused<T, true, false><<<grid, c->threads, c->smem, s>>>(A);
+        else if (c->threads <= 128) k_nr_fused<T, false, true><<<grid, c->threads, c->smem, s>>>(A);
+        else k_nr_fused<T, false, false><<<grid, c->threads, c->smem, s>>>(A);
         c->launches += 1;
     } else {
         A.t.level = c->level_one;

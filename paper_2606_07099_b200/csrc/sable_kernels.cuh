@@ -1,6 +1,6 @@
-// The fused persistent Newton-Raphson kernel: a CTA serves G scenario slots in lockstep and runs their whole NR loops
-// on chip; a slot whose scenario converged (or stopped) is refilled from an atomic queue at once, which is the
-// per-scenario convergence masking (a converged scenario costs nothing further).  Launched from sable_capi.cu.
+// The fused persistent Newton-Raphson kernel: a CTA takes groups of G scenarios from an atomic queue and runs the whole
+// NR loops of a group's scenarios in lockstep, with no host round trip; a scenario that converged (or stopped) is no
+// longer evaluated -- the per-scenario convergence masking.  Launched from sable_capi.cu.
 #pragma once
 #include "sable_stages.cuh"
 
@@ -14,8 +14,8 @@ struct SolveArgs {
     double *vm, *va, *final_norm;
     int32_t* iterations;
     uint8_t* converged;
-    char* factors;            // [max_batch + 1][fac_stride] bytes
-    char* work;               // [max_batch + 1][work_stride] bytes
+    char* factors;            // [groups + 1][fac_stride << gsh] bytes, group-interleaved (sable_device.cuh)
+    char* work;               // [groups + 1][work_stride << gsh] bytes
     int64_t fac_stride, work_stride;
     int32_t gsh, dg_cut, pr_cut, st_cut;                   // slots per CTA = 1 << gsh; placement cuts (nodes, pairs, nodes)
     int32_t ring_r, ring_slot, first_staged;               // level-blob ring: slots, bytes per slot, first streamed level
@@ -118,8 +118,11 @@ __device__ __forceinline__ int pop_group(const SolveArgs& A) {
 // A CTA takes one GROUP of G consecutive scenarios at a time from the atomic queue (slot g serves scenario
 // group * G + g, whose HBM slices are interleaved with the rest of its group) and advances its slots in lockstep; a slot
 // that has finished stops being evaluated (its lanes run along and write nothing that is read) until the group is done.
-template <typename T, bool kSmem>
-__global__ void __launch_bounds__(512, kSmem ? 1 : 2) k_nr_fused(const SolveArgs A) {
+// Register budgets (measured, profiles/r01_v2_sweeps.md): on chip 1 CTA of up to 512 threads (up to 128 registers); HBM
+// placement 2 x 512 threads (64 registers) or, kSmall, 7 x 128 threads (72 registers: the FP64 build then spills
+// 110 B instead of 190 B and cfg 3 runs 6 % faster).
+template <typename T, bool kSmem, bool kSmall>
+__global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? 7 : 2)) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;

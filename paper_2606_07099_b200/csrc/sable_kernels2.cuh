@@ -1,5 +1,6 @@
 // Staged kernels (one kernel per stage, state in HBM between stages -- the per-stage profiling mode), the adjoint /
-// linear-solve kernel on kept factors, and the debug kernels.  All of them serve one scenario per CTA (gsh = 0).
+// linear-solve kernel on kept factors, and the debug kernels.  The staged and debug kernels serve one scenario per CTA
+// (gsh = 0); the adjoint kernel serves one group per CTA in the layout the factors were written in.
 #pragma once
 #include "sable_kernels.cuh"
 
