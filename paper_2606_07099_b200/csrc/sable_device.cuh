@@ -204,6 +204,16 @@ struct BlobRing {
         if (threadIdx.x == 0) issue(use + (unsigned)R);
         ++use;
     }
+    // a backward sweep that is not run: its entries still pass through the ring (the producer runs R entries ahead),
+    // so consume them; contains barriers
+    __device__ __forceinline__ void skip_sweep() {
+        for (int l = n_level - 1; l >= first; --l) {
+            const int sl = (int)(use % (unsigned)R);
+            mbar_wait(mbar + sl, (use / (unsigned)R) & 1u);
+            __syncthreads();
+            release(l);
+        }
+    }
     __device__ __forceinline__ void drain() const {                    // before the CTA exits: no copy may be in flight
         if (first < n_level && threadIdx.x == 0)
             for (unsigned e = use; e < use + (unsigned)R; ++e) mbar_wait(mbar + (e % (unsigned)R), (e / (unsigned)R) & 1u);

@@ -189,8 +189,10 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? 7 : 
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
         stage_factor_forward<T, kSmem, true, true, false, false>(t, s, lv, ring);
-        stage_backward<T, kSmem, false>(t, s, lv, ring);
-        stage_update<T, kSmem>(t, s, tsub, nsub);
+        if (any_slot(b >= 0 && !fin)) {                    // a trip that only refactors for kept factors needs no solve
+            stage_backward<T, kSmem, false>(t, s, lv, ring);
+            stage_update<T, kSmem>(t, s, tsub, nsub);
+        } else ring.skip_sweep();
         if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
         if (b >= 0 && !fin) ++it;
         if (fin) {
