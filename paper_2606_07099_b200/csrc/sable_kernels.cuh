@@ -185,10 +185,10 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? 7 : 
         }
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
-        stage_fill_pairs<T, kSmem>(t, s, tsub, nsub);
+        stage_fill_pairs<T, kSmem, true>(t, s, tsub, nsub, lv[0].p1);
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
-        stage_factor_forward<T, kSmem, true, true, false, false>(t, s, lv, ring);
+        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv, ring);
         if (any_slot(b >= 0 && !fin)) {                    // a trip that only refactors for kept factors needs no solve
             stage_backward<T, kSmem, false>(t, s, lv, ring);
             stage_update<T, kSmem>(t, s, tsub, nsub);

@@ -47,12 +47,12 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     int st = 0;
     if (r <= A.tol) st = 1;
     else if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) st = 2;
-    if (st == 0 || A.keep) stage_fill_pairs<T, false>(A.t, s, threadIdx.x, blockDim.x);
+    if (st == 0 || A.keep) stage_fill_pairs<T, false, true>(A.t, s, threadIdx.x, blockDim.x, A.t.level[0].p1);
     if (st != 0) {
         scen_output<T, false>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
         __syncthreads();
         if (threadIdx.x == 0) A.status[b] = st;
-        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, false, true, false, false, false>(A.t, s, A.t.level, ring); }
+        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, false, true, false, false, true>(A.t, s, A.t.level, ring); }
     }
 }
 
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
     if (A.status[b] != 0) return;
     const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
     BlobRing ring = no_ring(A.t);
-    stage_factor_forward<T, false, true, true, false, false>(A.t, s, A.t.level, ring);
+    stage_factor_forward<T, false, true, true, false, true>(A.t, s, A.t.level, ring);
     stage_backward<T, false, false>(A.t, s, A.t.level, ring);
     stage_update<T, false>(A.t, s, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) A.it[b] += 1;
@@ -144,7 +144,7 @@ __global__ void k_debug(const DebugArgs A) {
         if (threadIdx.x == 0) A.norm[b] = r;
         return;
     }
-    stage_fill_pairs<T, false>(t, s, threadIdx.x, blockDim.x);
+    stage_fill_pairs<T, false, false>(t, s, threadIdx.x, blockDim.x, 0);
     __syncthreads();
     if (A.what == 1) {
         const T* dg = reinterpret_cast<const T*>(s.g_dg());

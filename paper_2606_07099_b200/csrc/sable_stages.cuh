@@ -75,12 +75,16 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kSmem>& s, int2 mj, doub
     L.a = T(l1);  L.b = T(l2 * ivm);  L.c = jpq ? T(-l2) : T(0);  L.d = jpq ? T(l1 * ivm) : T(0);
 }
 
-// separate a2 pass (staged mode and debug export): every pair slot of the filled pattern is written
-template <typename T, bool kSmem>
-__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
+// a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  kPrescale: the pairs owned by
+// level-0 nodes (p < leaf_p1; such a node has no earlier neighbour, so D_m = J(m,m) and its pairs have no terms) get
+// their final values here -- U(m,j) = J(m,j), L(j,m) = J(j,m) J(m,m)^-1 -- and the refactor skips them (kLeafDone).
+template <typename T, bool kSmem, bool kPrescale>
+__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub, int leaf_p1) {
     for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
-        fill_pair<T, kSmem>(s, t.pair_mj[p], t.pair_y[p], U, L);
+        const int2 mj = t.pair_mj[p];
+        fill_pair<T, kSmem>(s, mj, t.pair_y[p], U, L);
+        if (kPrescale && p < leaf_p1) L = mul(L, inv(s.ldD(mj.x & kIdxMask)));
         s.stU(p, U); s.stL(p, L);
     }
 }
@@ -89,9 +93,10 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slo
 // inverted), fused with the forward substitution L y = rhs which walks the same lists.  Contains barriers.
 //   diag target m :  D_m = J(m,m) - sum_k L(m,k) U(k,m);   y_m = rhs_m - sum_k L(m,k) y_k      (k: pairs (k,m))
 //   pair target p :  U(m,j) = J(m,j) - sum_k L(m,k) U(k,j);  L(j,m) = (J(j,m) - sum_k L(j,k) U(k,m)) D_m^-1
-// kInlineFill: J(m,j), J(j,m) are evaluated here (a2 fused into a4, the value array is written once, final).
+// kLeafDone: the pairs of level 0 already hold their final values (stage_fill_pairs<kPrescale>), level 0 then has
+// diagonal targets only and a single barrier.  A pair target without terms is not touched by the accumulate pass.
 // kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
-template <typename T, bool kSmem, bool kFactor, bool kSolve, bool kTransposed, bool kInlineFill>
+template <typename T, bool kSmem, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone>
 __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv, BlobRing& ring) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
@@ -103,7 +108,6 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
         const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
         const int2* tab = reinterpret_cast<const int2*>(lb + d.o_tab);
-        const double4* py = reinterpret_cast<const double4*>(lb + d.o_py);
         {
             const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
             const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
@@ -147,7 +151,7 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
                 }
             }
         }
-        if (kFactor) {
+        if (kFactor && !(kLeafDone && l == 0)) {
             // pair targets accumulate J - sum(terms) concurrently with the diagonal targets (they only need factors of
             // earlier levels); warps are taken from the other end so that a narrow level spreads over distinct warps
             const int ssh = d.sp, tsh = 5 - gsh - ssh, S = 1 << ssh;
@@ -155,14 +159,10 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
             for (int base = d.p0 + ((nwarps - 1 - warp) << tsh); base < d.p1; base += nwarps << tsh) {
                 const bool valid = base + tl < d.p1;
                 const int p = valid ? base + tl : d.p1 - 1;
-                const bool lead = valid && part == 0;
                 const int t0 = tptr[p - d.p0], t1 = valid ? tptr[p - d.p0 + 1] : t0;
-                const int2 mj = pmj[p - d.p0];
+                const bool lead = valid && part == 0 && t1 > t0;
                 Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
-                if (lead) {
-                    if (kInlineFill) fill_pair<T, kSmem>(s, mj, py[p - d.p0], U, L);
-                    else { U = s.ldU(p); L = s.ldL(p); }
-                }
+                if (lead) { U = s.ldU(p); L = s.ldL(p); }
                 for (int q = t0 + part; q < t1; q += S) {
                     const int2 ab = tab[q];
                     mulsub(U, s.ldL(ab.x), s.ldU(ab.y));
