@@ -213,7 +213,7 @@ static sable_status choose_launch(sable_ctx* ctx) {
         // slots per CTA (= scenarios whose HBM slices are interleaved): 4 / 2 / 1 by grid size, or SABLE_G
         int sg = 0;
         const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : nn <= 4000 ? 2 : 1);
-        while ((2 << sg) <= g_want && ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1)) ++sg;
+        while ((2 << sg) <= g_want && (g_env > 0 || ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1))) ++sg;
         if (cl < 0) { cl = 0; while (cl < nl && need(sg, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
         cl = std::min(cl, nl);
         const int nc = cl < nl ? T.level_ptr[cl] : nn;

@@ -385,6 +385,10 @@ def test_placements_and_group_layouts(env, monkeypatch):
     ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=12, method=1)
     for keep in (False, True):
         ctx = make_ctx(net, max_batch=256, keep_factors=keep)
+        if "SABLE_G" in env:
+            assert ctx.info["slots_per_cta"] == int(env["SABLE_G"])
+        if "SABLE_CUT" in env:
+            assert ctx.info["placement"] == 1
         res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
         check_solution(res, ref, c.tol, 1e-9)
         if keep:
