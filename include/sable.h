@@ -170,7 +170,8 @@ sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, const doubl
                                       double* x_p, double* x_q, void* cuda_stream);
 
 /* Per-phase cycle counters of CTA 0 of the fused kernel, accumulated since the last call (then reset).  Only when
- * the context was created with SABLE_TIMING=1 in the environment (else SABLE_ERR_STATE).  out[4 l + 0 / 1 / 2] = cycles
+ * the context was created with SABLE_TIMING=1 in the environment (else SABLE_ERR_STATE); the HBM-placement kernels
+ * carry the counters only when the library is built with -DSABLE_TIMING_ALL (they cost registers there).  out[4 l + 0 / 1 / 2] = cycles
  * in the diagonal-target / pair-target / backward phase of elimination level l; out[4 L] = cycles in decision +
  * output; out[4 L + 1] = loop trips; out[4 L + 2] = refill + init; out[4 L + 3] = mismatch + norm; L = n_level;
  * n = entries wanted, at most 4 L + 4 (HOST out). */

@@ -168,6 +168,7 @@ struct BlobRing {
     char* slots; unsigned long long* mbar;
     const char* gblob; const LevelDesc* lv;
     int R, slot_bytes, first, n_level;
+    bool on;                   // false (a compile-time constant in the HBM-placement kernels): blobs are read in place
     unsigned use;
     unsigned long long* tim;   // optional per-phase cycle counters of CTA 0 (sable_debug_timing); nullptr = off
     __device__ __forceinline__ void tick(int slot, long long& t0) const {   // thread 0 of CTA 0, right after a barrier
@@ -185,6 +186,7 @@ struct BlobRing {
     }
     __device__ __forceinline__ void start() {                          // all threads, once; contains a barrier
         use = 0;
+        if (!on) return;
         if (first < n_level && threadIdx.x == 0) {
             for (int i = 0; i < R; ++i) mbar_init(mbar + i, 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -193,20 +195,21 @@ struct BlobRing {
         if (first < n_level && threadIdx.x == 0) for (int i = 0; i < R; ++i) issue((unsigned)i);
     }
     __device__ __forceinline__ const char* acquire(int l, const LevelDesc& d) const {
-        if (l < first) return gblob + d.blob_off;
+        if (!on || l < first) return gblob + d.blob_off;
         const int sl = (int)(use % (unsigned)R);
         mbar_wait(mbar + sl, (use / (unsigned)R) & 1u);
         return slots + (size_t)sl * slot_bytes;
     }
     // after a CTA barrier that follows the last read of level l's blob
     __device__ __forceinline__ void release(int l) {
-        if (l < first) return;
+        if (!on || l < first) return;
         if (threadIdx.x == 0) issue(use + (unsigned)R);
         ++use;
     }
     // a backward sweep that is not run: its entries still pass through the ring (the producer runs R entries ahead),
     // so consume them; contains barriers
     __device__ __forceinline__ void skip_sweep() {
+        if (!on) return;
         for (int l = n_level - 1; l >= first; --l) {
             const int sl = (int)(use % (unsigned)R);
             mbar_wait(mbar + sl, (use / (unsigned)R) & 1u);
@@ -215,7 +218,7 @@ struct BlobRing {
         }
     }
     __device__ __forceinline__ void drain() const {                    // before the CTA exits: no copy may be in flight
-        if (first < n_level && threadIdx.x == 0)
+        if (on && first < n_level && threadIdx.x == 0)
             for (unsigned e = use; e < use + (unsigned)R; ++e) mbar_wait(mbar + (e % (unsigned)R), (e / (unsigned)R) & 1u);
     }
 };

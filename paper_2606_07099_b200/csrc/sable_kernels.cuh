@@ -121,8 +121,11 @@ __device__ __forceinline__ int pop_group(const SolveArgs& A) {
 // Register budgets (measured, profiles/r01_v2_sweeps.md): on chip 1 CTA of up to 512 threads (up to 128 registers); HBM
 // placement 2 x 512 threads (64 registers) or, kSmall, 7 x 128 threads (72 registers: the FP64 build then spills
 // 110 B instead of 190 B and cfg 3 runs 6 % faster).
+#ifndef SABLE_SMALL_B32
+#define SABLE_SMALL_B32 7
+#endif
 template <typename T, bool kSmem, bool kSmall>
-__global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? 7 : 2)) k_nr_fused(const SolveArgs A) {
+__global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? (sizeof(T) == 4 ? SABLE_SMALL_B32 : 7) : 2)) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
@@ -136,7 +139,12 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? 7 : 
     ring.mbar = reinterpret_cast<unsigned long long*>(smem + kRedBytes + 128);
     ring.gblob = t.blob; ring.lv = lv; ring.R = A.ring_r; ring.slot_bytes = A.ring_slot;
     ring.first = A.first_staged; ring.n_level = t.n_level;
+    ring.on = kSmem && A.ring_r > 0;
+#ifdef SABLE_TIMING_ALL
     ring.tim = blockIdx.x == 0 ? A.tim : nullptr;
+#else
+    ring.tim = (kSmem && blockIdx.x == 0) ? A.tim : nullptr;   // HBM-placement kernels: counters compiled out (registers)
+#endif
     long long tk = clock64();
     __syncthreads();                                       // lv[] complete before the producer reads it
     ring.start();

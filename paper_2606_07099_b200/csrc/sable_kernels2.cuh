@@ -22,7 +22,7 @@ __device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* f
 __device__ __forceinline__ BlobRing no_ring(const DevTemplate& t) {
     BlobRing r;
     r.slots = nullptr; r.mbar = nullptr; r.gblob = t.blob; r.lv = t.level; r.R = 0; r.slot_bytes = 0;
-    r.first = t.n_level; r.n_level = t.n_level; r.use = 0; r.tim = nullptr;
+    r.first = t.n_level; r.n_level = t.n_level; r.use = 0; r.tim = nullptr; r.on = false;
     return r;
 }
 
