@@ -68,8 +68,8 @@ typedef struct {
     int64_t bytes_iter_m0;  /* SURVEY.md §8(d) model M0: algorithmic HBM bytes per scenario per NR iteration */
     int64_t bytes_adjoint_m0; /* same for one adjoint solve */
     int32_t smem_bytes;     /* dynamic shared memory per CTA of the NR kernel */
-    int32_t placement;      /* 0: factors, V and rhs of every slot in shared memory; 1: elimination levels >= cut_level
-                               in shared memory, the wide early levels in the scenario's HBM workspace slice */
+    int32_t placement;      /* 0: factors, V and rhs of every slot in shared memory; 2: everything in the group-interleaved
+                               HBM workspace; 1 (only on request): elimination levels >= cut_level in shared memory */
     int32_t threads;        /* threads per CTA */
     int32_t ctas_per_sm;    /* occupancy the NR kernel was sized for */
     int32_t slots_per_cta;  /* scenarios a CTA of the NR kernel advances in lockstep */

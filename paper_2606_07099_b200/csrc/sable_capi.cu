@@ -72,10 +72,12 @@ static void fill_info(sable_ctx* c) {
     I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->cut_level;
 }
 
-static const void* fused_fn(bool mixed, bool all_smem, bool small) {
-    if (all_smem) return mixed ? (const void*)k_nr_fused<float, true, false> : (const void*)k_nr_fused<double, true, false>;
-    if (small) return mixed ? (const void*)k_nr_fused<float, false, true> : (const void*)k_nr_fused<double, false, true>;
-    return mixed ? (const void*)k_nr_fused<float, false, false> : (const void*)k_nr_fused<double, false, false>;
+// kernel variant: placement 0 = on chip, 1 = mixed (only on request: SABLE_CUT), 2 = HBM; small = up to 128 threads
+static const void* fused_fn(bool mixed, int place, bool small) {
+    if (place == 0) return mixed ? (const void*)k_nr_fused<float, 0, false> : (const void*)k_nr_fused<double, 0, false>;
+    if (place == 1) return mixed ? (const void*)k_nr_fused<float, 1, false> : (const void*)k_nr_fused<double, 1, false>;
+    if (small) return mixed ? (const void*)k_nr_fused<float, 2, true> : (const void*)k_nr_fused<double, 2, true>;
+    return mixed ? (const void*)k_nr_fused<float, 2, false> : (const void*)k_nr_fused<double, 2, false>;
 }
 
 static int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
@@ -200,29 +202,29 @@ static sable_status choose_launch(sable_ctx* ctx) {
     if (on_chip) {
         ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
     } else {
-        // split placement.  Measured (profiles/r01_v2_sweeps.md): for grids whose factors do not fit on chip, resident
-        // warps and a large L1 (which then holds the shared index program and Y_bus) buy more than shared-memory
-        // residency of a part of the factors: keep only a small top of the elimination tree on chip (<= 24 KB per
-        // CTA), read the level blobs in place (no ring), and let the register file set the CTA count (the split
-        // kernel is built for 64 registers: 1024 threads per SM).
+        // HBM placement.  Measured (profiles/r01_v2_sweeps.md): once the batch needs many waves, resident warps and a
+        // large L1 (which then holds the shared index program and Y_bus) buy more than shared-memory residency of the
+        // factors, and even a small on-chip top of the elimination tree is neutral to slightly negative: everything
+        // lives in the group-interleaved HBM workspace (placement 2, kernels without placement branches), the level
+        // blobs are read in place (no ring), and the register file sets the CTA count (72 registers for up to 128
+        // threads per CTA, 64 beyond).  SABLE_CUT=<level> asks for the mixed placement 1 (levels >= cut on chip).
         if (ctx->opt.threads <= 0 && env_int("SABLE_THREADS", 0) <= 0) th = nn <= 1200 ? 128 : nn <= 4000 ? 256 : 512;
         want_ctas = env_int("SABLE_CTAS", std::max(1, 1024 / th));
         set_ring(r_env >= 0 ? ropts[0] : RingOpt{0, 0});
-        const int64_t budget = std::min<int64_t>({(int64_t)max_optin, (int64_t)smem_sm / want_ctas - 2048, (int64_t)env_int("SABLE_SPLIT_SMEM", 24576)});
-        int cl = cut_env;
         // slots per CTA (= scenarios whose HBM slices are interleaved): 4 / 2 / 1 by grid size, or SABLE_G
         int sg = 0;
         const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : nn <= 4000 ? 2 : 1);
         while ((2 << sg) <= g_want && (g_env > 0 || ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1))) ++sg;
-        if (cl < 0) { cl = 0; while (cl < nl && need(sg, T.level_ptr[cl], T.pair_ptr[T.level_ptr[cl]], T.level_ptr[cl]) > budget) ++cl; }
-        cl = std::min(cl, nl);
+        const int cl = cut_env >= 0 ? std::min(cut_env, nl) : nl;
         const int nc = cl < nl ? T.level_ptr[cl] : nn;
-        ctx->placement = 1; ctx->gsh = sg; ctx->dg_cut = nc; ctx->st_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->cut_level = cl;
+        ctx->placement = cl < nl ? 1 : 2; ctx->gsh = sg; ctx->cut_level = cl;
+        ctx->dg_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->st_cut = cl < nl ? nc : nn + 1;
+        if (ctx->placement == 1 && th <= 128) th = 256;      // the mixed kernel is built in the large variant only
         if (need(sg, ctx->dg_cut, ctx->pr_cut, ctx->st_cut) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
     }
     ctx->threads = th;
     ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
-    const void* fn = fused_fn(mixed, ctx->placement == 0, th <= 128);
+    const void* fn = fused_fn(mixed, ctx->placement, th <= 128);
     CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)ctx->smem));
@@ -360,9 +362,10 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
         c->factor_gsh = c->gsh;
-        if (c->placement == 0) k_nr_fused<T, true, false><<<grid, c->threads, c->smem, s>>>(A);
-        else if (c->threads <= 128) k_nr_fused<T, false, true><<<grid, c->threads, c->smem, s>>>(A);
-        else k_nr_fused<T, false, false><<<grid, c->threads, c->smem, s>>>(A);
+        if (c->placement == 0) k_nr_fused<T, 0, false><<<grid, c->threads, c->smem, s>>>(A);
+        else if (c->placement == 1) k_nr_fused<T, 1, false><<<grid, c->threads, c->smem, s>>>(A);
+        else if (c->threads <= 128) k_nr_fused<T, 2, true><<<grid, c->threads, c->smem, s>>>(A);
+        else k_nr_fused<T, 2, false><<<grid, c->threads, c->smem, s>>>(A);
         c->launches += 1;
     } else {
         A.t.level = c->level_one;

@@ -102,8 +102,9 @@ __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
     *reinterpret_cast<float4*>(p) = make_float4(v.a, v.b, v.c, v.d);
 }
 
-// One thread's view of the slot it serves.  kSmem = true: everything is in shared memory (cuts are 0, no branches).
-template <typename T, bool kSmem> struct Slot {
+// One thread's view of the slot it serves.  kP = 0: everything in shared memory; 2: everything in the HBM workspace
+// (both without placement branches); 1: mixed, split at the cuts.
+template <typename T, int kP> struct Slot {
     static constexpr int VPB = (int)(4 * sizeof(T) / 16);      // 16-byte vectors per block: 2 (FP64) or 1 (FP32)
     // Three per-thread pointers (shared base, factor slice and state slice of the group, each offset by g * 16) plus
     // CTA-uniform byte offsets of the arrays behind them (uniform registers / constant bank: keeps the register count
@@ -123,7 +124,7 @@ template <typename T, bool kSmem> struct Slot {
     __device__ __forceinline__ char* g_rh() const { return gw + go_rh; }
 
     __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
-        if (kSmem || idx >= cut_blocks) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
+        if (kP == 0 || (kP == 1 && idx >= cut_blocks)) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
         vs = 16 << gsh; return reinterpret_cast<T*>(gb + (((size_t)idx * VPB) << (gsh + 4)));
     }
     __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); return ld_blk(p, vs); }
@@ -134,7 +135,7 @@ template <typename T, bool kSmem> struct Slot {
     __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
 
     __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
-        if (kSmem || m >= st_cut) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
+        if (kP == 0 || (kP == 1 && m >= st_cut)) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
         return reinterpret_cast<double2*>(gb + ((size_t)m << (gsh + 4)));
     }
     __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv(), g_vv(), m); }

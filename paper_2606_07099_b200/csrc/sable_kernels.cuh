@@ -43,9 +43,9 @@ template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, i
 }
 
 // shared-memory part of a slot view (fixed for the lifetime of the CTA)
-template <typename T, bool kSmem>
-__device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
-    Slot<T, kSmem> s;
+template <typename T, int kP>
+__device__ __forceinline__ Slot<T, kP> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
+    Slot<T, kP> s;
     char* p = reinterpret_cast<char*>(smem) + smem_fixed(n_level, ring_bytes) + g * 16;
     const unsigned ns = (unsigned)(((size_t)(n_node + 1 - st_cut) * 16) << gsh);
     s.sb = p; s.so_ma = ns; s.so_rh = 2 * ns; s.so_dg = 3 * ns;
@@ -57,16 +57,16 @@ __device__ __forceinline__ Slot<T, kSmem> carve(unsigned char* smem, int n_node,
     return s;
 }
 // HBM part: the slices of scenario b's group (b >> gsh), offset to lane b & (G - 1); strides are per scenario
-template <typename T, bool kSmem>
-__device__ __forceinline__ void bind(Slot<T, kSmem>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
+template <typename T, int kP>
+__device__ __forceinline__ void bind(Slot<T, kP>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
     const int gsh = s.gsh;
     const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
     s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
     s.gw = work + ((grp * (size_t)work_stride) << gsh) + lane16;
 }
 
-template <typename T, bool kSmem>
-__device__ __forceinline__ void scen_init(const SolveArgs& A, const Slot<T, kSmem>& s, int b, int tsub, int nsub) {
+template <typename T, int kP>
+__device__ __forceinline__ void scen_init(const SolveArgs& A, const Slot<T, kP>& s, int b, int tsub, int nsub) {
     const DevTemplate& t = A.t;
     const size_t o = (size_t)b * t.n_bus;
     for (int m = tsub; m <= t.n_node; m += nsub) {       // PAPER.md:287 flat start unless vm0/va0 given
@@ -80,8 +80,8 @@ __device__ __forceinline__ void scen_init(const SolveArgs& A, const Slot<T, kSme
     }
 }
 
-template <typename T, bool kSmem>
-__device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kSmem>& s, int b, int it, bool conv, double r, int tsub, int nsub) {
+template <typename T, int kP>
+__device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kP>& s, int b, int it, bool conv, double r, int tsub, int nsub) {
     const DevTemplate& t = A.t;
     const size_t o = (size_t)b * t.n_bus;
     for (int m = tsub; m <= t.n_node; m += nsub) {
@@ -98,9 +98,9 @@ __device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kS
 
 // kept factors (reading 16): the on-chip part of the factors of J1 at the final
 // iterate goes to the scenario's HBM slice, next to the part that already lives there
-template <typename T, bool kSmem>
-__device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
-    constexpr int VPB = Slot<T, kSmem>::VPB;
+template <typename T, int kP>
+__device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
+    constexpr int VPB = Slot<T, kP>::VPB;
     const int n_dg = (t.n_node - s.dg_cut) * VPB, n_pr = 2 * (t.n_pair - s.pr_cut) * VPB;
     char* gd = s.g_dg() + (((size_t)s.dg_cut * VPB) << (s.gsh + 4));
     char* gp = s.g_pr() + (((size_t)2 * s.pr_cut * VPB) << (s.gsh + 4));
@@ -124,8 +124,8 @@ __device__ __forceinline__ int pop_group(const SolveArgs& A) {
 #ifndef SABLE_SMALL_B32
 #define SABLE_SMALL_B32 7
 #endif
-template <typename T, bool kSmem, bool kSmall>
-__global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? (sizeof(T) == 4 ? SABLE_SMALL_B32 : 7) : 2)) k_nr_fused(const SolveArgs A) {
+template <typename T, int kP, bool kSmall>
+__global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? (sizeof(T) == 4 ? SABLE_SMALL_B32 : 7) : 2)) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
@@ -133,17 +133,17 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? (siz
     int* s_b = reinterpret_cast<int*>(smem + kRedBytes);
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
     for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
-    Slot<T, kSmem> s = carve<T, kSmem>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    Slot<T, kP> s = carve<T, kP>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
     BlobRing ring;
     ring.slots = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)t.n_level * (int64_t)sizeof(LevelDesc));
     ring.mbar = reinterpret_cast<unsigned long long*>(smem + kRedBytes + 128);
     ring.gblob = t.blob; ring.lv = lv; ring.R = A.ring_r; ring.slot_bytes = A.ring_slot;
     ring.first = A.first_staged; ring.n_level = t.n_level;
-    ring.on = kSmem && A.ring_r > 0;
+    ring.on = kP == 0 && A.ring_r > 0;
 #ifdef SABLE_TIMING_ALL
     ring.tim = blockIdx.x == 0 ? A.tim : nullptr;
 #else
-    ring.tim = (kSmem && blockIdx.x == 0) ? A.tim : nullptr;   // HBM-placement kernels: counters compiled out (registers)
+    ring.tim = (kP == 0 && blockIdx.x == 0) ? A.tim : nullptr;   // HBM-placement kernels: counters compiled out (registers)
 #endif
     long long tk = clock64();
     __syncthreads();                                       // lv[] complete before the producer reads it
@@ -167,17 +167,17 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? (siz
             const int grp = s_b[0];
             if (grp < 0) { ring.drain(); return; }
             const int bb = (grp << gsh) + g;
-            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, bb);
+            bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, bb);
             b = bb < A.batch ? bb : -1;
             it = 0; fin = false;
-            if (b < 0) bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
-            if (b >= 0) scen_init<T, kSmem>(A, s, b, tsub, nsub);
+            if (b < 0) bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
+            if (b >= 0) scen_init<T, kP>(A, s, b, tsub, nsub);
             __syncthreads();
         }
         ring.tick(4 * t.n_level + 2, tk);                  // group bookkeeping + init
         {
             const size_t row = (size_t)(b >= 0 ? b : 0) * t.n_bus;
-            const double loc = stage_mismatch<T, kSmem>(t, s, A.p_spec + row, A.q_spec + row, b >= 0);
+            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0);
             const double r = slot_max_nan(loc, red, gsh);
             ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
             if (b >= 0) {
@@ -185,28 +185,28 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kSmem ? 1 : (kSmall ? (siz
                 if (r <= A.tol) { done = true; conv = true; }
                 else if (it == A.max_it || !(fabs(r) < kInf)) done = true;
                 if (done) {
-                    scen_output<T, kSmem>(A, s, b, it, conv, r, tsub, nsub);
+                    scen_output<T, kP>(A, s, b, it, conv, r, tsub, nsub);
                     if (A.keep) fin = true;
-                    else { b = -1; bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g); }
+                    else { b = -1; bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g); }
                 }
             }
         }
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
-        stage_fill_pairs<T, kSmem, true>(t, s, tsub, nsub, lv[0].p1);
+        stage_fill_pairs<T, kP, true>(t, s, tsub, nsub, lv[0].p1);
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
-        stage_factor_forward<T, kSmem, true, true, false, true>(t, s, lv, ring);
+        stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring);
         if (any_slot(b >= 0 && !fin)) {                    // a trip that only refactors for kept factors needs no solve
-            stage_backward<T, kSmem, false>(t, s, lv, ring);
-            stage_update<T, kSmem>(t, s, tsub, nsub);
+            stage_backward<T, kP, false>(t, s, lv, ring);
+            stage_update<T, kP>(t, s, tsub, nsub);
         } else ring.skip_sweep();
         if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
         if (b >= 0 && !fin) ++it;
         if (fin) {
-            store_top_factors<T, kSmem>(t, s, tsub, nsub);
+            store_top_factors<T, kP>(t, s, tsub, nsub);
             b = -1; fin = false;                           // the kept factors stay untouched: run along on the spare group
-            bind<T, kSmem>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
+            bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
         }
     }
 }

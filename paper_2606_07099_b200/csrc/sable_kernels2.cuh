@@ -7,14 +7,14 @@
 namespace sable {
 
 // everything in the scenario's HBM slices
-template <typename T>
-__device__ __forceinline__ Slot<T, false> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
-    Slot<T, false> s;
+template <typename T, int kP = 2>
+__device__ __forceinline__ Slot<T, kP> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
+    Slot<T, kP> s;
     s.sb = nullptr; s.so_ma = s.so_rh = s.so_dg = s.so_pr = 0;
     s.go_pr = (unsigned)(((size_t)t.n_node * 4 * sizeof(T)) << gsh);
     s.go_ma = (unsigned)(((size_t)(t.n_node + 1) * 16) << gsh); s.go_rh = 2 * s.go_ma;
     s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = gsh;
-    bind<T, false>(s, factors, fac_stride, work, work_stride, t.n_node, b);
+    bind<T, kP>(s, factors, fac_stride, work, work_stride, t.n_node, b);
     return s;
 }
 
@@ -29,8 +29,8 @@ __device__ __forceinline__ BlobRing no_ring(const DevTemplate& t) {
 template <typename T>
 __global__ void k_st_init(const SolveArgs A) {
     const int b = blockIdx.x;
-    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    scen_init<T, false>(A, s, b, threadIdx.x, blockDim.x);
+    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    scen_init<T, 2>(A, s, b, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) { A.status[b] = 0; A.it[b] = 0; }
 }
 
@@ -41,18 +41,18 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     __shared__ double red[32 * 32];
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
-    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    const double r = slot_max_nan(stage_mismatch<T, false>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true), red, 0);
+    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true), red, 0);
     const int it = A.it[b];
     int st = 0;
     if (r <= A.tol) st = 1;
     else if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) st = 2;
-    if (st == 0 || A.keep) stage_fill_pairs<T, false, true>(A.t, s, threadIdx.x, blockDim.x, A.t.level[0].p1);
+    if (st == 0 || A.keep) stage_fill_pairs<T, 2, true>(A.t, s, threadIdx.x, blockDim.x, A.t.level[0].p1);
     if (st != 0) {
-        scen_output<T, false>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
+        scen_output<T, 2>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
         __syncthreads();
         if (threadIdx.x == 0) A.status[b] = st;
-        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, false, true, false, false, true>(A.t, s, A.t.level, ring); }
+        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, 2, true, false, false, true>(A.t, s, A.t.level, ring); }
     }
 }
 
@@ -61,11 +61,11 @@ template <typename T>
 __global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;
-    const Slot<T, false> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
     BlobRing ring = no_ring(A.t);
-    stage_factor_forward<T, false, true, true, false, true>(A.t, s, A.t.level, ring);
-    stage_backward<T, false, false>(A.t, s, A.t.level, ring);
-    stage_update<T, false>(A.t, s, threadIdx.x, blockDim.x);
+    stage_factor_forward<T, 2, true, true, false, true>(A.t, s, A.t.level, ring);
+    stage_backward<T, 2, false>(A.t, s, A.t.level, ring);
+    stage_update<T, 2>(A.t, s, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) A.it[b] += 1;
 }
 
@@ -88,7 +88,7 @@ __global__ void k_linsolve(const LinArgs A) {
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
     const int bb = (blockIdx.x << gsh) + g;
     const bool act = bb < A.batch;
-    Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
+    Slot<T, 1> s = hbm_slot<T, 1>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
     if (A.rhs_in_smem) { s.st_cut = 0; s.sb = reinterpret_cast<char*>(smem) + g * 16; s.so_rh = 0; }   // only rh is touched
     const size_t o = (size_t)(act ? bb : 0) * t.n_bus;
     for (int m = tsub; m < t.n_node; m += nsub) {
@@ -97,8 +97,8 @@ __global__ void k_linsolve(const LinArgs A) {
     }
     __syncthreads();
     BlobRing ring = no_ring(t);
-    if (A.transposed) { stage_factor_forward<T, false, false, true, true, false>(t, s, t.level, ring); stage_backward<T, false, true>(t, s, t.level, ring); }
-    else              { stage_factor_forward<T, false, false, true, false, false>(t, s, t.level, ring); stage_backward<T, false, false>(t, s, t.level, ring); }
+    if (A.transposed) { stage_factor_forward<T, 1, false, true, true, false>(t, s, t.level, ring); stage_backward<T, 1, true>(t, s, t.level, ring); }
+    else              { stage_factor_forward<T, 1, false, true, false, false>(t, s, t.level, ring); stage_backward<T, 1, false>(t, s, t.level, ring); }
     if (act)
         for (int m = tsub; m <= t.n_node; m += nsub) {
             const int bus = t.node_bus[m];
@@ -123,7 +123,7 @@ __global__ void k_debug(const DebugArgs A) {
     __shared__ double red[32 * 32];
     const DevTemplate& t = A.t;
     const int b = blockIdx.x;
-    const Slot<T, false> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
     const size_t o = (size_t)b * t.n_bus;
     for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
@@ -133,7 +133,7 @@ __global__ void k_debug(const DebugArgs A) {
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = slot_max_nan(stage_mismatch<T, false>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];
@@ -144,7 +144,7 @@ __global__ void k_debug(const DebugArgs A) {
         if (threadIdx.x == 0) A.norm[b] = r;
         return;
     }
-    stage_fill_pairs<T, false, false>(t, s, threadIdx.x, blockDim.x, 0);
+    stage_fill_pairs<T, 2, false>(t, s, threadIdx.x, blockDim.x, 0);
     __syncthreads();
     if (A.what == 1) {
         const T* dg = reinterpret_cast<const T*>(s.g_dg());
@@ -154,7 +154,7 @@ __global__ void k_debug(const DebugArgs A) {
         return;
     }
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, false, true, false, false, false>(t, s, t.level, ring);
+    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring);
 }
 
 }  // namespace sable

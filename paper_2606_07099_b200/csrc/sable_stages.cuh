@@ -10,8 +10,8 @@ namespace sable {
 // a1 (+ diagonal case of a2): S = V o conj(Ybus V), F1 rows (eq. 6), real form of
 // PAPER.md:201-207; writes rh = -F1 and the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated
 // P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
-template <typename T, bool kSmem>
-__device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kSmem>& s, const double* p_row,
+template <typename T, int kP>
+__device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kP>& s, const double* p_row,
                                                  const double* q_row, bool act) {
     // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
     // the evaluation (act = false) takes part in the shuffles and writes nothing
@@ -62,8 +62,8 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
 // theta_mj = theta_m - theta_j:  a = Vm_m Vm_j cos theta_mj,  b = Vm_m Vm_j sin theta_mj
 //   dP_m/dth_j = G b - B a     dP_m/dVm_j = (G a + B b)/Vm_j     dQ_m/dth_j = -(G a + B b)     dQ_m/dVm_j = (G b - B a)/Vm_j
 // evaluated in FP64 and rounded to T (Table I: value update DP, solver copy SP).  Fill pairs get zeros.
-template <typename T, bool kSmem>
-__device__ __forceinline__ void fill_pair(const Slot<T, kSmem>& s, int2 mj, double4 y, Blk<T>& U, Blk<T>& L) {
+template <typename T, int kP>
+__device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4 y, Blk<T>& U, Blk<T>& L) {
     const int m = mj.x & kIdxMask, j = mj.y & kIdxMask;
     const bool mpq = mj.x >> 30, jpq = mj.y >> 30;
     const double2 vm_ = s.vv(m), vj = s.vv(j);
@@ -78,12 +78,12 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kSmem>& s, int2 mj, doub
 // a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  kPrescale: the pairs owned by
 // level-0 nodes (p < leaf_p1; such a node has no earlier neighbour, so D_m = J(m,m) and its pairs have no terms) get
 // their final values here -- U(m,j) = J(m,j), L(j,m) = J(j,m) J(m,m)^-1 -- and the refactor skips them (kLeafDone).
-template <typename T, bool kSmem, bool kPrescale>
-__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub, int leaf_p1) {
+template <typename T, int kP, bool kPrescale>
+__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub, int leaf_p1) {
     for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
         const int2 mj = t.pair_mj[p];
-        fill_pair<T, kSmem>(s, mj, t.pair_y[p], U, L);
+        fill_pair<T, kP>(s, mj, t.pair_y[p], U, L);
         if (kPrescale && p < leaf_p1) L = mul(L, inv(s.ldD(mj.x & kIdxMask)));
         s.stU(p, U); s.stL(p, L);
     }
@@ -96,8 +96,8 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slo
 // kLeafDone: the pairs of level 0 already hold their final values (stage_fill_pairs<kPrescale>), level 0 then has
 // diagonal targets only and a single barrier.  A pair target without terms is not touched by the accumulate pass.
 // kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
-template <typename T, bool kSmem, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone>
-__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv, BlobRing& ring) {
+template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone>
+__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
     for (int l = 0; l < t.n_level; ++l) {
@@ -188,8 +188,8 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
 
 // backward half of a5: U x = y, i.e. x_m = D_m^-1 (y_m - sum_j U(m,j) x_j) over the pairs owned by m, levels
 // descending.  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
-template <typename T, bool kSmem, bool kTransposed>
-__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kSmem>& s, const LevelDesc* lv, BlobRing& ring) {
+template <typename T, int kP, bool kTransposed>
+__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
     for (int l = t.n_level - 1; l >= 0; --l) {
@@ -229,8 +229,8 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
 
 // Newton update of PAPER.md:90 for every node, accumulated in FP64; one wide pass (the sincos is kept
 // off the level-by-level critical path of the backward sweep).  No barrier.
-template <typename T, bool kSmem>
-__device__ __forceinline__ void stage_update(const DevTemplate& t, const Slot<T, kSmem>& s, int tsub, int nsub) {
+template <typename T, int kP>
+__device__ __forceinline__ void stage_update(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
     for (int m = tsub; m < t.n_node; m += nsub) {
         const double2 a = s.ma(m), x = s.rh(m);
         const double th = a.y + x.x;

@@ -387,8 +387,8 @@ def test_placements_and_group_layouts(env, monkeypatch):
         ctx = make_ctx(net, max_batch=256, keep_factors=keep)
         if "SABLE_G" in env:
             assert ctx.info["slots_per_cta"] == int(env["SABLE_G"])
-        if "SABLE_CUT" in env:
-            assert ctx.info["placement"] == 1
+        if "SABLE_CUT" in env:      # mixed placement below the last level, plain HBM placement beyond
+            assert ctx.info["placement"] == (1 if int(env["SABLE_CUT"]) < ctx.info["n_level"] else 2)
         res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
         check_solution(res, ref, c.tol, 1e-9)
         if keep:
