@@ -211,9 +211,9 @@ static sable_status choose_launch(sable_ctx* ctx) {
         if (ctx->opt.threads <= 0 && env_int("SABLE_THREADS", 0) <= 0) th = nn <= 1200 ? 128 : nn <= 4000 ? 256 : 512;
         want_ctas = env_int("SABLE_CTAS", std::max(1, 1024 / th));
         set_ring(r_env >= 0 ? ropts[0] : RingOpt{0, 0});
-        // slots per CTA (= scenarios whose HBM slices are interleaved): 4 / 2 / 1 by grid size, or SABLE_G
+        // slots per CTA (= scenarios whose HBM slices are interleaved): 4 for small grids, else 1 (measured), or SABLE_G
         int sg = 0;
-        const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : nn <= 4000 ? 2 : 1);
+        const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : 1);
         while ((2 << sg) <= g_want && (g_env > 0 || ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1))) ++sg;
         const int cl = cut_env >= 0 ? std::min(cut_env, nl) : nl;
         const int nc = cl < nl ? T.level_ptr[cl] : nn;
