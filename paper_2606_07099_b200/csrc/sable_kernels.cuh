@@ -119,13 +119,9 @@ __device__ __forceinline__ int pop_group(const SolveArgs& A) {
 // group * G + g, whose HBM slices are interleaved with the rest of its group) and advances its slots in lockstep; a slot
 // that has finished stops being evaluated (its lanes run along and write nothing that is read) until the group is done.
 // Register budgets (measured, profiles/r01_v2_sweeps.md): on chip 1 CTA of up to 512 threads (up to 128 registers); HBM
-// placement 2 x 512 threads (64 registers) or, kSmall, 7 x 128 threads (72 registers: the FP64 build then spills
-// 110 B instead of 190 B and cfg 3 runs 6 % faster).
-#ifndef SABLE_SMALL_B32
-#define SABLE_SMALL_B32 7
-#endif
+// placement 2 x 512 threads (64 registers) or, kSmall, 7 x 128 threads (72 registers, no spills).
 template <typename T, int kP, bool kSmall>
-__global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? (sizeof(T) == 4 ? SABLE_SMALL_B32 : 7) : 2)) k_nr_fused(const SolveArgs A) {
+__global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 : 2)) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
