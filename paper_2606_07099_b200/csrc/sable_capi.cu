@@ -313,7 +313,7 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     {
         std::vector<LevelDesc> lf = build_levels(T, c->lv_host, c->threads, c->gsh, c->first_staged);
         std::vector<LevelDesc> l1 = build_levels(T, c->lv_host, c->threads1, 0, T.n_level);
-        c->threads_lin = env_int("SABLE_THREADS_LIN", std::min(512, std::max(c->threads1 << c->gsh, 32)));
+        c->threads_lin = env_int("SABLE_THREADS_LIN", std::min(512, std::max(32 << c->gsh, 64)));   // 32 targets in flight per slot (measured)
         std::vector<LevelDesc> ll = build_levels(T, c->lv_host, c->threads_lin, c->gsh, T.n_level);
         up(lf, &c->level_fused); up(l1, &c->level_one); up(ll, &c->level_lin); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
