@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
         ring.tick(4 * t.n_level + 2, tk);                  // group bookkeeping + init
         {
             const size_t row = (size_t)(b >= 0 ? b : 0) * t.n_bus;
-            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0);
+            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0, lv[0].m1);
             const double r = slot_max_nan(loc, red, gsh);
             ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
             if (b >= 0) {

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     const int b = blockIdx.x;
     if (A.status[b] != 0) return;                                   // masked: no loads, no stores
     const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    const double r = slot_max_nan(stage_mismatch<T, 2>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true, A.t.level[0].m1), red, 0);
     const int it = A.it[b];
     int st = 0;
     if (r <= A.tol) st = 1;
@@ -133,7 +133,7 @@ __global__ void k_debug(const DebugArgs A) {
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];

@@ -12,7 +12,9 @@ namespace sable {
 // P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
 template <typename T, int kP>
 __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kP>& s, const double* p_row,
-                                                 const double* q_row, bool act) {
+                                                 const double* q_row, bool act, int leaf_m1) {
+    // leaf_m1: nodes m < leaf_m1 (level 0: no earlier neighbour, so D_m = J(m,m) and y_m = rhs_m) get their pivot inverse
+    // stored right here -- with stage_fill_pairs<kPrescale> and kLeafDone the refactor has nothing left to do at level 0
     // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
     // the evaluation (act = false) takes part in the shuffles and writes nothing
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
@@ -51,7 +53,7 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
                 d.a = T(-Q - yd.y * v2);
                 if (pq) { d.b = T(P * iv + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q * iv - yd.y * vm); }
                 else    { d.b = T(0); d.c = T(0); d.d = T(1); }
-                s.stD(m, d);
+                s.stD(m, m < leaf_m1 ? inv(d) : d);
             }
         }
     }
@@ -77,14 +79,15 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4
 
 // a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  kPrescale: the pairs owned by
 // level-0 nodes (p < leaf_p1; such a node has no earlier neighbour, so D_m = J(m,m) and its pairs have no terms) get
-// their final values here -- U(m,j) = J(m,j), L(j,m) = J(j,m) J(m,m)^-1 -- and the refactor skips them (kLeafDone).
+// their final values here -- U(m,j) = J(m,j), L(j,m) = J(j,m) J(m,m)^-1 (the inverse comes from stage_mismatch) -- and
+// the refactor skips level 0 altogether (kLeafDone).
 template <typename T, int kP, bool kPrescale>
 __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub, int leaf_p1) {
     for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
         const int2 mj = t.pair_mj[p];
         fill_pair<T, kP>(s, mj, t.pair_y[p], U, L);
-        if (kPrescale && p < leaf_p1) L = mul(L, inv(s.ldD(mj.x & kIdxMask)));
+        if (kPrescale && p < leaf_p1) L = mul(L, s.ldD(mj.x & kIdxMask));       // D^-1 left there by stage_mismatch
         s.stU(p, U); s.stL(p, L);
     }
 }
@@ -108,7 +111,7 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
         const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
         const int2* tab = reinterpret_cast<const int2*>(lb + d.o_tab);
-        {
+        if (!(kLeafDone && l == 0)) {
             const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
             const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
             for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
@@ -180,6 +183,7 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
                 s.stL(p, mul(s.ldL(p), s.ldD(pmj[i].x & kIdxMask)));
             }
         }
+        if (kLeafDone && l == 0 && !ring.on) continue;   // nothing was done at level 0: no barrier needed
         __syncthreads();
         ring.tick(4 * l + 1, tk);
         ring.release(l);
