@@ -36,7 +36,7 @@ WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward"
             5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
 # captures (profiles/r01_v4_README.md); None where no capture exists
-NCU_TRAFFIC = {2: 2.998016e6, 3: 3.696919e9 + 3.666356e9, 4: 2.279826e9 + 3.435172e9, 5: 8.564032e9 + 4.487271e9}
+NCU_TRAFFIC = {2: 2.991616e6, 3: 3.284000e9 + 3.239069e9, 4: 2.073546e9 + 3.073361e9, 5: 8.367077e9 + 4.186991e9}
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 

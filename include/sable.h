@@ -118,6 +118,17 @@ sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double* p_spec, co
 sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm,
                            double* lam_p, double* lam_q, void* cuda_stream);
 
+/* Step-2 explicit recovery (PAPER.md:80 eq. 5, :95-99 eq. 9: with dF2/dz2 = I the block z2 = [p_g at the slack; q_g at
+ * PV and slack buses] is read off the mismatch rows that Step 1 does not use).  Returns the calculated net injections
+ * P_i(V), Q_i(V) of S = V o conj(Y_bus V) for EVERY bus at the given voltages (normally the vm, va of sable_solve):
+ * p_inj at the slack is the recovered slack injection, q_inj at PV / slack buses the recovered reactive injections
+ * (generation = injection + load); at the other rows they equal the specified values up to the final
+ * mismatch.  All DEVICE pointers, [batch][n_bus]; asynchronous on the stream; uses the workspace only for grids above
+ * 10 240 buses (then it overwrites the state of the last solve, not the kept factors).
+ * Errors: INVALID_ARG, STATE, CUDA. */
+sable_status sable_recover(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* p_inj,
+                           double* q_inj, void* cuda_stream);
+
 /* Host-buffer convenience wrappers: same semantics with HOST pointers; they copy in, run on the context's
  * device and copy out (synchronous).  Used for the end-to-end measurement. */
 sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,

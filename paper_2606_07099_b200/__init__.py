@@ -46,7 +46,7 @@ class Info(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_solve_host", "sable_adjoint_host",
+EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
            "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing"]
 
@@ -161,6 +161,15 @@ class Context:
             out = (torch.empty_like(g_va), torch.empty_like(g_vm))
         self._check(lib().sable_adjoint(self._h, C.c_int32(batch), _dp(g_va), _dp(g_vm), _dp(out[0]), _dp(out[1]),
                                         _stream()))
+        return out
+
+    def recover(self, vm, va, out=None):
+        """sable_recover (Step-2 explicit recovery).  Returns (p_inj, q_inj): calculated net injections at every bus."""
+        import torch
+        batch = int(vm.shape[0])
+        if out is None:
+            out = (torch.empty_like(vm), torch.empty_like(vm))
+        self._check(lib().sable_recover(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(out[0]), _dp(out[1]), _stream()))
         return out
 
     # -- host-buffer calls (numpy) ----------------------------------------------------------------------

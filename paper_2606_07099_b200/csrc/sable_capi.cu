@@ -19,6 +19,7 @@ struct sable_ctx {
     std::vector<void*> dev_allocs;
     char* factors = nullptr;  char* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
     double* zeros = nullptr;
+    const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
     unsigned long long* tim = nullptr;                       // SABLE_TIMING=1: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
     // launch plan of the fused kernel (choose_launch) and of the one-scenario-per-CTA kernels
@@ -303,6 +304,11 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     }
     bool ok = true;
     auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
+{
+        std::vector<double2> fgb(T.fcol.size());
+        for (size_t k = 0; k < fgb.size(); ++k) fgb[k] = make_double2(T.fg[k], T.fb[k]);
+        up(T.fptr, &c->fptr); up(T.fcol, &c->fcol); up(fgb, &c->fgb);
+    }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
     up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(pmj, &d.pair_mj); up(py, &d.pair_y);
     if (!ok) return bail(SABLE_ERR_ALLOC);
@@ -445,6 +451,28 @@ extern "C" sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const doubl
     if (batch == 0) return SABLE_OK;
     CU(cudaSetDevice(ctx->opt.device));
     return launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, (cudaStream_t)cuda_stream);
+}
+
+// ---- Step-2 explicit recovery ---------------------------------------------------------------------------------------
+extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* p_inj,
+                                      double* q_inj, void* cuda_stream) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
+    if (batch == 0) return SABLE_OK;
+    if (!vm || !va || !p_inj || !q_inj) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    CU(cudaSetDevice(ctx->opt.device));
+    RecoverArgs R{};
+    R.n_bus = ctx->T.n_bus; R.batch = batch; R.fptr = ctx->fptr; R.fcol = ctx->fcol; R.fgb = ctx->fgb;
+    R.vm = vm; R.va = va; R.p_inj = p_inj; R.q_inj = q_inj; R.work = ctx->work; R.work_stride = ctx->work_stride;
+    const size_t sm = (size_t)ctx->T.n_bus * 16;
+    R.v_in_smem = sm <= 160 * 1024;            // else the scenario's workspace slice (>= 3 (n_bus) 16 bytes) holds V
+    if (R.v_in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_recover, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    k_recover<<<batch, th, R.v_in_smem ? sm : 0, (cudaStream_t)cuda_stream>>>(R);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    return SABLE_OK;
 }
 
 // ---- host-buffer wrappers (end-to-end path: H2D, solve, D2H; synchronous) ------------------------------------------

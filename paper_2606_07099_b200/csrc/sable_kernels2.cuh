@@ -108,6 +108,45 @@ __global__ void k_linsolve(const LinArgs A) {
         }
 }
 
+// ---- Step-2 explicit recovery (PAPER.md:80 eq. 5, :95-99 eq. 9): with dF2/dz2 = I the block z2 = [p_g at the slack;
+// q_g at PV and slack buses] is read off the calculated injections S = V o conj(Y_bus V) at the solved voltages.
+// The kernel returns P_i(V), Q_i(V) for EVERY bus (net injection = generation - load); the caller picks
+// the slack / PV rows.  One CTA per scenario: V in rectangular form goes to shared memory (or to the scenario's
+// workspace slice when the grid is too large), then one row of Y_bus per thread.
+struct RecoverArgs {
+    int32_t n_bus, batch, v_in_smem;
+    const int32_t *fptr, *fcol;
+    const double2* fgb;                // (G, B) per stored entry, bus order
+    const double *vm, *va;             // [batch][n_bus]
+    double *p_inj, *q_inj;             // [batch][n_bus]
+    char* work; int64_t work_stride;   // used when V does not fit shared memory
+};
+
+__global__ void k_recover(const RecoverArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int b = blockIdx.x;
+    const size_t o = (size_t)b * A.n_bus;
+    double2* v = A.v_in_smem ? reinterpret_cast<double2*>(smem) : reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
+    for (int i = threadIdx.x; i < A.n_bus; i += blockDim.x) {
+        double sn, cs; sincos(A.va[o + i], &sn, &cs);
+        const double m = A.vm[o + i];
+        v[i] = make_double2(m * cs, m * sn);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < A.n_bus; i += blockDim.x) {
+        double ire = 0.0, iim = 0.0;
+        const int k1 = A.fptr[i + 1];
+        for (int k = A.fptr[i]; k < k1; ++k) {
+            const double2 y = A.fgb[k], x = v[A.fcol[k]];
+            ire += y.x * x.x - y.y * x.y;
+            iim += y.y * x.x + y.x * x.y;
+        }
+        const double2 vi = v[i];
+        A.p_inj[o + i] = vi.x * ire + vi.y * iim;
+        A.q_inj[o + i] = vi.y * ire - vi.x * iim;
+    }
+}
+
 // ---- debug: state from caller's (vm, va), mismatch / Jacobian / refactor at that state ---------------------------
 struct DebugArgs {
     DevTemplate t;

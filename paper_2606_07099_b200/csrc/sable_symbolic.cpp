@@ -71,6 +71,11 @@ int build_template(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx
     }
     T.nnz_y = 0;
     for (int i = 0; i < n_bus; ++i) T.nnz_y += (int64_t)rows[i].size();
+    T.fptr.assign(n_bus + 1, 0); T.fcol.clear(); T.fg.clear(); T.fb.clear();
+    for (int i = 0; i < n_bus; ++i) {
+        for (const YEntry& e : rows[i]) { T.fcol.push_back(e.c); T.fg.push_back(e.g); T.fb.push_back(e.b); }
+        T.fptr[i + 1] = (int32_t)T.fcol.size();
+    }
 
     // ---- 2. every bus must reach the slack (otherwise J1 is structurally singular) ---------------------------
     {

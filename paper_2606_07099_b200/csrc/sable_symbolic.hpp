@@ -29,6 +29,10 @@ struct Template {
     std::vector<double>  yg, yb;
     std::vector<int32_t> ydiag;         // [n_node] slot of Y(m,m)
 
+    // canonical Y_bus of ALL buses in bus order (Step-2 recovery of the slack / PV injections)
+    std::vector<int32_t> fptr, fcol;    // [n_bus+1], [nnz_y]
+    std::vector<double>  fg, fb;
+
     // filled block pattern: pair p owned by node m couples m with a later node j:  {U(m,j), L(j,m)}
     std::vector<int32_t> pair_ptr;      // [n_node+1]
     std::vector<int32_t> pair_row;      // [n_pair] m

@@ -400,3 +400,38 @@ def test_placements_and_group_layouts(env, monkeypatch):
             assert (np.abs(lp - rp).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
             assert (np.abs(lq - rq).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
         ctx.close()
+
+
+# ---- NEXT row 1: Step-2 explicit recovery ---------------------------------------------------------
+@pytest.mark.parametrize("cfg,batch", [(1, 64), (2, 50), (3, 17), (5, 3)])
+def test_step2_recovery(cfg, batch):
+    """sable_recover returns S = V o conj(Ybus V) at every bus: checked against the oracle's injections (pinned by the
+    complex form and by power balance in tests/test_oracle_pins.py), against the specified injections at the rows
+    Step 1 solved, and by power balance (sum of injections = sum of branch losses, an identity for any V)."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, keep_factors=False)
+    res = ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it)
+    p_inj, q_inj = ctx.recover(res["vm"], res["va"])
+    vm, va = res["vm"].cpu().numpy(), res["va"].cpu().numpy()
+    p_inj, q_inj = p_inj.cpu().numpy(), q_inj.cpu().numpy()
+    conv = res["converged"].cpu().numpy() == 1
+    assert conv.all()
+    sc = row_scale(Y, vm)
+    for b in range(batch):
+        P, Q = oracle.injections(Y, vm[b], va[b])
+        assert (np.abs(p_inj[b] - P) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+        assert (np.abs(q_inj[b] - Q) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+    nonslack = net.bus_type != S.SLACK
+    pq = net.bus_type == S.PQ
+    assert np.abs(p_inj[:, nonslack] - ps[:, nonslack]).max() <= c.tol * (1 + 1e-6)
+    assert np.abs(q_inj[:, pq] - qs[:, pq]).max() <= c.tol * (1 + 1e-6)
+    # power balance against the branch list (independent of Y_bus): S_ft + S_tf per branch
+    V = vm * np.exp(1j * va)
+    y = 1.0 / (net.r + 1j * net.x)
+    Vf, Vt = V[:, net.f], V[:, net.t]
+    loss = (Vf * np.conj((y + 0.5j * net.b) * Vf - y * Vt) + Vt * np.conj((y + 0.5j * net.b) * Vt - y * Vf)).sum(axis=1)
+    tot = (p_inj + 1j * q_inj).sum(axis=1)
+    assert np.abs(tot - loss).max() <= 1e-10 * max(1.0, sc.max())
+    ctx.close()
