@@ -185,3 +185,61 @@ def adjoint_batch(Y, bus_type, vm, va, g_va, g_vm, method=1, mixed=False, n_thre
                                       _p(va, C.c_double), _p(g_va, C.c_double), _p(g_vm, C.c_double), int(method),
                                       int(bool(mixed)), int(n_threads), _p(lp, C.c_double), _p(lq, C.c_double))
     return lp, lq, used
+
+
+# ---- NEXT row 2: implicit-layer backward (eqs. 10-16) -----------------------------------------------
+def full_jacobians(Y, vm, va):
+    """Dense dS/dtheta and dS/dVm of S = V o conj(Ybus V) for ALL buses (complex n_bus x n_bus), by the complex-matrix
+    identities  dS/dtheta = j diag(V) conj(diag(I) - Y diag(V)),  dS/dVm = diag(V) conj(Y diag(V/|V|)) + conj(diag(I)) diag(V/|V|).
+    The base Jacobian of eq. (2) is made of their real / imaginary parts."""
+    row_ptr, col, g, bb = Y
+    nb = vm.shape[0]
+    Yd = np.zeros((nb, nb), dtype=complex)
+    for i in range(nb):
+        sl = slice(row_ptr[i], row_ptr[i + 1])
+        np.add.at(Yd[i], col[sl], g[sl] + 1j * bb[sl])
+    V = vm * np.exp(1j * va)
+    I = Yd @ V
+    E = V / np.abs(V)
+    dS_dth = 1j * np.diag(V) @ np.conj(np.diag(I) - Yd @ np.diag(V))
+    dS_dvm = np.diag(V) @ np.conj(Yd @ np.diag(E)) + np.conj(np.diag(I)) @ np.diag(E)
+    return dS_dth, dS_dvm
+
+
+def layer_backward(Y, bus_type, vm, va, gl_pg, gl_qg, gl_vm, gl_va):
+    """dL/dx of the embedded PF layer for ONE scenario at the converged (vm, va), following PAPER.md eqs. (10)-(16).
+
+    Layer: input x = [p_g at PV buses; Vm at PV and slack buses] (eq. 3); Step 1 solves F1 = 0 for
+    z1 = [Vm at PQ; theta at non-slack] (eq. 4, 6); Step 2 reads z2 = [p_g at the slack; q_g at PV and slack] off the
+    unused rows (eq. 5, 9): p_g = P(V) + p_d, q_g = Q(V) + q_d.  Given the partials of a scalar loss w.r.t. the output
+    buffer y -- gl_pg (used at PV and slack), gl_qg (PV and slack), gl_vm (all buses), gl_va (non-slack) -- returns
+    (dx_pg [n_bus], nonzero at PV; dx_vm [n_bus], nonzero at PV and slack).
+
+    Sign convention of this repository: F = S_calc - S_spec, so dz2/dv = +d(S_calc rows)/dv and dF1/dp_g = -1; the
+    paper writes F = spec - calc, which flips the sign of lambda and of J2, J3 but not of dL/dx."""
+    bus_type = np.asarray(bus_type)
+    nb = vm.shape[0]
+    pq = bus_type == 0
+    pv = bus_type == 1
+    sl = bus_type == 2
+    nonslack = ~sl
+    gen = pv | sl                                   # B \\ D
+    dS_dth, dS_dvm = full_jacobians(Y, vm, va)
+    dP_dth, dQ_dth, dP_dvm, dQ_dvm = dS_dth.real, dS_dth.imag, dS_dvm.real, dS_dvm.imag
+    # eq. (11)-(12): Step-2 contribution on the voltage coordinates, v2 = (dz2/dv)^T dL/dz2
+    v2_th = dP_dth[sl].T @ gl_pg[sl] + dQ_dth[gen].T @ gl_qg[gen]
+    v2_vm = dP_dvm[sl].T @ gl_pg[sl] + dQ_dvm[gen].T @ gl_qg[gen]
+    # eq. (13)
+    g_th = np.where(nonslack, gl_va + v2_th, 0.0)
+    g_vm = gl_vm + v2_vm
+    # eq. (14): J1^T lambda = g_z1, unknown / equation order [theta non-slack; Vm PQ] / [P non-slack; Q PQ]
+    ns, pqi = np.flatnonzero(nonslack), np.flatnonzero(pq)
+    J1 = np.block([[dP_dth[np.ix_(ns, ns)], dP_dvm[np.ix_(ns, pqi)]], [dQ_dth[np.ix_(pqi, ns)], dQ_dvm[np.ix_(pqi, pqi)]]])
+    lam = np.linalg.solve(J1.T, np.concatenate([g_th[ns], g_vm[pqi]]))
+    lam_p = np.zeros(nb); lam_q = np.zeros(nb)
+    lam_p[ns] = lam[: len(ns)]; lam_q[pqi] = lam[len(ns):]
+    # eq. (15)-(16): dF1/dp_g,PV = -I on the P rows of PV buses; J3 = dF1/dVm at PV and slack buses
+    dx_pg = np.where(pv, gl_pg + lam_p, 0.0)
+    J3T_lam = dP_dvm[ns].T @ lam_p[ns] + dQ_dvm[pqi].T @ lam_q[pqi]
+    dx_vm = np.where(gen, g_vm - J3T_lam, 0.0)
+    return dx_pg, dx_vm
