@@ -129,6 +129,23 @@ sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const double* g_va, co
 sable_status sable_recover(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* p_inj,
                            double* q_inj, void* cuda_stream);
 
+/* Implicit-layer backward (eqs. 10-16): total derivative dL/dx of a scalar loss w.r.t. the layer input
+ * x = [p_g at PV buses; Vm at PV and slack buses] (eq. 3), given the partials of L w.r.t. the completed buffer
+ * y = [p_g, q_g at PV and slack buses; Vm; theta] (eq. 1) at the solution of the last sable_solve (keep_factors = 1):
+ * one transposed SpMV with J2 (eq. 12), the adjoint solve of eq. 14 on the kept factors, one transposed SpMV with J3 and
+ * the selector term (eq. 16).  With this library's sign F = S_calc - S_spec:  dL/dp_g,k = dL/dp_g,k|direct + lambda_P,k.
+ *   vm, va                the vm, va returned by that sable_solve
+ *   gl_pg, gl_qg          dL/dp_g,i and dL/dq_g,i: read at PV and slack buses (gl_pg at a PV bus is the direct partial
+ *                         w.r.t. the input itself; at the slack it multiplies the recovered slack injection)
+ *   gl_vm, gl_va          dL/dVm_i (all buses), dL/dtheta_i (slack entry ignored)
+ *   dx_pg, dx_vm          out: dL/dp_g (nonzero at PV buses), dL/dVm (nonzero at PV and slack buses)
+ * All DEVICE pointers, [batch][n_bus]; batch must equal the batch of the last solve; asynchronous on the stream; for
+ * grids above 5 120 buses the state part of the workspace is used as scratch (the kept factors stay intact).
+ * Errors: INVALID_ARG, STATE, CUDA. */
+sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                  const double* gl_pg, const double* gl_qg, const double* gl_vm, const double* gl_va,
+                                  double* dx_pg, double* dx_vm, void* cuda_stream);
+
 /* Host-buffer convenience wrappers: same semantics with HOST pointers; they copy in, run on the context's
  * device and copy out (synchronous).  Used for the end-to-end measurement. */
 sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,

@@ -8,7 +8,8 @@ follows); this file only compiles it with gcc and marshals numpy arrays through 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): 2-bus closed form, hand-derived 3-bus example
 (tests/golden/), Jacobian vs central finite differences and vs the complex-matrix identities,
 power balance vs branch losses, adjoint vs finite-difference sensitivities, dense vs sparse vs scipy
-solves, permutation / batch-composition invariance.  No function of this oracle is "parity unpinned".
+solves, permutation / batch-composition invariance; the implicit-layer backward (numpy, below) is pinned by finite
+differences of the whole layer (tests/test_oracle_layer.py).  No function of this oracle is "parity unpinned".
 """
 from __future__ import annotations
 

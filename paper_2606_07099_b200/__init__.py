@@ -46,7 +46,7 @@ class Info(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_solve_host", "sable_adjoint_host",
+EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_layer_backward", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
            "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing"]
 
@@ -170,6 +170,16 @@ class Context:
         if out is None:
             out = (torch.empty_like(vm), torch.empty_like(vm))
         self._check(lib().sable_recover(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(out[0]), _dp(out[1]), _stream()))
+        return out
+
+    def layer_backward(self, vm, va, gl_pg, gl_qg, gl_vm, gl_va, out=None):
+        """sable_layer_backward (eqs. 10-16).  Returns (dx_pg, dx_vm)."""
+        import torch
+        batch = int(vm.shape[0])
+        if out is None:
+            out = (torch.empty_like(vm), torch.empty_like(vm))
+        self._check(lib().sable_layer_backward(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(gl_pg), _dp(gl_qg),
+                                               _dp(gl_vm), _dp(gl_va), _dp(out[0]), _dp(out[1]), _stream()))
         return out
 
     # -- host-buffer calls (numpy) ----------------------------------------------------------------------

@@ -20,6 +20,7 @@ struct sable_ctx {
     char* factors = nullptr;  char* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
     double* zeros = nullptr;
     const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
+    const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward
     unsigned long long* tim = nullptr;                       // SABLE_TIMING=1: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
     // launch plan of the fused kernel (choose_launch) and of the one-scenario-per-CTA kernels
@@ -308,6 +309,15 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         std::vector<double2> fgb(T.fcol.size());
         for (size_t k = 0; k < fgb.size(); ++k) fgb[k] = make_double2(T.fg[k], T.fb[k]);
         up(T.fptr, &c->fptr); up(T.fcol, &c->fcol); up(fgb, &c->fgb);
+        std::vector<int32_t> tpos(T.fcol.size());
+        for (int i = 0; i < T.n_bus; ++i)
+            for (int k = T.fptr[i]; k < T.fptr[i + 1]; ++k) {
+                const int j = T.fcol[k];
+                auto bj = T.fcol.begin() + T.fptr[j], ej = T.fcol.begin() + T.fptr[j + 1];
+                tpos[k] = (int32_t)(std::lower_bound(bj, ej, i) - T.fcol.begin());   // the pattern is symmetric (canonicalised)
+            }
+        std::vector<uint8_t> bt(bus_type, bus_type + n_bus);
+        up(tpos, &c->ftpos); up(bt, &c->d_bus_type);
     }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
     up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(pmj, &d.pair_mj); up(py, &d.pair_y);
@@ -336,7 +346,8 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     const size_t G = (size_t)1 << c->gsh, mb_alloc = (mb + G - 1) / G * G + G;
     if (!dmalloc((void**)&c->factors, mb_alloc * c->fac_stride) || !dmalloc((void**)&c->work, mb_alloc * c->work_stride) ||
         !dmalloc((void**)&c->ints, (2 * mb + 4) * 4) || !dmalloc((void**)&c->hbuf, 9 * mb * nb * 8 + mb * 8) ||
-        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb) || !dmalloc((void**)&c->zeros, nb * 8))
+        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb) || !dmalloc((void**)&c->zeros, nb * 8) ||
+        !dmalloc((void**)&c->lbuf, 4 * mb * nb * 8))
         return bail(SABLE_ERR_ALLOC);
     if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work, 0, mb_alloc * c->work_stride) != cudaSuccess ||
         cudaMemset(c->factors, 0, mb_alloc * c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
@@ -471,6 +482,40 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
     k_recover<<<batch, th, R.v_in_smem ? sm : 0, (cudaStream_t)cuda_stream>>>(R);
     ctx->launches += 1;
+    CU(cudaGetLastError());
+    return SABLE_OK;
+}
+
+// ---- implicit-layer backward ----------------------------------------------------------------------------------------
+extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                             const double* gl_pg, const double* gl_qg, const double* gl_vm, const double* gl_va,
+                                             double* dx_pg, double* dx_vm, void* cuda_stream) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (!ctx->have_factors) return fail(ctx, SABLE_ERR_STATE, "no kept factors: call sable_solve with keep_factors = 1 first");
+    if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
+    if (!vm || !va || !gl_pg || !gl_qg || !gl_vm || !gl_va || !dx_pg || !dx_vm) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    if (batch == 0) return SABLE_OK;
+    CU(cudaSetDevice(ctx->opt.device));
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus;
+    LayerArgs L{};
+    L.n_bus = ctx->T.n_bus; L.batch = batch; L.fptr = ctx->fptr; L.fcol = ctx->fcol; L.ftpos = ctx->ftpos; L.fgb = ctx->fgb;
+    L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_pg = gl_pg; L.gl_qg = gl_qg; L.gl_vm = gl_vm; L.gl_va = gl_va;
+    L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.lam_p = ctx->lbuf + 2 * n; L.lam_q = ctx->lbuf + 3 * n;
+    L.dx_pg = dx_pg; L.dx_vm = dx_vm; L.work = ctx->work; L.work_stride = ctx->work_stride;
+    const size_t sm = (size_t)ctx->T.n_bus * 32;
+    L.in_smem = sm <= 160 * 1024;          // else the scenario's workspace slice (48 n_bus bytes) holds V and (P, Q)
+    if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    L.post = 0;
+    k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
+    CU(cudaGetLastError());
+    sable_status st = launch_lin(ctx, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, s);
+    if (st != SABLE_OK) return st;
+    L.post = 1;
+    k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
+    ctx->launches += 2;
     CU(cudaGetLastError());
     return SABLE_OK;
 }

@@ -147,6 +147,95 @@ __global__ void k_recover(const RecoverArgs A) {
     }
 }
 
+// ---- implicit-layer backward (eqs. 10-16) around the adjoint solve ---------------------------------
+// Layer: x = [p_g at PV; Vm at PV and slack] -> y = [p_g, q_g at PV and slack; Vm; theta] through Step 1 (F1 = 0) and
+// Step 2 (recovery).  With F = S_calc - S_spec (this repository's sign):
+//   pre : g_theta_j = dL/dtheta_j + sum_i [a_i dP_i/dtheta_j + c_i dQ_i/dtheta_j],  g_Vm_j likewise            (eq. 11-13)
+//         with a_i = dL/dp_g,i at the slack, c_i = dL/dq_g,i at PV and slack buses (the rows of z2, eq. 5)
+//   solve J1^T lambda = [g_theta (non-slack); g_Vm (PQ)]                                                        (eq. 14)
+//   post: dL/dp_g,k = dL/dp_g,k + lambda_P,k (PV);  dL/dVm_k = g_Vm_k - sum_i [lambda_P,i dP_i/dVm_k + lambda_Q,i dQ_i/dVm_k]  (eq. 15-16)
+// Jacobian entries are evaluated on the fly from Y_bus and V with the Alg. 1 formulas (the rows / columns needed here are
+// not part of J1).  One CTA per scenario; V and (P, Q) per bus in shared memory, or in the scenario's workspace slice.
+struct LayerArgs {
+    int32_t n_bus, batch, in_smem, post;
+    const int32_t *fptr, *fcol, *ftpos;      // full Y_bus CSR (bus order) and the position of each entry's transpose
+    const double2* fgb;
+    const uint8_t* bus_type;
+    const double *vm, *va;                   // [batch][n_bus] solved state
+    const double *gl_pg, *gl_qg, *gl_vm, *gl_va;   // loss partials w.r.t. the output buffer y
+    double *g_va, *g_vm;                     // pre: out (right-hand side of eq. 14 and the Vm part of g_x); post: in
+    const double *lam_p, *lam_q;             // post: in
+    double *dx_pg, *dx_vm;                   // post: out
+    char* work; int64_t work_stride;
+};
+
+__device__ __forceinline__ void jac_entry(double2 y, double2 vi, double2 vj, double vmj, double& dP_dth, double& dP_dvm,
+                                          double& dQ_dth, double& dQ_dvm) {   // off-diagonal, theta_ij = theta_i - theta_j
+    const double a = vi.x * vj.x + vi.y * vj.y, b = vi.y * vj.x - vi.x * vj.y;
+    const double u1 = y.x * b - y.y * a, u2 = y.x * a + y.y * b, iv = 1.0 / vmj;
+    dP_dth = u1; dP_dvm = u2 * iv; dQ_dth = -u2; dQ_dvm = u1 * iv;
+}
+
+__global__ void k_layer(const LayerArgs A) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int b = blockIdx.x, nb = A.n_bus;
+    const size_t o = (size_t)b * nb;
+    double2* v = A.in_smem ? reinterpret_cast<double2*>(smem) : reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
+    double2* pq = v + nb;
+    const double* vm = A.vm + o;
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) {
+        double sn, cs; sincos(A.va[o + i], &sn, &cs);
+        v[i] = make_double2(vm[i] * cs, vm[i] * sn);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) {
+        double ire = 0.0, iim = 0.0;
+        for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
+            const double2 y = A.fgb[k], x = v[A.fcol[k]];
+            ire += y.x * x.x - y.y * x.y;  iim += y.y * x.x + y.x * x.y;
+        }
+        pq[i] = make_double2(v[i].x * ire + v[i].y * iim, v[i].y * ire - v[i].x * iim);
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < nb; j += blockDim.x) {
+        const int tj = A.bus_type[j];
+        const double vmj = vm[j];
+        if (!A.post) {
+            double vth = 0.0, vvm = 0.0;
+            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+                const int i = A.fcol[k], ti = A.bus_type[i];
+                const double ai = ti == 2 ? A.gl_pg[o + i] : 0.0, ci = ti != 0 ? A.gl_qg[o + i] : 0.0;
+                if (ti == 0) continue;                                   // rows of z2 sit at PV and slack buses only
+                double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+                if (i == j) {
+                    const double2 y = A.fgb[k], s = pq[i];
+                    dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
+                    dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
+                } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+                vth += ai * dP_dth + ci * dQ_dth;
+                vvm += ai * dP_dvm + ci * dQ_dvm;
+            }
+            A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + vth : 0.0;
+            A.g_vm[o + j] = A.gl_vm[o + j] + vvm;
+        } else {
+            double sacc = 0.0;
+            if (tj != 0)
+                for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+                    const int i = A.fcol[k], ti = A.bus_type[i];
+                    const double lp = ti != 2 ? A.lam_p[o + i] : 0.0, lq = ti == 0 ? A.lam_q[o + i] : 0.0;
+                    double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+                    if (i == j) {
+                        const double2 y = A.fgb[k], s = pq[i];
+                        dP_dvm = s.x / vmj + y.x * vmj;  dQ_dvm = s.y / vmj - y.y * vmj;
+                    } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+                    sacc += lp * dP_dvm + lq * dQ_dvm;
+                }
+            A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - sacc : 0.0;
+            A.dx_pg[o + j] = tj == 1 ? A.gl_pg[o + j] + A.lam_p[o + j] : 0.0;
+        }
+    }
+}
+
 // ---- debug: state from caller's (vm, va), mismatch / Jacobian / refactor at that state ---------------------------
 struct DebugArgs {
     DevTemplate t;

@@ -435,3 +435,34 @@ def test_step2_recovery(cfg, batch):
     tot = (p_inj + 1j * q_inj).sum(axis=1)
     assert np.abs(tot - loss).max() <= 1e-10 * max(1.0, sc.max())
     ctx.close()
+
+
+# ---- NEXT row 2: implicit-layer backward (eqs. 10-16) ------------------------------------------------------------
+@pytest.mark.parametrize("cfg,batch", [(1, 16), (2, 12), (3, 6)])
+def test_layer_backward(cfg, batch):
+    """dL/dx of the embedded PF layer against the oracle (pinned by finite differences of the whole layer in
+    tests/test_oracle_layer.py), evaluated at the GPU's returned state."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    rng = np.random.Generator(np.random.PCG64(31 + cfg))
+    gl = [rng.standard_normal((batch, net.n_bus)) for _ in range(4)]       # dL/dp_g, dL/dq_g, dL/dVm, dL/dtheta
+    ctx = make_ctx(net, max_batch=batch, keep_factors=True)
+    res = ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it)
+    dx_pg, dx_vm = ctx.layer_backward(res["vm"], res["va"], *[dev(a) for a in gl])
+    vm, va = res["vm"].cpu().numpy(), res["va"].cpu().numpy()
+    dx_pg, dx_vm = dx_pg.cpu().numpy(), dx_vm.cpu().numpy()
+    assert (res["converged"].cpu().numpy() == 1).all()
+    pv = net.bus_type == S.PV
+    gen = net.bus_type != S.PQ
+    for b in range(batch):
+        rp, rv = oracle.layer_backward(Y, net.bus_type, vm[b], va[b], gl[0][b], gl[1][b], gl[2][b], gl[3][b])
+        sc = max(1.0, np.abs(rp).max(), np.abs(rv).max())
+        assert np.abs(dx_pg[b] - rp).max() <= 1e-8 * sc, (b, np.abs(dx_pg[b] - rp).max())
+        assert np.abs(dx_vm[b] - rv).max() <= 1e-8 * sc, (b, np.abs(dx_vm[b] - rv).max())
+        assert (dx_pg[b][~pv] == 0).all() and (dx_vm[b][~gen] == 0).all()
+    # needs kept factors of a solve of the same batch
+    with pytest.raises(sb.SableError) as e:
+        ctx.layer_backward(res["vm"][:2], res["va"][:2], *[dev(a[:2]) for a in gl])
+    assert e.value.status == 1
+    ctx.close()
