@@ -466,3 +466,24 @@ def test_layer_backward(cfg, batch):
         ctx.layer_backward(res["vm"][:2], res["va"][:2], *[dev(a[:2]) for a in gl])
     assert e.value.status == 1
     ctx.close()
+
+
+# ---- NEXT row 3 (part): FP32 adjoint solve on the mixed-precision factors (Table I: backward LU solve in SP) ------
+@pytest.mark.parametrize("cfg,batch", [(2, 64), (4, 16)])
+def test_adjoint_mixed_precision(cfg, batch):
+    """In SABLE_MIXED mode the kept factors are FP32 and sable_adjoint solves with them (Table I).
+    Against the FP64 oracle the multipliers agree to FP32-factor accuracy: 5e-4 relative (cond(J1) ~ 1e3-1e4 x 6e-8)."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, precision=sb.MIXED, keep_factors=True)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    assert (res["converged"] == 1).all()
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    assert (np.abs(lp - rp).max(axis=1) <= 5e-4 * scale).all(), (np.abs(lp - rp).max(axis=1) / scale).max()
+    assert (np.abs(lq - rq).max(axis=1) <= 5e-4 * scale).all()
+    ctx.close()
