@@ -146,6 +146,18 @@ sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* v
                                   const double* gl_pg, const double* gl_qg, const double* gl_vm, const double* gl_va,
                                   double* dx_pg, double* dx_vm, void* cuda_stream);
 
+/* Adjoint of eq. 14 with FP64 iterative refinement on the kept factors (Table I runs the backward LU in single
+ * precision; this call brings lambda back to FP64 accuracy without an FP64 factorisation):
+ *   lambda_0 = solve(g);  repeat `sweeps` times:  r = g - J1^T lambda (FP64, the entries of J1 evaluated on the fly from
+ *   vm, va with the Alg. 1 formulas);  lambda += solve(r)   (solve = the transposed sweeps of sable_adjoint, in the
+ *   precision of the kept factors).
+ * sweeps = 0 is sable_adjoint.  vm, va = the vm, va returned by the last sable_solve; other arguments, layout and errors
+ * as sable_adjoint (sweeps outside [0, 16]: INVALID_ARG).  All DEVICE pointers; asynchronous on the stream; for grids
+ * above 5 120 buses the state part of the workspace is used as scratch (the kept factors stay intact). */
+sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                   const double* g_va, const double* g_vm, int32_t sweeps, double* lam_p,
+                                   double* lam_q, void* cuda_stream);
+
 /* Host-buffer convenience wrappers: same semantics with HOST pointers; they copy in, run on the context's
  * device and copy out (synchronous).  Used for the end-to-end measurement. */
 sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,

@@ -46,7 +46,7 @@ class Info(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_layer_backward", "sable_solve_host", "sable_adjoint_host",
+EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_layer_backward", "sable_adjoint_refined", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
            "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing"]
 
@@ -161,6 +161,16 @@ class Context:
             out = (torch.empty_like(g_va), torch.empty_like(g_vm))
         self._check(lib().sable_adjoint(self._h, C.c_int32(batch), _dp(g_va), _dp(g_vm), _dp(out[0]), _dp(out[1]),
                                         _stream()))
+        return out
+
+    def adjoint_refined(self, vm, va, g_va, g_vm, sweeps=2, out=None):
+        """sable_adjoint_refined: the adjoint of eq. 14 with `sweeps` FP64 refinement sweeps.  Returns (lam_p, lam_q)."""
+        import torch
+        batch = int(g_va.shape[0])
+        if out is None:
+            out = (torch.empty_like(g_va), torch.empty_like(g_vm))
+        self._check(lib().sable_adjoint_refined(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(g_va), _dp(g_vm),
+                                                C.c_int32(int(sweeps)), _dp(out[0]), _dp(out[1]), _stream()))
         return out
 
     def recover(self, vm, va, out=None):

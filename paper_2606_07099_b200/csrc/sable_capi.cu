@@ -520,6 +520,42 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     return SABLE_OK;
 }
 
+// ---- adjoint with FP64 iterative refinement -------------------------------------------------------------------------
+extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
+                                              const double* g_va, const double* g_vm, int32_t sweeps, double* lam_p,
+                                              double* lam_q, void* cuda_stream) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (!ctx->have_factors) return fail(ctx, SABLE_ERR_STATE, "no kept factors: call sable_solve with keep_factors = 1 first");
+    if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
+    if (!vm || !va || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
+    if (sweeps < 0 || sweeps > 16) return fail(ctx, SABLE_ERR_INVALID_ARG, "sweeps out of range [0, 16]");
+    if (batch == 0) return SABLE_OK;
+    CU(cudaSetDevice(ctx->opt.device));
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    sable_status st = launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, s);
+    if (st != SABLE_OK || sweeps == 0) return st;
+    const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus, nb = (size_t)batch * ctx->T.n_bus;
+    LayerArgs L{};
+    L.n_bus = ctx->T.n_bus; L.batch = batch; L.fptr = ctx->fptr; L.fcol = ctx->fcol; L.ftpos = ctx->ftpos; L.fgb = ctx->fgb;
+    L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_va = g_va; L.gl_vm = g_vm; L.lam_p = lam_p; L.lam_q = lam_q;
+    L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.work = ctx->work; L.work_stride = ctx->work_stride; L.post = 2;
+    const size_t sm = (size_t)ctx->T.n_bus * 32;
+    L.in_smem = sm <= 160 * 1024;
+    if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    for (int it = 0; it < sweeps; ++it) {
+        k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);                                   // r = g - J1^T lambda   (FP64)
+        CU(cudaGetLastError());
+        st = launch_lin(ctx, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, s);   // J1^T d = r  (kept factors)
+        if (st != SABLE_OK) return st;
+        k_add2<<<(int)std::min<size_t>((nb + 255) / 256, 4096), 256, 0, s>>>(lam_p, lam_q, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, nb);
+        CU(cudaGetLastError());
+        ctx->launches += 2;
+    }
+    return SABLE_OK;
+}
+
 // ---- host-buffer wrappers (end-to-end path: H2D, solve, D2H; synchronous) ------------------------------------------
 extern "C" sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
                                          const double* v_set, const double* vm0, const double* va0, double tol,

@@ -217,6 +217,26 @@ __global__ void k_layer(const LayerArgs A) {
             }
             A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + vth : 0.0;
             A.g_vm[o + j] = A.gl_vm[o + j] + vvm;
+        } else if (A.post == 2) {
+            // residual of eq. 14 in FP64, r = g - J1^T lambda (here gl_va / gl_vm = g, output g_va / g_vm = r): column
+            // theta_j of every non-slack bus, column Vm_j of every PQ bus; rows P_i (non-slack), Q_i (PQ)
+            double sth = 0.0, svm = 0.0;
+            if (tj != 2)
+                for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+                    const int i = A.fcol[k], ti = A.bus_type[i];
+                    if (ti == 2) continue;
+                    const double lp = A.lam_p[o + i], lq = ti == 0 ? A.lam_q[o + i] : 0.0;
+                    double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+                    if (i == j) {
+                        const double2 y = A.fgb[k], s = pq[i];
+                        dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
+                        dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
+                    } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+                    sth += lp * dP_dth + lq * dQ_dth;
+                    svm += lp * dP_dvm + lq * dQ_dvm;
+                }
+            A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] - sth : 0.0;
+            A.g_vm[o + j] = tj == 0 ? A.gl_vm[o + j] - svm : 0.0;
         } else {
             double sacc = 0.0;
             if (tj != 0)
@@ -233,6 +253,13 @@ __global__ void k_layer(const LayerArgs A) {
             A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - sacc : 0.0;
             A.dx_pg[o + j] = tj == 1 ? A.gl_pg[o + j] + A.lam_p[o + j] : 0.0;
         }
+    }
+}
+
+// lambda += correction (iterative refinement of the adjoint, sable_adjoint_refined)
+__global__ void k_add2(double* xp, double* xq, const double* dp, const double* dq, size_t n) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        xp[i] += dp[i]; xq[i] += dq[i];
     }
 }
 

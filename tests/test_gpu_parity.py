@@ -487,3 +487,38 @@ def test_adjoint_mixed_precision(cfg, batch):
     assert (np.abs(lp - rp).max(axis=1) <= 5e-4 * scale).all(), (np.abs(lp - rp).max(axis=1) / scale).max()
     assert (np.abs(lq - rq).max(axis=1) <= 5e-4 * scale).all()
     ctx.close()
+
+
+@pytest.mark.parametrize("cfg,batch,precision", [(3, 96, "mixed"), (4, 24, "mixed"), (5, 3, "mixed"), (3, 37, "fp64")])
+def test_adjoint_refined(cfg, batch, precision):
+    """sable_adjoint_refined: FP64 residual g - J1^T lambda (J1 on the fly, Alg. 1 formulas) + correction solves on the kept
+    factors.  With FP32 factors (Table I: backward LU in SP) two sweeps bring lambda from ~1e-4 relative to the 1e-9
+    relative of the FP64 adjoint parity test; sweeps = 0 is sable_adjoint bit for bit; on FP64 factors a sweep does no
+    harm.  Reference: the FP64 oracle at the CUDA path's own returned iterate (as in test_adjoint_parity)."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, precision=sb.MIXED if precision == "mixed" else sb.FP64, keep_factors=True)
+    out = ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it)
+    res = to_np(out)
+    assert (res["converged"] == 1).all()
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    err = lambda l, r: (np.abs(l.cpu().numpy() - r).max(axis=1) / scale).max()
+    l0 = ctx.adjoint(dev(gva), dev(gvm))
+    z0 = ctx.adjoint_refined(out["vm"], out["va"], dev(gva), dev(gvm), sweeps=0)
+    assert torch.equal(l0[0], z0[0]) and torch.equal(l0[1], z0[1])
+    l2 = ctx.adjoint_refined(out["vm"], out["va"], dev(gva), dev(gvm), sweeps=2)
+    e0, e2 = max(err(l0[0], rp), err(l0[1], rq)), max(err(l2[0], rp), err(l2[1], rq))
+    assert e2 <= 1e-9, (e0, e2)
+    if precision == "mixed":
+        assert e0 > 1e-8                          # the unrefined FP32 solve is visibly less accurate: the sweeps did the work
+        l1 = ctx.adjoint_refined(out["vm"], out["va"], dev(gva), dev(gvm), sweeps=1)
+        assert max(err(l1[0], rp), err(l1[1], rq)) < 1e-2 * e0 + 1e-12
+    # PV buses carry no Q multiplier, the slack none at all
+    bt = np.asarray(net.bus_type)
+    assert (l2[1].cpu().numpy()[:, bt != 0] == 0).all() and (l2[0].cpu().numpy()[:, bt == 2] == 0).all()
+    with pytest.raises(sb.SableError):
+        ctx.adjoint_refined(out["vm"], out["va"], dev(gva), dev(gvm), sweeps=17)
+    ctx.close()
