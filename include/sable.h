@@ -74,6 +74,9 @@ typedef struct {
     int32_t ctas_per_sm;    /* occupancy the NR kernel was sized for */
     int32_t slots_per_cta;  /* scenarios a CTA of the NR kernel advances in lockstep */
     int32_t cut_level;      /* placement 1: first elimination level kept in shared memory */
+    int32_t front_k;        /* placement 2: nodes of the dense top front (the last elimination levels, factored as one dense
+                               block matrix in shared memory); 0 = none */
+    int32_t front_level;    /* first elimination level of that front (n_level if none) */
 } sable_info;
 
 /* Build the shared fixed-pattern template for one network (host symbolic phase, run once; PAPER.md:185-197:

@@ -40,7 +40,8 @@ class Info(C.Structure):
                 ("n_term", C.c_int64), ("n_term_diag", C.c_int64), ("lu_flops", C.c_int64),
                 ("factor_bytes", C.c_int64), ("bytes_iter_m0", C.c_int64), ("bytes_adjoint_m0", C.c_int64),
                 ("smem_bytes", C.c_int32), ("placement", C.c_int32), ("threads", C.c_int32),
-                ("ctas_per_sm", C.c_int32), ("slots_per_cta", C.c_int32), ("cut_level", C.c_int32)]
+                ("ctas_per_sm", C.c_int32), ("slots_per_cta", C.c_int32), ("cut_level", C.c_int32),
+                ("front_k", C.c_int32), ("front_level", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -240,7 +241,8 @@ class Context:
         self._check(lib().sable_debug_timing(self._h, C.c_void_p(buf.ctypes.data), C.c_int32(buf.size)))
         return (buf[:4 * L].reshape(L, 4)[:, :3].astype(np.int64),
                 dict(decide_output=int(buf[4 * L]), trips=int(buf[4 * L + 1]), refill_init=int(buf[4 * L + 2]),
-                     mismatch_norm=int(buf[4 * L + 3])))
+                     mismatch_norm=int(buf[4 * L + 3]), front_assemble=int(buf[3]), front_factor=int(buf[7]) if L > 1 else 0,
+                     front_backward=int(buf[11]) if L > 2 else 0))
 
     def debug_mismatch(self, p_spec, q_spec, vm, va):
         import torch

@@ -33,6 +33,7 @@ struct sable_ctx {
     std::vector<LevelDesc> lv_host;                          // blob offsets per level (splits filled per kernel family)
     std::vector<char> blob_host;
     int ring_r = 0, ring_slot = 0, first_staged = 0;
+    int front_k = 0, front_f0 = 0, front_level = 0; int64_t front_off = 0; LevelDesc front{};   // dense top front (sable_front.cuh)
     int last_batch = -1;  bool have_factors = false;
     int64_t launches = 0;
     std::string err;
@@ -72,6 +73,7 @@ static void fill_info(sable_ctx* c) {
     I.bytes_adjoint_m0 = w * T.nnz_lu + 16 * (int64_t)I.n;
     I.smem_bytes = c->smem; I.placement = c->placement; I.threads = c->threads;
     I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->cut_level;
+    I.front_k = c->front_k; I.front_level = c->front_k > 0 ? c->front_level : T.n_level;
 }
 
 // kernel variant: placement 0 = on chip, 1 = mixed (only on request: SABLE_CUT), 2 = HBM; small = up to 128 threads
@@ -148,6 +150,60 @@ static std::vector<LevelDesc> build_levels(const Template& T, const std::vector<
         d.staged = l >= first_staged;
     }
     return lv;
+}
+
+// Dense top front (sable_front.cuh): the nodes of the last elimination levels, as many levels as keep the K x K block
+// matrix within `budget` bytes of shared memory per CTA (K <= kcap).  Appends the assembly lists (the front targets'
+// multiply-subtract terms whose eliminated node k lies below the front) to the blob and fills ctx->front*.
+static void build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap) {
+    const Template& T = c->T;
+    const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
+    const bool mixed = c->opt.precision == SABLE_MIXED;
+    c->front_k = 0; c->front_f0 = nn; c->front_level = nl; c->front = LevelDesc{};
+    auto bytes = [&](int K) { return mixed ? front_bytes<float>(K, gsh) : front_bytes<double>(K, gsh); };
+    int lc = nl;
+    while (lc > 1 && nn - T.level_ptr[lc - 1] <= kcap && bytes(nn - T.level_ptr[lc - 1]) <= budget) --lc;
+    if (nl - lc < 2) return;                                 // merging fewer than two levels saves nothing
+    const int f0 = T.level_ptr[lc], K = nn - f0;
+    LevelDesc d{};
+    d.m0 = f0; d.m1 = nn; d.p0 = T.pair_ptr[f0]; d.p1 = np;
+    const int nm = K, npr = d.p1 - d.p0;
+    std::vector<int32_t> dptr(nm + 1, 0), tptr(npr + 1, 0);
+    std::vector<int2> dak, tab, pmj(npr);
+    int maxd = 0, maxt = 0;
+    for (int i = 0; i < nm; ++i) {
+        for (int q = T.dterm_ptr[f0 + i]; q < T.dterm_ptr[f0 + i + 1]; ++q) {
+            const int a = T.dterm[q], k = T.pair_row[a];
+            if (k < f0) dak.push_back(make_int2(a, k));
+        }
+        dptr[i + 1] = (int32_t)dak.size(); maxd = std::max(maxd, dptr[i + 1] - dptr[i]);
+    }
+    for (int i = 0; i < npr; ++i) {
+        const int p = d.p0 + i;
+        for (int q = T.term_ptr[p]; q < T.term_ptr[p + 1]; ++q)
+            if (T.pair_row[T.term_a[q]] < f0) tab.push_back(make_int2(T.term_a[q], T.term_b[q]));
+        tptr[i + 1] = (int32_t)tab.size(); maxt = std::max(maxt, tptr[i + 1] - tptr[i]);
+        const int m = T.pair_row[p], j = T.pair_col[p];
+        pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
+    }
+    auto al = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
+    size_t o = 0;
+    o += (size_t)(nm + 1) * 4; d.o_tptr = (int32_t)o;
+    o += (size_t)(npr + 1) * 4; d.o_pptr = (int32_t)o; o = al(o, 8); d.o_dak = (int32_t)o;
+    o += dak.size() * 8; d.o_pmj = (int32_t)o;
+    o += (size_t)npr * 8; d.o_tab = (int32_t)o;
+    o += tab.size() * 8; o = al(o, 128); d.o_py = (int32_t)o;
+    d.blob_off = (int32_t)c->blob_host.size(); d.blob_bytes = (int32_t)o;
+    c->blob_host.resize(c->blob_host.size() + o, 0);
+    char* base = c->blob_host.data() + d.blob_off;
+    memcpy(base, dptr.data(), dptr.size() * 4);
+    memcpy(base + d.o_tptr, tptr.data(), tptr.size() * 4);
+    if (!dak.empty()) memcpy(base + d.o_dak, dak.data(), dak.size() * 8);
+    if (!pmj.empty()) memcpy(base + d.o_pmj, pmj.data(), pmj.size() * 8);
+    if (!tab.empty()) memcpy(base + d.o_tab, tab.data(), tab.size() * 8);
+    d.sd = pick_split(nm, maxd, threads, gsh);
+    d.sp = pick_split(npr, maxt, threads, gsh);
+    c->front = d; c->front_k = K; c->front_f0 = f0; c->front_level = lc;
 }
 
 // Launch plan of the fused kernel: as many scenario slots per CTA as fit entirely in shared
@@ -233,6 +289,17 @@ static sable_status choose_launch(sable_ctx* ctx) {
     }
     ctx->threads = th;
     ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
+    ctx->front_k = 0; ctx->front_level = nl; ctx->front_f0 = nn;
+    if (ctx->placement == 2) {
+        // dense top front: shared memory that still leaves most of the L1 to the resident CTAs (measured budgets)
+        const int kcap = env_int("SABLE_FRONT", 64);
+        const int64_t budget = env_int("SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : 16) * 1024LL;
+        if (kcap >= 2) build_front(ctx, th, ctx->gsh, budget, std::min(kcap, 96));
+        if (ctx->front_k > 0) {
+            ctx->front_off = align16(ctx->smem);
+            ctx->smem = (int)(ctx->front_off + (mixed ? front_bytes<float>(ctx->front_k, ctx->gsh) : front_bytes<double>(ctx->front_k, ctx->gsh)));
+        }
+    }
     const void* fn = fused_fn(mixed, ctx->placement, th <= 128);
     CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem));
     int occ = 0;
@@ -383,6 +450,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         A.gsh = c->gsh; A.dg_cut = c->dg_cut; A.pr_cut = c->pr_cut; A.st_cut = c->st_cut;
         A.ring_r = c->ring_r; A.ring_slot = c->ring_slot; A.first_staged = c->first_staged;
         A.trash_grp = (c->opt.max_batch + (1 << c->gsh) - 1) >> c->gsh;
+        A.front_k = c->front_k; A.front_f0 = c->front_f0; A.front_level = c->front_level; A.front_off = c->front_off; A.front = c->front;
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
         c->factor_gsh = c->gsh;

@@ -3,6 +3,7 @@
 // longer evaluated -- the per-scenario convergence masking.  Launched from sable_capi.cu.
 #pragma once
 #include "sable_stages.cuh"
+#include "sable_front.cuh"
 
 namespace sable {
 
@@ -19,6 +20,9 @@ struct SolveArgs {
     int64_t fac_stride, work_stride;
     int32_t gsh, dg_cut, pr_cut, st_cut;                   // slots per CTA = 1 << gsh; placement cuts (nodes, pairs, nodes)
     int32_t ring_r, ring_slot, first_staged;               // level-blob ring: slots, bytes per slot, first streamed level
+    int32_t front_k, front_f0, front_level;                // dense top front (sable_front.cuh): K nodes from f0 = levels >= front_level; 0 = off
+    int64_t front_off;                                     // its byte offset in the CTA's dynamic shared memory
+    LevelDesc front;                                       // assembly lists of the front
     unsigned long long* tim;  // optional cycle counters (sable_debug_timing), else nullptr
     int32_t* queue;           // persistent-kernel scenario counter
     int32_t* status;          // staged mode: [batch] 0 = active, 1 = converged, 2 = stopped
@@ -130,6 +134,7 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
     for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
     Slot<T, kP> s = carve<T, kP>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    Front<T> F = carve_front<T>(smem, A.front_off, A.front_k, A.front_f0, gsh, g);
     BlobRing ring;
     ring.slots = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)t.n_level * (int64_t)sizeof(LevelDesc));
     ring.mbar = reinterpret_cast<unsigned long long*>(smem + kRedBytes + 128);
@@ -190,13 +195,31 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
         stage_fill_pairs<T, kP, true>(t, s, tsub, nsub, lv[0].p1);
+        if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub, nsub);
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
-        stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring);
-        if (any_slot(b >= 0 && !fin)) {                    // a trip that only refactors for kept factors needs no solve
-            stage_backward<T, kP, false>(t, s, lv, ring);
-            stage_update<T, kP>(t, s, tsub, nsub);
-        } else ring.skip_sweep();
+        if (kP == 2 && A.front_k > 0) {
+            // levels below the front level by level, the front itself as one dense block in shared memory
+            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, A.front_level);
+            tk = clock64();
+            front_assemble<T, kP, true>(t, s, F, A.front);
+            ring.tick(3, tk);
+            front_factor<T, true>(F, tsub, nsub);
+            ring.tick(7, tk);
+            if (any_slot(b >= 0 && !fin)) {
+                front_backward<T, kP>(s, F, tsub, nsub);
+                ring.tick(11, tk);
+                stage_backward<T, kP, false>(t, s, lv, ring, A.front_level);
+                stage_update<T, kP>(t, s, tsub, nsub);
+            }
+            if (fin) front_store<T, kP>(t, s, F, A.front, tsub, nsub);
+        } else {
+            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, t.n_level);
+            if (any_slot(b >= 0 && !fin)) {                // a trip that only refactors for kept factors needs no solve
+                stage_backward<T, kP, false>(t, s, lv, ring, t.n_level);
+                stage_update<T, kP>(t, s, tsub, nsub);
+            } else ring.skip_sweep();
+        }
         if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
         if (b >= 0 && !fin) ++it;
         if (fin) {

@@ -370,9 +370,12 @@ def test_host_buffer_calls_match_device_calls():
                                  dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="64"),
                                  dict(SABLE_G="32", SABLE_CUT="99", SABLE_THREADS="128"),
                                  dict(SABLE_G="2", SABLE_CUT="2", SABLE_RING_R="2", SABLE_RING_SLOT="4096"),
-                                 dict(SABLE_RING_R="0")])
+                                 dict(SABLE_RING_R="0"),
+                                 dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="128", SABLE_FRONT="13", SABLE_FRONT_KB="64"),
+                                 dict(SABLE_G="1", SABLE_CUT="99", SABLE_THREADS="256", SABLE_FRONT="33", SABLE_FRONT_KB="200"),
+                                 dict(SABLE_G="2", SABLE_CUT="99", SABLE_THREADS="64", SABLE_FRONT="0")])
 def test_placements_and_group_layouts(env, monkeypatch):
-    for k in ("SABLE_G", "SABLE_CUT", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT"):
+    for k in ("SABLE_G", "SABLE_CUT", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT", "SABLE_FRONT", "SABLE_FRONT_KB"):
         monkeypatch.delenv(k, raising=False)
     for k, v in env.items():
         monkeypatch.setenv(k, v)
@@ -389,6 +392,9 @@ def test_placements_and_group_layouts(env, monkeypatch):
             assert ctx.info["slots_per_cta"] == int(env["SABLE_G"])
         if "SABLE_CUT" in env:      # mixed placement below the last level, plain HBM placement beyond
             assert ctx.info["placement"] == (1 if int(env["SABLE_CUT"]) < ctx.info["n_level"] else 2)
+        if "SABLE_FRONT" in env:    # dense top front: the last levels whose nodes fit the cap (cfg 2: 13 -> levels 4-7, 33 -> 2-7)
+            want = {"13": (13, 4), "33": (33, 2), "0": (0, ctx.info["n_level"])}[env["SABLE_FRONT"]]
+            assert (ctx.info["front_k"], ctx.info["front_level"]) == want
         res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
         check_solution(res, ref, c.tol, 1e-9)
         if keep:
@@ -521,4 +527,45 @@ def test_adjoint_refined(cfg, batch, precision):
     assert (l2[1].cpu().numpy()[:, bt != 0] == 0).all() and (l2[0].cpu().numpy()[:, bt == 2] == 0).all()
     with pytest.raises(sb.SableError):
         ctx.adjoint_refined(out["vm"], out["va"], dev(gva), dev(gvm), sweeps=17)
+    ctx.close()
+
+
+# ---- dense top front of the fused HBM-placement kernel (csrc/sable_front.cuh) ------------------------------------------
+@pytest.mark.parametrize("cfg,batch,precision,front", [(3, 150, "fp64", "13"), (4, 40, "mixed", "35"), (5, 5, "fp64", "47"),
+                                                       (5, 3, "mixed", "20"), (3, 33, "fp64", "0")])
+def test_dense_front(cfg, batch, precision, front, monkeypatch):
+    """The last elimination levels factored as one dense block matrix in shared memory (Schur complement of the sparse
+    part, right-looking block LU with the same 2x2 pivots, substitutions fused in) give the NR results of the
+    level-by-level code -- parity with the oracle at the usual tolerances -- and the factors written back into the sparse
+    slots serve sable_adjoint (1e-8 relative in FP64, FP32-factor accuracy in mixed mode)."""
+    monkeypatch.setenv("SABLE_FRONT", front)
+    monkeypatch.setenv("SABLE_FRONT_KB", "200")
+    monkeypatch.setenv("SABLE_CUT", "99")          # HBM placement also for these small batches, in the bench's launch shapes
+    monkeypatch.setenv("SABLE_G", "4" if cfg == 3 else "1")
+    monkeypatch.setenv("SABLE_THREADS", {3: "128", 4: "256", 5: "512"}[cfg])
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    mixed = precision == "mixed"
+    ctx = make_ctx(net, max_batch=batch, precision=sb.MIXED if mixed else sb.FP64, keep_factors=True)
+    assert ctx.info["placement"] == 2
+    assert (ctx.info["front_k"] > 1) == (front != "0") and ctx.info["front_k"] <= int(front)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    if mixed:      # acceptance as in test_nr_parity_mixed_precision
+        assert np.array_equal(res["converged"], ref["converged"])
+        assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+        ok = res["converged"] == 1
+        assert (res["final_norm"][ok] <= c.tol).all()
+        assert np.abs(res["vm"] - ref["vm"])[ok].max() <= 1e-7 and np.abs(res["va"] - ref["va"])[ok].max() <= 1e-7
+    else:
+        check_solution(res, ref, c.tol, 1e-9)
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    tol = 5e-4 if mixed else 1e-8
+    assert (np.abs(lp - rp).max(axis=1) <= tol * scale).all(), (np.abs(lp - rp).max(axis=1) / scale).max()
+    assert (np.abs(lq - rq).max(axis=1) <= tol * scale).all()
     ctx.close()
