@@ -198,25 +198,27 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
         if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub, nsub);
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
-        if (kP == 2 && A.front_k > 0) {
-            // levels below the front level by level, the front itself as one dense block in shared memory
-            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, A.front_level);
-            tk = clock64();
-            front_assemble<T, kP, true>(t, s, F, A.front);
-            ring.tick(3, tk);
-            front_factor<T, true>(F, tsub, nsub);
-            ring.tick(7, tk);
-            if (any_slot(b >= 0 && !fin)) {
-                front_backward<T, kP>(s, F, tsub, nsub);
-                ring.tick(11, tk);
-                stage_backward<T, kP, false>(t, s, lv, ring, A.front_level);
+        if (kP == 2) {
+            // HBM placement: the levels below the dense top front level by level (all of them if there is no front:
+            // front_level = n_level), the front itself as one dense block in shared memory (sable_front.cuh)
+            stage_factor_forward<T, kP, true, true, false, true, false>(t, s, lv, ring, A.front_level);
+            if (A.front_k > 0) {
+                tk = clock64();
+                front_assemble<T, kP, true>(t, s, F, A.front);
+                ring.tick(3, tk);
+                front_factor<T, true>(F, tsub, nsub);
+                ring.tick(7, tk);
+            }
+            if (any_slot(b >= 0 && !fin)) {                // a trip that only refactors for kept factors needs no solve
+                if (A.front_k > 0) { front_backward<T, kP>(s, F, tsub, nsub); ring.tick(11, tk); }
+                stage_backward<T, kP, false, false>(t, s, lv, ring, A.front_level);
                 stage_update<T, kP>(t, s, tsub, nsub);
             }
-            if (fin) front_store<T, kP>(t, s, F, A.front, tsub, nsub);
+            if (fin && A.front_k > 0) front_store<T, kP>(t, s, F, A.front, tsub, nsub);
         } else {
-            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, t.n_level);
-            if (any_slot(b >= 0 && !fin)) {                // a trip that only refactors for kept factors needs no solve
-                stage_backward<T, kP, false>(t, s, lv, ring, t.n_level);
+            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring);
+            if (any_slot(b >= 0 && !fin)) {
+                stage_backward<T, kP, false>(t, s, lv, ring);
                 stage_update<T, kP>(t, s, tsub, nsub);
             } else ring.skip_sweep();
         }

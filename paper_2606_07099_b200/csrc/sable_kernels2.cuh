@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
         scen_output<T, 2>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
         __syncthreads();
         if (threadIdx.x == 0) A.status[b] = st;
-        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, 2, true, false, false, true>(A.t, s, A.t.level, ring, A.t.n_level); }
+        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, 2, true, false, false, true>(A.t, s, A.t.level, ring); }
     }
 }
 
@@ -63,8 +63,8 @@ __global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
     if (A.status[b] != 0) return;
     const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
     BlobRing ring = no_ring(A.t);
-    stage_factor_forward<T, 2, true, true, false, true>(A.t, s, A.t.level, ring, A.t.n_level);
-    stage_backward<T, 2, false>(A.t, s, A.t.level, ring, A.t.n_level);
+    stage_factor_forward<T, 2, true, true, false, true>(A.t, s, A.t.level, ring);
+    stage_backward<T, 2, false>(A.t, s, A.t.level, ring);
     stage_update<T, 2>(A.t, s, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0) A.it[b] += 1;
 }
@@ -97,8 +97,8 @@ __global__ void k_linsolve(const LinArgs A) {
     }
     __syncthreads();
     BlobRing ring = no_ring(t);
-    if (A.transposed) { stage_factor_forward<T, 1, false, true, true, false>(t, s, t.level, ring, t.n_level); stage_backward<T, 1, true>(t, s, t.level, ring, t.n_level); }
-    else              { stage_factor_forward<T, 1, false, true, false, false>(t, s, t.level, ring, t.n_level); stage_backward<T, 1, false>(t, s, t.level, ring, t.n_level); }
+    if (A.transposed) { stage_factor_forward<T, 1, false, true, true, false>(t, s, t.level, ring); stage_backward<T, 1, true>(t, s, t.level, ring); }
+    else              { stage_factor_forward<T, 1, false, true, false, false>(t, s, t.level, ring); stage_backward<T, 1, false>(t, s, t.level, ring); }
     if (act)
         for (int m = tsub; m <= t.n_node; m += nsub) {
             const int bus = t.node_bus[m];
@@ -309,7 +309,7 @@ __global__ void k_debug(const DebugArgs A) {
         return;
     }
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring, t.n_level);
+    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring);
 }
 
 }  // namespace sable

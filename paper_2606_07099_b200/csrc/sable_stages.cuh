@@ -99,9 +99,10 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slo
 // kLeafDone: the pairs of level 0 already hold their final values (stage_fill_pairs<kPrescale>), level 0 then has
 // diagonal targets only and a single barrier.  A pair target without terms is not touched by the accumulate pass.
 // kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
-// nl: levels [0, nl) are processed (t.n_level, or the first level of the dense top front: sable_front.cuh).
-template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone>
-__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl) {
+// kAll = false: only the levels [0, nl_) are processed (those below the dense top front: sable_front.cuh).
+template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone, bool kAll = true>
+__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl_ = 0) {
+    const int nl = kAll ? t.n_level : nl_;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
     for (int l = 0; l < nl; ++l) {
@@ -193,8 +194,9 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
 
 // backward half of a5: U x = y, i.e. x_m = D_m^-1 (y_m - sum_j U(m,j) x_j) over the pairs owned by m, levels
 // descending.  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
-template <typename T, int kP, bool kTransposed>
-__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl) {
+template <typename T, int kP, bool kTransposed, bool kAll = true>
+__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl_ = 0) {
+    const int nl = kAll ? t.n_level : nl_;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
     for (int l = nl - 1; l >= 0; --l) {
