@@ -35,8 +35,8 @@ WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward"
             4: "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
             5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
-# captures (profiles/r01_v4_README.md); None where no capture exists
-NCU_TRAFFIC = {2: 2.991616e6, 3: 3.284000e9 + 3.239069e9, 4: 2.073546e9 + 3.073361e9, 5: 8.367077e9 + 4.186991e9}
+# captures (profiles/r01_v5_README.md); None where no capture exists
+NCU_TRAFFIC = {2: 2.991872e6, 3: 3.302762e9 + 3.165931e9, 4: 2.096229e9 + 3.065290e9, 5: 8.386075e9 + 4.177006e9}
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 
@@ -184,7 +184,7 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
                         "achieved": alg / kern_s / 1e9, "peak": peak, "unit": "GB/s", "frac": alg / kern_s / 1e9 / peak,
                         "traffic": NCU_TRAFFIC.get(cfg_id) if mode == 0 else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                         "note": "achieved = model-M0 bytes (DESIGN.md section 8) / kernel time; traffic = ncu dram bytes of one such "
-                                "launch (profiles/r01_v4_README.md); configs 1-2 run on chip, so their traffic is far below M0"},
+                                "launch (profiles/r01_v5_README.md); configs 1-2 run on chip, so their traffic is far below M0"},
            "launches": launches, "create_s": create_s, "info": {k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level",
                                                                                    "placement", "threads", "smem_bytes", "bytes_iter_m0")},
            "clocks": sampler.summary() if sampler else None}
