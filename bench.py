@@ -186,8 +186,23 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
                         "note": "achieved = model-M0 bytes (DESIGN.md section 8) / kernel time; traffic = ncu dram bytes of one such "
                                 "launch (profiles/r01_v5_README.md); configs 1-2 run on chip, so their traffic is far below M0"},
            "launches": launches, "create_s": create_s, "info": {k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level",
-                                                                                   "placement", "threads", "smem_bytes", "bytes_iter_m0")},
+                                                                                   "placement", "threads", "smem_bytes", "front_k", "bytes_iter_m0")},
            "clocks": sampler.summary() if sampler else None}
+    # the NEXT rows of DESIGN.md section 0 (outside the timed region above; CUDA events, L2 flushed between calls)
+    def timed(fn, reps=5):
+        ts = []
+        for _ in range(reps + 1):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return float(np.mean(ts[1:]))
+    pq = (torch.empty_like(out["vm"]), torch.empty_like(out["vm"]))
+    res["next_rows_ms"] = {"recover": timed(lambda: ctx.recover(out["vm"], out["va"], out=pq))}
+    if c.adjoint:
+        res["next_rows_ms"]["layer_backward"] = timed(lambda: ctx.layer_backward(out["vm"], out["va"], dga, dgm, dgm, dga, out=pq))
+        res["next_rows_ms"]["adjoint_refined_2_sweeps"] = timed(lambda: ctx.adjoint_refined(out["vm"], out["va"], dga, dgm, sweeps=2, out=lam))
     if e2e:
         pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory().numpy()
         hps, hqs, hvs, hga, hgm = pin(ps), pin(qs), pin(vs), pin(gva), pin(gvm)
@@ -360,7 +375,7 @@ def main():
             "dtype": "f64" if not cfg.precision else "f64+f32", "data": "synthetic", "config": config,
             "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["launches"], "roofline": res["roofline"],
             "converged": res["converged"], "iterations_hist": res["iterations_hist"], "solve_ms": res["solve_ms"],
-            "adjoint_ms": res["adjoint_ms"], "create_s": res["create_s"], "info": res["info"]}
+            "adjoint_ms": res["adjoint_ms"], "next_rows_ms": res["next_rows_ms"], "create_s": res["create_s"], "info": res["info"]}
     if rank == 0 and world == 1:
         line["cpu_baseline"], _, _ = run_oracle(a.config, inputs)
         if not a.no_sweep:
@@ -370,7 +385,7 @@ def main():
                 per[S.CONFIGS[k].name] = {"solves_per_s": r["value"], "ms_per_step": r["ms_per_step"], "solve_ms": r["solve_ms"],
                                           "adjoint_ms": r["adjoint_ms"], "converged": r["converged"], "batch": r["batch"],
                                           "iterations_hist": r["iterations_hist"], "roofline_frac": r["roofline"]["frac"],
-                                          "achieved_gbs": r["roofline"]["achieved"], "info": r["info"]}
+                                          "achieved_gbs": r["roofline"]["achieved"], "next_rows_ms": r["next_rows_ms"], "info": r["info"]}
             line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))

@@ -143,7 +143,7 @@ sable_status sable_recover(sable_ctx* ctx, int32_t batch, const double* vm, cons
  *   gl_vm, gl_va          dL/dVm_i (all buses), dL/dtheta_i (slack entry ignored)
  *   dx_pg, dx_vm          out: dL/dp_g (nonzero at PV buses), dL/dVm (nonzero at PV and slack buses)
  * All DEVICE pointers, [batch][n_bus]; batch must equal the batch of the last solve; asynchronous on the stream; for
- * grids above 5 120 buses the state part of the workspace is used as scratch (the kept factors stay intact).
+ * grids above 3 413 buses the state part of the workspace is used as scratch (the kept factors stay intact).
  * Errors: INVALID_ARG, STATE, CUDA. */
 sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
                                   const double* gl_pg, const double* gl_qg, const double* gl_vm, const double* gl_va,
@@ -156,7 +156,7 @@ sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* v
  *   precision of the kept factors).
  * sweeps = 0 is sable_adjoint.  vm, va = the vm, va returned by the last sable_solve; other arguments, layout and errors
  * as sable_adjoint (sweeps outside [0, 16]: INVALID_ARG).  All DEVICE pointers; asynchronous on the stream; for grids
- * above 5 120 buses the state part of the workspace is used as scratch (the kept factors stay intact). */
+ * above 3 413 buses the state part of the workspace is used as scratch (the kept factors stay intact). */
 sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
                                    const double* g_va, const double* g_vm, int32_t sweeps, double* lam_p,
                                    double* lam_q, void* cuda_stream);

@@ -84,6 +84,14 @@ static const void* fused_fn(bool mixed, int place, bool small) {
     return mixed ? (const void*)k_nr_fused<float, 2, false> : (const void*)k_nr_fused<double, 2, false>;
 }
 
+// threads per CTA of the one-thread-per-bus kernels (recover, layer): whole rounds with no idle tail (300 buses -> 160
+// threads x 2 rounds, not 256 x 2 with the second round 85 % idle), 64 for small grids, 512 for large ones
+static int bus_threads(int n_bus) {
+    if (n_bus <= 256) return 64;
+    const int cap = n_bus <= 4096 ? 256 : 512, rounds = (n_bus + cap - 1) / cap;
+    return std::min(cap, ((n_bus + rounds - 1) / rounds + 31) / 32 * 32);
+}
+
 static int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
 
 // lanes per target (log2) for a level with n targets whose longest list has max_len entries: as many as keep every
@@ -547,7 +555,7 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     const size_t sm = (size_t)ctx->T.n_bus * 16;
     R.v_in_smem = sm <= 160 * 1024;            // else the scenario's workspace slice (>= 3 (n_bus) 16 bytes) holds V
     if (R.v_in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_recover, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    const int th = bus_threads(ctx->T.n_bus);
     k_recover<<<batch, th, R.v_in_smem ? sm : 0, (cudaStream_t)cuda_stream>>>(R);
     ctx->launches += 1;
     CU(cudaGetLastError());
@@ -572,10 +580,10 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_pg = gl_pg; L.gl_qg = gl_qg; L.gl_vm = gl_vm; L.gl_va = gl_va;
     L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.lam_p = ctx->lbuf + 2 * n; L.lam_q = ctx->lbuf + 3 * n;
     L.dx_pg = dx_pg; L.dx_vm = dx_vm; L.work = ctx->work; L.work_stride = ctx->work_stride;
-    const size_t sm = (size_t)ctx->T.n_bus * 32;
-    L.in_smem = sm <= 160 * 1024;          // else the scenario's workspace slice (48 n_bus bytes) holds V and (P, Q)
+    const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
+    L.in_smem = sm <= 160 * 1024;          // else the scenario's workspace slice (48 n_bus bytes) holds them
     if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    const int th = bus_threads(ctx->T.n_bus);
     L.post = 0;
     k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
     CU(cudaGetLastError());
@@ -608,10 +616,10 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
     L.n_bus = ctx->T.n_bus; L.batch = batch; L.fptr = ctx->fptr; L.fcol = ctx->fcol; L.ftpos = ctx->ftpos; L.fgb = ctx->fgb;
     L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_va = g_va; L.gl_vm = g_vm; L.lam_p = lam_p; L.lam_q = lam_q;
     L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.work = ctx->work; L.work_stride = ctx->work_stride; L.post = 2;
-    const size_t sm = (size_t)ctx->T.n_bus * 32;
+    const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
     L.in_smem = sm <= 160 * 1024;
     if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const int th = ctx->T.n_bus <= 256 ? 64 : ctx->T.n_bus <= 4096 ? 256 : 512;
+    const int th = bus_threads(ctx->T.n_bus);
     for (int it = 0; it < sweeps; ++it) {
         k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);                                   // r = g - J1^T lambda   (FP64)
         CU(cudaGetLastError());

@@ -182,10 +182,14 @@ __global__ void k_layer(const LayerArgs A) {
     const size_t o = (size_t)b * nb;
     double2* v = A.in_smem ? reinterpret_cast<double2*>(smem) : reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
     double2* pq = v + nb;
+    double2* w = pq + nb;                  // per bus i: the two row weights the transposed products gather (coalesced here)
     const double* vm = A.vm + o;
     for (int i = threadIdx.x; i < nb; i += blockDim.x) {
         double sn, cs; sincos(A.va[o + i], &sn, &cs);
         v[i] = make_double2(vm[i] * cs, vm[i] * sn);
+        const int ti = A.bus_type[i];
+        if (!A.post) w[i] = make_double2(ti == 2 ? A.gl_pg[o + i] : 0.0, ti != 0 ? A.gl_qg[o + i] : 0.0);   // rows of z2: P at the slack, Q at PV / slack
+        else         w[i] = make_double2(ti != 2 ? A.lam_p[o + i] : 0.0, ti == 0 ? A.lam_q[o + i] : 0.0);   // rows of J1: P non-slack, Q at PQ
     }
     __syncthreads();
     for (int i = threadIdx.x; i < nb; i += blockDim.x) {
@@ -204,8 +208,8 @@ __global__ void k_layer(const LayerArgs A) {
             double vth = 0.0, vvm = 0.0;
             for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
                 const int i = A.fcol[k], ti = A.bus_type[i];
-                const double ai = ti == 2 ? A.gl_pg[o + i] : 0.0, ci = ti != 0 ? A.gl_qg[o + i] : 0.0;
                 if (ti == 0) continue;                                   // rows of z2 sit at PV and slack buses only
+                const double ai = w[i].x, ci = w[i].y;
                 double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
                 if (i == j) {
                     const double2 y = A.fgb[k], s = pq[i];
@@ -225,7 +229,7 @@ __global__ void k_layer(const LayerArgs A) {
                 for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
                     const int i = A.fcol[k], ti = A.bus_type[i];
                     if (ti == 2) continue;
-                    const double lp = A.lam_p[o + i], lq = ti == 0 ? A.lam_q[o + i] : 0.0;
+                    const double lp = w[i].x, lq = w[i].y;
                     double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
                     if (i == j) {
                         const double2 y = A.fgb[k], s = pq[i];
@@ -242,7 +246,7 @@ __global__ void k_layer(const LayerArgs A) {
             if (tj != 0)
                 for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
                     const int i = A.fcol[k], ti = A.bus_type[i];
-                    const double lp = ti != 2 ? A.lam_p[o + i] : 0.0, lq = ti == 0 ? A.lam_q[o + i] : 0.0;
+                    const double lp = w[i].x, lq = w[i].y;
                     double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
                     if (i == j) {
                         const double2 y = A.fgb[k], s = pq[i];
