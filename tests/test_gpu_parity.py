@@ -373,6 +373,7 @@ def test_host_buffer_calls_match_device_calls():
                                  dict(SABLE_RING_R="0"),
                                  dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="128", SABLE_FRONT="13", SABLE_FRONT_KB="64"),
                                  dict(SABLE_G="1", SABLE_CUT="99", SABLE_THREADS="256", SABLE_FRONT="33", SABLE_FRONT_KB="200"),
+                                 dict(SABLE_G="1", SABLE_CUT="99", SABLE_THREADS="256", SABLE_FRONT="57", SABLE_FRONT_KB="200"),
                                  dict(SABLE_G="2", SABLE_CUT="99", SABLE_THREADS="64", SABLE_FRONT="0")])
 def test_placements_and_group_layouts(env, monkeypatch):
     for k in ("SABLE_G", "SABLE_CUT", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT", "SABLE_FRONT", "SABLE_FRONT_KB"):
@@ -393,7 +394,7 @@ def test_placements_and_group_layouts(env, monkeypatch):
         if "SABLE_CUT" in env:      # mixed placement below the last level, plain HBM placement beyond
             assert ctx.info["placement"] == (1 if int(env["SABLE_CUT"]) < ctx.info["n_level"] else 2)
         if "SABLE_FRONT" in env:    # dense top front: the last levels whose nodes fit the cap (cfg 2: 13 -> levels 4-7, 33 -> 2-7)
-            want = {"13": (13, 4), "33": (33, 2), "0": (0, ctx.info["n_level"])}[env["SABLE_FRONT"]]
+            want = {"13": (13, 4), "33": (33, 2), "57": (57, 1), "0": (0, ctx.info["n_level"])}[env["SABLE_FRONT"]]   # 57: all but level 0
             assert (ctx.info["front_k"], ctx.info["front_level"]) == want
         res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=12))
         check_solution(res, ref, c.tol, 1e-9)
