@@ -118,14 +118,13 @@ static void build_blobs(const Template& T, std::vector<LevelDesc>& lv, std::vect
         o += (size_t)(nm + 1) * 4; o = al(o, 8); d.o_dak = (int32_t)o;
         o += (size_t)nd * 8; d.o_pmj = (int32_t)o;
         o += (size_t)np * 8; d.o_tab = (int32_t)o;
-        o += (size_t)nt * 8; o = al(o, 32); d.o_py = (int32_t)o;
-        o += (size_t)np * 32; o = al(o, 128);
+        o += (size_t)nt * 8; d.o_py = (int32_t)o;              // (the Y values of the pairs live in DevTemplate::pair_y)
+        o = al(o, 128);
         d.blob_off = (int32_t)blob.size(); d.blob_bytes = (int32_t)o;
         blob.resize(blob.size() + o, 0);
         char* base = blob.data() + d.blob_off;
         int32_t* dptr = (int32_t*)base; int32_t* tptr = (int32_t*)(base + d.o_tptr); int32_t* pptr = (int32_t*)(base + d.o_pptr);
         int2* dak = (int2*)(base + d.o_dak); int2* pmj = (int2*)(base + d.o_pmj); int2* tab = (int2*)(base + d.o_tab);
-        double4* py = (double4*)(base + d.o_py);
         for (int i = 0; i <= nm; ++i) {
             dptr[i] = T.dterm_ptr[d.m0 + i] - T.dterm_ptr[d.m0];
             pptr[i] = (T.pair_ptr[d.m0 + i] - d.p0) | ((i < nm && T.node_pq[d.m0 + i]) ? 1 << 30 : 0);
@@ -134,9 +133,8 @@ static void build_blobs(const Template& T, std::vector<LevelDesc>& lv, std::vect
         for (int q = 0; q < nd; ++q) { const int a = T.dterm[T.dterm_ptr[d.m0] + q]; dak[q] = make_int2(a, T.pair_row[a]); }
         for (int q = 0; q < nt; ++q) tab[q] = make_int2(T.term_a[T.term_ptr[d.p0] + q], T.term_b[T.term_ptr[d.p0] + q]);
         for (int i = 0; i < np; ++i) {
-            const int p = d.p0 + i, m = T.pair_row[p], j = T.pair_col[p], su = T.pair_yu[p], sl = T.pair_yl[p];
+            const int p = d.p0 + i, m = T.pair_row[p], j = T.pair_col[p];
             pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
-            py[i] = make_double4(su >= 0 ? T.yg[su] : 0.0, su >= 0 ? T.yb[su] : 0.0, sl >= 0 ? T.yg[sl] : 0.0, sl >= 0 ? T.yb[sl] : 0.0);
         }
     }
 }

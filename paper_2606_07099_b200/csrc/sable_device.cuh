@@ -33,7 +33,6 @@ namespace sable {
 //   int2  dak[]        (pair (k,m), node k)                                  at o_dak
 //   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                      at o_pmj
 //   int2  tab[]        (pair (k,m), pair (k,j))                              at o_tab
-//   double4 py[np]     (G_mj, B_mj, G_jm, B_jm), zeros for a fill pair       at o_py
 // Narrow levels (staged = 1) are streamed through a shared-memory ring by cp.async.bulk one or two levels ahead of
 // use, so that no index load of the latency-critical top of the elimination tree goes to L2; wide levels are read
 // in place (their latency hides behind the many targets in flight).
@@ -41,7 +40,7 @@ struct LevelDesc {
     int32_t m0, m1, p0, p1;
     uint8_t sd, sp, sb, staged;   // diag / pair / backward lane splits (lanes per target = 1 << s)
     int32_t blob_off, blob_bytes; // slice of DevTemplate::blob (16-byte aligned, size a multiple of 16)
-    int32_t o_tptr, o_pptr, o_dak, o_pmj, o_tab, o_py;
+    int32_t o_tptr, o_pptr, o_dak, o_pmj, o_tab, o_py;   // o_py: end of the lists (the front's descriptor keeps one more list there)
     int32_t pad;
 };
 

@@ -245,7 +245,7 @@ __global__ void k_layer(const LayerArgs A) {
             double sacc = 0.0;
             if (tj != 0)
                 for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
-                    const int i = A.fcol[k], ti = A.bus_type[i];
+                    const int i = A.fcol[k];
                     const double lp = w[i].x, lq = w[i].y;
                     double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
                     if (i == j) {
