@@ -122,9 +122,12 @@ template <typename T, int kP> struct Slot {
     __device__ __forceinline__ char* g_ma() const { return gw + go_ma; }
     __device__ __forceinline__ char* g_rh() const { return gw + go_rh; }
 
+    // byte offsets are 32-bit: a group's slice (and shared memory) is far below 4 GB
     __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
-        if (kP == 0 || (kP == 1 && idx >= cut_blocks)) { vs = 16 << gsh; return reinterpret_cast<T*>(sb + (((size_t)(idx - cut_blocks) * VPB) << (gsh + 4))); }
-        vs = 16 << gsh; return reinterpret_cast<T*>(gb + (((size_t)idx * VPB) << (gsh + 4)));
+        vs = 16 << gsh;
+        if (kP == 0) return reinterpret_cast<T*>(sb + ((unsigned)(idx * VPB) << (gsh + 4)));
+        if (kP == 1 && idx >= cut_blocks) return reinterpret_cast<T*>(sb + ((unsigned)((idx - cut_blocks) * VPB) << (gsh + 4)));
+        return reinterpret_cast<T*>(gb + ((unsigned)(idx * VPB) << (gsh + 4)));
     }
     __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); return ld_blk(p, vs); }
     __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); st_blk(p, vs, v); }
@@ -134,8 +137,9 @@ template <typename T, int kP> struct Slot {
     __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
 
     __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
-        if (kP == 0 || (kP == 1 && m >= st_cut)) return reinterpret_cast<double2*>(sb + ((size_t)(m - st_cut) << (gsh + 4)));
-        return reinterpret_cast<double2*>(gb + ((size_t)m << (gsh + 4)));
+        if (kP == 0) return reinterpret_cast<double2*>(sb + ((unsigned)m << (gsh + 4)));
+        if (kP == 1 && m >= st_cut) return reinterpret_cast<double2*>(sb + ((unsigned)(m - st_cut) << (gsh + 4)));
+        return reinterpret_cast<double2*>(gb + ((unsigned)m << (gsh + 4)));
     }
     __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv(), g_vv(), m); }
     __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma(), g_ma(), m); }
