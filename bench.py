@@ -36,7 +36,7 @@ WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward"
             5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
 # captures (profiles/r01_v5_README.md); None where no capture exists
-NCU_TRAFFIC = {2: 2.991872e6, 3: 3.302762e9 + 3.165931e9, 4: 2.096229e9 + 3.065290e9, 5: 8.386075e9 + 4.177006e9}
+NCU_TRAFFIC = {2: 2.990848e6, 3: 3.282664e9 + 3.159225e9, 4: 2.215608e9 + 3.034042e9, 5: 8.344635e9 + 4.143312e9}
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 
