@@ -1,21 +1,29 @@
 #!/usr/bin/env python
 """bench.py -- converged power-flow solves/s of the batched Newton-Raphson hot path on B200 (one JSON line).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference] [--no-sweep]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5|mesh] [--impl ours|reference] [--no-sweep]
 
 A "step" is one pass of the whole hot path over one batch of synthetic scenarios of a BASELINE.json config:
 sable_solve (mismatch + norm, masking, Jacobian fill, LU refactor, triangular solves, update -- until every scenario
-converged or stopped) and, for configs that ask for it, sable_adjoint on the kept factors.  Default workload:
-BASELINE.json configs[1] (118 buses, 1024 scenarios); `--config k` picks configs[k-1]; unless --no-sweep the line also
-carries a short measurement of all five configs under "per_config" (HBM-roofline fractions are meaningful for
-configs 3-5 only: configs 1-2 are L2-resident).
+converged or stopped) and, for configs that ask for it, sable_adjoint on the kept factors.  Default (headline) workload:
+BASELINE.json configs[4] (9241 buses x 256 scenarios, FP64 forward + adjoint), the largest single-GPU config and the
+shape of the paper's own headline rows; `--config k` picks configs[k-1]; unless --no-sweep the line
+also carries a measurement of all five configs plus a higher-fill mesh stand-in under "per_config", each with its own
+clock sample, end-to-end figure and roofline object.
 
 Timing: W >= 3 warm-up steps, then K steps each bracketed by CUDA events on the launching stream (torch's current
 stream, which is the stream handed to the library); L2 is flushed (256 MiB memset) between steps, outside the timed
 region; barrier + synchronize on both sides; max over ranks.  N > 1: scenarios shard with no collective (weak
 scaling: every rank solves its own batch of the config with its own scenario seed).
+
+Roofline: `achieved` = algorithmic (model M0) bytes of the executed scenario-iterations / the mean
+CUDA-event duration of the dominant kernel (the one k_nr_fused launch of sable_solve); `traffic` = ncu dram bytes of one
+such launch read from the committed capture table profiles/r02_ncu_traffic.csv (null when the table has no row for the
+workload).  When the capture shows LESS DRAM traffic than the model (the batch is served from shared memory / L2), the
+model bytes were never moved: the line then says bound = "l2/latency" and quotes the DRAM-moved rate, never the model.
 """
 import argparse
+import csv
 import json
 import os
 import sys
@@ -29,14 +37,13 @@ sys.path.insert(0, ROOT)
 
 import sable_synth as S  # noqa: E402
 
-WORKLOAD = {1: "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward",
-            2: "BASELINE.json configs[1]: 118 buses x 1024 scenarios, FP64 forward",
-            3: "BASELINE.json configs[2]: 300 buses x 8192 scenarios, FP64 forward + adjoint",
-            4: "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
-            5: "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint"}
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_nr_fused launch of the full batch, from the committed ncu --set full
-# captures (profiles/r01_v5_README.md); None where no capture exists
-NCU_TRAFFIC = {2: 2.990848e6, 3: 3.282664e9 + 3.159225e9, 4: 2.215608e9 + 3.034042e9, 5: 8.344635e9 + 4.143312e9}
+WORKLOAD = {"1": "BASELINE.json configs[0]: 14 buses x 64 scenarios, FP64 forward",
+            "2": "BASELINE.json configs[1]: 118 buses x 1024 scenarios, FP64 forward",
+            "3": "BASELINE.json configs[2]: 300 buses x 8192 scenarios, FP64 forward + adjoint",
+            "4": "BASELINE.json configs[3]: 2000 buses x 2048 scenarios, FP64 mismatch / FP32 LU",
+            "5": "BASELINE.json configs[4]: 9241 buses x 256 scenarios, FP64 forward + adjoint",
+            "mesh": "higher-fill stand-in (not a BASELINE.json config): 30 x 30 lattice mesh, 900 buses x 512 scenarios, FP64 forward + adjoint"}
+TRAFFIC_TABLE = os.path.join("profiles", "r02_ncu_traffic.csv")
 METRIC = "converged PF solves/sec at batch B per grid size; % of B200 HBM roofline"
 UNIT = "solves/s"
 
@@ -48,8 +55,21 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(cfg_key, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on the full batch of the workload, from the
+    committed capture table (written from `ncu --set full` captures; profiles/r02_README.md names the commands)."""
+    path = os.path.join(ROOT, TRAFFIC_TABLE)
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        for row in csv.DictReader(fh):
+            if row["config"] == str(cfg_key) and row["kernel"] == kernel:
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return None
+
+
 class ClockSampler:
-    """SM clock and throttle reasons sampled through NVML every ~2 ms DURING the timed region (the quantities of the
+    """SM clock and throttle reasons sampled through NVML every ~0.5 ms DURING the timed region (the quantities of the
     nvidia-smi clocks line in B200_PROFILING.md: clocks.sm, clocks.max.sm, clocks_event_reasons.*)."""
 
     def __init__(self, index):
@@ -94,13 +114,26 @@ class ClockSampler:
                 "reasons": [k for k, bit in names.items() if self.reasons & bit], "samples": len(self.sm)}
 
 
-def make_inputs(cfg_id, seed_offset=0):
-    net = S.make_network(cfg_id)
+def make_net(cfg_key):
+    return S.mesh_network(30, 30, kappa=0.3) if cfg_key == "mesh" else S.make_network(int(cfg_key))
+
+
+def net_adjoint(net, cfg_key):
+    return True if cfg_key == "mesh" else net.cfg.adjoint
+
+
+def make_inputs(cfg_key, seed_offset=0):
+    net = make_net(cfg_key)
     ps, qs, vs = S.make_scenarios(net, seed=10_000 + net.extra["s_net"] + 1000 * seed_offset)
     gva = gvm = None
-    if net.cfg.adjoint:
+    if net_adjoint(net, cfg_key):
         gva, gvm = S.make_adjoint_rhs(net)
     return net, ps, qs, vs, gva, gvm
+
+
+def ybus_csr(net):
+    """Harness-side Y_bus CSR of the pi-model branch list (the library takes Y_bus as given)."""
+    return S.ybus_triplets(net.n_bus, net.f, net.t, net.r, net.x, net.b)
 
 
 def algorithmic_bytes(info, iterations, batch, keep, w):
@@ -113,18 +146,31 @@ def algorithmic_bytes(info, iterations, batch, keep, w):
     return b
 
 
-def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
+def roofline_obj(kernel, alg, kern_s, traffic, peak, peak_src):
+    """One kernel's roofline object.  alg = algorithmic bytes per launch, traffic = ncu DRAM bytes per launch or None."""
+    served_on_chip = traffic is not None and traffic < alg
+    moved = traffic if served_on_chip else alg
+    return {"bound": "l2/latency" if served_on_chip else "hbm", "kernel": kernel, "achieved": moved / kern_s / 1e9, "peak": peak,
+            "unit": "GB/s", "frac": moved / kern_s / 1e9 / peak, "traffic": traffic, "algorithmic_bytes_per_launch": alg,
+            "kernel_ms": kern_s * 1e3, "peak_source": peak_src, "traffic_source": TRAFFIC_TABLE if traffic is not None else None,
+            "note": ("ncu DRAM traffic of this launch is below the model bytes (the batch is served from shared memory / L2): achieved = "
+                     "DRAM-moved bytes / kernel time, not an HBM-bound figure") if served_on_chip else
+                    "achieved = model-M0 bytes (DESIGN.md section 8) / kernel time; traffic = ncu dram bytes of one such launch"}
+
+
+def run_ours(cfg_key, steps, warmup, rank, world, e2e=True, clocks=True, mode=0, stages=True):
     import torch
     import paper_2606_07099_b200 as sb
     import torch.distributed as dist
     from paper_2606_07099_b200.sharding import reduce_job
-    net, ps, qs, vs, gva, gvm = make_inputs(cfg_id, seed_offset=rank)
+    net, ps, qs, vs, gva, gvm = make_inputs(cfg_key, seed_offset=rank)
     c = net.cfg
+    adjoint = net_adjoint(net, cfg_key)
     B = c.batch
-    Yh = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+    Yh = ybus_csr(net)
     t0 = time.perf_counter()
     ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=B, precision=c.precision,
-                     keep_factors=c.adjoint, mode=mode, device=torch.cuda.current_device())
+                     keep_factors=adjoint, mode=mode, device=torch.cuda.current_device())
     create_s = time.perf_counter() - t0
     info = ctx.info
     dev = torch.device("cuda", torch.cuda.current_device())
@@ -133,12 +179,12 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
     out = dict(vm=torch.empty((B, net.n_bus), dtype=torch.float64, device=dev), va=torch.empty((B, net.n_bus), dtype=torch.float64, device=dev),
                iterations=torch.empty(B, dtype=torch.int32, device=dev), converged=torch.empty(B, dtype=torch.uint8, device=dev),
                final_norm=torch.empty(B, dtype=torch.float64, device=dev))
-    lam = (torch.empty_like(out["vm"]), torch.empty_like(out["vm"])) if c.adjoint else None
+    lam = (torch.empty_like(out["vm"]), torch.empty_like(out["vm"])) if adjoint else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
 
     def step():
         ctx.solve(dps, dqs, dvs, tol=c.tol, max_it=c.max_it, out=out)
-        if c.adjoint:
+        if adjoint:
             ctx.adjoint(dga, dgm, out=lam)
 
     for _ in range(max(warmup, 3)):
@@ -159,12 +205,10 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
         a.record()
         ctx.solve(dps, dqs, dvs, tol=c.tol, max_it=c.max_it, out=out)
         m.record()
-        if c.adjoint:
+        if adjoint:
             ctx.adjoint(dga, dgm, out=lam)
         b.record()
     torch.cuda.synchronize()
-    if sampler:
-        sampler.__exit__()
     launches = ctx.launch_count() - l0
     if world > 1:
         dist.barrier()
@@ -174,20 +218,40 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
     conv = int(out["converged"].sum().item())
     secs, conv_all, solves_all = reduce_job(sum(step_ms) / 1e3, conv * steps, B * steps, device=dev)
     w = 4 if c.precision == 1 else 8
-    alg = algorithmic_bytes(info, its, B, c.adjoint, w)
+    alg = algorithmic_bytes(info, its, B, adjoint, w)
     peak, peak_src = peaks()
     kern_s = float(np.mean(solve_ms)) / 1e3
+    fused_name = "k_nr_fused" if mode == 0 else "staged"
+    roof = roofline_obj("k_nr_fused (one launch = the whole NR loop of the batch)" if mode == 0 else
+                        "staged: k_st_mismatch_fill + k_st_factor_solve per iteration (time = whole sable_solve)",
+                        alg, kern_s, ncu_traffic(cfg_key, fused_name) if mode == 0 else None, peak, peak_src)
     res = {"value": conv_all / secs, "ms_per_step": 1e3 * secs / steps, "converged": conv, "batch": B,
            "iterations_hist": np.bincount(its).tolist(), "solve_ms": float(np.mean(solve_ms)),
-           "adjoint_ms": float(np.mean(step_ms) - np.mean(solve_ms)) if c.adjoint else None,
-           "roofline": {"bound": "hbm", "kernel": "k_nr_fused (one launch = the whole NR loop of the batch)" if mode == 0 else "staged: k_st_mismatch_fill + k_st_factor_solve per iteration (time = whole sable_solve)",
-                        "achieved": alg / kern_s / 1e9, "peak": peak, "unit": "GB/s", "frac": alg / kern_s / 1e9 / peak,
-                        "traffic": NCU_TRAFFIC.get(cfg_id) if mode == 0 else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
-                        "note": "achieved = model-M0 bytes (DESIGN.md section 8) / kernel time; traffic = ncu dram bytes of one such "
-                                "launch (profiles/r01_v5_README.md); configs 1-2 run on chip, so their traffic is far below M0"},
-           "launches": launches, "create_s": create_s, "info": {k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level",
-                                                                                   "placement", "threads", "smem_bytes", "front_k", "bytes_iter_m0")},
-           "clocks": sampler.summary() if sampler else None}
+           "adjoint_ms": float(np.mean(step_ms) - np.mean(solve_ms)) if adjoint else None,
+           "roofline": roof, "launches": launches, "create_s": create_s,
+           "info": dict({k: info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level", "placement", "threads", "slots_per_cta", "ctas_per_sm",
+                                              "smem_bytes", "front_k", "bytes_iter_m0", "bytes_adjoint_m0")},
+                        fill=info["nnz_lu"] / info["nnz_j"])}
+    if adjoint:
+        adj_s = max(res["adjoint_ms"], 1e-6) / 1e3
+        res["roofline_adjoint"] = roofline_obj("k_linsolve (transposed sweeps on the kept factors)",
+                                               info["bytes_adjoint_m0"] * B + 4 * 8 * info["n_bus"] * B, adj_s,
+                                               ncu_traffic(cfg_key, "k_linsolve"), peak, peak_src)
+    # per-stage figures in the default (group-interleaved) layout: the fused kernel's own stage routines launched one
+    # stage per kernel on the state the last solve left (sable_debug_stage_times; outside the timed region)
+    if stages and mode == 0 and hasattr(ctx, "stage_times"):
+        try:
+            st = ctx.stage_times(dps, dqs, dvs, reps=5)
+            nJ, nLU, nB, n = info["nnz_j"], info["nnz_lu"], info["n_bus"], info["n"]
+            b_fill = (8 * nJ if w == 8 else 4 * nJ) + 8 * (6 * nB + n) + 8 * 4 * nB       # a1 + a2: state, spec, F, J values written
+            b_fact = w * nJ + 2 * w * nLU + 8 * (3 * n)                                       # a4 + a5: J read, LU written, LU read, rhs/state
+            res["stages"] = {"mismatch_fill_ms": st["mismatch_fill_ms"], "factor_solve_ms": st["factor_solve_ms"],
+                             "mismatch_fill_frac": b_fill * B / (st["mismatch_fill_ms"] / 1e3) / 1e9 / peak,
+                             "factor_solve_frac": b_fact * B / (st["factor_solve_ms"] / 1e3) / 1e9 / peak,
+                             "bytes_mismatch_fill": b_fill * B, "bytes_factor_solve": b_fact * B,
+                             "note": "one iteration of the whole batch, every scenario active; model-M0 bytes of the stage / its CUDA-event time / peak"}
+        except Exception as exc:   # the export is a debug surface: its absence must not void the bench line
+            res["stages"] = {"error": str(exc)}
     # the NEXT rows of DESIGN.md section 0 (outside the timed region above; CUDA events, L2 flushed between calls)
     def timed(fn, reps=5):
         ts = []
@@ -200,7 +264,7 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
         return float(np.mean(ts[1:]))
     pq = (torch.empty_like(out["vm"]), torch.empty_like(out["vm"]))
     res["next_rows_ms"] = {"recover": timed(lambda: ctx.recover(out["vm"], out["va"], out=pq))}
-    if c.adjoint:
+    if adjoint:
         res["next_rows_ms"]["layer_backward"] = timed(lambda: ctx.layer_backward(out["vm"], out["va"], dga, dgm, dgm, dga, out=pq))
         res["next_rows_ms"]["adjoint_refined_2_sweeps"] = timed(lambda: ctx.adjoint_refined(out["vm"], out["va"], dga, dgm, sweeps=2, out=lam))
     if e2e:
@@ -208,11 +272,11 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
         hps, hqs, hvs, hga, hgm = pin(ps), pin(qs), pin(vs), pin(gva), pin(gvm)
         hout = dict(vm=pin(np.empty((B, net.n_bus))), va=pin(np.empty((B, net.n_bus))), iterations=pin(np.empty(B, np.int32)),
                     converged=pin(np.empty(B, np.uint8)), final_norm=pin(np.empty(B)))
-        hlam = (pin(np.empty((B, net.n_bus))), pin(np.empty((B, net.n_bus)))) if c.adjoint else None
+        hlam = (pin(np.empty((B, net.n_bus))), pin(np.empty((B, net.n_bus)))) if adjoint else None
 
         def estep():
             ctx.solve_host(hps, hqs, hvs, tol=c.tol, max_it=c.max_it, out=hout)
-            if c.adjoint:
+            if adjoint:
                 ctx.adjoint_host(hga, hgm, out=hlam)
         for _ in range(3):
             estep()
@@ -227,18 +291,25 @@ def run_ours(cfg_id, steps, warmup, rank, world, e2e=True, clocks=True, mode=0):
         econv = int(hout["converged"].sum())
         es, econv_all, _ = reduce_job(es, econv * steps, B * steps, device=dev)
         nb8 = B * net.n_bus * 8
-        res["e2e"] = {"value": econv_all / es, "unit": UNIT, "h2d_bytes_per_step": (3 + (2 if c.adjoint else 0)) * nb8,
-                      "d2h_bytes_per_step": (2 + (2 if c.adjoint else 0)) * nb8 + B * 13}
+        res["e2e"] = {"value": econv_all / es, "unit": UNIT, "ms_per_step": 1e3 * es / steps,
+                      "h2d_bytes_per_step": (3 + (2 if adjoint else 0)) * nb8,
+                      "d2h_bytes_per_step": (2 + (2 if adjoint else 0)) * nb8 + B * 13}
+    if sampler:
+        sampler.__exit__()
+        res["clocks"] = sampler.summary()
+    else:
+        res["clocks"] = None
     ctx.close()
     return res, (net, ps, qs, vs, gva, gvm)
 
 
-def run_oracle(cfg_id, inputs=None, budget_s=12.0):
-    """The oracle as it stands on the host cores, on a bounded sample of the workload: the first m scenarios, passed
-    over `reps` times when one pass is shorter than the budget (about 10-30 s of CPU work in total)."""
+def run_oracle(cfg_key, inputs=None, budget_s=12.0):
+    """The oracle as it stands (never tuned for this) on the host cores, on a bounded sample of the workload: the first m
+    scenarios, passed over `reps` times when one pass is shorter than the budget (about 10-30 s of CPU work in total)."""
     import oracle
-    net, ps, qs, vs, gva, gvm = inputs or make_inputs(cfg_id)
+    net, ps, qs, vs, gva, gvm = inputs or make_inputs(cfg_key)
     c = net.cfg
+    adjoint = net_adjoint(net, cfg_key)
     Y = oracle.ybus(net.n_bus, net.f, net.t, net.r, net.x, net.b)
     cores = os.cpu_count() or 1
     probe = min(c.batch, cores)
@@ -251,14 +322,15 @@ def run_oracle(cfg_id, inputs=None, budget_s=12.0):
     t0 = time.perf_counter()
     for _ in range(reps):
         r = oracle.nr_batch(Y, net.bus_type, ps[:m], qs[:m], vs[:m], tol=c.tol, max_it=c.max_it, method=1)
-        if c.adjoint:
+        if adjoint:
             oracle.adjoint_batch(Y, net.bus_type, r["vm"], r["va"], gva[:m], gvm[:m], method=1)
         conv += int(r["converged"].sum())
         threads = int(r["threads"])
     dt = time.perf_counter() - t0
     return {"value": conv / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "tuned": False, "what": "unoptimised textbook oracle (plain C, FP64, sparse row elimination with partial pivoting): a reported baseline, not a tuned CPU solver",
             "sample": f"first {m} of {c.batch} scenarios of the same workload x {reps} passes, FP64 sparse-LU oracle"
-                      f"{' + adjoint' if c.adjoint else ''}, {dt:.2f} s wall on {threads} threads"}, dt / reps, m
+                      f"{' + adjoint' if adjoint else ''}, {dt:.2f} s wall on {threads} threads"}, dt / reps, m
 
 
 def paper_sweep(reps=7):
@@ -266,22 +338,17 @@ def paper_sweep(reps=7):
     Table II (other hardware, other networks: context only).  The paper's case files are not
     available and are not reconstructed: the stand-ins are drawn by sable_synth's recipe with
     +-10 % i.i.d. load perturbation per scenario and load (eq. 20).  Network seed: the first of 1..8 on which
-    the library converges >= 99 % of 64 scenarios from the flat start."""
+    the library converges >= 99 % of 64 scenarios from the flat start.  (Parity of the stand-ins against the oracle:
+    tests/test_gpu_parity.py::test_paper_standins.)"""
     import torch
     import paper_2606_07099_b200 as sb
     out = {}
     dev = torch.device("cuda", torch.cuda.current_device())
     for nb in (1354, 3120, 9241, 25000):
-        big = nb > 5000
-        base = dict(n_bus=nb, n_pv=int(round(0.18 * nb)), n_branch=int(round(1.6 * nb)),
-                    r_range=(0.0005, 0.02) if big else (0.001, 0.03), x_ratio=(4.0, 12.0) if big else (4.0, 10.0),
-                    b_range=(0.0, 0.06), load=("lognormal", float(np.log(0.05 if big else 0.1)), 0.8 if big else 0.7),
-                    q_ratio=(0.2, 0.5), gen_share=0.7, vset_range=(0.98, 1.05), slack_vm=1.0, scale_range=(0.9, 1.1),
-                    scale_per_bus=True, batch=256, max_it=30)
         chosen = None
         for seed in range(1, 9):
-            net = S.make_network(S.GridConfig(name=f"standin{nb}", s_net=seed, **base), s_net=seed, kappa=1.0)
-            Yh = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+            net = S.make_network(S.standin_config(nb), s_net=seed, kappa=1.0)
+            Yh = ybus_csr(net)
             ps, qs, vs = S.make_scenarios(net, batch=256)
             d = lambda a: torch.from_numpy(a).to(dev)
             ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=256, keep_factors=False, device=dev.index)
@@ -317,14 +384,23 @@ def paper_sweep(reps=7):
     return out
 
 
+def config_obj(cfg_key, net, world, mode):
+    cfg = net.cfg
+    return {"workload": WORKLOAD[cfg_key], "name": cfg.name, "batch_per_gpu": cfg.batch, "tol": cfg.tol,
+            "max_it": cfg.max_it, "precision": "fp64 mismatch + fp32 LU" if cfg.precision else "fp64",
+            "adjoint": net_adjoint(net, cfg_key), "network_seed": cfg.s_net, "load_scale_kappa": cfg.kappa,
+            "parallelism": f"scenario sharding x{world}, no collective", "launch_mode": mode, "cache": "L2 flushed between steps (256 MiB memset)"}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", default="5", choices=["1", "2", "3", "4", "5", "mesh"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--sweep-steps", type=int, default=20)
     ap.add_argument("--paper-sweep", action="store_true", help="batch 4..256 on paper-sized stand-in grids (context for Table II); prints its own JSON")
     ap.add_argument("--mode", default="fused", choices=["fused", "staged"],
                     help="staged = one kernel per stage (mismatch+fill / refactor+solve), state in HBM between: per-stage profiling")
@@ -332,11 +408,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    cfg = S.CONFIGS[a.config]
-    config = {"workload": WORKLOAD[a.config], "name": cfg.name, "batch_per_gpu": cfg.batch, "tol": cfg.tol,
-              "max_it": cfg.max_it, "precision": "fp64 mismatch + fp32 LU" if cfg.precision else "fp64",
-              "adjoint": cfg.adjoint, "network_seed": cfg.s_net, "load_scale_kappa": cfg.kappa,
-              "parallelism": f"scenario sharding x{world}, no collective", "launch_mode": a.mode, "cache": "L2 flushed between steps (256 MiB memset)"}
+    net0 = make_net(a.config)
+    cfg = net0.cfg
+    config = config_obj(a.config, net0, world, a.mode)
 
     if a.impl == "reference":
         if rank != 0:
@@ -374,18 +448,20 @@ def main():
             "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if not cfg.precision else "f64+f32", "data": "synthetic", "config": config,
             "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["launches"], "roofline": res["roofline"],
+            "roofline_adjoint": res.get("roofline_adjoint"), "stages": res.get("stages"),
             "converged": res["converged"], "iterations_hist": res["iterations_hist"], "solve_ms": res["solve_ms"],
             "adjoint_ms": res["adjoint_ms"], "next_rows_ms": res["next_rows_ms"], "create_s": res["create_s"], "info": res["info"]}
     if rank == 0 and world == 1:
         line["cpu_baseline"], _, _ = run_oracle(a.config, inputs)
         if not a.no_sweep:
             per = {}
-            for k in (1, 2, 3, 4, 5):
-                r, _ = run_ours(k, 5, 3, 0, 1, e2e=False, clocks=False)
-                per[S.CONFIGS[k].name] = {"solves_per_s": r["value"], "ms_per_step": r["ms_per_step"], "solve_ms": r["solve_ms"],
-                                          "adjoint_ms": r["adjoint_ms"], "converged": r["converged"], "batch": r["batch"],
-                                          "iterations_hist": r["iterations_hist"], "roofline_frac": r["roofline"]["frac"],
-                                          "achieved_gbs": r["roofline"]["achieved"], "next_rows_ms": r["next_rows_ms"], "info": r["info"]}
+            for k in ("1", "2", "3", "4", "5", "mesh"):
+                r, _ = run_ours(k, max(a.sweep_steps, 20), 3, 0, 1)
+                per[WORKLOAD[k].split(":")[0] if k != "mesh" else "mesh30x30"] = {
+                    "workload": WORKLOAD[k], "solves_per_s": r["value"], "ms_per_step": r["ms_per_step"], "solve_ms": r["solve_ms"],
+                    "adjoint_ms": r["adjoint_ms"], "converged": r["converged"], "batch": r["batch"], "steps": max(a.sweep_steps, 20),
+                    "iterations_hist": r["iterations_hist"], "roofline": r["roofline"], "roofline_adjoint": r.get("roofline_adjoint"),
+                    "stages": r.get("stages"), "e2e": r["e2e"], "clocks": r["clocks"], "next_rows_ms": r["next_rows_ms"], "info": r["info"]}
             line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))

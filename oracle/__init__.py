@@ -244,3 +244,55 @@ def layer_backward(Y, bus_type, vm, va, gl_pg, gl_qg, gl_vm, gl_va):
     J3T_lam = dP_dvm[ns].T @ lam_p[ns] + dQ_dvm[pqi].T @ lam_q[pqi]
     dx_vm = np.where(gen, g_vm - J3T_lam, 0.0)
     return dx_pg, dx_vm
+
+
+def full_jacobians_sparse(Y, vm, va):
+    """The same complex-matrix identities as full_jacobians, as scipy.sparse matrices (for grids where the dense
+    n_bus x n_bus form does not fit): dS/dtheta = j diag(V) conj(diag(I) - Y diag(V)),
+    dS/dVm = diag(V) conj(Y diag(V/|V|)) + conj(diag(I)) diag(V/|V|)."""
+    import scipy.sparse as sp
+    row_ptr, col, g, bb = Y
+    nb = vm.shape[0]
+    Ys = sp.csr_matrix((g + 1j * bb, col, row_ptr), shape=(nb, nb))
+    V = vm * np.exp(1j * va)
+    I = Ys @ V
+    E = V / np.abs(V)
+    dg = lambda v: sp.diags(v, format="csr")
+    dS_dth = (1j * dg(V) @ (dg(I) - Ys @ dg(V)).conj()).tocsr()
+    dS_dvm = (dg(V) @ (Ys @ dg(E)).conj() + dg(np.conj(I)) @ dg(E)).tocsr()
+    return dS_dth, dS_dvm
+
+
+def layer_backward_sparse(Y, bus_type, vm, va, gl_pg, gl_qg, gl_vm, gl_va):
+    """layer_backward (eqs. 10-16) restated line by line on scipy.sparse matrices, with the adjoint system of
+    eq. (14) solved by scipy's SuperLU; for grids where the dense form is too large.  Pinned against the dense form on
+    configs 1-3 and by finite differences of the whole layer on config 4 (tests/test_oracle_layer.py)."""
+    import scipy.sparse as sp
+    import scipy.sparse.linalg as spla
+    bus_type = np.asarray(bus_type)
+    nb = vm.shape[0]
+    pq = bus_type == 0
+    pv = bus_type == 1
+    sl = bus_type == 2
+    nonslack = ~sl
+    gen = pv | sl
+    dS_dth, dS_dvm = full_jacobians_sparse(Y, vm, va)
+    dP_dth, dQ_dth, dP_dvm, dQ_dvm = dS_dth.real.tocsr(), dS_dth.imag.tocsr(), dS_dvm.real.tocsr(), dS_dvm.imag.tocsr()
+    sli, geni = np.flatnonzero(sl), np.flatnonzero(gen)
+    ns, pqi = np.flatnonzero(nonslack), np.flatnonzero(pq)
+    # eq. (11)-(12)
+    v2_th = dP_dth[sli].T @ gl_pg[sli] + dQ_dth[geni].T @ gl_qg[geni]
+    v2_vm = dP_dvm[sli].T @ gl_pg[sli] + dQ_dvm[geni].T @ gl_qg[geni]
+    # eq. (13)
+    g_th = np.where(nonslack, gl_va + v2_th, 0.0)
+    g_vm = gl_vm + v2_vm
+    # eq. (14)
+    J1 = sp.bmat([[dP_dth[ns][:, ns], dP_dvm[ns][:, pqi]], [dQ_dth[pqi][:, ns], dQ_dvm[pqi][:, pqi]]], format="csc")
+    lam = spla.splu(J1.T.tocsc()).solve(np.concatenate([g_th[ns], g_vm[pqi]]))
+    lam_p = np.zeros(nb); lam_q = np.zeros(nb)
+    lam_p[ns] = lam[: len(ns)]; lam_q[pqi] = lam[len(ns):]
+    # eq. (15)-(16)
+    dx_pg = np.where(pv, gl_pg + lam_p, 0.0)
+    J3T_lam = dP_dvm[ns].T @ lam_p[ns] + dQ_dvm[pqi].T @ lam_q[pqi]
+    dx_vm = np.where(gen, g_vm - J3T_lam, 0.0)
+    return dx_pg, dx_vm

@@ -273,19 +273,3 @@ class Context:
 
 def sable_create(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt) -> Context:
     return Context(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt)
-
-
-def ybus_from_branches(n_bus, f, t, r, x, b):
-    """Harness-side Y_bus CSR (pi-model; the paper takes Y_bus as given) -- unsorted triplets with
-    duplicates, which sable_create canonicalises.  Returns (row_ptr, col, G, B)."""
-    f = np.asarray(f, np.int64); t = np.asarray(t, np.int64)
-    y = 1.0 / (np.asarray(r, float) + 1j * np.asarray(x, float))
-    sh = 0.5j * np.asarray(b, float)
-    rows = np.concatenate([f, t, f, t]); cols = np.concatenate([f, t, t, f])
-    vals = np.concatenate([y + sh, y + sh, -y, -y])
-    order = np.argsort(rows, kind="stable")
-    rows, cols, vals = rows[order], cols[order], vals[order]
-    row_ptr = np.zeros(n_bus + 1, np.int64)
-    np.add.at(row_ptr, rows + 1, 1)
-    row_ptr = np.cumsum(row_ptr).astype(np.int32)
-    return row_ptr, cols.astype(np.int32), np.ascontiguousarray(vals.real), np.ascontiguousarray(vals.imag)

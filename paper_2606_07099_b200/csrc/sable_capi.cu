@@ -41,10 +41,21 @@ struct sable_ctx {
     double* hbuf = nullptr; int32_t* hbuf_it = nullptr; uint8_t* hbuf_cv = nullptr;
 };
 
-static std::string g_create_err;
+static thread_local std::string g_create_err;   // message of the last failed sable_create on this host thread
 
 static sable_status fail(sable_ctx* c, sable_status s, const std::string& m) { if (c) c->err = m; else g_create_err = m; return s; }
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, e_ == cudaErrorMemoryAllocation ? SABLE_ERR_ALLOC : SABLE_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+
+// the library switches to the context's device for the duration of a call and restores the caller's device on return
+struct DeviceGuard {
+    int prev = -1; cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != dev) err = cudaSetDevice(dev); else if (err == cudaSuccess) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE(ctx) DeviceGuard guard_((ctx)->opt.device); CU(guard_.err)
 
 template <typename V>
 static cudaError_t upload(sable_ctx* c, const std::vector<V>& h, const V** out) {
@@ -460,6 +471,9 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
         const int G = 1 << c->gsh;
         const int grid = std::min((A.batch + G - 1) / G, c->grid);
         c->factor_gsh = c->gsh;
+        // the attribute is per-function state shared by every live context: set it for THIS context right before the launch
+        e = cudaFuncSetAttribute(fused_fn(sizeof(T) == 4, c->placement, c->threads <= 128), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem);
+        if (e != cudaSuccess) return e;
         if (c->placement == 0) k_nr_fused<T, 0, false><<<grid, c->threads, c->smem, s>>>(A);
         else if (c->placement == 1) k_nr_fused<T, 1, false><<<grid, c->threads, c->smem, s>>>(A);
         else if (c->threads <= 128) k_nr_fused<T, 2, true><<<grid, c->threads, c->smem, s>>>(A);
@@ -490,7 +504,7 @@ extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double*
     if (batch == 0) return SABLE_OK;                       /* empty batch: nothing is read or written */
     if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
         return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     SolveArgs A{};
     A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.tol = tol;
     A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
@@ -534,7 +548,7 @@ extern "C" sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const doubl
     if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
     if (!g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (batch == 0) return SABLE_OK;
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     return launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, (cudaStream_t)cuda_stream);
 }
 
@@ -546,7 +560,7 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
     if (batch == 0) return SABLE_OK;
     if (!vm || !va || !p_inj || !q_inj) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     RecoverArgs R{};
     R.n_bus = ctx->T.n_bus; R.batch = batch; R.fptr = ctx->fptr; R.fcol = ctx->fcol; R.fgb = ctx->fgb;
     R.vm = vm; R.va = va; R.p_inj = p_inj; R.q_inj = q_inj; R.work = ctx->work; R.work_stride = ctx->work_stride;
@@ -570,7 +584,7 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
     if (!vm || !va || !gl_pg || !gl_qg || !gl_vm || !gl_va || !dx_pg || !dx_vm) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (batch == 0) return SABLE_OK;
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus;
     LayerArgs L{};
@@ -605,7 +619,7 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
     if (!vm || !va || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (sweeps < 0 || sweeps > 16) return fail(ctx, SABLE_ERR_INVALID_ARG, "sweeps out of range [0, 16]");
     if (batch == 0) return SABLE_OK;
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     sable_status st = launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, s);
     if (st != SABLE_OK || sweeps == 0) return st;
@@ -641,7 +655,7 @@ extern "C" sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const do
     if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
         return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (batch == 0) { ctx->have_factors = false; ctx->last_batch = 0; return SABLE_OK; }
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
     double* d = ctx->hbuf;       // slots: 0 p, 1 q, 2 vset, 3 vm0, 4 va0, 5 vm, 6 va, (7, 8 adjoint), then norm
     double* dn = ctx->hbuf + 9 * (size_t)ctx->opt.max_batch * ctx->T.n_bus;
@@ -667,7 +681,7 @@ extern "C" sable_status sable_adjoint_host(sable_ctx* ctx, int32_t batch, const 
     if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
     if (batch < 0 || batch > ctx->opt.max_batch || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "bad argument");
     if (batch == 0) return SABLE_OK;
-    CU(cudaSetDevice(ctx->opt.device));
+    ON_DEVICE(ctx);
     const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
     double* d = ctx->hbuf;
     CU(cudaMemcpyAsync(d, g_va, bytes, cudaMemcpyHostToDevice, 0));
@@ -716,7 +730,6 @@ static sable_status debug_check(sable_ctx* ctx, int batch) {
     if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
     if (batch < 1 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
     ctx->have_factors = false;
-    CU(cudaSetDevice(ctx->opt.device));
     return SABLE_OK;
 }
 
@@ -724,6 +737,7 @@ extern "C" sable_status sable_debug_mismatch(sable_ctx* ctx, int32_t batch, cons
                                              const double* vm, const double* va, double* f_p, double* f_q, double* norm,
                                              void* cuda_stream) {
     sable_status st = debug_check(ctx, batch); if (st) return st;
+    ON_DEVICE(ctx);
     if (!p_spec || !q_spec || !vm || !va || !f_p || !f_q || !norm) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     DebugArgs D{}; D.batch = batch; D.what = 0; D.p_spec = p_spec; D.q_spec = q_spec; D.vm = vm; D.va = va; D.f_p = f_p; D.f_q = f_q; D.norm = norm;
     return launch_debug(ctx, D, (cudaStream_t)cuda_stream);
@@ -732,6 +746,7 @@ extern "C" sable_status sable_debug_mismatch(sable_ctx* ctx, int32_t batch, cons
 extern "C" sable_status sable_debug_jacobian(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* diag,
                                              double* pairs, void* cuda_stream) {
     sable_status st = debug_check(ctx, batch); if (st) return st;
+    ON_DEVICE(ctx);
     if (!vm || !va || !diag || !pairs) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     DebugArgs D{}; D.batch = batch; D.what = 1; D.vm = vm; D.va = va; D.diag = diag; D.pairs = pairs;
     return launch_debug(ctx, D, (cudaStream_t)cuda_stream);
@@ -741,6 +756,7 @@ extern "C" sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, 
                                                  const double* rhs_p, const double* rhs_q, int32_t transpose, double* x_p,
                                                  double* x_q, void* cuda_stream) {
     sable_status st = debug_check(ctx, batch); if (st) return st;
+    ON_DEVICE(ctx);
     if (!vm || !va || !rhs_p || !rhs_q || !x_p || !x_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     DebugArgs D{}; D.batch = batch; D.what = 2; D.vm = vm; D.va = va;
     st = launch_debug(ctx, D, (cudaStream_t)cuda_stream); if (st) return st;

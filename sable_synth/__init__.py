@@ -234,3 +234,104 @@ def tiny_network(n_bus: int, n_extra: int, n_pv: int, seed: int, load=(0.05, 0.3
                      (0.0, 0.05), ("uniform", load[0], load[1]), (0.2, 0.5), 0.6 if n_pv else 0.0,
                      (1.00, 1.06), 1.04, (0.9, 1.1), True, 8, 20)
     return make_network(cfg, s_net=seed, kappa=1.0)
+
+
+def standin_config(n_bus: int, batch: int = 256) -> GridConfig:
+    """Paper-shaped stand-ins: synthetic grids of the sizes of the paper's cases
+    (1 354 / 3 120 / 9 241 / 25 000 buses) drawn by the recipe above with +-10 % i.i.d. load
+    perturbation per scenario and load (eq. 20).  Nothing of the pandapower case files is reproduced."""
+    big = n_bus > 5000
+    return GridConfig(name=f"standin{n_bus}", n_bus=n_bus, n_pv=int(round(0.18 * n_bus)), n_branch=int(round(1.6 * n_bus)),
+                      r_range=(0.0005, 0.02) if big else (0.001, 0.03), x_ratio=(4.0, 12.0) if big else (4.0, 10.0),
+                      b_range=(0.0, 0.06), load=("lognormal", float(np.log(0.05 if big else 0.1)), 0.8 if big else 0.7),
+                      q_ratio=(0.2, 0.5), gen_share=0.7, vset_range=(0.98, 1.05), slack_vm=1.0, scale_range=(0.9, 1.1),
+                      scale_per_bus=True, batch=batch, max_it=30)
+
+
+def mesh_network(nx: int, ny: int, seed: int = 1, kappa: float = 0.3, n_pv_frac: float = 0.15, batch: int = 512) -> Network:
+    """Higher-fill stand-in: an nx x ny lattice (every bus joined to its right and lower neighbour) with a fraction of
+    the lattice edges removed at random while keeping the graph connected, plus a few diagonal ties.  Minimum-degree
+    fill on such meshes is 2-4x nnz(J1) (transmission grids sit between this and the tree-like configs 1-5), so the
+    launch policy is exercised away from its low-fill tuning points.  Same impedance / load recipe as config 4;
+    `kappa` scales the loads so that the flat start converges (meshes of long lines are weak)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = nx * ny
+    idx = lambda i, j: i * ny + j
+    edges = []
+    for i in range(nx):
+        for j in range(ny):
+            if j + 1 < ny:
+                edges.append((idx(i, j), idx(i, j + 1)))
+            if i + 1 < nx:
+                edges.append((idx(i, j), idx(i + 1, j)))
+    edges = [edges[k] for k in rng.permutation(len(edges))]
+    # spanning tree first (union-find), then 70 % of the remaining lattice edges, then n/20 diagonal ties
+    root = list(range(n))
+
+    def find(a):
+        while root[a] != a:
+            root[a] = root[root[a]]
+            a = root[a]
+        return a
+    tree, rest = [], []
+    for a, b in edges:
+        ra, rb = find(a), find(b)
+        if ra != rb:
+            root[ra] = rb
+            tree.append((a, b))
+        else:
+            rest.append((a, b))
+    keep = tree + rest[: int(0.7 * len(rest))]
+    have = set((min(a, b), max(a, b)) for a, b in keep)
+    for _ in range(n // 20):
+        i, j = int(rng.integers(0, nx - 1)), int(rng.integers(0, ny - 1))
+        e = (idx(i, j), idx(i + 1, j + 1))
+        if e not in have:
+            have.add(e)
+            keep.append(e)
+    n_pv = int(round(n_pv_frac * n))
+    cfg = GridConfig(name=f"mesh{nx}x{ny}", n_bus=n, n_pv=n_pv, n_branch=len(keep), r_range=(0.001, 0.03), x_ratio=(4.0, 10.0),
+                     b_range=(0.0, 0.08), load=("lognormal", float(np.log(0.1)), 0.7), q_ratio=(0.2, 0.5), gen_share=0.7,
+                     vset_range=(0.98, 1.05), slack_vm=1.0, scale_range=(0.9, 1.1), scale_per_bus=True, batch=batch, max_it=20,
+                     s_net=seed, kappa=kappa)
+    f = np.array([e[0] for e in keep], dtype=np.int64)
+    t = np.array([e[1] for e in keep], dtype=np.int64)
+    nb = f.shape[0]
+    r = rng.uniform(cfg.r_range[0], cfg.r_range[1], nb)
+    x = r * rng.uniform(cfg.x_ratio[0], cfg.x_ratio[1], nb)
+    b = rng.uniform(cfg.b_range[0], cfg.b_range[1], nb)
+    bus_type = np.zeros(n, dtype=np.uint8)
+    slack = idx(nx // 2, ny // 2)
+    bus_type[slack] = SLACK
+    others = np.array([i for i in range(n) if i != slack])
+    pv = rng.choice(others, size=n_pv, replace=False)
+    bus_type[pv] = PV
+    v_set = np.ones(n)
+    v_set[np.sort(pv)] = rng.uniform(cfg.vset_range[0], cfg.vset_range[1], n_pv)
+    pq = np.flatnonzero(bus_type == PQ)
+    pl = rng.lognormal(cfg.load[1], cfg.load[2], pq.shape[0])
+    ql = pl * rng.uniform(cfg.q_ratio[0], cfg.q_ratio[1], pq.shape[0])
+    p_load = np.zeros(n); q_load = np.zeros(n)
+    p_load[pq] = kappa * pl; q_load[pq] = kappa * ql
+    w = rng.uniform(0.5, 1.5, n_pv)
+    p_gen = np.zeros(n)
+    p_gen[np.sort(pv)] = cfg.gen_share * p_load.sum() * w / w.sum()
+    return Network(cfg, n, f.astype(np.int32), t.astype(np.int32), r, x, b, bus_type, int(slack), v_set, p_load, q_load, p_gen,
+                   {"s_net": seed, "kappa": kappa})
+
+
+def ybus_triplets(n_bus, f, t, r, x, b):
+    """Harness-side input preparation for the CUDA library only (the oracle assembles its own Y_bus in C and never calls
+    this): the pi-model branch list as Y_bus CSR triplets -- unsorted, with duplicates, which sable_create canonicalises.
+    The paper takes Y_bus as given.  Returns (row_ptr, col, G, B)."""
+    f = np.asarray(f, np.int64); t = np.asarray(t, np.int64)
+    y = 1.0 / (np.asarray(r, float) + 1j * np.asarray(x, float))
+    sh = 0.5j * np.asarray(b, float)
+    rows = np.concatenate([f, t, f, t]); cols = np.concatenate([f, t, t, f])
+    vals = np.concatenate([y + sh, y + sh, -y, -y])
+    order = np.argsort(rows, kind="stable")
+    rows, cols, vals = rows[order], cols[order], vals[order]
+    row_ptr = np.zeros(n_bus + 1, np.int64)
+    np.add.at(row_ptr, rows + 1, 1)
+    row_ptr = np.cumsum(row_ptr).astype(np.int32)
+    return row_ptr, cols.astype(np.int32), np.ascontiguousarray(vals.real), np.ascontiguousarray(vals.imag)

@@ -12,7 +12,7 @@ import pytest
 
 import oracle
 import sable_synth as S
-from util import dev, gpu_jacobian_dense, make_ctx, oracle_Y, random_state
+from util import dev, gpu_jacobian_coo, gpu_jacobian_dense, make_ctx, oracle_Y, random_state
 
 torch = pytest.importorskip("torch")
 pytestmark = [pytest.mark.gpu, pytest.mark.timeout(240)]
@@ -117,6 +117,37 @@ def test_jacobian_fill_kernel(cfg, batch):
     ctx.close()
 
 
+def test_jacobian_fill_kernel_cfg5_sparse():
+    """Config 5 (n = 17 036): entry-by-entry through COO triplets (the dense form would need 2.3 GB)."""
+    import scipy.sparse as sp
+    net, Y = get_net(5)
+    batch = 2
+    vm, va = random_state(net, batch, 177 + 5)
+    ctx = make_ctx(net, max_batch=batch)
+    diag, pairs = ctx.debug_jacobian(dev(vm), dev(va))
+    diag, pairs = diag.cpu().numpy(), pairs.cpu().numpy()
+    sc = row_scale(Y, vm)
+    n, th, vmx = oracle.index_maps(net.bus_type)
+    rs = np.zeros((batch, n))
+    for i in range(net.n_bus):
+        if th[i] >= 0:
+            rs[:, th[i]] = sc[:, i]
+        if vmx[i] >= 0:
+            rs[:, vmx[i]] = sc[:, i]
+    for b in range(batch):
+        gr, gc, gv, pad_ok = gpu_jacobian_coo(ctx, net, diag[b], pairs[b])
+        assert pad_ok
+        _, jr, jc, jv = oracle.jacobian(Y, net.bus_type, vm[b], va[b])
+        Jg = sp.coo_matrix((gv, (gr, gc)), shape=(n, n)).tocsr()
+        Jo = sp.coo_matrix((jv, (jr, jc)), shape=(n, n)).tocsr()
+        slots = sp.coo_matrix((np.ones_like(gv), (gr, gc)), shape=(n, n)).tocsr()
+        assert (slots[jr, jc] >= 1).all(), "a structural J1 entry has no slot in the template"
+        D = (Jg - Jo).tocoo()                       # fill slots hold exact zeros, so they drop out of the difference
+        assert (np.abs(D.data) <= 1e-13 * np.maximum(rs[b][D.row], 1.0) / 0.9).all(), np.abs(D.data).max()
+        assert Jo.nnz == ctx.info["nnz_j"]
+    ctx.close()
+
+
 # ---- a4 + a5 (+ transposed, a7): one linear solve on the static pattern ---------------------------------------------
 @pytest.mark.parametrize("cfg,batch,precision", [(1, 4, sb.FP64), (2, 3, sb.FP64), (3, 3, sb.FP64), (4, 2, sb.FP64),
                                                  (5, 2, sb.FP64), (2, 3, sb.MIXED), (4, 2, sb.MIXED)])
@@ -156,7 +187,7 @@ def test_refactor_and_triangular_solves(cfg, batch, precision, transpose):
 
 
 # ---- whole path: NR loop with masking, both launch modes ------------------------------------------------------------
-def check_solution(res, ref, tol, v_tol, conv_only=True):
+def check_solution(res, ref, tol, v_tol, conv_only=True, max_edge_frac=None, label=""):
     it, cv = res["iterations"], res["converged"]
     assert np.array_equal(cv, ref["converged"]), "converged flags differ"
     assert (np.abs(it.astype(int) - ref["iterations"].astype(int)) <= 1).all()
@@ -167,10 +198,18 @@ def check_solution(res, ref, tol, v_tol, conv_only=True):
     dva = np.abs(res["va"] - ref["va"]).max(axis=1)
     assert (dvm[same] <= v_tol).all() and (dva[same] <= v_tol).all(), (dvm[same].max(), dva[same].max())
     # a scenario whose mismatch lands within rounding of tol may take one more / one fewer update (DESIGN.md reading
-    # 22): both iterates satisfy ||F|| <= tol; they differ by the size of that last step
+    # 22): both iterates satisfy ||F|| <= tol; they differ by the size of that last step.  Such a scenario is accepted
+    # only if the side that stopped one update earlier did so with a norm within 10 % of tol (i.e. the decision really
+    # was a rounding matter), and each one is listed.
     edge = ok & ~same
-    if edge.any():
-        assert (dvm[edge] <= 1e-7).all() and (dva[edge] <= 1e-7).all()
+    for b in np.flatnonzero(edge):
+        early = res["final_norm"][b] if it[b] < ref["iterations"][b] else ref["final_norm"][b]
+        print(f"{label} borderline scenario {b}: iterations gpu {it[b]} / oracle {ref['iterations'][b]}, accepting norm of the earlier side "
+              f"{early:.6e} (tol {tol:.1e}), |dVm| {dvm[b]:.2e}, |dtheta| {dva[b]:.2e}")
+        assert 0.9 * tol <= early <= tol, (b, early)
+        assert dvm[b] <= 1e-7 and dva[b] <= 1e-7
+    if max_edge_frac is not None:
+        assert edge.sum() <= max_edge_frac * max(1, ok.sum()), (int(edge.sum()), int(ok.sum()))
     return int(same.sum()), int(edge.sum())
 
 
@@ -317,35 +356,115 @@ def test_two_bus_closed_form_on_gpu():
     ctx.close()
 
 
-# ---- full BASELINE.json sizes, in the launch configuration bench.py times (fused, max_batch = batch) -----------------
-@pytest.mark.parametrize("cfg,sample", [(2, 1024), (3, 2048), (4, 256), (5, 24)])
-def test_full_size_sampled_parity(cfg, sample):
+# ---- full BASELINE.json sizes, in the launch configuration bench.py times (fused, max_batch = batch): the WHOLE batch ------
+@pytest.mark.timeout(900)
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_batch_parity(cfg):
+    """Every scenario of the full BASELINE.json batch against the oracle (about 0.1 / 1.5 / 2.5 / 20 s of oracle time on
+    16 threads), forward and (configs 3, 5) adjoint.  Borderline (+-1 iteration) scenarios: at most 1 % of the batch,
+    each listed with its accepting norm (check_solution)."""
     net, Y = get_net(cfg)
     c = net.cfg
     ps, qs, vs = S.make_scenarios(net)
     ctx = make_ctx(net, max_batch=c.batch, precision=c.precision, keep_factors=c.adjoint)
     res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
-    rng = np.random.Generator(np.random.PCG64(99))
-    idx = np.unique(np.concatenate([[0, c.batch - 1], rng.choice(c.batch, size=min(sample, c.batch), replace=False)]))
-    ref = oracle.nr_batch(Y, net.bus_type, ps[idx], qs[idx], vs[idx], tol=c.tol, max_it=c.max_it, method=1)
-    sub = {k: v[idx] for k, v in res.items()}
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
     if c.precision == sb.FP64:
-        check_solution(sub, ref, c.tol, 1e-9)
+        check_solution(res, ref, c.tol, 1e-9, max_edge_frac=0.01, label=f"cfg{cfg}")
     else:
-        assert np.array_equal(sub["converged"], ref["converged"])
-        assert (np.abs(sub["iterations"].astype(int) - ref["iterations"]) <= 1).all()
-        assert np.abs(sub["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(sub["va"] - ref["va"]).max() <= 1e-7
-    # properties that hold at any size: every converged scenario satisfies the tolerance; masking froze nothing early
+        # mixed precision (DESIGN.md section 5): a different Newton sequence accepted at the same FP64 tolerance
+        assert np.array_equal(res["converged"], ref["converged"])
+        assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+        assert np.abs(res["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(res["va"] - ref["va"]).max() <= 1e-7
     assert (res["final_norm"][res["converged"] == 1] <= c.tol).all()
     assert res["converged"].mean() >= 0.99
     if c.adjoint:
         gva, gvm = S.make_adjoint_rhs(net)
         lp, lq = ctx.adjoint(dev(gva), dev(gvm))
-        lp, lq = lp.cpu().numpy()[idx], lq.cpu().numpy()[idx]
-        rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, sub["vm"], sub["va"], gva[idx], gvm[idx], method=1)
+        lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+        rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
         scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
         assert (np.abs(lp - rp).max(axis=1) <= 1e-8 * scale).all()
         assert (np.abs(lq - rq).max(axis=1) <= 1e-8 * scale).all()
+    ctx.close()
+
+
+def test_two_live_contexts():
+    """Two contexts that map to the same kernel instantiation with different shared-memory sizes (the dynamic
+    shared-memory attribute is per-function state): create cfg 2 (83 KB per CTA), create cfg 1 (7 KB), solve on the first."""
+    net2, Y2 = get_net(2)
+    net1, Y1 = get_net(1)
+    a = make_ctx(net2, max_batch=256, keep_factors=False)
+    b = make_ctx(net1, max_batch=64, keep_factors=False)
+    assert a.info["placement"] == 0 and b.info["placement"] == 0 and a.info["smem_bytes"] > 48 * 1024 > b.info["smem_bytes"]
+    ps, qs, vs = S.make_scenarios(net2, batch=256)
+    res = to_np(a.solve(dev(ps), dev(qs), dev(vs), tol=net2.cfg.tol, max_it=net2.cfg.max_it))
+    ref = oracle.nr_batch(Y2, net2.bus_type, ps, qs, vs, tol=net2.cfg.tol, max_it=net2.cfg.max_it, method=1)
+    check_solution(res, ref, net2.cfg.tol, 1e-9)
+    ps, qs, vs = S.make_scenarios(net1, batch=64)
+    res = to_np(b.solve(dev(ps), dev(qs), dev(vs), tol=net1.cfg.tol, max_it=net1.cfg.max_it))
+    ref = oracle.nr_batch(Y1, net1.bus_type, ps, qs, vs, tol=net1.cfg.tol, max_it=net1.cfg.max_it, method=1)
+    check_solution(res, ref, net1.cfg.tol, 1e-9)
+    a.close(); b.close()
+
+
+# ---- grids between / beyond the tuning points of the launch policy -------------------------------------------------------
+@pytest.mark.timeout(900)
+@pytest.mark.parametrize("n_bus", [1354, 3120, 9241, 25000])
+def test_paper_standins(n_bus):
+    """The stand-in grids of bench.py --paper-sweep (paper-sized; drawn by sable_synth, nothing of the case
+    files reproduced): 8 scenarios per grid against the oracle, FP64 and mixed."""
+    chosen = None
+    for seed in range(1, 9):
+        net = S.make_network(S.standin_config(n_bus), s_net=seed, kappa=1.0)
+        ps, qs, vs = S.make_scenarios(net, batch=8)
+        Y = oracle_Y(net)
+        ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=1e-8, max_it=30, method=1)
+        if ref["converged"].all():
+            chosen = (net, Y, ps, qs, vs, ref)
+            break
+    assert chosen is not None, "no stand-in seed in 1..8 converges from the flat start"
+    net, Y, ps, qs, vs, ref = chosen
+    for precision in (sb.FP64, sb.MIXED):
+        ctx = make_ctx(net, max_batch=8, precision=precision, keep_factors=False)
+        res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=1e-8, max_it=30))
+        if precision == sb.FP64:
+            check_solution(res, ref, 1e-8, 1e-9, label=f"standin{n_bus}")
+        else:
+            assert np.array_equal(res["converged"], ref["converged"])
+            assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+            assert (res["final_norm"] <= 1e-8).all()
+            assert np.abs(res["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(res["va"] - ref["va"]).max() <= 1e-7
+        ctx.close()
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+def test_mesh_standin(precision):
+    """Higher-fill stand-in (30 x 30 lattice mesh, LU fill ~3x, 67 elimination levels, 12x the multiply-subtract terms of
+    config 4 per unknown): forward + adjoint against the oracle."""
+    net = S.mesh_network(30, 30, kappa=0.3)
+    Y = oracle_Y(net)
+    batch = 48
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    mixed = precision == "mixed"
+    ctx = make_ctx(net, max_batch=batch, precision=sb.MIXED if mixed else sb.FP64, keep_factors=True)
+    assert ctx.info["nnz_lu"] >= 2.5 * ctx.info["nnz_j"]
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=1e-8, max_it=20))
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=1e-8, max_it=20, method=1)
+    if mixed:
+        assert np.array_equal(res["converged"], ref["converged"]) and ref["converged"].all()
+        assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+        assert np.abs(res["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(res["va"] - ref["va"]).max() <= 1e-7
+    else:
+        check_solution(res, ref, 1e-8, 1e-9, label="mesh")
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    tol = 5e-4 if mixed else 1e-8
+    assert (np.abs(lp - rp).max(axis=1) <= tol * scale).all() and (np.abs(lq - rq).max(axis=1) <= tol * scale).all()
     ctx.close()
 
 
@@ -444,6 +563,24 @@ def test_step2_recovery(cfg, batch):
     ctx.close()
 
 
+def test_step2_recovery_large_grid():
+    """A grid above 10 240 buses: V no longer fits the CTA's shared memory and lives in the scenario's workspace slice.
+    The injections are an identity in V, so an arbitrary (non-solved) state serves."""
+    net = S.make_network(S.standin_config(11000), s_net=1, kappa=1.0)
+    Y = oracle_Y(net)
+    batch = 3
+    vm, va = random_state(net, batch, 1234)
+    ctx = make_ctx(net, max_batch=batch, keep_factors=False)
+    p_inj, q_inj = ctx.recover(dev(vm), dev(va))
+    p_inj, q_inj = p_inj.cpu().numpy(), q_inj.cpu().numpy()
+    sc = row_scale(Y, vm)
+    for b in range(batch):
+        P, Q = oracle.injections(Y, vm[b], va[b])
+        assert (np.abs(p_inj[b] - P) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+        assert (np.abs(q_inj[b] - Q) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+    ctx.close()
+
+
 # ---- NEXT row 2: implicit-layer backward (PAPER.md eqs. 10-16) ------------------------------------------------------------
 @pytest.mark.parametrize("cfg,batch", [(1, 16), (2, 12), (3, 6)])
 def test_layer_backward(cfg, batch):
@@ -472,6 +609,39 @@ def test_layer_backward(cfg, batch):
     with pytest.raises(sb.SableError) as e:
         ctx.layer_backward(res["vm"][:2], res["va"][:2], *[dev(a[:2]) for a in gl])
     assert e.value.status == 1
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,batch", [(4, 4), (5, 3)])
+def test_layer_backward_large_grids(cfg, batch):
+    """Configs 4 and 5 (config 5 takes the workspace path of k_layer: 48 n_bus bytes exceed the shared-memory budget)
+    against the scipy.sparse restatement of the oracle (pinned against the dense form and by finite differences in
+    tests/test_oracle_layer.py), in FP64."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    rng = np.random.Generator(np.random.PCG64(131 + cfg))
+    gl = [rng.standard_normal((batch, net.n_bus)) for _ in range(4)]
+    ctx = make_ctx(net, max_batch=batch, keep_factors=True)
+    res = ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it)
+    dx_pg, dx_vm = ctx.layer_backward(res["vm"], res["va"], *[dev(a) for a in gl])
+    vm, va = res["vm"].cpu().numpy(), res["va"].cpu().numpy()
+    dx_pg, dx_vm = dx_pg.cpu().numpy(), dx_vm.cpu().numpy()
+    assert (res["converged"].cpu().numpy() == 1).all()
+    pv = net.bus_type == S.PV
+    gen = net.bus_type != S.PQ
+    for b in range(batch):
+        rp, rv = oracle.layer_backward_sparse(Y, net.bus_type, vm[b], va[b], gl[0][b], gl[1][b], gl[2][b], gl[3][b])
+        sc = max(1.0, np.abs(rp).max(), np.abs(rv).max())
+        assert np.abs(dx_pg[b] - rp).max() <= 1e-8 * sc, (b, np.abs(dx_pg[b] - rp).max())
+        assert np.abs(dx_vm[b] - rv).max() <= 1e-8 * sc, (b, np.abs(dx_vm[b] - rv).max())
+        assert (dx_pg[b][~pv] == 0).all() and (dx_vm[b][~gen] == 0).all()
+    # the kept factors survive the call (the workspace path uses the state part only): a second adjoint still matches
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, vm, va, gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    assert (np.abs(lp.cpu().numpy() - rp).max(axis=1) <= 1e-8 * scale).all()
     ctx.close()
 
 

@@ -64,3 +64,56 @@ def test_layer_backward_reduces_to_adjoint_when_loss_sees_only_z1():
     dx_pg, dx_vm = oracle.layer_backward(Y, net.bus_type, res["vm"][0], res["va"][0], z, z, gvm[0], gva[0])
     pv = net.bus_type == S.PV
     assert np.abs(dx_pg[pv] - lp[0][pv]).max() <= 1e-10 * max(1.0, np.abs(lp).max())
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_sparse_layer_backward_equals_dense(cfg):
+    """The scipy.sparse restatement (used for configs 4-5, where the dense form does not fit) against the dense form."""
+    net = S.make_network(cfg)
+    Y = oracle_Y(net)
+    ps, qs, vs = S.make_scenarios(net, batch=2)
+    res = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=1e-10, max_it=30, method=1)
+    rng = np.random.Generator(np.random.PCG64(50 + cfg))
+    for b in range(2):
+        gl = [rng.standard_normal(net.n_bus) for _ in range(4)]
+        d = oracle.layer_backward(Y, net.bus_type, res["vm"][b], res["va"][b], *gl)
+        s = oracle.layer_backward_sparse(Y, net.bus_type, res["vm"][b], res["va"][b], *gl)
+        sc = max(1.0, np.abs(d[0]).max(), np.abs(d[1]).max())
+        assert np.abs(d[0] - s[0]).max() <= 1e-10 * sc and np.abs(d[1] - s[1]).max() <= 1e-10 * sc
+
+
+def test_sparse_layer_backward_vs_finite_differences_cfg4():
+    """Finite differences of the whole layer on the 2 000-bus config (a few input coordinates): pins the sparse form at
+    a size where the dense one is not used."""
+    net = S.make_network(4)
+    Y = oracle_Y(net)
+    nb = net.n_bus
+    rng = np.random.Generator(np.random.PCG64(9))
+    pv = net.bus_type == S.PV
+    gen = net.bus_type != S.PQ
+    w_pg, w_qg, w_vm, w_va = (rng.standard_normal(nb) for _ in range(4))
+    w_pg[~gen] = 0; w_qg[~gen] = 0; w_va[net.bus_type == S.SLACK] = 0
+
+    def loss(p_gen, v_set):
+        pg, qg, vm, va = layer_forward(net, Y, p_gen, v_set, net.p_load, net.q_load)
+        return w_pg @ pg + w_qg @ qg + w_vm @ vm + w_va @ va
+
+    def layer_forward(net, Y, p_gen, v_set, p_load, q_load):
+        res = oracle.nr_batch(Y, net.bus_type, (p_gen - p_load)[None, :], (-q_load)[None, :], v_set[None, :], tol=1e-12, max_it=40, method=1)
+        assert res["converged"][0]
+        vm, va = res["vm"][0], res["va"][0]
+        P, Q = oracle.injections(Y, vm, va)
+        return P + p_load, Q + q_load, vm, va
+
+    pg0, vs0 = net.p_gen.copy(), net.v_set.copy()
+    _, _, vm, va = layer_forward(net, Y, pg0, vs0, net.p_load, net.q_load)
+    dx_pg, dx_vm = oracle.layer_backward_sparse(Y, net.bus_type, vm, va, w_pg, w_qg, w_vm, w_va)
+    h = 1e-5
+    for i in np.flatnonzero(pv)[[0, 7, 123]]:
+        e = np.zeros(nb); e[i] = h
+        fd = (loss(pg0 + e, vs0) - loss(pg0 - e, vs0)) / (2 * h)
+        assert abs(fd - dx_pg[i]) <= 5e-5 * max(1.0, abs(fd), np.abs(dx_pg).max()), (i, fd, dx_pg[i])
+    for i in np.flatnonzero(gen)[[0, 5, 200]]:
+        e = np.zeros(nb); e[i] = h
+        fd = (loss(pg0, vs0 + e) - loss(pg0, vs0 - e)) / (2 * h)
+        assert abs(fd - dx_vm[i]) <= 5e-5 * max(1.0, abs(fd), np.abs(dx_vm).max()), (i, fd, dx_vm[i])

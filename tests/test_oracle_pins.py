@@ -259,6 +259,27 @@ def test_linear_solvers_against_numpy_and_scipy(cfg):
         assert np.abs(xt - np.linalg.solve(A.toarray().T, rhs)).max() <= 1e-10 * np.abs(xt).max()
 
 
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_sparse_solver_against_scipy_at_large_sizes(cfg):
+    """Configs 4-5 (n = 3 598 / 17 036): the sparse elimination is the only oracle path used there, so it is cross-checked
+    against scipy's SuperLU (plain and transposed) and by the residual at exactly those sizes."""
+    net = S.make_network(cfg)
+    Y = net_Y(net)
+    rng = np.random.default_rng(11 + cfg)
+    vm, va = random_state(net, rng)
+    n, jr, jc, jv = oracle.jacobian(Y, net.bus_type, vm, va)
+    A = sp.coo_matrix((jv, (jr, jc)), shape=(n, n)).tocsc()
+    rhs = rng.standard_normal(n)
+    lu = spla.splu(A)
+    for transpose in (False, True):
+        x_sp = lu.solve(rhs, trans="T" if transpose else "N")
+        x = oracle.linear_solve(n, jr, jc, jv, rhs, method=1, transpose=transpose)
+        scale = np.abs(x_sp).max()
+        assert np.abs(x - x_sp).max() <= 1e-9 * scale
+        M = A.T if transpose else A
+        assert np.abs(M @ x - rhs).max() <= 1e-11 * max(1.0, np.abs(A).max() * scale)
+
+
 def test_sparse_solver_pivots_when_needed():
     """A matrix whose natural diagonal is zero needs row exchanges; duplicates in COO are summed."""
     A = np.array([[0.0, 2.0, 0.0, 1.0], [1.0, 0.0, 3.0, 0.0], [0.0, 1e-9, 0.0, 4.0], [2.0, 0.0, 1.0, 0.0]])

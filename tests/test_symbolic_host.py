@@ -196,7 +196,7 @@ def test_fill_pattern_on_a_ring():
         f = np.array([0, 1, 2, 3, 4, 5] + ([1] if chord else []), np.int32)
         t = np.array([1, 2, 3, 4, 5, 0] + ([5] if chord else []), np.int32)
         k = len(f)
-        Y = sb.ybus_from_branches(6, f, t, np.full(k, 0.01), np.full(k, 0.1), np.zeros(k))
+        Y = S.ybus_triplets(6, f, t, np.full(k, 0.01), np.full(k, 0.1), np.zeros(k))
         return sb.Context(6, *Y, np.array([2, 0, 0, 0, 0, 0], np.uint8), 0, max_batch=1, device=-1)
     a, b = ring_ctx(False), ring_ctx(True)
     assert a.info["n_pair"] == 4 and a.info["n_pair_j"] == 4 and a.info["n_term"] == 0
@@ -207,7 +207,7 @@ def test_fill_pattern_on_a_ring():
 
 def test_create_rejects_bad_input():
     net = S.make_network(1)
-    rp, ci, g, b = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+    rp, ci, g, b = S.ybus_triplets(net.n_bus, net.f, net.t, net.r, net.x, net.b)
     bt = net.bus_type
 
     def status(*a, **k):
@@ -226,7 +226,7 @@ def test_create_rejects_bad_input():
     assert status(1, rp[:2], ci, g, b, bt[:1], 0) == 1                        # n_bus < 2
     # an island: bus 13 cut off
     keep = (net.f != 13) & (net.t != 13)
-    Y = sb.ybus_from_branches(net.n_bus, net.f[keep], net.t[keep], net.r[keep], net.x[keep], net.b[keep])
+    Y = S.ybus_triplets(net.n_bus, net.f[keep], net.t[keep], net.r[keep], net.x[keep], net.b[keep])
     assert status(net.n_bus, *Y, bt, 0) == 2
     with pytest.raises(sb.SableError) as e:
         sb.Context(net.n_bus, rp, ci, g, b, bt, 0, max_batch=0, device=-1)

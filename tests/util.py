@@ -15,7 +15,7 @@ def oracle_Y(net):
 def make_ctx(net, **opt):
     """sable_create on the harness-side Y_bus (unsorted triplets with duplicates: the library canonicalises)."""
     import paper_2606_07099_b200 as sb
-    Y = sb.ybus_from_branches(net.n_bus, net.f, net.t, net.r, net.x, net.b)
+    Y = S.ybus_triplets(net.n_bus, net.f, net.t, net.r, net.x, net.b)
     return sb.Context(net.n_bus, *Y, net.bus_type, net.slack, **opt)
 
 
@@ -66,3 +66,28 @@ def gpu_jacobian_dense(ctx, net, diag, pairs):
             put(nb[m], nb[j], pairs[p][0:4])
             put(nb[j], nb[m], pairs[p][4:8])
     return J, seen, pad_ok
+
+
+def gpu_jacobian_coo(ctx, net, diag, pairs):
+    """The library's padded block layout as COO triplets in the oracle's J1 ordering (for grids where the dense form
+    does not fit).  Returns (rows, cols, vals, padding_ok)."""
+    n, th, vmx = oracle.index_maps(net.bus_type)
+    pat = ctx.debug_pattern()
+    nb = pat["node_bus"].astype(np.int64)
+    nn = nb.shape[0]
+    prow = np.repeat(np.arange(nn), np.diff(pat["pair_ptr"]))
+    pcol = pat["pair_col"].astype(np.int64)
+    bi = np.concatenate([nb, nb[prow], nb[pcol]])
+    bj = np.concatenate([nb, nb[pcol], nb[prow]])
+    blk = np.concatenate([diag.reshape(nn, 4), pairs[:, 0:4], pairs[:, 4:8]])
+    is_diag = np.concatenate([np.ones(nn, bool), np.zeros(2 * prow.shape[0], bool)])
+    rows, cols, vals = [], [], []
+    pad_ok = True
+    for a, rmap in enumerate((th, vmx)):
+        for c, cmap in enumerate((th, vmx)):
+            r, cc, v = rmap[bi], cmap[bj], blk[:, 2 * a + c]
+            real = (r >= 0) & (cc >= 0)
+            rows.append(r[real]); cols.append(cc[real]); vals.append(v[real])
+            want = np.where(is_diag & (a == 1) & (c == 1), 1.0, 0.0)
+            pad_ok = pad_ok and bool((v[~real] == want[~real]).all())
+    return np.concatenate(rows), np.concatenate(cols), np.concatenate(vals), pad_ok
