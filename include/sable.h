@@ -38,18 +38,45 @@ enum { SABLE_BUS_PQ = 0, SABLE_BUS_PV = 1, SABLE_BUS_SLACK = 2 };
 enum { SABLE_FP64 = 0, SABLE_MIXED = 1 };    /* MIXED: FP64 mismatch / state, FP32 Jacobian factors and solves (Table I) */
 enum { SABLE_MODE_FUSED = 0, SABLE_MODE_STAGED = 1 };
 
+/* Launch tuning.  Every field has an "automatic" value (what sable_default_options() returns); the library then chooses
+ * from the grid size, the level structure and max_batch.  For experiments each field can also be
+ * overridden through the environment variable named beside it (read at sable_create, only when the field is left automatic;
+ * values are clamped to the stated range). */
+typedef struct {
+    int32_t group;            /* scenarios a CTA advances in lockstep = group size of the interleaved workspace: 1, 2, 4 ... 32;
+                                 0 = automatic                                                        (SABLE_G) */
+    int32_t ctas_per_sm;      /* cap on resident CTAs per SM of the NR kernel, 1 ... 32; 0 = automatic  (SABLE_CTAS) */
+    int32_t on_chip;          /* 1 = all arrays of every slot in shared memory (if they fit), 0 = HBM workspace,
+                                 -1 = automatic                                                       (SABLE_ONCHIP) */
+    int32_t ring_slots;       /* on-chip placement: slots of the level-blob ring, 0 ... 8 (0 = off); -1 = automatic  (SABLE_RING_R) */
+    int32_t ring_slot_bytes;  /* bytes per ring slot, 256 ... 65536; -1 = automatic                     (SABLE_RING_SLOT) */
+    int32_t front_nodes;      /* HBM placement: cap on the nodes of the dense top front, 0 ... 96 (0 = off); -1 = automatic  (SABLE_FRONT) */
+    int32_t front_kb;         /* shared-memory budget of the front per CTA in KB, 0 ... 220; -1 = automatic  (SABLE_FRONT_KB) */
+    int32_t threads_stage;    /* threads per CTA of the staged kernels, 32 ... 512; 0 = automatic       (SABLE_THREADS1) */
+    int32_t threads_lin;      /* threads per CTA of the adjoint kernel, 32 ... 1024; 0 = automatic      (SABLE_THREADS_LIN) */
+    int32_t timing;           /* 1 = per-phase cycle counters of CTA 0 (sable_debug_timing)            (SABLE_TIMING) */
+} sable_tuning;
+
 typedef struct {
     int32_t max_batch;      /* scenarios per sable_solve call; all device buffers are sized for it at create time */
     int32_t precision;      /* SABLE_FP64 or SABLE_MIXED */
     int32_t keep_factors;   /* 1: after the NR loop, J1 is re-factored at the final iterate and the factors are kept
                                for sable_adjoint (reading 16) */
-    int32_t mode;           /* SABLE_MODE_FUSED: one persistent kernel runs the whole NR loops of the batch on chip;
-                               SABLE_MODE_STAGED: one kernel per stage (mismatch / fill / refactor / solve), state in HBM
-                               between stages -- used for per-stage profiling */
+    int32_t mode;           /* SABLE_MODE_FUSED: one persistent kernel runs the whole NR loops of the batch;
+                               SABLE_MODE_STAGED: one kernel per stage (mismatch + fill / refactor + solve), state in HBM
+                               between stages, host check of the active count -- used for per-stage profiling */
     int32_t device;         /* CUDA device ordinal; -1 = host-only context (symbolic phase only: sable_get_info and the
                                sable_debug_* pattern queries work, solve / adjoint return SABLE_ERR_STATE) */
-    int32_t threads;        /* threads per CTA for the NR kernels; 0 = library default for the grid size */
+    int32_t threads;        /* threads per CTA for the NR kernel; 0 = library default for the grid size  (SABLE_THREADS) */
+    int32_t ir_sweeps;      /* inner iterative-refinement sweeps of the forward linear solve in SABLE_MIXED mode.  Must be 0:
+                               the paper's scheme has none (Table I) -- the Newton loop with its FP64
+                               residual and FP64 state accumulation is the refinement (reading 15).  FP64
+                               refinement of the ADJOINT solve on FP32 factors: sable_adjoint_refined. */
+    sable_tuning tune;
 } sable_options;
+
+/* Options with every field at its default / automatic value: max_batch 1, FP64, keep_factors 1, fused, device 0. */
+sable_options sable_default_options(void);
 
 typedef struct {
     int32_t n_bus, n_pq, n_pv;
@@ -69,14 +96,16 @@ typedef struct {
     int64_t bytes_adjoint_m0; /* same for one adjoint solve */
     int32_t smem_bytes;     /* dynamic shared memory per CTA of the NR kernel */
     int32_t placement;      /* 0: factors, V and rhs of every slot in shared memory; 2: everything in the group-interleaved
-                               HBM workspace; 1 (only on request): elimination levels >= cut_level in shared memory */
+                               HBM workspace */
     int32_t threads;        /* threads per CTA */
     int32_t ctas_per_sm;    /* occupancy the NR kernel was sized for */
     int32_t slots_per_cta;  /* scenarios a CTA of the NR kernel advances in lockstep */
-    int32_t cut_level;      /* placement 1: first elimination level kept in shared memory */
+    int32_t cut_level;      /* first elimination level kept in shared memory: 0 (placement 0) or n_level (placement 2) */
     int32_t front_k;        /* placement 2: nodes of the dense top front (the last elimination levels, factored as one dense
                                block matrix in shared memory); 0 = none */
     int32_t front_level;    /* first elimination level of that front (n_level if none) */
+    int32_t threads_lin;    /* threads per CTA of the adjoint kernel */
+    int32_t threads_stage;  /* threads per CTA of the staged kernels */
 } sable_info;
 
 /* Build the shared fixed-pattern template for one network (host symbolic phase, run once; PAPER.md:185-197:
@@ -87,7 +116,8 @@ typedef struct {
  *   row_ptr[n_bus+1], col_idx[nnz], y_re[nnz], y_im[nnz]   HOST.  Y_bus = G + jB in CSR; columns may be unsorted,
  *                    duplicates are summed, a missing diagonal or transpose entry is added with value 0.
  *   bus_type[n_bus]  HOST.  SABLE_BUS_PQ / PV / SLACK; exactly one slack, and it must equal `slack`.
- *   opt              may be NULL (defaults: max_batch 1, FP64, keep_factors 1, fused, device 0).
+ *   opt              may be NULL (= sable_default_options()).  Start from sable_default_options() and change fields:
+ *                    a zero-initialised struct is NOT the default (on_chip / ring / front fields use -1 for automatic).
  *   out              receives the context.  The input arrays are not referenced after the call returns.
  * Errors: INVALID_ARG, STRUCTURE, ALLOC, CUDA.  On error *out = NULL (message via sable_last_error(NULL)). */
 sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx,
@@ -117,9 +147,20 @@ sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double* p_spec, co
  * i.e. J1 at that call's final iterates; only transposed triangular solves run.
  *   g_va [batch][n_bus]  dl/dtheta_i (slack entry ignored);   g_vm [batch][n_bus]  dl/dVm_i (PQ entries used)
  *   lam_p, lam_q [batch][n_bus]  out: multipliers of the P_i / Q_i equations; 0 at the slack / off PQ buses.
+ * A scenario whose kept factors carry a tiny-pivot flag (sable_get_pivot_flags, bit 1) gets NaN in every entry: static
+ * pivoting failed there and, unlike the forward path, nothing downstream would reveal a wrong lambda.
  * All DEVICE pointers.  batch must equal the batch of the last solve.  Errors: INVALID_ARG, STATE, CUDA. */
 sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const double* g_va, const double* g_vm,
                            double* lam_p, double* lam_q, void* cuda_stream);
+
+/* Tiny-pivot flags of the last sable_solve (the paper's cuDSS path pivots internally; this library uses static
+ * 2x2 block-diagonal pivots in a fixed order, shared by the batch): flags[b] bit 0 = in some refactorisation of scenario b a
+ * pivot block D had |det D| <= eps * max|D_ij|^2 (eps = 1e-10 in FP64, 1e-6 with FP32 factors) or a non-finite
+ * determinant; bit 1 = that happened in the LAST refactorisation (with keep_factors: in the kept factors).  A flagged
+ * scenario that still converged is fine (the FP64 residual test protects the forward path); a flagged scenario that did not
+ * converge should be re-solved by a pivoting solver.  flags [batch] int32 DEVICE out; asynchronous on the stream.
+ * Errors: INVALID_ARG (batch differs from the last solve), STATE, CUDA. */
+sable_status sable_get_pivot_flags(sable_ctx* ctx, int32_t batch, int32_t* flags, void* cuda_stream);
 
 /* Step-2 explicit recovery (PAPER.md:80 eq. 5, :95-99 eq. 9: with dF2/dz2 = I the block z2 = [p_g at the slack; q_g at
  * PV and slack buses] is read off the mismatch rows that Step 1 does not use).  Returns the calculated net injections
@@ -161,8 +202,10 @@ sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, const double* 
                                    const double* g_va, const double* g_vm, int32_t sweeps, double* lam_p,
                                    double* lam_q, void* cuda_stream);
 
-/* Host-buffer convenience wrappers: same semantics with HOST pointers; they copy in, run on the context's
- * device and copy out (synchronous).  Used for the end-to-end measurement. */
+/* Host-buffer convenience wrappers: same semantics with HOST pointers (pinned memory for full copy speed); they copy in,
+ * run on the context's device and copy out, synchronously.  The batch is cut into up to four chunks of whole scenario
+ * groups, each on its own internal stream, so that the copies of one chunk overlap the kernels of the others.  The device
+ * staging buffers are allocated at the first such call.  Used for the end-to-end measurement. */
 sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
                               const double* v_set, const double* vm0, const double* va0, double tol,
                               int32_t max_it, double* vm, double* va, int32_t* iterations, uint8_t* converged,
@@ -212,10 +255,17 @@ sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, const doubl
                                       const double* rhs_p, const double* rhs_q, int32_t transpose,
                                       double* x_p, double* x_q, void* cuda_stream);
 
+/* Per-stage times in the default workspace layout: runs the fused kernel's own stage routines one stage per launch
+ * (mismatch + norm + decision + Jacobian fill / refactor + triangular solves + update) for three Newton iterations from the
+ * flat start on the given batch (DEVICE pointers, [batch][n_bus]) and returns the mean CUDA-event time of each launch in ms
+ * (HOST out).  Synchronous; overwrites the workspace, so kept factors are gone afterwards. */
+sable_status sable_debug_stage_times(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                     const double* v_set, double* ms_mismatch_fill, double* ms_factor_solve, void* cuda_stream);
+
 /* Per-phase cycle counters of CTA 0 of the fused kernel, accumulated since the last call (then reset).  Only when
- * the context was created with SABLE_TIMING=1 in the environment (else SABLE_ERR_STATE); the HBM-placement kernels
- * carry the counters only when the library is built with -DSABLE_TIMING_ALL (they cost registers there).  out[4 l + 0 / 1 / 2] = cycles
- * in the diagonal-target / pair-target / backward phase of elimination level l; out[4 L] = cycles in decision +
+ * the context was created with tune.timing = 1 (else SABLE_ERR_STATE); the HBM-placement kernels
+ * carry the counters only when the library is built with -DSABLE_TIMING_ALL (they cost registers there).  out[4 l + 0 / 2] = cycles
+ * in the accumulate (factor + forward) / backward phase of elimination level l; out[4 L] = cycles in decision +
  * output; out[4 L + 1] = loop trips; out[4 L + 2] = refill + init; out[4 L + 3] = mismatch + norm; L = n_level;
  * n = entries wanted, at most 4 L + 4 (HOST out). */
 sable_status sable_debug_timing(sable_ctx* ctx, uint64_t* out, int32_t n);

@@ -28,9 +28,16 @@ class SableError(RuntimeError):
         self.status = status
 
 
+class Tuning(C.Structure):
+    _fields_ = [("group", C.c_int32), ("ctas_per_sm", C.c_int32), ("on_chip", C.c_int32), ("ring_slots", C.c_int32),
+                ("ring_slot_bytes", C.c_int32), ("front_nodes", C.c_int32), ("front_kb", C.c_int32),
+                ("threads_stage", C.c_int32), ("threads_lin", C.c_int32), ("timing", C.c_int32)]
+
+
 class Options(C.Structure):
     _fields_ = [("max_batch", C.c_int32), ("precision", C.c_int32), ("keep_factors", C.c_int32),
-                ("mode", C.c_int32), ("device", C.c_int32), ("threads", C.c_int32)]
+                ("mode", C.c_int32), ("device", C.c_int32), ("threads", C.c_int32), ("ir_sweeps", C.c_int32),
+                ("tune", Tuning)]
 
 
 class Info(C.Structure):
@@ -41,15 +48,17 @@ class Info(C.Structure):
                 ("factor_bytes", C.c_int64), ("bytes_iter_m0", C.c_int64), ("bytes_adjoint_m0", C.c_int64),
                 ("smem_bytes", C.c_int32), ("placement", C.c_int32), ("threads", C.c_int32),
                 ("ctas_per_sm", C.c_int32), ("slots_per_cta", C.c_int32), ("cut_level", C.c_int32),
-                ("front_k", C.c_int32), ("front_level", C.c_int32)]
+                ("front_k", C.c_int32), ("front_level", C.c_int32), ("threads_lin", C.c_int32), ("threads_stage", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-EXPORTS = ["sable_create", "sable_solve", "sable_adjoint", "sable_recover", "sable_layer_backward", "sable_adjoint_refined", "sable_solve_host", "sable_adjoint_host",
+EXPORTS = ["sable_create", "sable_default_options", "sable_solve", "sable_adjoint", "sable_get_pivot_flags", "sable_recover",
+           "sable_layer_backward", "sable_adjoint_refined", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
-           "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing"]
+           "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing",
+           "sable_debug_stage_times"]
 
 
 def lib():
@@ -65,6 +74,8 @@ def lib():
         L.sable_launch_count.argtypes = [C.c_void_p]
         L.sable_destroy.restype = None
         L.sable_destroy.argtypes = [C.c_void_p]
+        L.sable_default_options.restype = Options
+        L.sable_default_options.argtypes = []
         _lib = L
     return _lib
 
@@ -75,11 +86,19 @@ def _hp(a, dtype):
     return a, a.ctypes.data_as(C.c_void_p)
 
 
-def _dp(t):
-    """torch CUDA tensor (or None) -> device pointer."""
+def _dp(t, shape=None, dtype=None, device=None):
+    """torch CUDA tensor (or None) -> device pointer.  With `shape` / `dtype` / `device` given the tensor is checked
+    against them first: the kernels trust the boundary arrays' sizes."""
     if t is None:
         return C.c_void_p(0)
-    assert t.is_cuda and t.is_contiguous(), "device arrays must be contiguous CUDA tensors"
+    if not (t.is_cuda and t.is_contiguous()):
+        raise ValueError("device arrays must be contiguous CUDA tensors")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    if device is not None and t.device.index != device:
+        raise ValueError(f"tensor lives on cuda:{t.device.index}, the context on cuda:{device}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -92,7 +111,9 @@ class Context:
     """Owns one `sable_ctx*`.  Method names follow the C calls (sable_solve -> .solve, ...)."""
 
     def __init__(self, n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, max_batch=1, precision=FP64,
-                 keep_factors=True, mode=FUSED, device=0, threads=0):
+                 keep_factors=True, mode=FUSED, device=0, threads=0, **tune):
+        """`tune`: fields of sable_tuning (group, ctas_per_sm, on_chip, ring_slots, ring_slot_bytes, front_nodes, front_kb,
+        threads_stage, threads_lin, timing); anything not given stays automatic."""
         L = lib()
         keep = []
         ptrs = []
@@ -101,7 +122,13 @@ class Context:
             arr, p = _hp(a, dt)
             keep.append(arr)
             ptrs.append(p)
-        opt = Options(int(max_batch), int(precision), int(bool(keep_factors)), int(mode), int(device), int(threads))
+        opt = L.sable_default_options()
+        opt.max_batch, opt.precision, opt.keep_factors = int(max_batch), int(precision), int(bool(keep_factors))
+        opt.mode, opt.device, opt.threads = int(mode), int(device), int(threads)
+        for k, v in tune.items():
+            if not hasattr(opt.tune, k):
+                raise TypeError(f"unknown tuning field {k!r}")
+            setattr(opt.tune, k, int(v))
         self._h = C.c_void_p(0)
         st = L.sable_create(C.c_int32(int(n_bus)), *ptrs, C.c_int32(int(slack)), C.byref(opt), C.byref(self._h))
         if st != 0:
@@ -136,11 +163,21 @@ class Context:
         return int(lib().sable_launch_count(self._h))
 
     # -- device-pointer calls (torch CUDA tensors, float64 [batch][n_bus]) ------------------------------
+    def _bn(self, t):
+        """pointer of a float64 [batch][n_bus] tensor on this context's device (batch read from the first argument)."""
+        return _dp(t, (self._batch, self.n_bus), self._f64, self.device)
+
+    def _begin(self, first):
+        import torch
+        self._f64 = torch.float64
+        self._batch = int(first.shape[0])
+        return self._batch
+
     def solve(self, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, out=None):
         """sable_solve.  Returns dict(vm, va, iterations, converged, final_norm) of torch CUDA tensors.
         Asynchronous on torch's current stream."""
         import torch
-        batch = int(p_spec.shape[0])
+        batch = self._begin(p_spec)
         dev = p_spec.device
         if out is None:
             out = dict(vm=torch.empty((batch, self.n_bus), dtype=torch.float64, device=dev),
@@ -148,50 +185,72 @@ class Context:
                        iterations=torch.empty(batch, dtype=torch.int32, device=dev),
                        converged=torch.empty(batch, dtype=torch.uint8, device=dev),
                        final_norm=torch.empty(batch, dtype=torch.float64, device=dev))
-        self._check(lib().sable_solve(self._h, C.c_int32(batch), _dp(p_spec), _dp(q_spec), _dp(v_set), _dp(vm0),
-                                      _dp(va0), C.c_double(tol), C.c_int32(int(max_it)), _dp(out["vm"]),
-                                      _dp(out["va"]), _dp(out["iterations"]), _dp(out["converged"]),
-                                      _dp(out["final_norm"]), _stream()))
+        self._check(lib().sable_solve(self._h, C.c_int32(batch), self._bn(p_spec), self._bn(q_spec), self._bn(v_set), self._bn(vm0),
+                                      self._bn(va0), C.c_double(tol), C.c_int32(int(max_it)), self._bn(out["vm"]),
+                                      self._bn(out["va"]), _dp(out["iterations"], (batch,), torch.int32, self.device),
+                                      _dp(out["converged"], (batch,), torch.uint8, self.device),
+                                      _dp(out["final_norm"], (batch,), torch.float64, self.device), _stream()))
         return out
+
+    def pivot_flags(self, batch):
+        """sable_get_pivot_flags of the last solve: int32 [batch], bit 0 = a tiny pivot in some refactorisation, bit 1 = in the last."""
+        import torch
+        flags = torch.empty(int(batch), dtype=torch.int32, device=torch.device("cuda", self.device))
+        self._check(lib().sable_get_pivot_flags(self._h, C.c_int32(int(batch)), _dp(flags), _stream()))
+        return flags
 
     def adjoint(self, g_va, g_vm, out=None):
         """sable_adjoint.  Returns (lam_p, lam_q)."""
         import torch
-        batch = int(g_va.shape[0])
+        batch = self._begin(g_va)
         if out is None:
             out = (torch.empty_like(g_va), torch.empty_like(g_vm))
-        self._check(lib().sable_adjoint(self._h, C.c_int32(batch), _dp(g_va), _dp(g_vm), _dp(out[0]), _dp(out[1]),
+        self._check(lib().sable_adjoint(self._h, C.c_int32(batch), self._bn(g_va), self._bn(g_vm), self._bn(out[0]), self._bn(out[1]),
                                         _stream()))
         return out
 
     def adjoint_refined(self, vm, va, g_va, g_vm, sweeps=2, out=None):
         """sable_adjoint_refined: the adjoint of eq. 14 with `sweeps` FP64 refinement sweeps.  Returns (lam_p, lam_q)."""
         import torch
-        batch = int(g_va.shape[0])
+        batch = self._begin(g_va)
         if out is None:
             out = (torch.empty_like(g_va), torch.empty_like(g_vm))
-        self._check(lib().sable_adjoint_refined(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(g_va), _dp(g_vm),
-                                                C.c_int32(int(sweeps)), _dp(out[0]), _dp(out[1]), _stream()))
+        self._check(lib().sable_adjoint_refined(self._h, C.c_int32(batch), self._bn(vm), self._bn(va), self._bn(g_va), self._bn(g_vm),
+                                                C.c_int32(int(sweeps)), self._bn(out[0]), self._bn(out[1]), _stream()))
         return out
 
     def recover(self, vm, va, out=None):
         """sable_recover (Step-2 explicit recovery).  Returns (p_inj, q_inj): calculated net injections at every bus."""
         import torch
-        batch = int(vm.shape[0])
+        batch = self._begin(vm)
         if out is None:
             out = (torch.empty_like(vm), torch.empty_like(vm))
-        self._check(lib().sable_recover(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(out[0]), _dp(out[1]), _stream()))
+        self._check(lib().sable_recover(self._h, C.c_int32(batch), self._bn(vm), self._bn(va), self._bn(out[0]), self._bn(out[1]), _stream()))
         return out
 
     def layer_backward(self, vm, va, gl_pg, gl_qg, gl_vm, gl_va, out=None):
         """sable_layer_backward (eqs. 10-16).  Returns (dx_pg, dx_vm)."""
         import torch
-        batch = int(vm.shape[0])
+        batch = self._begin(vm)
         if out is None:
             out = (torch.empty_like(vm), torch.empty_like(vm))
-        self._check(lib().sable_layer_backward(self._h, C.c_int32(batch), _dp(vm), _dp(va), _dp(gl_pg), _dp(gl_qg),
-                                               _dp(gl_vm), _dp(gl_va), _dp(out[0]), _dp(out[1]), _stream()))
+        self._check(lib().sable_layer_backward(self._h, C.c_int32(batch), self._bn(vm), self._bn(va), self._bn(gl_pg), self._bn(gl_qg),
+                                               self._bn(gl_vm), self._bn(gl_va), self._bn(out[0]), self._bn(out[1]), _stream()))
         return out
+
+    def stage_times(self, p_spec, q_spec, v_set, reps=1):
+        """sable_debug_stage_times: mean ms of the mismatch + fill launch and of the refactor + solve launch over three Newton
+        iterations of the whole batch in the default workspace layout (averaged over `reps` calls)."""
+        batch = self._begin(p_spec)
+        a, b = C.c_double(0), C.c_double(0)
+        ta = tb = 0.0
+        for _ in range(max(1, int(reps))):
+            self._check(lib().sable_debug_stage_times(self._h, C.c_int32(batch), self._bn(p_spec), self._bn(q_spec), self._bn(v_set),
+                                                      C.byref(a), C.byref(b), _stream()))
+            ta += a.value
+            tb += b.value
+        n = max(1, int(reps))
+        return {"mismatch_fill_ms": ta / n, "factor_solve_ms": tb / n}
 
     # -- host-buffer calls (numpy) ----------------------------------------------------------------------
     def solve_host(self, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, out=None):
@@ -234,12 +293,12 @@ class Context:
         return a
 
     def debug_timing(self):
-        """Per-phase cycle counters of CTA 0 (needs SABLE_TIMING=1 at create).
-        Returns (per_level [L][3], dict(decide_output, trips, refill_init, mismatch_norm))."""
+        """Per-phase cycle counters of CTA 0 (needs timing=1 at create).
+        Returns (per_level [L][2] = accumulate / backward cycles, dict(decide_output, trips, refill_init, mismatch_norm, front_*))."""
         L = self.info["n_level"]
         buf = np.zeros(4 * L + 4, np.uint64)
         self._check(lib().sable_debug_timing(self._h, C.c_void_p(buf.ctypes.data), C.c_int32(buf.size)))
-        return (buf[:4 * L].reshape(L, 4)[:, :3].astype(np.int64),
+        return (buf[:4 * L].reshape(L, 4)[:, [0, 2]].astype(np.int64),
                 dict(decide_output=int(buf[4 * L]), trips=int(buf[4 * L + 1]), refill_init=int(buf[4 * L + 2]),
                      mismatch_norm=int(buf[4 * L + 3]), front_assemble=int(buf[3]), front_factor=int(buf[7]) if L > 1 else 0,
                      front_backward=int(buf[11]) if L > 2 else 0))

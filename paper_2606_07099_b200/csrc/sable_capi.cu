@@ -17,19 +17,20 @@ struct sable_ctx {
     sable_info info{};
     DevTemplate d{};
     std::vector<void*> dev_allocs;
-    char* factors = nullptr;  char* work = nullptr;  int32_t* ints = nullptr;   // ints: queue[1] status[mb] it[mb]
+    char* factors = nullptr;  char* work = nullptr;
+    int32_t* ints = nullptr;                                 // queue[kMaxChunk] status[mb] it[mb] pivot[mb] active[kMaxActive]
     double* zeros = nullptr;
     const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
-    const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward
-    unsigned long long* tim = nullptr;                       // SABLE_TIMING=1: per-phase cycle counters of CTA 0
+    const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward (lbuf: lazily allocated)
+    unsigned long long* tim = nullptr;                       // tuning.timing: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
-    // launch plan of the fused kernel (choose_launch) and of the one-scenario-per-CTA kernels
-    int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1;
-    int dg_cut = 0, pr_cut = 0, st_cut = 0, cut_level = 0;
-    int threads1 = 0;                                        // staged / adjoint / debug kernels
+    // launch plan of the fused kernel (choose_launch) and of the other kernel families
+    int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1, variant = 0;
+    int big_off = 0, slot_off = 0;
+    int threads_stage = 0, threads_lin = 0, threads1 = 0;    // staged kernels (group layout), adjoint kernel, one-scenario debug kernels
     int factor_gsh = 0;                                      // group layout of the factors currently in the workspace
-    const LevelDesc* level_fused = nullptr; const LevelDesc* level_one = nullptr; const LevelDesc* level_lin = nullptr;
-    int threads_lin = 0;                                     // adjoint kernel on group-interleaved factors
+    const LevelDesc* level_fused = nullptr; const LevelDesc* level_stage = nullptr;
+    const LevelDesc* level_lin = nullptr; const LevelDesc* level_one = nullptr;
     std::vector<LevelDesc> lv_host;                          // blob offsets per level (splits filled per kernel family)
     std::vector<char> blob_host;
     int ring_r = 0, ring_slot = 0, first_staged = 0;
@@ -37,9 +38,12 @@ struct sable_ctx {
     int last_batch = -1;  bool have_factors = false;
     int64_t launches = 0;
     std::string err;
-    // host wrapper staging (device)
+    // host wrappers: staging buffers (lazily allocated) and the streams / events of the chunk pipeline
     double* hbuf = nullptr; int32_t* hbuf_it = nullptr; uint8_t* hbuf_cv = nullptr;
+    cudaStream_t hstream[4] = {nullptr, nullptr, nullptr, nullptr};
 };
+constexpr int kMaxChunk = 4;      // chunks of the host-buffer pipeline (each with its own queue counter and stream)
+constexpr int kMaxActive = 64;    // staged mode: active-scenario counters, one per mismatch pass
 
 static thread_local std::string g_create_err;   // message of the last failed sable_create on this host thread
 
@@ -83,17 +87,28 @@ static void fill_info(sable_ctx* c) {
     I.bytes_iter_m0 = 8 * T.nnz_j + w * T.nnz_j + 2 * w * T.nnz_lu + 8 * (10 * (int64_t)T.n_bus + 4 * (int64_t)I.n);
     I.bytes_adjoint_m0 = w * T.nnz_lu + 16 * (int64_t)I.n;
     I.smem_bytes = c->smem; I.placement = c->placement; I.threads = c->threads;
-    I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->cut_level;
+    I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->placement == 0 ? 0 : T.n_level;
     I.front_k = c->front_k; I.front_level = c->front_k > 0 ? c->front_level : T.n_level;
+    I.threads_lin = c->threads_lin; I.threads_stage = c->threads_stage;
 }
 
-// kernel variant: placement 0 = on chip, 1 = mixed (only on request: SABLE_CUT), 2 = HBM; small = up to 128 threads
-static const void* fused_fn(bool mixed, int place, bool small) {
-    if (place == 0) return mixed ? (const void*)k_nr_fused<float, 0, false> : (const void*)k_nr_fused<double, 0, false>;
-    if (place == 1) return mixed ? (const void*)k_nr_fused<float, 1, false> : (const void*)k_nr_fused<double, 1, false>;
-    if (small) return mixed ? (const void*)k_nr_fused<float, 2, true> : (const void*)k_nr_fused<double, 2, true>;
-    return mixed ? (const void*)k_nr_fused<float, 2, false> : (const void*)k_nr_fused<double, 2, false>;
+// kernel variants of the fused kernel: (placement, max threads per CTA, CTAs per SM the registers are budgeted for)
+struct Variant { int place, threads, ctas; };
+static const Variant kVariants[] = {{0, 512, 1}, {2, 128, 7}, {2, 256, 4}, {2, 512, 2}, {2, 1024, 1}};
+static int pick_variant(int place, int th) {
+    if (place == 0) return 0;
+    return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : 4;
 }
+template <typename T> static const void* fused_fn_t(int v) {
+    switch (v) {
+        case 0: return (const void*)k_nr_fused<T, 0, 512, 1>;
+        case 1: return (const void*)k_nr_fused<T, 2, 128, 7>;
+        case 2: return (const void*)k_nr_fused<T, 2, 256, 4>;
+        case 3: return (const void*)k_nr_fused<T, 2, 512, 2>;
+        default: return (const void*)k_nr_fused<T, 2, 1024, 1>;
+    }
+}
+static const void* fused_fn(bool mixed, int v) { return mixed ? fused_fn_t<float>(v) : fused_fn_t<double>(v); }
 
 // threads per CTA of the one-thread-per-bus kernels (recover, layer): whole rounds with no idle tail (300 buses -> 160
 // threads x 2 rounds, not 256 x 2 with the second round 85 % idle), 64 for small grids, 512 for large ones
@@ -103,76 +118,158 @@ static int bus_threads(int n_bus) {
     return std::min(cap, ((n_bus + rounds - 1) / rounds + 31) / 32 * 32);
 }
 
-static int env_int(const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; }
+// A tuning value: the option field if set, else the (debug) environment override, else the default; clamped to [lo, hi].
+static int tune(int opt_value, int unset, const char* env, int dflt, int lo, int hi) {
+    int v = opt_value != unset ? opt_value : dflt;
+    if (opt_value == unset) { const char* e = getenv(env); if (e && *e) v = atoi(e); }
+    return std::min(hi, std::max(lo, v));
+}
+static bool tune_given(int opt_value, int unset, const char* env) { const char* e = getenv(env); return opt_value != unset || (e && *e); }
+static int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
 
-// lanes per target (log2) for a level with n targets whose longest list has max_len entries: as many as keep every
-// thread busy at most once, never more than a warp's share per slot
-static uint8_t pick_split(int n, int max_len, int threads, int gsh) {
+// level slices of the index program (layout: LevelDesc in sable_device.cuh).  `d` carries m0, m1, p0, p1; targets are the
+// nodes / pairs of that range; only items whose eliminated node k is below k_limit are listed (the front's assembly lists).
+struct LevelLists { std::vector<int> dlen, tlen; };   // list lengths in sorted order (for the class cuts)
+static LevelLists pack_level(const Template& T, LevelDesc& d, int k_limit, std::vector<char>& blob) {
+    auto al = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
+    const int nm = d.m1 - d.m0, np = d.p1 - d.p0;
+    // item lists per target, filtered
+    std::vector<std::vector<int2>> dl(nm);
+    std::vector<std::vector<int4>> tl(np);
+    for (int i = 0; i < nm; ++i)
+        for (int q = T.dterm_ptr[d.m0 + i]; q < T.dterm_ptr[d.m0 + i + 1]; ++q) {
+            const int a = T.dterm[q], k = T.pair_row[a];
+            if (k < k_limit) dl[i].push_back(make_int2(a, k));
+        }
+    for (int i = 0; i < np; ++i)
+        for (int q = T.term_ptr[d.p0 + i]; q < T.term_ptr[d.p0 + i + 1]; ++q) {
+            const int a = T.term_a[q], b = T.term_b[q], k = T.pair_row[a];
+            if (k < k_limit) tl[i].push_back(make_int4(a, b, k, 0));
+        }
+    std::vector<int32_t> dord(nm), tord(np);
+    for (int i = 0; i < nm; ++i) dord[i] = i;
+    for (int i = 0; i < np; ++i) tord[i] = i;
+    std::stable_sort(dord.begin(), dord.end(), [&](int a, int b) { return dl[a].size() > dl[b].size(); });
+    std::stable_sort(tord.begin(), tord.end(), [&](int a, int b) { return tl[a].size() > tl[b].size(); });
+    size_t nd = 0, nt = 0;
+    for (auto& v : dl) nd += v.size();
+    for (auto& v : tl) nt += v.size();
+    size_t o = 0;
+    o += (size_t)(nm + 1) * 4; d.o_dord = (int32_t)o;
+    o += (size_t)nm * 4; d.o_tptr = (int32_t)o;
+    o += (size_t)(np + 1) * 4; d.o_tord = (int32_t)o;
+    o += (size_t)np * 4; d.o_pptr = (int32_t)o;
+    o += (size_t)(nm + 1) * 4; o = al(o, 8); d.o_dak = (int32_t)o;
+    o += nd * 8; d.o_pmj = (int32_t)o;
+    o += (size_t)np * 8; o = al(o, 16); d.o_tab = (int32_t)o;
+    o += nt * 16;
+    o = al(o, 128);
+    d.blob_off = (int32_t)blob.size(); d.blob_bytes = (int32_t)o;
+    blob.resize(blob.size() + o, 0);
+    char* base = blob.data() + d.blob_off;
+    int32_t* dptr = (int32_t*)base; int32_t* dor = (int32_t*)(base + d.o_dord); int32_t* tptr = (int32_t*)(base + d.o_tptr);
+    int32_t* tor = (int32_t*)(base + d.o_tord); int32_t* pptr = (int32_t*)(base + d.o_pptr);
+    int2* dak = (int2*)(base + d.o_dak); int2* pmj = (int2*)(base + d.o_pmj); int4* tab = (int4*)(base + d.o_tab);
+    LevelLists L;
+    int32_t q = 0;
+    for (int i = 0; i < nm; ++i) {
+        dptr[i] = q; dor[i] = dord[i];
+        for (const int2& e : dl[dord[i]]) dak[q++] = e;
+        L.dlen.push_back((int)dl[dord[i]].size());
+    }
+    dptr[nm] = q; q = 0;
+    for (int i = 0; i < np; ++i) {
+        tptr[i] = q; tor[i] = tord[i];
+        for (const int4& e : tl[tord[i]]) tab[q++] = e;
+        L.tlen.push_back((int)tl[tord[i]].size());
+    }
+    tptr[np] = q;
+    for (int i = 0; i <= nm; ++i) pptr[i] = T.pair_ptr[d.m0 + i] - d.p0;
+    for (int i = 0; i < np; ++i) {
+        const int p = d.p0 + i, m = T.pair_row[p], j = T.pair_col[p];
+        pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
+    }
+    return L;
+}
+
+// Class cuts of one target kind for a kernel family with `lanes` lanes per slot and at most `wmax` lanes of one warp per
+// target: targets are sorted by descending list length `len`; a class is a run of targets that get the same number of
+// lanes 2^ssh.  A target asks for enough lanes to leave at most kSerial items per lane; when the level has more lanes than
+// its targets ask for, every target gets proportionally more (up to its list length), so that a narrow level spreads over
+// the whole CTA.  `unit` = lanes one target position stands for (2 for pair targets: two block-targets each).
+static int cut_classes(const std::vector<int>& len, int first, int count, int unit, int lanes, int wmax, Cls* cls) {
+    constexpr int kSerial = 2;
+    auto want = [&](int n, int boost) {
+        int s = 0;
+        while ((1 << s) < wmax && (n + (1 << s) - 1) / (1 << s) > kSerial) ++s;
+        while (boost > 0 && (2 << s) <= wmax && (2 << s) <= std::max(1, n)) { ++s; --boost; }
+        return s;
+    };
+    if (count <= 0) return 0;
+    int boost = 0;
+    for (;; ++boost) {          // largest boost that still fits the CTA in one round
+        int64_t need = 0;
+        for (int i = first; i < first + count; ++i) need += (int64_t)unit << want(len[i], boost + 1);
+        bool grew = false;
+        for (int i = first; i < first + count && !grew; ++i) grew = want(len[i], boost + 1) > want(len[i], boost);
+        if (need > lanes || !grew || boost >= 5) break;
+    }
+    std::vector<int> ssh(count);
+    for (int i = 0; i < count; ++i) ssh[i] = want(len[first + i], boost);
+    // at most kMaxCls classes: merge the smallest neighbouring runs upwards (a merged run takes the larger split)
+    std::vector<std::pair<int, int>> runs;      // (end index, ssh)
+    for (int i = 0; i < count; ++i) {
+        if (!runs.empty() && runs.back().second == ssh[i]) runs.back().first = i + 1;
+        else runs.push_back({i + 1, ssh[i]});
+    }
+    while ((int)runs.size() > kMaxCls) {
+        int best = 1; int bestlen = 1 << 30;
+        for (size_t r = 1; r < runs.size(); ++r) {
+            const int l = runs[r].first - runs[r - 1].first;
+            if (l < bestlen) { bestlen = l; best = (int)r; }
+        }
+        runs[best - 1].first = runs[best].first;      // run `best` joins its predecessor (larger or equal split: lists are sorted descending)
+        runs.erase(runs.begin() + best);
+    }
+    for (size_t r = 0; r < runs.size(); ++r) cls[r] = Cls{(first + runs[r].first) * unit, runs[r].second};
+    return (int)runs.size();
+}
+
+// lanes per target (log2) for the backward sweep of a level with n targets whose longest list has max_len entries
+static uint8_t pick_split(int n, int max_len, int lanes, int wmax) {
     int s = 0;
-    while ((2 << s) <= (32 >> gsh) && (int64_t)n * (2 << s) <= (threads >> gsh) && (2 << s) <= std::max(1, max_len)) ++s;
+    while ((2 << s) <= wmax && (int64_t)n * (2 << s) <= lanes && (2 << s) <= std::max(1, max_len)) ++s;
     return (uint8_t)s;
 }
 
-// level slices of the index program (layout: LevelDesc in sable_device.cuh)
-static void build_blobs(const Template& T, std::vector<LevelDesc>& lv, std::vector<char>& blob) {
-    lv.assign(T.n_level, LevelDesc{});
-    blob.clear();
-    auto al = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
-    for (int l = 0; l < T.n_level; ++l) {
-        LevelDesc& d = lv[l];
-        d.m0 = T.level_ptr[l]; d.m1 = T.level_ptr[l + 1]; d.p0 = T.pair_ptr[d.m0]; d.p1 = T.pair_ptr[d.m1];
-        const int nm = d.m1 - d.m0, np = d.p1 - d.p0;
-        const int nd = T.dterm_ptr[d.m1] - T.dterm_ptr[d.m0], nt = T.term_ptr[d.p1] - T.term_ptr[d.p0];
-        size_t o = 0;
-        o += (size_t)(nm + 1) * 4; d.o_tptr = (int32_t)o;
-        o += (size_t)(np + 1) * 4; d.o_pptr = (int32_t)o;
-        o += (size_t)(nm + 1) * 4; o = al(o, 8); d.o_dak = (int32_t)o;
-        o += (size_t)nd * 8; d.o_pmj = (int32_t)o;
-        o += (size_t)np * 8; d.o_tab = (int32_t)o;
-        o += (size_t)nt * 8; d.o_py = (int32_t)o;              // (the Y values of the pairs live in DevTemplate::pair_y)
-        o = al(o, 128);
-        d.blob_off = (int32_t)blob.size(); d.blob_bytes = (int32_t)o;
-        blob.resize(blob.size() + o, 0);
-        char* base = blob.data() + d.blob_off;
-        int32_t* dptr = (int32_t*)base; int32_t* tptr = (int32_t*)(base + d.o_tptr); int32_t* pptr = (int32_t*)(base + d.o_pptr);
-        int2* dak = (int2*)(base + d.o_dak); int2* pmj = (int2*)(base + d.o_pmj); int2* tab = (int2*)(base + d.o_tab);
-        for (int i = 0; i <= nm; ++i) {
-            dptr[i] = T.dterm_ptr[d.m0 + i] - T.dterm_ptr[d.m0];
-            pptr[i] = (T.pair_ptr[d.m0 + i] - d.p0) | ((i < nm && T.node_pq[d.m0 + i]) ? 1 << 30 : 0);
-        }
-        for (int i = 0; i <= np; ++i) tptr[i] = T.term_ptr[d.p0 + i] - T.term_ptr[d.p0];
-        for (int q = 0; q < nd; ++q) { const int a = T.dterm[T.dterm_ptr[d.m0] + q]; dak[q] = make_int2(a, T.pair_row[a]); }
-        for (int q = 0; q < nt; ++q) tab[q] = make_int2(T.term_a[T.term_ptr[d.p0] + q], T.term_b[T.term_ptr[d.p0] + q]);
-        for (int i = 0; i < np; ++i) {
-            const int p = d.p0 + i, m = T.pair_row[p], j = T.pair_col[p];
-            pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
-        }
-    }
+// splits / classes of one level descriptor for a kernel family (threads per CTA, slots per CTA)
+static void plan_level(const Template& T, LevelDesc& d, const LevelLists& L, int threads, int gsh, bool allow_big, bool staged) {
+    const int lanes = std::max(1, threads >> gsh), wmax = std::max(1, 32 >> gsh), nm = d.m1 - d.m0;
+    int nbig = 0;
+    if (allow_big && lanes >= 2 * wmax) while (nbig < nm && nbig < 4 && L.dlen[nbig] >= 3 * wmax && L.dlen[nbig] >= 64) ++nbig;
+    d.n_big = nbig;
+    d.n_dcls = (uint8_t)cut_classes(L.dlen, nbig, nm - nbig, 1, lanes, wmax, d.dcls);
+    int with_terms = 0;
+    while (with_terms < (int)L.tlen.size() && L.tlen[with_terms] > 0) ++with_terms;
+    d.n_tcls = (uint8_t)cut_classes(L.tlen, 0, with_terms, 2, lanes, wmax, d.tcls);
+    int maxb = 0;
+    for (int m = d.m0; m < d.m1; ++m) maxb = std::max(maxb, T.pair_ptr[m + 1] - T.pair_ptr[m]);
+    d.sb = pick_split(nm, maxb, lanes, wmax);
+    d.staged = staged;
 }
 
-// lane splits for a kernel family (threads per CTA, slots per CTA) and the streamed-level flag
-static std::vector<LevelDesc> build_levels(const Template& T, const std::vector<LevelDesc>& base, int threads, int gsh, int first_staged) {
-    std::vector<LevelDesc> lv(base);
-    for (int l = 0; l < T.n_level; ++l) {
-        LevelDesc& d = lv[l];
-        int maxd = 0, maxt = 0, maxb = 0;
-        for (int m = d.m0; m < d.m1; ++m) {
-            maxd = std::max(maxd, T.dterm_ptr[m + 1] - T.dterm_ptr[m]);
-            maxb = std::max(maxb, T.pair_ptr[m + 1] - T.pair_ptr[m]);
-        }
-        for (int p = d.p0; p < d.p1; ++p) maxt = std::max(maxt, T.term_ptr[p + 1] - T.term_ptr[p]);
-        d.sd = pick_split(d.m1 - d.m0, maxd, threads, gsh);
-        d.sp = pick_split(d.p1 - d.p0, maxt, threads, gsh);
-        d.sb = pick_split(d.m1 - d.m0, maxb, threads, gsh);
-        d.staged = l >= first_staged;
-    }
+struct LevelPack { std::vector<LevelDesc> lv; std::vector<LevelLists> lists; };
+
+static std::vector<LevelDesc> build_levels(const Template& T, const LevelPack& P, int threads, int gsh, bool allow_big, int first_staged) {
+    std::vector<LevelDesc> lv(P.lv);
+    for (int l = 0; l < T.n_level; ++l) plan_level(T, lv[l], P.lists[l], threads, gsh, allow_big, l >= first_staged);
     return lv;
 }
 
 // Dense top front (sable_front.cuh): the nodes of the last elimination levels, as many levels as keep the K x K block
 // matrix within `budget` bytes of shared memory per CTA (K <= kcap).  Appends the assembly lists (the front targets'
-// multiply-subtract terms whose eliminated node k lies below the front) to the blob and fills ctx->front*.
-static void build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap) {
+// items whose eliminated node k lies below the front) to the blob and fills ctx->front*.
+static void build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap, bool allow_big) {
     const Template& T = c->T;
     const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
     const bool mixed = c->opt.precision == SABLE_MIXED;
@@ -181,53 +278,18 @@ static void build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int 
     int lc = nl;
     while (lc > 1 && nn - T.level_ptr[lc - 1] <= kcap && bytes(nn - T.level_ptr[lc - 1]) <= budget) --lc;
     if (nl - lc < 2) return;                                 // merging fewer than two levels saves nothing
-    const int f0 = T.level_ptr[lc], K = nn - f0;
+    const int f0 = T.level_ptr[lc];
     LevelDesc d{};
     d.m0 = f0; d.m1 = nn; d.p0 = T.pair_ptr[f0]; d.p1 = np;
-    const int nm = K, npr = d.p1 - d.p0;
-    std::vector<int32_t> dptr(nm + 1, 0), tptr(npr + 1, 0);
-    std::vector<int2> dak, tab, pmj(npr);
-    int maxd = 0, maxt = 0;
-    for (int i = 0; i < nm; ++i) {
-        for (int q = T.dterm_ptr[f0 + i]; q < T.dterm_ptr[f0 + i + 1]; ++q) {
-            const int a = T.dterm[q], k = T.pair_row[a];
-            if (k < f0) dak.push_back(make_int2(a, k));
-        }
-        dptr[i + 1] = (int32_t)dak.size(); maxd = std::max(maxd, dptr[i + 1] - dptr[i]);
-    }
-    for (int i = 0; i < npr; ++i) {
-        const int p = d.p0 + i;
-        for (int q = T.term_ptr[p]; q < T.term_ptr[p + 1]; ++q)
-            if (T.pair_row[T.term_a[q]] < f0) tab.push_back(make_int2(T.term_a[q], T.term_b[q]));
-        tptr[i + 1] = (int32_t)tab.size(); maxt = std::max(maxt, tptr[i + 1] - tptr[i]);
-        const int m = T.pair_row[p], j = T.pair_col[p];
-        pmj[i] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
-    }
-    auto al = [](size_t x, size_t a) { return (x + a - 1) / a * a; };
-    size_t o = 0;
-    o += (size_t)(nm + 1) * 4; d.o_tptr = (int32_t)o;
-    o += (size_t)(npr + 1) * 4; d.o_pptr = (int32_t)o; o = al(o, 8); d.o_dak = (int32_t)o;
-    o += dak.size() * 8; d.o_pmj = (int32_t)o;
-    o += (size_t)npr * 8; d.o_tab = (int32_t)o;
-    o += tab.size() * 8; o = al(o, 128); d.o_py = (int32_t)o;
-    d.blob_off = (int32_t)c->blob_host.size(); d.blob_bytes = (int32_t)o;
-    c->blob_host.resize(c->blob_host.size() + o, 0);
-    char* base = c->blob_host.data() + d.blob_off;
-    memcpy(base, dptr.data(), dptr.size() * 4);
-    memcpy(base + d.o_tptr, tptr.data(), tptr.size() * 4);
-    if (!dak.empty()) memcpy(base + d.o_dak, dak.data(), dak.size() * 8);
-    if (!pmj.empty()) memcpy(base + d.o_pmj, pmj.data(), pmj.size() * 8);
-    if (!tab.empty()) memcpy(base + d.o_tab, tab.data(), tab.size() * 8);
-    d.sd = pick_split(nm, maxd, threads, gsh);
-    d.sp = pick_split(npr, maxt, threads, gsh);
-    c->front = d; c->front_k = K; c->front_f0 = f0; c->front_level = lc;
+    const LevelLists L = pack_level(T, d, f0, c->blob_host);
+    plan_level(T, d, L, threads, gsh, allow_big, false);
+    c->front = d; c->front_k = nn - f0; c->front_f0 = f0; c->front_level = lc;
 }
 
-// Launch plan of the fused kernel: as many scenario slots per CTA as fit entirely in shared
-// memory (G = 8, 4, 2, 1); if not even one fits, one slot per CTA with the top of the elimination tree (levels >=
-// cut_level) on chip and the wide early levels in the scenario's HBM slice.
-static sable_status choose_launch(sable_ctx* ctx) {
+// Launch plan of the fused kernel (DESIGN.md "Placement" and "Launch policy").
+static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     const Template& T = ctx->T;
+    const sable_tuning& tu = ctx->opt.tune;
     const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
     const bool mixed = ctx->opt.precision == SABLE_MIXED;
     int dev = 0; CU(cudaGetDevice(&dev));
@@ -235,96 +297,108 @@ static sable_status choose_launch(sable_ctx* ctx) {
     CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     CU(cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+    const int mb = ctx->opt.max_batch;
     int ring_bytes = 0;
-    auto need = [&](int gsh, int dgc, int prc, int stc) {
-        return mixed ? smem_need<float>(nn, np, nl, ring_bytes, gsh, dgc, prc, stc) : smem_need<double>(nn, np, nl, ring_bytes, gsh, dgc, prc, stc);
+    auto need = [&](int th, int gsh, bool on_chip) {
+        const int big = (int)big_bytes(th, gsh);
+        return mixed ? smem_need<float>(nn, np, nl, ring_bytes, big, gsh, on_chip) : smem_need<double>(nn, np, nl, ring_bytes, big, gsh, on_chip);
     };
     // ring candidates (slots, slot capacity): the streamed levels are the trailing run of levels whose blobs fit a slot
     struct RingOpt { int r, cap; };
-    const int r_env = env_int("SABLE_RING_R", -1), cap_env = env_int("SABLE_RING_SLOT", -1);
+    const bool ring_given = tune_given(tu.ring_slots, -1, "SABLE_RING_R") || tune_given(tu.ring_slot_bytes, -1, "SABLE_RING_SLOT");
     std::vector<RingOpt> ropts = {{3, 8192}, {2, 8192}, {3, 4096}, {2, 4096}, {2, 2048}, {0, 0}};
-    if (r_env >= 0 || cap_env >= 0) ropts = {{r_env >= 0 ? r_env : 3, cap_env >= 0 ? cap_env : 8192}, {0, 0}};
+    if (ring_given) ropts = {{tune(tu.ring_slots, -1, "SABLE_RING_R", 3, 0, kMaxRing), tune(tu.ring_slot_bytes, -1, "SABLE_RING_SLOT", 8192, 256, 65536) / 16 * 16}, {0, 0}};
     auto set_ring = [&](const RingOpt& o) {
         int first = nl, slot = 0;
-        if (o.r > 0) while (first > 0 && ctx->lv_host[first - 1].blob_bytes <= o.cap) { --first; slot = std::max(slot, ctx->lv_host[first].blob_bytes); }
+        if (o.r > 0) while (first > 0 && P.lv[first - 1].blob_bytes <= o.cap) { --first; slot = std::max(slot, P.lv[first].blob_bytes); }
         if (first == nl) { ctx->ring_r = 0; ctx->ring_slot = 0; ctx->first_staged = nl; ring_bytes = 0; return; }
         ctx->ring_r = o.r; ctx->ring_slot = slot; ctx->first_staged = first; ring_bytes = o.r * slot;
     };
-    int th = ctx->opt.threads;
-    if (th <= 0) th = nn <= 64 ? 64 : nn <= 200 ? 256 : (nn > 1200 && nn <= 4000) ? 256 : 512;   // measured: profiles/r01_v2_sweeps.md
-    th = env_int("SABLE_THREADS", th);
-    th = std::min(512, std::max(32, (th + 31) / 32 * 32));
-    const int mb = ctx->opt.max_batch;
-    int gsh = -1, want_ctas = 1;
-    const int g_env = env_int("SABLE_G", 0);
-    for (int cand = 3; cand >= 0 && gsh < 0; --cand) {
-        if (g_env > 0 && (1 << cand) != g_env) continue;
+    const bool th_given = ctx->opt.threads > 0 || tune_given(0, 0, "SABLE_THREADS");
+    const bool g_given = tune_given(tu.group, 0, "SABLE_G");
+    const int g_want = pow2_floor(tune(tu.group, 0, "SABLE_G", 1, 1, 32));
+    const int want_chip = tune(tu.on_chip, -1, "SABLE_ONCHIP", -1, -1, 1);
+    // ---- on-chip candidate: as many scenario slots per CTA as fit entirely in shared memory (G = 8, 4, 2, 1) ----------
+    int th0 = ctx->opt.threads > 0 ? ctx->opt.threads : nn <= 64 ? 64 : nn <= 200 ? 256 : 512;
+    th0 = std::min(512, std::max(32, (tune(0, 0, "SABLE_THREADS", th0, 32, 512) + 31) / 32 * 32));
+    int gsh0 = -1;
+    for (int cand = 3; cand >= 0 && gsh0 < 0 && want_chip != 0; --cand) {
+        if (g_given && (1 << cand) != g_want) continue;
         // do not group more scenarios per CTA than leaves every SM a CTA (small batches stay spread out)
-        if (g_env <= 0 && cand > 0 && (int64_t)n_sm * (1 << cand) > (int64_t)mb) continue;
-        // the blob ring pays only where the slots leave no L1 for the index program (measured: cfg 2 with 57 KB of L1
-        // left runs 0.133 ms without the ring, 0.147 ms with it; cfg 3 on chip with 21 KB left 4.9 ms vs 4.4 ms)
-        if (r_env < 0 && cap_env < 0) {
+        if (!g_given && cand > 0 && (int64_t)n_sm * (1 << cand) > (int64_t)mb) continue;
+        if ((th0 >> cand) < 8) continue;
+        // the blob ring pays only where the slots leave no L1 for the index program (measured in round 1: cfg 2 with
+        // 57 KB of L1 left runs 0.133 ms without the ring, 0.147 ms with it; cfg 3 on chip with 21 KB left 4.9 vs 4.4 ms)
+        if (!ring_given) {
             set_ring(RingOpt{0, 0});
-            const int64_t n0 = need(cand, 0, 0, 0) + 1024;
-            if (n0 <= max_optin && smem_sm - (smem_sm / n0) * n0 >= 32 * 1024) { gsh = cand; break; }
+            const int64_t n0 = need(th0, cand, true) + 1024;
+            if (n0 <= max_optin && smem_sm - (smem_sm / n0) * n0 >= 32 * 1024) { gsh0 = cand; break; }
         }
         for (const RingOpt& o : ropts) {
             set_ring(o);
-            if (need(cand, 0, 0, 0) <= max_optin) { gsh = cand; break; }
+            if (need(th0, cand, true) <= max_optin) { gsh0 = cand; break; }
         }
     }
-    const int cut_env = env_int("SABLE_CUT", -1);
     // all on chip only while the SMs can hold a good part of the batch at once; a batch of many waves runs faster from
-    // the group-interleaved HBM workspace with many small CTAs (cfg 3: 3.5 ms vs 4.4 ms, profiles/r01_v2_sweeps.md)
-    bool on_chip = gsh >= 0 && cut_env < 0;
-    if (on_chip && g_env <= 0 && env_int("SABLE_THREADS", 0) <= 0) {
-        const int64_t slots_sm = (int64_t)std::max<int64_t>(1, smem_sm / (need(gsh, 0, 0, 0) + 1024)) << gsh;
+    // the group-interleaved HBM workspace with many small CTAs (round 1: cfg 3 3.5 ms vs 4.4 ms)
+    bool on_chip = gsh0 >= 0;
+    if (on_chip && want_chip < 0 && !g_given && !th_given) {
+        const int64_t slots_sm = (int64_t)std::max<int64_t>(1, smem_sm / (need(th0, gsh0, true) + 1024)) << gsh0;
         if (slots_sm * n_sm * 2 < (int64_t)mb) on_chip = false;
     }
+    int th, gsh;
     if (on_chip) {
-        ctx->placement = 0; ctx->gsh = gsh; ctx->dg_cut = ctx->pr_cut = ctx->st_cut = 0; ctx->cut_level = 0;
+        ctx->placement = 0; th = th0; gsh = gsh0;
     } else {
-        // HBM placement.  Measured (profiles/r01_v2_sweeps.md): once the batch needs many waves, resident warps and a
-        // large L1 (which then holds the shared index program and Y_bus) buy more than shared-memory residency of the
-        // factors, and even a small on-chip top of the elimination tree is neutral to slightly negative: everything
-        // lives in the group-interleaved HBM workspace (placement 2, kernels without placement branches), the level
-        // blobs are read in place (no ring), and the register file sets the CTA count (72 registers for up to 128
-        // threads per CTA, 64 beyond).  SABLE_CUT=<level> asks for the mixed placement 1 (levels >= cut on chip).
-        if (ctx->opt.threads <= 0 && env_int("SABLE_THREADS", 0) <= 0) th = nn <= 1200 ? 128 : nn <= 4000 ? 256 : 512;
-        want_ctas = env_int("SABLE_CTAS", std::max(1, 1024 / th));
-        set_ring(r_env >= 0 ? ropts[0] : RingOpt{0, 0});
-        // slots per CTA (= scenarios whose HBM slices are interleaved): 4 for small grids, else 1 (measured), or SABLE_G
-        int sg = 0;
-        const int g_want = g_env > 0 ? g_env : (nn <= 1200 ? 4 : 1);
-        while ((2 << sg) <= g_want && (g_env > 0 || ((int64_t)n_sm << (sg + 1)) <= (int64_t)std::max(mb, 1))) ++sg;
-        const int cl = cut_env >= 0 ? std::min(cut_env, nl) : nl;
-        const int nc = cl < nl ? T.level_ptr[cl] : nn;
-        ctx->placement = cl < nl ? 1 : 2; ctx->gsh = sg; ctx->cut_level = cl;
-        ctx->dg_cut = nc; ctx->pr_cut = T.pair_ptr[nc]; ctx->st_cut = cl < nl ? nc : nn + 1;
-        if (ctx->placement == 1 && th <= 128) th = 256;      // the mixed kernel is built in the large variant only
-        if (need(sg, ctx->dg_cut, ctx->pr_cut, ctx->st_cut) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
+        // ---- HBM placement (everything in the group-interleaved workspace, blobs read in place, no ring) --------------
+        // Occupancy model: the path is latency-bound, so the SM should hold as many independent elimination chains
+        // (scenarios) as its registers allow, each with enough lanes for the wide levels.  Lanes per scenario
+        // L = 2^floor(log2(n_node / 8)) in [32, 512] (a level-1 target per lane or so); slots per CTA G such that a CTA
+        // has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72 registers) but never so many that
+        // the batch leaves SMs without a CTA.
+        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
+        int G = std::max(1, 128 / L);
+        if (g_given) G = g_want;
+        else while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
+        gsh = 0; while ((2 << gsh) <= G) ++gsh;
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : L << gsh;
+        th = std::min(1024, std::max(32 << 0, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
+        if ((th >> gsh) < 1) gsh = 0;
+        ctx->placement = 2;
+        set_ring(RingOpt{0, 0});
+        if (need(th, gsh, false) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
     }
-    ctx->threads = th;
-    ctx->smem = (int)need(ctx->gsh, ctx->dg_cut, ctx->pr_cut, ctx->st_cut);
+    ctx->threads = th; ctx->gsh = gsh;
+    ctx->variant = pick_variant(ctx->placement, th);
+    const int big = (int)big_bytes(th, gsh);
+    ctx->big_off = (int)(smem_fixed(nl, ring_bytes, 0));
+    ctx->slot_off = (int)smem_fixed(nl, ring_bytes, big);
+    ctx->smem = (int)need(th, gsh, on_chip);
     ctx->front_k = 0; ctx->front_level = nl; ctx->front_f0 = nn;
     if (ctx->placement == 2) {
-        // dense top front: shared memory that still leaves most of the L1 to the resident CTAs (measured budgets)
-        const int kcap = env_int("SABLE_FRONT", 64);
-        const int64_t budget = env_int("SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : 16) * 1024LL;
-        if (kcap >= 2) build_front(ctx, th, ctx->gsh, budget, std::min(kcap, 96));
+        // dense top front: shared memory that still leaves most of the L1 to the resident CTAs
+        const int kcap = tune(tu.front_nodes, -1, "SABLE_FRONT", 64, 0, 96);
+        const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : 16, 0, 220) * 1024LL;
+        if (kcap >= 2) build_front(ctx, th, gsh, budget, kcap, true);
         if (ctx->front_k > 0) {
             ctx->front_off = align16(ctx->smem);
-            ctx->smem = (int)(ctx->front_off + (mixed ? front_bytes<float>(ctx->front_k, ctx->gsh) : front_bytes<double>(ctx->front_k, ctx->gsh)));
+            ctx->smem = (int)(ctx->front_off + (mixed ? front_bytes<float>(ctx->front_k, gsh) : front_bytes<double>(ctx->front_k, gsh)));
         }
     }
-    const void* fn = fused_fn(mixed, ctx->placement, th <= 128);
+    if (ctx->smem > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "launch plan does not fit shared memory");
+    const void* fn = fused_fn(mixed, ctx->variant);
     CU(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->smem));
     int occ = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)ctx->smem));
     if (occ < 1) return fail(ctx, SABLE_ERR_CUDA, "NR kernel does not fit on an SM");
-    occ = std::min(occ, env_int("SABLE_CTAS", occ));
+    occ = std::min(occ, tune(tu.ctas_per_sm, 0, "SABLE_CTAS", occ, 1, 32));
     ctx->ctas_per_sm = occ; ctx->grid = occ * n_sm;
-    ctx->threads1 = env_int("SABLE_THREADS1", nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512);
+    // the other kernel families: staged kernels (same group layout; the fused kernel's own shape when it is an HBM kernel),
+    // the adjoint kernel (32 targets in flight per slot measured best in round 1), one-scenario debug kernels
+    const int Ls = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
+    ctx->threads_stage = (tune(tu.threads_stage, 0, "SABLE_THREADS1", ctx->placement == 2 ? std::min(th, 512) : std::min(512, Ls << gsh), 32, 512) + 31) / 32 * 32;
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     return SABLE_OK;
 }
 
@@ -334,11 +408,12 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     sable_ctx* ctx = nullptr;      // CU() reports into g_create_err while ctx is null
     if (!out) return fail(nullptr, SABLE_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
-    sable_options o{1, SABLE_FP64, 1, SABLE_MODE_FUSED, 0, 0};
+    sable_options o = sable_default_options();
     if (opt) o = *opt;
     if (o.max_batch < 1 || (o.precision != SABLE_FP64 && o.precision != SABLE_MIXED) ||
-        (o.mode != SABLE_MODE_FUSED && o.mode != SABLE_MODE_STAGED) || o.device < -1 || o.threads < 0)
-        return fail(nullptr, SABLE_ERR_INVALID_ARG, "bad option value");
+        (o.mode != SABLE_MODE_FUSED && o.mode != SABLE_MODE_STAGED) || o.device < -1 || o.threads < 0 || o.ir_sweeps != 0)
+        return fail(nullptr, SABLE_ERR_INVALID_ARG, o.ir_sweeps != 0 ? "ir_sweeps must be 0: the forward Newton loop (FP64 residual, FP32 correction) is the "
+                    "refinement (DESIGN.md reading 15); inner sweeps exist for the adjoint only (sable_adjoint_refined)" : "bad option value");
     sable_ctx* c = new (std::nothrow) sable_ctx;
     if (!c) return fail(nullptr, SABLE_ERR_ALLOC, "host allocation failed");
     c->opt = o;
@@ -350,8 +425,8 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     const Template& T = c->T;
     const int nn = T.n_node, np = (int)T.pair_col.size();
     auto bail = [&](sable_status s) { std::string m = c->err; sable_destroy(c); g_create_err = m; return s; };
-    cudaError_t e = cudaSetDevice(o.device);
-    if (e != cudaSuccess) { c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(e); return bail(SABLE_ERR_CUDA); }
+    DeviceGuard guard(o.device);
+    if (guard.err != cudaSuccess) { c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(guard.err); return bail(SABLE_ERR_CUDA); }
     // packed device arrays
     std::vector<int32_t> node_bus(T.node_bus); node_bus.push_back(T.slack);
     std::vector<double2> ygb(T.ycol.size()), ydg(nn);
@@ -389,7 +464,7 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     }
     bool ok = true;
     auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
-{
+    {
         std::vector<double2> fgb(T.fcol.size());
         for (size_t k = 0; k < fgb.size(); ++k) fgb[k] = make_double2(T.fg[k], T.fb[k]);
         up(T.fptr, &c->fptr); up(T.fcol, &c->fcol); up(fgb, &c->fgb);
@@ -407,15 +482,22 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(pmj, &d.pair_mj); up(py, &d.pair_y);
     if (!ok) return bail(SABLE_ERR_ALLOC);
     ctx = c;
-    build_blobs(T, c->lv_host, c->blob_host);
-    sable_status st = choose_launch(c);
+    LevelPack P;
+    P.lv.assign(T.n_level, LevelDesc{});
+    for (int l = 0; l < T.n_level; ++l) {
+        LevelDesc& ld = P.lv[l];
+        ld.m0 = T.level_ptr[l]; ld.m1 = T.level_ptr[l + 1]; ld.p0 = T.pair_ptr[ld.m0]; ld.p1 = T.pair_ptr[ld.m1];
+        P.lists.push_back(pack_level(T, ld, nn, c->blob_host));
+    }
+    c->lv_host = P.lv;
+    sable_status st = choose_launch(c, P);
     if (st != SABLE_OK) return bail(st);
     {
-        std::vector<LevelDesc> lf = build_levels(T, c->lv_host, c->threads, c->gsh, c->first_staged);
-        std::vector<LevelDesc> l1 = build_levels(T, c->lv_host, c->threads1, 0, T.n_level);
-        c->threads_lin = env_int("SABLE_THREADS_LIN", std::min(512, std::max(32 << c->gsh, 64)));   // 32 targets in flight per slot (measured)
-        std::vector<LevelDesc> ll = build_levels(T, c->lv_host, c->threads_lin, c->gsh, T.n_level);
-        up(lf, &c->level_fused); up(l1, &c->level_one); up(ll, &c->level_lin); up(c->blob_host, &d.blob);
+        std::vector<LevelDesc> lf = build_levels(T, P, c->threads, c->gsh, true, c->first_staged);
+        std::vector<LevelDesc> ls = build_levels(T, P, c->threads_stage, c->gsh, ((c->threads_stage >> 5) << c->gsh) <= 256, T.n_level);
+        std::vector<LevelDesc> ll = build_levels(T, P, c->threads_lin, c->gsh, true, T.n_level);
+        std::vector<LevelDesc> l1 = build_levels(T, P, c->threads1, 0, true, T.n_level);
+        up(lf, &c->level_fused); up(ls, &c->level_stage); up(ll, &c->level_lin); up(l1, &c->level_one); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
     }
     const bool mixed = o.precision == SABLE_MIXED;
@@ -426,16 +508,17 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         c->dev_allocs.push_back(*p); return true;
     };
     const size_t mb = (size_t)o.max_batch, nb = (size_t)T.n_bus;
-    // workspace for whole groups of 1 << gsh scenarios (fused mode interleaves a group's slices; staged mode: gsh 0)
+    // workspace for whole groups of 1 << gsh scenarios + one spare group that absorbs the stores of finished slots
     const size_t G = (size_t)1 << c->gsh, mb_alloc = (mb + G - 1) / G * G + G;
+    const size_t n_ints = kMaxChunk + 3 * mb + kMaxActive;
     if (!dmalloc((void**)&c->factors, mb_alloc * c->fac_stride) || !dmalloc((void**)&c->work, mb_alloc * c->work_stride) ||
-        !dmalloc((void**)&c->ints, (2 * mb + 4) * 4) || !dmalloc((void**)&c->hbuf, 9 * mb * nb * 8 + mb * 8) ||
-        !dmalloc((void**)&c->hbuf_it, mb * 4) || !dmalloc((void**)&c->hbuf_cv, mb) || !dmalloc((void**)&c->zeros, nb * 8) ||
-        !dmalloc((void**)&c->lbuf, 4 * mb * nb * 8))
+        !dmalloc((void**)&c->ints, n_ints * 4) || !dmalloc((void**)&c->zeros, nb * 8))
         return bail(SABLE_ERR_ALLOC);
     if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work, 0, mb_alloc * c->work_stride) != cudaSuccess ||
-        cudaMemset(c->factors, 0, mb_alloc * c->fac_stride) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
-    if (env_int("SABLE_TIMING", 0)) {
+        cudaMemset(c->factors, 0, mb_alloc * c->fac_stride) != cudaSuccess || cudaMemset(c->ints, 0, n_ints * 4) != cudaSuccess) {
+        c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA);
+    }
+    if (tune(o.tune.timing, 0, "SABLE_TIMING", 0, 0, 1)) {
         const size_t tb = (4 * (size_t)T.n_level + 4) * 8;
         if (!dmalloc((void**)&c->tim, tb)) return bail(SABLE_ERR_ALLOC);
         cudaMemset(c->tim, 0, tb);
@@ -445,9 +528,21 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     return SABLE_OK;
 }
 
+extern "C" sable_options sable_default_options(void) {
+    sable_options o{};
+    o.max_batch = 1; o.precision = SABLE_FP64; o.keep_factors = 1; o.mode = SABLE_MODE_FUSED; o.device = 0; o.threads = 0; o.ir_sweeps = 0;
+    o.tune.group = 0; o.tune.ctas_per_sm = 0; o.tune.on_chip = -1; o.tune.ring_slots = -1; o.tune.ring_slot_bytes = -1;
+    o.tune.front_nodes = -1; o.tune.front_kb = -1; o.tune.threads_stage = 0; o.tune.threads_lin = 0; o.tune.timing = 0;
+    return o;
+}
+
 extern "C" void sable_destroy(sable_ctx* c) {
     if (!c) return;
-    for (void* p : c->dev_allocs) cudaFree(p);
+    if (c->opt.device >= 0) {
+        DeviceGuard guard(c->opt.device);
+        for (cudaStream_t s : c->hstream) if (s) cudaStreamDestroy(s);
+        for (void* p : c->dev_allocs) cudaFree(p);
+    }
     delete c;
 }
 extern "C" const char* sable_last_error(const sable_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
@@ -458,83 +553,147 @@ extern "C" sable_status sable_get_info(const sable_ctx* c, sable_info* info) {
 }
 
 // ---- solve -------------------------------------------------------------------------------------------------------
+static int32_t* ctx_status(sable_ctx* c) { return c->ints + kMaxChunk; }
+static int32_t* ctx_it(sable_ctx* c) { return c->ints + kMaxChunk + c->opt.max_batch; }
+static int32_t* ctx_pivot(sable_ctx* c) { return c->ints + kMaxChunk + 2 * (size_t)c->opt.max_batch; }
+static int32_t* ctx_active(sable_ctx* c) { return c->ints + kMaxChunk + 3 * (size_t)c->opt.max_batch; }
+
 template <typename T>
-static cudaError_t launch_solve(sable_ctx* c, SolveArgs& A, cudaStream_t s) {
+static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s) {
+    const int G = 1 << c->gsh, grid = std::min((A.batch + G - 1) / G, c->grid);
+    switch (c->variant) {
+        case 0: k_nr_fused<T, 0, 512, 1><<<grid, c->threads, c->smem, s>>>(A); break;
+        case 1: k_nr_fused<T, 2, 128, 7><<<grid, c->threads, c->smem, s>>>(A); break;
+        case 2: k_nr_fused<T, 2, 256, 4><<<grid, c->threads, c->smem, s>>>(A); break;
+        case 3: k_nr_fused<T, 2, 512, 2><<<grid, c->threads, c->smem, s>>>(A); break;
+        default: k_nr_fused<T, 2, 1024, 1><<<grid, c->threads, c->smem, s>>>(A); break;
+    }
+    return cudaGetLastError();
+}
+
+// Scenarios [b0, b0 + nb) of the caller's arrays (b0 a multiple of the group size) on stream s, with queue counter `chunk`.
+template <typename T>
+static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int chunk, cudaStream_t s) {
+    const size_t o = (size_t)b0 * c->T.n_bus;
+    const int G = 1 << c->gsh, g0 = b0 >> c->gsh;
+    A.batch = nb;
+    A.p_spec += o; A.q_spec += o; A.v_set += o; if (A.vm0) { A.vm0 += o; A.va0 += o; }
+    A.vm += o; A.va += o; A.iterations += b0; A.converged += b0; if (A.final_norm) A.final_norm += b0;
+    A.pivot = ctx_pivot(c) + b0; A.status = ctx_status(c) + b0; A.it = ctx_it(c) + b0; A.active = ctx_active(c);
+    A.factors = c->factors + (size_t)g0 * G * c->fac_stride; A.work = c->work + (size_t)g0 * G * c->work_stride;
+    A.trash_grp = ((c->opt.max_batch + G - 1) >> c->gsh) - g0;
+    A.gsh = c->gsh; c->factor_gsh = c->gsh;
     if (c->opt.mode == SABLE_MODE_FUSED) {
+        A.queue = c->ints + chunk;
         cudaError_t e = cudaMemsetAsync(A.queue, 0, 4, s);
         if (e != cudaSuccess) return e;
         A.t.level = c->level_fused;
-        A.gsh = c->gsh; A.dg_cut = c->dg_cut; A.pr_cut = c->pr_cut; A.st_cut = c->st_cut;
         A.ring_r = c->ring_r; A.ring_slot = c->ring_slot; A.first_staged = c->first_staged;
-        A.trash_grp = (c->opt.max_batch + (1 << c->gsh) - 1) >> c->gsh;
+        A.big_off = c->big_off; A.slot_off = c->slot_off;
         A.front_k = c->front_k; A.front_f0 = c->front_f0; A.front_level = c->front_level; A.front_off = c->front_off; A.front = c->front;
-        const int G = 1 << c->gsh;
-        const int grid = std::min((A.batch + G - 1) / G, c->grid);
-        c->factor_gsh = c->gsh;
         // the attribute is per-function state shared by every live context: set it for THIS context right before the launch
-        e = cudaFuncSetAttribute(fused_fn(sizeof(T) == 4, c->placement, c->threads <= 128), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem);
+        e = cudaFuncSetAttribute(fused_fn(sizeof(T) == 4, c->variant), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem);
         if (e != cudaSuccess) return e;
-        if (c->placement == 0) k_nr_fused<T, 0, false><<<grid, c->threads, c->smem, s>>>(A);
-        else if (c->placement == 1) k_nr_fused<T, 1, false><<<grid, c->threads, c->smem, s>>>(A);
-        else if (c->threads <= 128) k_nr_fused<T, 2, true><<<grid, c->threads, c->smem, s>>>(A);
-        else k_nr_fused<T, 2, false><<<grid, c->threads, c->smem, s>>>(A);
+        e = launch_fused<T>(c, A, s);
         c->launches += 1;
-    } else {
-        A.t.level = c->level_one;
-        A.gsh = 0; c->factor_gsh = 0;
-        k_st_init<T><<<A.batch, c->threads1, 0, s>>>(A);
-        for (int i = 0; i <= A.max_it; ++i) {
-            k_st_mismatch_fill<T><<<A.batch, c->threads1, 0, s>>>(A);
-            if (i < A.max_it) k_st_factor_solve<T><<<A.batch, c->threads1, 0, s>>>(A);
+        return e;
+    }
+    // staged mode: one launch per stage; after three iterations the host reads the count of still-active scenarios after
+    // every mismatch pass and stops launching when it is zero (this mode synchronises; it exists for per-stage profiling)
+    A.t.level = c->level_stage;
+    const int grid = (nb + G - 1) / G, th = c->threads_stage;
+    cudaError_t e = cudaMemsetAsync(A.active, 0, kMaxActive * 4, s);
+    if (e != cudaSuccess) return e;
+    k_st_init<T><<<grid, th, 0, s>>>(A);
+    c->launches += 1;
+    for (int i = 0; i <= A.max_it; ++i) {
+        A.stage_it = std::min(i, kMaxActive - 1);
+        if (i >= kMaxActive - 1) cudaMemsetAsync(A.active + A.stage_it, 0, 4, s);
+        k_st_mismatch_fill<T><<<grid, th, 0, s>>>(A);
+        c->launches += 1;
+        if (i >= 3 || i == A.max_it) {
+            int32_t left = 0;
+            e = cudaMemcpyAsync(&left, A.active + A.stage_it, 4, cudaMemcpyDeviceToHost, s);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+            if (e != cudaSuccess) return e;
+            if (left == 0) break;
         }
-        c->launches += 2 + 2 * (int64_t)A.max_it;
+        if (i < A.max_it) { k_st_factor_solve<T><<<grid, th, 0, s>>>(A); c->launches += 1; }
     }
     return cudaGetLastError();
+}
+
+static sable_status check_solve_args(sable_ctx* ctx, int32_t batch, const void* p_spec, const void* q_spec, const void* v_set,
+                                     const void* vm0, const void* va0, double tol, int32_t max_it, const void* vm, const void* va,
+                                     const void* iterations, const void* converged) {
+    if (!ctx) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
+    if (max_it < 0 || !(tol >= 0.0)) return fail(ctx, SABLE_ERR_INVALID_ARG, "max_it < 0 or tol < 0");
+    if (batch > 0 && (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr))))
+        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
+    return SABLE_OK;
+}
+
+static SolveArgs base_args(sable_ctx* ctx, const double* p_spec, const double* q_spec, const double* v_set, const double* vm0,
+                           const double* va0, double tol, int32_t max_it, double* vm, double* va, int32_t* iterations,
+                           uint8_t* converged, double* final_norm) {
+    SolveArgs A{};
+    A.t = ctx->d; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.tol = tol;
+    A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
+    A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
+    A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride; A.tim = ctx->tim;
+    return A;
 }
 
 extern "C" sable_status sable_solve(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
                                     const double* v_set, const double* vm0, const double* va0, double tol, int32_t max_it,
                                     double* vm, double* va, int32_t* iterations, uint8_t* converged, double* final_norm,
                                     void* cuda_stream) {
-    if (!ctx) return SABLE_ERR_INVALID_ARG;
-    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
-    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
-    if (max_it < 0 || !(tol >= 0.0)) return fail(ctx, SABLE_ERR_INVALID_ARG, "max_it < 0 or tol < 0");
+    sable_status st = check_solve_args(ctx, batch, p_spec, q_spec, v_set, vm0, va0, tol, max_it, vm, va, iterations, converged);
+    if (st != SABLE_OK) return st;
     ctx->have_factors = false; ctx->last_batch = batch;
     if (batch == 0) return SABLE_OK;                       /* empty batch: nothing is read or written */
-    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
-        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array (vm0 and va0 must both be given or both be NULL)");
     ON_DEVICE(ctx);
-    SolveArgs A{};
-    A.t = ctx->d; A.batch = batch; A.max_it = max_it; A.keep = ctx->opt.keep_factors; A.tol = tol;
-    A.p_spec = p_spec; A.q_spec = q_spec; A.v_set = v_set; A.vm0 = vm0; A.va0 = va0;
-    A.vm = vm; A.va = va; A.final_norm = final_norm; A.iterations = iterations; A.converged = converged;
-    A.factors = ctx->factors; A.work = ctx->work; A.fac_stride = ctx->fac_stride; A.work_stride = ctx->work_stride;
-    A.tim = ctx->tim;
-    A.queue = ctx->ints; A.status = ctx->ints + 4; A.it = ctx->ints + 4 + ctx->opt.max_batch;
+    const SolveArgs A = base_args(ctx, p_spec, q_spec, v_set, vm0, va0, tol, max_it, vm, va, iterations, converged, final_norm);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    CU(ctx->opt.precision == SABLE_MIXED ? launch_solve<float>(ctx, A, s) : launch_solve<double>(ctx, A, s));
+    CU(ctx->opt.precision == SABLE_MIXED ? launch_solve<float>(ctx, A, 0, batch, 0, s) : launch_solve<double>(ctx, A, 0, batch, 0, s));
     ctx->have_factors = ctx->opt.keep_factors != 0;
     return SABLE_OK;
 }
 
+extern "C" sable_status sable_get_pivot_flags(sable_ctx* ctx, int32_t batch, int32_t* flags, void* cuda_stream) {
+    if (!ctx || !flags) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch != ctx->last_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch differs from the last sable_solve");
+    if (batch == 0) return SABLE_OK;
+    ON_DEVICE(ctx);
+    CU(cudaMemcpyAsync(flags, ctx_pivot(ctx), (size_t)batch * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return SABLE_OK;
+}
+
 // ---- adjoint / linear solves on kept factors ---------------------------------------------------------------------
-static sable_status launch_lin(sable_ctx* ctx, int batch, const double* rp, const double* rq, int transposed, double* xp,
-                               double* xq, cudaStream_t s) {
+static sable_status launch_lin(sable_ctx* ctx, int b0, int batch, const double* rp, const double* rq, int transposed, double* xp,
+                               double* xq, bool use_flags, cudaStream_t s) {
     LinArgs L{};
-    const int gsh = ctx->factor_gsh, G = 1 << gsh;
+    const int gsh = ctx->factor_gsh, G = 1 << gsh, g0 = b0 >> gsh;
+    const size_t o = (size_t)b0 * ctx->T.n_bus;
     L.t = ctx->d;
     L.t.level = gsh == 0 ? ctx->level_one : ctx->level_lin;
-    L.batch = batch; L.transposed = transposed; L.gsh = gsh; L.rhs_p = rp; L.rhs_q = rq; L.x_p = xp; L.x_q = xq;
-    L.factors = ctx->factors; L.fac_stride = ctx->fac_stride; L.work = ctx->work; L.work_stride = ctx->work_stride;
-    const size_t sm = ((size_t)ctx->T.n_node * 16) << gsh;
-    int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
-    L.rhs_in_smem = sm <= std::min<size_t>((size_t)max_optin, 64 * 1024);
-    const void* lin = ctx->opt.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
-    if (L.rhs_in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    L.batch = batch; L.transposed = transposed; L.gsh = gsh; L.rhs_p = rp + o; L.rhs_q = rq + o; L.x_p = xp + o; L.x_q = xq + o;
+    L.pivot = use_flags ? ctx_pivot(ctx) + b0 : nullptr;
+    L.factors = ctx->factors + (size_t)g0 * G * ctx->fac_stride; L.fac_stride = ctx->fac_stride;
+    L.work = ctx->work + (size_t)g0 * G * ctx->work_stride; L.work_stride = ctx->work_stride;
     const int th = gsh == 0 ? ctx->threads1 : ctx->threads_lin, grid = (batch + G - 1) / G;
-    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<grid, th, L.rhs_in_smem ? sm : 0, s>>>(L);
-    else k_linsolve<double><<<grid, th, L.rhs_in_smem ? sm : 0, s>>>(L);
+    L.big_off = (int)align16(big_bytes(th, gsh));
+    const size_t rhs = ((size_t)ctx->T.n_node * 16) << gsh;
+    int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
+    L.rhs_in_smem = L.big_off + rhs <= std::min<size_t>((size_t)max_optin, 64 * 1024);
+    const size_t sm = L.big_off + (L.rhs_in_smem ? rhs : 0);
+    const void* lin = ctx->opt.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
+    CU(cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(sm, 48 * 1024)));
+    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<grid, th, sm, s>>>(L);
+    else k_linsolve<double><<<grid, th, sm, s>>>(L);
     ctx->launches += 1;
     CU(cudaGetLastError());
     return SABLE_OK;
@@ -549,7 +708,7 @@ extern "C" sable_status sable_adjoint(sable_ctx* ctx, int32_t batch, const doubl
     if (!g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (batch == 0) return SABLE_OK;
     ON_DEVICE(ctx);
-    return launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, (cudaStream_t)cuda_stream);
+    return launch_lin(ctx, 0, batch, g_va, g_vm, 1, lam_p, lam_q, true, (cudaStream_t)cuda_stream);
 }
 
 // ---- Step-2 explicit recovery ---------------------------------------------------------------------------------------
@@ -574,6 +733,15 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     return SABLE_OK;
 }
 
+// scratch of the layer / refinement calls: four [max_batch][n_bus] arrays, allocated at the first such call
+static sable_status need_lbuf(sable_ctx* ctx) {
+    if (ctx->lbuf) return SABLE_OK;
+    void* p = nullptr;
+    CU(cudaMalloc(&p, 4 * (size_t)ctx->opt.max_batch * ctx->T.n_bus * 8));
+    ctx->dev_allocs.push_back(p); ctx->lbuf = (double*)p;
+    return SABLE_OK;
+}
+
 // ---- implicit-layer backward ----------------------------------------------------------------------------------------
 extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, const double* vm, const double* va,
                                              const double* gl_pg, const double* gl_qg, const double* gl_vm, const double* gl_va,
@@ -585,6 +753,7 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     if (!vm || !va || !gl_pg || !gl_qg || !gl_vm || !gl_va || !dx_pg || !dx_vm) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     if (batch == 0) return SABLE_OK;
     ON_DEVICE(ctx);
+    sable_status st = need_lbuf(ctx); if (st != SABLE_OK) return st;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus;
     LayerArgs L{};
@@ -599,7 +768,7 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     L.post = 0;
     k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
     CU(cudaGetLastError());
-    sable_status st = launch_lin(ctx, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, s);
+    st = launch_lin(ctx, 0, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, true, s);
     if (st != SABLE_OK) return st;
     L.post = 1;
     k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
@@ -621,8 +790,9 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
     if (batch == 0) return SABLE_OK;
     ON_DEVICE(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    sable_status st = launch_lin(ctx, batch, g_va, g_vm, 1, lam_p, lam_q, s);
+    sable_status st = launch_lin(ctx, 0, batch, g_va, g_vm, 1, lam_p, lam_q, true, s);
     if (st != SABLE_OK || sweeps == 0) return st;
+    st = need_lbuf(ctx); if (st != SABLE_OK) return st;
     const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus, nb = (size_t)batch * ctx->T.n_bus;
     LayerArgs L{};
     L.n_bus = ctx->T.n_bus; L.batch = batch; L.fptr = ctx->fptr; L.fcol = ctx->fcol; L.ftpos = ctx->ftpos; L.fgb = ctx->fgb;
@@ -635,7 +805,7 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
     for (int it = 0; it < sweeps; ++it) {
         k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);                                   // r = g - J1^T lambda   (FP64)
         CU(cudaGetLastError());
-        st = launch_lin(ctx, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, s);   // J1^T d = r  (kept factors)
+        st = launch_lin(ctx, 0, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, false, s);   // J1^T d = r  (kept factors)
         if (st != SABLE_OK) return st;
         k_add2<<<(int)std::min<size_t>((nb + 255) / 256, 4096), 256, 0, s>>>(lam_p, lam_q, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, nb);
         CU(cudaGetLastError());
@@ -645,33 +815,62 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
 }
 
 // ---- host-buffer wrappers (end-to-end path: H2D, solve, D2H; synchronous) ------------------------------------------
+// The batch is cut into up to kMaxChunk chunks of whole groups, each on its own stream: copy in, kernel, copy out.  The
+// copies of one chunk overlap the kernels of the others (and the kernels one another: every chunk has its own queue
+// counter and its own part of the workspace), so the exposed copy time is about that of one chunk.
+static sable_status need_hbuf(sable_ctx* ctx) {
+    if (ctx->hbuf) return SABLE_OK;
+    const size_t mb = (size_t)ctx->opt.max_batch, nb = (size_t)ctx->T.n_bus;
+    void *a = nullptr, *b = nullptr, *c = nullptr;
+    CU(cudaMalloc(&a, 9 * mb * nb * 8 + mb * 8)); ctx->dev_allocs.push_back(a); ctx->hbuf = (double*)a;
+    CU(cudaMalloc(&b, mb * 4)); ctx->dev_allocs.push_back(b); ctx->hbuf_it = (int32_t*)b;
+    CU(cudaMalloc(&c, mb)); ctx->dev_allocs.push_back(c); ctx->hbuf_cv = (uint8_t*)c;
+    for (int i = 0; i < kMaxChunk; ++i) CU(cudaStreamCreateWithFlags(&ctx->hstream[i], cudaStreamNonBlocking));
+    return SABLE_OK;
+}
+static int host_chunks(const sable_ctx* ctx, int batch, int* per) {
+    const int G = 1 << ctx->gsh, groups = (batch + G - 1) / G;
+    // a chunk should still give every SM its CTAs; a staged-mode solve synchronises inside, so it is not cut
+    int n = ctx->opt.mode == SABLE_MODE_STAGED ? 1 : std::max(1, std::min(kMaxChunk, groups / std::max(1, ctx->grid / 4)));
+    n = std::max(1, std::min(n, groups));
+    *per = (groups + n - 1) / n * G;
+    return (batch + *per - 1) / *per;
+}
+
 extern "C" sable_status sable_solve_host(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
                                          const double* v_set, const double* vm0, const double* va0, double tol,
                                          int32_t max_it, double* vm, double* va, int32_t* iterations, uint8_t* converged,
                                          double* final_norm) {
-    if (!ctx) return SABLE_ERR_INVALID_ARG;
-    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
-    if (batch < 0 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
-    if (!p_spec || !q_spec || !v_set || !vm || !va || !iterations || !converged || ((vm0 == nullptr) != (va0 == nullptr)))
-        return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
-    if (batch == 0) { ctx->have_factors = false; ctx->last_batch = 0; return SABLE_OK; }
-    ON_DEVICE(ctx);
-    const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
-    double* d = ctx->hbuf;       // slots: 0 p, 1 q, 2 vset, 3 vm0, 4 va0, 5 vm, 6 va, (7, 8 adjoint), then norm
-    double* dn = ctx->hbuf + 9 * (size_t)ctx->opt.max_batch * ctx->T.n_bus;
-    CU(cudaMemcpyAsync(d, p_spec, bytes, cudaMemcpyHostToDevice, 0));
-    CU(cudaMemcpyAsync(d + n, q_spec, bytes, cudaMemcpyHostToDevice, 0));
-    CU(cudaMemcpyAsync(d + 2 * n, v_set, bytes, cudaMemcpyHostToDevice, 0));
-    if (vm0) { CU(cudaMemcpyAsync(d + 3 * n, vm0, bytes, cudaMemcpyHostToDevice, 0)); CU(cudaMemcpyAsync(d + 4 * n, va0, bytes, cudaMemcpyHostToDevice, 0)); }
-    sable_status st = sable_solve(ctx, batch, d, d + n, d + 2 * n, vm0 ? d + 3 * n : nullptr, vm0 ? d + 4 * n : nullptr, tol, max_it,
-                                  d + 5 * n, d + 6 * n, ctx->hbuf_it, ctx->hbuf_cv, dn, nullptr);
+    sable_status st = check_solve_args(ctx, batch, p_spec, q_spec, v_set, vm0, va0, tol, max_it, vm, va, iterations, converged);
     if (st != SABLE_OK) return st;
-    CU(cudaMemcpyAsync(vm, d + 5 * n, bytes, cudaMemcpyDeviceToHost, 0));
-    CU(cudaMemcpyAsync(va, d + 6 * n, bytes, cudaMemcpyDeviceToHost, 0));
-    CU(cudaMemcpyAsync(iterations, ctx->hbuf_it, (size_t)batch * 4, cudaMemcpyDeviceToHost, 0));
-    CU(cudaMemcpyAsync(converged, ctx->hbuf_cv, (size_t)batch, cudaMemcpyDeviceToHost, 0));
-    if (final_norm) CU(cudaMemcpyAsync(final_norm, dn, (size_t)batch * 8, cudaMemcpyDeviceToHost, 0));
-    CU(cudaStreamSynchronize(0));
+    ctx->have_factors = false; ctx->last_batch = batch;
+    if (batch == 0) return SABLE_OK;
+    ON_DEVICE(ctx);
+    st = need_hbuf(ctx); if (st != SABLE_OK) return st;
+    const size_t nbus = (size_t)ctx->T.n_bus, n = (size_t)ctx->opt.max_batch * nbus;
+    double* d = ctx->hbuf;       // slots: 0 p, 1 q, 2 vset, 3 vm0, 4 va0, 5 vm, 6 va, (7, 8 adjoint), then norm
+    double* dn = ctx->hbuf + 9 * n;
+    const SolveArgs A = base_args(ctx, d, d + n, d + 2 * n, vm0 ? d + 3 * n : nullptr, vm0 ? d + 4 * n : nullptr, tol, max_it,
+                                  d + 5 * n, d + 6 * n, ctx->hbuf_it, ctx->hbuf_cv, dn);
+    int per = 0;
+    const int nch = host_chunks(ctx, batch, &per);
+    for (int c = 0; c < nch; ++c) {
+        const int b0 = c * per, nb = std::min(per, batch - b0);
+        const size_t o = (size_t)b0 * nbus, bytes = (size_t)nb * nbus * 8;
+        cudaStream_t s = ctx->hstream[c];
+        CU(cudaMemcpyAsync(d + o, p_spec + o, bytes, cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(d + n + o, q_spec + o, bytes, cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(d + 2 * n + o, v_set + o, bytes, cudaMemcpyHostToDevice, s));
+        if (vm0) { CU(cudaMemcpyAsync(d + 3 * n + o, vm0 + o, bytes, cudaMemcpyHostToDevice, s)); CU(cudaMemcpyAsync(d + 4 * n + o, va0 + o, bytes, cudaMemcpyHostToDevice, s)); }
+        CU(ctx->opt.precision == SABLE_MIXED ? launch_solve<float>(ctx, A, b0, nb, c, s) : launch_solve<double>(ctx, A, b0, nb, c, s));
+        CU(cudaMemcpyAsync(vm + o, d + 5 * n + o, bytes, cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(va + o, d + 6 * n + o, bytes, cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(iterations + b0, ctx->hbuf_it + b0, (size_t)nb * 4, cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(converged + b0, ctx->hbuf_cv + b0, (size_t)nb, cudaMemcpyDeviceToHost, s));
+        if (final_norm) CU(cudaMemcpyAsync(final_norm + b0, dn + b0, (size_t)nb * 8, cudaMemcpyDeviceToHost, s));
+    }
+    for (int c = 0; c < nch; ++c) CU(cudaStreamSynchronize(ctx->hstream[c]));
+    ctx->have_factors = ctx->opt.keep_factors != 0;
     return SABLE_OK;
 }
 
@@ -679,18 +878,77 @@ extern "C" sable_status sable_adjoint_host(sable_ctx* ctx, int32_t batch, const 
                                            double* lam_p, double* lam_q) {
     if (!ctx) return SABLE_ERR_INVALID_ARG;
     if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
-    if (batch < 0 || batch > ctx->opt.max_batch || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "bad argument");
+    if (!ctx->have_factors) return fail(ctx, SABLE_ERR_STATE, "no kept factors: call sable_solve_host with keep_factors = 1 first");
+    if (batch != ctx->last_batch || !g_va || !g_vm || !lam_p || !lam_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "bad argument");
     if (batch == 0) return SABLE_OK;
     ON_DEVICE(ctx);
-    const size_t n = (size_t)batch * ctx->T.n_bus, bytes = n * 8;
+    sable_status st = need_hbuf(ctx); if (st != SABLE_OK) return st;
+    const size_t nbus = (size_t)ctx->T.n_bus, n = (size_t)ctx->opt.max_batch * nbus;
     double* d = ctx->hbuf;
-    CU(cudaMemcpyAsync(d, g_va, bytes, cudaMemcpyHostToDevice, 0));
-    CU(cudaMemcpyAsync(d + n, g_vm, bytes, cudaMemcpyHostToDevice, 0));
-    sable_status st = sable_adjoint(ctx, batch, d, d + n, d + 7 * n, d + 8 * n, nullptr);
-    if (st != SABLE_OK) return st;
-    CU(cudaMemcpyAsync(lam_p, d + 7 * n, bytes, cudaMemcpyDeviceToHost, 0));
-    CU(cudaMemcpyAsync(lam_q, d + 8 * n, bytes, cudaMemcpyDeviceToHost, 0));
-    CU(cudaStreamSynchronize(0));
+    int per = 0;
+    const int nch = host_chunks(ctx, batch, &per);
+    for (int c = 0; c < nch; ++c) {
+        const int b0 = c * per, nb = std::min(per, batch - b0);
+        const size_t o = (size_t)b0 * nbus, bytes = (size_t)nb * nbus * 8;
+        cudaStream_t s = ctx->hstream[c];
+        CU(cudaMemcpyAsync(d + o, g_va + o, bytes, cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(d + n + o, g_vm + o, bytes, cudaMemcpyHostToDevice, s));
+        st = launch_lin(ctx, b0, nb, d, d + n, 1, d + 7 * n, d + 8 * n, true, s);
+        if (st != SABLE_OK) return st;
+        CU(cudaMemcpyAsync(lam_p + o, d + 7 * n + o, bytes, cudaMemcpyDeviceToHost, s));
+        CU(cudaMemcpyAsync(lam_q + o, d + 8 * n + o, bytes, cudaMemcpyDeviceToHost, s));
+    }
+    for (int c = 0; c < nch; ++c) CU(cudaStreamSynchronize(ctx->hstream[c]));
+    return SABLE_OK;
+}
+
+// ---- per-stage times in the default workspace layout (debug / measurement) ------------------------------------------------
+// Runs the staged kernels (the fused kernel's own stage routines, one stage per launch, group-interleaved workspace) for
+// three Newton iterations from the flat start on the given batch and returns the mean CUDA-event time of the mismatch +
+// fill launch and of the refactor + solve launch (ms) -- all scenarios are still active in those iterations.  Synchronous;
+// overwrites the workspace (kept factors are gone).
+extern "C" sable_status sable_debug_stage_times(sable_ctx* ctx, int32_t batch, const double* p_spec, const double* q_spec,
+                                                const double* v_set, double* ms_mismatch_fill, double* ms_factor_solve, void* cuda_stream) {
+    if (!ctx || !ms_mismatch_fill || !ms_factor_solve) return SABLE_ERR_INVALID_ARG;
+    if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
+    if (batch < 1 || batch > ctx->opt.max_batch || !p_spec || !q_spec || !v_set) return fail(ctx, SABLE_ERR_INVALID_ARG, "bad argument");
+    ON_DEVICE(ctx);
+    sable_status st = need_lbuf(ctx); if (st != SABLE_OK) return st;     // outputs nobody reads: vm, va -> lbuf
+    ctx->have_factors = false;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)ctx->opt.max_batch * ctx->T.n_bus;
+    SolveArgs A = base_args(ctx, p_spec, q_spec, v_set, nullptr, nullptr, 0.0, 1000, ctx->lbuf, ctx->lbuf + n, ctx_it(ctx), (uint8_t*)(ctx->lbuf + 2 * n), nullptr);
+    A.iterations = (int32_t*)(ctx->lbuf + 3 * n);
+    A.keep = 0; A.batch = batch;
+    A.pivot = ctx_pivot(ctx); A.status = ctx_status(ctx); A.it = ctx_it(ctx); A.active = ctx_active(ctx); A.stage_it = 0;
+    A.factors = ctx->factors; A.work = ctx->work;
+    const int G = 1 << ctx->gsh;
+    A.trash_grp = (ctx->opt.max_batch + G - 1) >> ctx->gsh; A.gsh = ctx->gsh; ctx->factor_gsh = ctx->gsh;
+    A.t.level = ctx->level_stage;
+    const int grid = (batch + G - 1) / G, th = ctx->threads_stage;
+    const bool mixed = ctx->opt.precision == SABLE_MIXED;
+    cudaEvent_t ev[7];
+    for (auto& e : ev) CU(cudaEventCreate(&e));
+    if (mixed) k_st_init<float><<<grid, th, 0, s>>>(A); else k_st_init<double><<<grid, th, 0, s>>>(A);
+    for (int i = 0; i < 3; ++i) {
+        CU(cudaEventRecord(ev[2 * i], s));
+        if (mixed) k_st_mismatch_fill<float><<<grid, th, 0, s>>>(A); else k_st_mismatch_fill<double><<<grid, th, 0, s>>>(A);
+        CU(cudaEventRecord(ev[2 * i + 1], s));
+        if (mixed) k_st_factor_solve<float><<<grid, th, 0, s>>>(A); else k_st_factor_solve<double><<<grid, th, 0, s>>>(A);
+    }
+    CU(cudaEventRecord(ev[6], s));
+    CU(cudaStreamSynchronize(s));
+    CU(cudaGetLastError());
+    ctx->launches += 7;
+    double a = 0, b = 0;
+    for (int i = 0; i < 3; ++i) {
+        float x = 0, y = 0;
+        CU(cudaEventElapsedTime(&x, ev[2 * i], ev[2 * i + 1]));
+        CU(cudaEventElapsedTime(&y, ev[2 * i + 1], ev[2 * i + 2]));
+        a += x / 3.0; b += y / 3.0;
+    }
+    for (auto& e : ev) cudaEventDestroy(e);
+    *ms_mismatch_fill = a; *ms_factor_solve = b;
     return SABLE_OK;
 }
 
@@ -717,7 +975,7 @@ extern "C" sable_status sable_debug_pattern(const sable_ctx* c, int32_t* node_bu
 }
 
 static sable_status launch_debug(sable_ctx* ctx, DebugArgs& D, cudaStream_t s) {
-    D.t = ctx->d; D.t.level = ctx->level_one; D.zeros = ctx->zeros; ctx->factor_gsh = 0;
+    D.t = ctx->d; D.t.level = ctx->level_one; D.zeros = ctx->zeros; ctx->factor_gsh = 0; D.pivot = D.what == 2 ? ctx_pivot(ctx) : nullptr;
     D.factors = ctx->factors; D.work = ctx->work; D.fac_stride = ctx->fac_stride; D.work_stride = ctx->work_stride;
     if (ctx->opt.precision == SABLE_MIXED) k_debug<float><<<D.batch, ctx->threads1, 0, s>>>(D);
     else k_debug<double><<<D.batch, ctx->threads1, 0, s>>>(D);
@@ -729,7 +987,7 @@ static sable_status debug_check(sable_ctx* ctx, int batch) {
     if (!ctx) return SABLE_ERR_INVALID_ARG;
     if (ctx->opt.device < 0) return fail(ctx, SABLE_ERR_STATE, "host-only context");
     if (batch < 1 || batch > ctx->opt.max_batch) return fail(ctx, SABLE_ERR_INVALID_ARG, "batch out of range");
-    ctx->have_factors = false;
+    ctx->have_factors = false; ctx->last_batch = batch;
     return SABLE_OK;
 }
 
@@ -760,5 +1018,5 @@ extern "C" sable_status sable_debug_linear_solve(sable_ctx* ctx, int32_t batch, 
     if (!vm || !va || !rhs_p || !rhs_q || !x_p || !x_q) return fail(ctx, SABLE_ERR_INVALID_ARG, "null array");
     DebugArgs D{}; D.batch = batch; D.what = 2; D.vm = vm; D.va = va;
     st = launch_debug(ctx, D, (cudaStream_t)cuda_stream); if (st) return st;
-    return launch_lin(ctx, batch, rhs_p, rhs_q, transpose ? 1 : 0, x_p, x_q, (cudaStream_t)cuda_stream);
+    return launch_lin(ctx, 0, batch, rhs_p, rhs_q, transpose ? 1 : 0, x_p, x_q, false, (cudaStream_t)cuda_stream);
 }

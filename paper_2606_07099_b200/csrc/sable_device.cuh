@@ -2,46 +2,56 @@
 //
 // Block conventions.  Every non-slack bus is a node with a 2x2 block: rows (P_m, Q_m), columns (theta_m, Vm_m),
 // stored row-major [dP/dth, dP/dVm, dQ/dth, dQ/dVm].  A PV node keeps the block with the Q row and Vm column padded
-// (0 off the diagonal, 1 on it).  Per scenario the factor storage is, in units of one block (4 values of T):
-//   dg[n_node]     : J(m,m), then after refactor the INVERSE of the pivot block D_m
-//   pr[2*n_pair]   : pair p = (m,j), m < j:  pr[2p] = J(m,j) -> U(m,j);  pr[2p+1] = J(j,m) -> L(j,m)
-// and the state, three 16-byte records per node (index n_node = slack):
-//   vv = (V_re, V_im)   ma = (|V|, theta)   rh = (rhs_P/theta, rhs_Q/Vm): -F, then y, then dz (g, w, lambda: adjoint)
+// (0 off the diagonal, 1 on it).  The factorisation is kept in the form  J1 = L' D^-1 U  (L' = the UNSCALED lower
+// blocks, U upper blocks, D the pivot blocks):  per scenario, in units of one block (4 values of T),
+//   dg[n_node]   : J(m,m), then after refactor the INVERSE of the pivot block D_m
+//   pu[n_pair]   : pair p = (m,j), m < j:  J(m,j) -> U(m,j)
+//   pl[n_pair]   :                         J(j,m) -> L'(j,m) = J(j,m) - sum_k L'(j,k) D_k^-1 U(k,m)
+// (U and L' in two separate arrays: a triangular sweep streams whole sectors of the one it needs) and the state,
+// three 16-byte records per node (index n_node = slack):
+//   vv = (V_re, V_im)   ma = (|V|, theta)   rh = (rhs_P/theta, rhs_Q/Vm): -F, then z = D^-1 y, then dz (g, w, lambda: adjoint)
+// Keeping L' unscaled removes the "scale by D_m^-1" phase (and its barrier) from every elimination level: a consumer
+// multiplies by D_k^-1 of the eliminated node k on the fly (one more L1-resident block per term).
 //
-// Placement.  A CTA works on G = 2^gsh scenarios in lockstep ("slots"; thread tid serves slot g = tid % G).  The late
-// part of every array (nodes >= cut, pairs >= cut: the top of the elimination tree, where levels are narrow and
-// latency decides) lives in shared memory, interleaved over the slots in 16-byte vectors:
+// Placement.  A CTA works on G = 2^gsh scenarios in lockstep ("slots"; thread tid serves slot g = tid % G).  Either
+// every array of every slot lives in shared memory (kP = 0), interleaved over the slots in 16-byte vectors:
 //   address = base + ((index_in_vectors << gsh) + g) * 16
-// so that the G lanes serving one target read consecutive 16-byte words (conflict-free LDS.128).  The early part lives
-// in the HBM workspace of the scenario's GROUP (scenarios b with equal b >> gsh), interleaved over the group in the same
-// way -- a warp then touches 16 G contiguous bytes per target instead of 32 scattered sectors (coalesced LDG.128; the
-// L1 wavefront count, which bounded the scenario-major layout at 65 % of its peak, drops by up to G) -- and that is also
-// where kept factors are handed to sable_adjoint.  With gsh = 0 (staged / debug kernels) this is a plain contiguous
-// slice per scenario.
+// so that the G lanes serving one target read consecutive 16-byte words (conflict-free LDS.128), or (kP = 2) in the HBM
+// workspace of the scenario's GROUP (scenarios b with equal b >> gsh), interleaved over the group in the same way -- a
+// warp then touches 16 G contiguous bytes per target instead of 32 scattered sectors (coalesced LDG.128) -- and that is
+// also where kept factors are handed to sable_adjoint.  With gsh = 0 this is a plain contiguous slice per scenario.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
 
 namespace sable {
 
-// One elimination level: node range [m0, m1), the pairs those nodes own [p0, p1), the lane split per target, and the
-// level's slice of the index program ("blob": everything the factor / forward / backward phases of this level read
-// besides values).  Blob layout (byte offsets from the blob start; counts nm = m1 - m0, np = p1 - p0):
-//   int32 dptr[nm+1]   diag target i subtracts the terms dak[dptr[i] .. dptr[i+1])
-//   int32 tptr[np+1]   pair target i subtracts the terms tab[tptr[i] .. tptr[i+1])
-//   int32 pptr[nm+1]   node i owns the pairs p0 + [pptr[i] & kIdxMask, pptr[i+1] & kIdxMask); bit 30 of pptr[i] = PQ node
-//   int2  dak[]        (pair (k,m), node k)                                  at o_dak
-//   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                      at o_pmj
-//   int2  tab[]        (pair (k,m), pair (k,j))                              at o_tab
-// Narrow levels (staged = 1) are streamed through a shared-memory ring by cp.async.bulk one or two levels ahead of
-// use, so that no index load of the latency-critical top of the elimination tree goes to L2; wide levels are read
-// in place (their latency hides behind the many targets in flight).
+// Targets of one kind (diagonal targets or pair block-targets) of a level, sorted by descending list length, are cut
+// into classes; the targets [i0, i1) of a class are served by 1 << ssh lanes each (per slot).
+struct Cls { int32_t i1; int32_t ssh; };
+constexpr int kMaxCls = 4;
+
+// One elimination level: node range [m0, m1), the pairs those nodes own [p0, p1), and the level's slice of the index
+// program ("blob": everything the factor / forward / backward phases of this level read besides values).  Blob layout
+// (byte offsets from the blob start; counts nm = m1 - m0, np = p1 - p0):
+//   int32 dptr[nm+1]   the diag target at SORTED position i (descending list length) subtracts dak[dptr[i] .. dptr[i+1])
+//   int32 dord[nm]     local node index (m - m0) of sorted position i                       at o_dord
+//   int32 tptr[np+1]   the pair target at SORTED position i (descending list length) subtracts tab[tptr[i] .. tptr[i+1])
+//   int32 tord[np]     local pair index (p - p0) of sorted position i                       at o_tord
+//   int32 pptr[nm+1]   node i owns the pairs p0 + [pptr[i], pptr[i+1])                        at o_pptr
+//   int2  dak[]        (pair a = (k,m), node k)                                             at o_dak
+//   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                                     at o_pmj
+//   int4  tab[]        (pair a = (k,m), pair b = (k,j), node k, 0)                          at o_tab
+// A pair target is two BLOCK-targets bt = 2 i + h:  h = 0: U(m,j) -= L'(a) D_k^-1 U(b);  h = 1: L'(j,m) -= L'(b) D_k^-1 U(a)
+// -- one uniform item  acc -= A D_k^-1 B  with three operand blocks, served by neighbouring lane groups.
 struct LevelDesc {
     int32_t m0, m1, p0, p1;
-    uint8_t sd, sp, sb, staged;   // diag / pair / backward lane splits (lanes per target = 1 << s)
-    int32_t blob_off, blob_bytes; // slice of DevTemplate::blob (16-byte aligned, size a multiple of 16)
-    int32_t o_tptr, o_pptr, o_dak, o_pmj, o_tab, o_py;   // o_py: end of the lists (the front's descriptor keeps one more list there)
-    int32_t pad;
+    int32_t blob_off, blob_bytes;     // slice of DevTemplate::blob (16-byte aligned, size a multiple of 16)
+    int32_t o_dord, o_tptr, o_tord, o_pptr, o_dak, o_pmj, o_tab;
+    uint8_t sb, n_dcls, n_tcls, staged;   // backward lane split; class counts; staged: streamed through the blob ring
+    int32_t n_big;                    // the first n_big diag targets are "big": served by every warp of the CTA in turn
+    Cls dcls[kMaxCls];                // diag classes over the targets [n_big, nm)
+    Cls tcls[kMaxCls];                // block-target classes over bt in [0, 2 x (pair targets with at least one term))
 };
 
 struct RowClass { int32_t i0, i1, ssh; };   // rows mm_order[i0 .. i1) of the mismatch pass are served by 1 << ssh lanes each
@@ -59,8 +69,8 @@ struct DevTemplate {
     const int32_t* ycol;        // node positions (slack = n_node)
     const double2* ygb;         // (G, B) per stored Y entry
     const double2* ydiag_gb;    // [n_node] (G_mm, B_mm)
-    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)   (separate fill pass only)
-    const double4* pair_y;      // [n_pair]                                     (separate fill pass only)
+    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)   (fill pass)
+    const double4* pair_y;      // [n_pair]                                     (fill pass)
 };
 constexpr int kIdxMask = 0x3fffffff;
 
@@ -74,8 +84,18 @@ template <typename T> __device__ __forceinline__ void mulsub(Blk<T>& acc, const 
 template <typename T> __device__ __forceinline__ Blk<T> mul(const Blk<T>& x, const Blk<T>& y) {
     return {x.a * y.a + x.b * y.c, x.a * y.b + x.b * y.d, x.c * y.a + x.d * y.c, x.c * y.b + x.d * y.d};
 }
-template <typename T> __device__ __forceinline__ Blk<T> inv(const Blk<T>& x) {
-    T det = x.a * x.d - x.b * x.c, r = T(1) / det;
+// Inverse of a pivot block.  There is no pivot search (the pattern is shared by the batch): a block whose determinant
+// is tiny against its largest entry squared -- |det| <= eps * max|entry|^2, i.e. a condition number above 1 / eps, or a
+// non-finite determinant -- is FLAGGED through `bad` and the caller reports it per scenario (sable.h:
+// sable_get_pivot_flags).  eps = 1e-10 in FP64, 1e-6 with FP32 factors (the identity-padded block of a PV node has the
+// condition number |dP/dtheta| <= ~1e4, which must not trip the flag).
+template <typename T> __device__ __forceinline__ T pivot_eps();
+template <> __device__ __forceinline__ double pivot_eps<double>() { return 1e-10; }
+template <> __device__ __forceinline__ float pivot_eps<float>() { return 1e-6f; }
+template <typename T> __device__ __forceinline__ Blk<T> inv(const Blk<T>& x, bool& bad) {
+    const T det = x.a * x.d - x.b * x.c, r = T(1) / det;
+    const T n = fmax(fmax(fabs(x.a), fabs(x.b)), fmax(fabs(x.c), fabs(x.d)));
+    bad |= !(fabs(det) > pivot_eps<T>() * n * n);
     return {x.d * r, -x.b * r, -x.c * r, x.a * r};
 }
 template <typename T> __device__ __forceinline__ T shx(T v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
@@ -102,51 +122,41 @@ __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
 }
 
 // One thread's view of the slot it serves.  kP = 0: everything in shared memory; 2: everything in the HBM workspace
-// (both without placement branches); 1: mixed, split at the cuts.
+// (two kernel families without placement branches).
 template <typename T, int kP> struct Slot {
     static constexpr int VPB = (int)(4 * sizeof(T) / 16);      // 16-byte vectors per block: 2 (FP64) or 1 (FP32)
-    // Three per-thread pointers (shared base, factor slice and state slice of the group, each offset by g * 16) plus
-    // CTA-uniform byte offsets of the arrays behind them (uniform registers / constant bank: keeps the register count
-    // of the persistent kernel down).  Shared order: vv | ma | rh | dg | pr.  HBM: factors = dg | pr, state = vv | ma | rh.
+    // Per-thread base pointers (shared base; factor slice and state slice of the group; each offset by g * 16) plus
+    // CTA-uniform byte offsets of the arrays behind them.  Order in both memories: factors = dg | pu | pl, state = vv | ma | rh
+    // (shared: state first, then factors).
     char *sb, *gf, *gw;
-    unsigned so_ma, so_rh, so_dg, so_pr, go_pr, go_ma, go_rh;
-    int dg_cut, pr_cut, st_cut, gsh;                          // node cut of dg, pair cut of pr, node cut of vv/ma/rh
-    __device__ __forceinline__ char* s_vv() const { return sb; }
-    __device__ __forceinline__ char* s_ma() const { return sb + so_ma; }
-    __device__ __forceinline__ char* s_rh() const { return sb + so_rh; }
-    __device__ __forceinline__ char* s_dg() const { return sb + so_dg; }
-    __device__ __forceinline__ char* s_pr() const { return sb + so_pr; }
-    __device__ __forceinline__ char* g_dg() const { return gf; }
-    __device__ __forceinline__ char* g_pr() const { return gf + go_pr; }
-    __device__ __forceinline__ char* g_vv() const { return gw; }
-    __device__ __forceinline__ char* g_ma() const { return gw + go_ma; }
-    __device__ __forceinline__ char* g_rh() const { return gw + go_rh; }
-
+    unsigned so_ma, so_rh, so_dg, so_pu, so_pl, go_pu, go_pl, go_ma, go_rh;
+    int gsh;
     // byte offsets are 32-bit: a group's slice (and shared memory) is far below 4 GB
-    __device__ __forceinline__ T* blk_ptr(char* sb, char* gb, int idx, int cut_blocks, int& vs) const {
+    __device__ __forceinline__ T* blk_ptr(unsigned so, unsigned go, int idx, int& vs) const {
         vs = 16 << gsh;
-        if (kP == 0) return reinterpret_cast<T*>(sb + ((unsigned)(idx * VPB) << (gsh + 4)));
-        if (kP == 1 && idx >= cut_blocks) return reinterpret_cast<T*>(sb + ((unsigned)((idx - cut_blocks) * VPB) << (gsh + 4)));
-        return reinterpret_cast<T*>(gb + ((unsigned)(idx * VPB) << (gsh + 4)));
+        if (kP == 0) return reinterpret_cast<T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4))));
+        return reinterpret_cast<T*>(gf + (go + ((unsigned)(idx * VPB) << (gsh + 4))));
     }
-    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); return ld_blk(p, vs); }
-    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(s_dg(), g_dg(), m, dg_cut, vs); st_blk(p, vs, v); }
-    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(s_pr(), g_pr(), 2 * p, 2 * pr_cut, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p, 2 * pr_cut, vs); st_blk(q, vs, v); }
-    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(s_pr(), g_pr(), 2 * p + 1, 2 * pr_cut, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(so_dg, 0u, m, vs); return ld_blk(p, vs); }
+    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(so_dg, 0u, m, vs); st_blk(p, vs, v); }
+    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(so_pu, go_pu, p, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(so_pl, go_pl, p, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(so_pu, go_pu, p, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(so_pl, go_pl, p, vs); st_blk(q, vs, v); }
+    // h = 0: the U block of pair p, h = 1: the L' block (block-targets, sable_stages.cuh)
+    __device__ __forceinline__ Blk<T> ldP(int p, int h) const { int vs; const T* q = blk_ptr(h ? so_pl : so_pu, h ? go_pl : go_pu, p, vs); return ld_blk(q, vs); }
+    __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { int vs; T* q = blk_ptr(h ? so_pl : so_pu, h ? go_pl : go_pu, p, vs); st_blk(q, vs, v); }
 
-    __device__ __forceinline__ double2* st_ptr(char* sb, char* gb, int m) const {
-        if (kP == 0) return reinterpret_cast<double2*>(sb + ((unsigned)m << (gsh + 4)));
-        if (kP == 1 && m >= st_cut) return reinterpret_cast<double2*>(sb + ((unsigned)(m - st_cut) << (gsh + 4)));
-        return reinterpret_cast<double2*>(gb + ((unsigned)m << (gsh + 4)));
+    __device__ __forceinline__ double2* st_ptr(unsigned so, unsigned go, int m) const {
+        if (kP == 0) return reinterpret_cast<double2*>(sb + (so + ((unsigned)m << (gsh + 4))));
+        return reinterpret_cast<double2*>(gw + (go + ((unsigned)m << (gsh + 4))));
     }
-    __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(s_vv(), g_vv(), m); }
-    __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(s_ma(), g_ma(), m); }
-    __device__ __forceinline__ double2 rh(int m) const { return *st_ptr(s_rh(), g_rh(), m); }
-    __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(s_vv(), g_vv(), m) = v; }
-    __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(s_ma(), g_ma(), m) = v; }
-    __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(s_rh(), g_rh(), m) = v; }
+    __device__ __forceinline__ double2 vv(int m) const { return *st_ptr(0u, 0u, m); }
+    __device__ __forceinline__ double2 ma(int m) const { return *st_ptr(so_ma, go_ma, m); }
+    __device__ __forceinline__ double2 rh(int m) const { return *st_ptr(so_rh, go_rh, m); }
+    __device__ __forceinline__ void set_vv(int m, double2 v) const { *st_ptr(0u, 0u, m) = v; }
+    __device__ __forceinline__ void set_ma(int m, double2 v) const { *st_ptr(so_ma, go_ma, m) = v; }
+    __device__ __forceinline__ void set_rh(int m, double2 v) const { *st_ptr(so_rh, go_rh, m) = v; }
 };
 
 // ---- level-blob ring: cp.async.bulk (TMA 1-D bulk copy) + mbarrier ------------------------------------------------
@@ -165,6 +175,8 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, uint32_t parity
     asm volatile("{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
                  ::"r"(smem_u32(b)), "r"(parity) : "memory");
 }
+
+constexpr int kMaxRing = 8;     // ring slots (mbarriers in the shared-memory header)
 
 // The staged levels [first, n_level) are visited forward then backward, once per sweep pair; entry e of that endless
 // sequence lives in ring slot e % R.  Thread 0 is the producer; every thread consumes and tracks `use` itself.
@@ -210,7 +222,7 @@ struct BlobRing {
         if (threadIdx.x == 0) issue(use + (unsigned)R);
         ++use;
     }
-    // a backward sweep that is not run: its entries still pass through the ring (the producer runs R entries ahead),
+    // a sweep that is not run: its entries still pass through the ring (the producer runs R entries ahead),
     // so consume them; contains barriers
     __device__ __forceinline__ void skip_sweep() {
         if (!on) return;

@@ -11,12 +11,12 @@
 //   factor     right-looking block LU with the same 2x2 pivots D_r in the same order, one barrier per step:
 //              M[c][c'] -= (M[c][r] D_r^-1) M[r][c'],   y_c -= (M[c][r] D_r^-1) y_r        (forward solve fused in)
 //   backward   x_c = D_c^-1 y_c;  y_r -= M[r][c] x_c  (r < c),  c descending, one barrier per step
-//   write-back (kept factors only)  D^-1, U(m,j) = M[r][c], L(j,m) = M[c][r] D_r^-1 into the sparse slots that
-//              sable_adjoint's transposed sweeps read.
+//   write-back (kept factors only)  D^-1, U(m,j) = M[r][c], L'(j,m) = M[c][r] (unscaled, sable_device.cuh) into the sparse
+//              slots that sable_adjoint's transposed sweeps read.
 // Entries outside the static pattern are zero and stay zero (the pattern is closed under fill), so the arithmetic is
 // that of the sparse code up to the order of the sums.
 #pragma once
-#include "sable_device.cuh"
+#include "sable_stages.cuh"
 
 namespace sable {
 
@@ -56,79 +56,53 @@ __device__ __forceinline__ void front_zero(const Front<T>& F, int tsub, int nsub
     for (int i = tsub; i < F.K * F.K; i += nsub) { int vs; T* p = F.bp(0, i, vs); st_blk(p, vs, z); }
 }
 
-// Assembly: the accumulate phase of stage_factor_forward for all front targets at once, term lists filtered to sparse
-// k (LevelDesc d: m0 = f0, m1 = n_node, p0 .. p1 = the pairs owned by front nodes), results into M and y.  Ends with a
-// barrier.  The lead lane of the first front node also leaves D_0^-1.
+// Assembly: the accumulate phase of a level (accumulate_level, sable_stages.cuh) for all front targets at once, item lists
+// filtered to sparse k (LevelDesc d: m0 = f0, m1 = n_node, p0 .. p1 = the pairs owned by front nodes, with its own target
+// classes), results into M and y instead of the sparse slots.  The lead lane of the first front node also leaves D_0^-1.
+template <typename T> struct FrontSink {
+    const Front<T>& F;
+    const PivotFlag& pf;
+    static constexpr bool kInvert = false;      // pivots are inverted by front_factor, in elimination order
+    __device__ __forceinline__ void diag(int m, const Blk<T>& D, T y0, T y1, bool, bool solve) const {
+        const int r = m - F.f0;
+        F.stM(r, r, D);
+        if (r == 0) { bool bad = false; F.stI(0, inv(D, bad)); if (bad) pf.raise(); }
+        if (solve) *F.yp(r) = make_double2(double(y0), double(y1));
+    }
+    __device__ __forceinline__ void pair(int, int h, int2 mj, const Blk<T>& v) const {
+        const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
+        if (h) F.stM(c, r, v); else F.stM(r, c, v);
+    }
+};
+
+// Fills M and y of the front: entries with terms through accumulate_level, the others straight from the sparse slots
+// (where stage_fill_pairs / stage_mismatch left J).  Ends with a barrier.
 template <typename T, int kP, bool kSolve>
-__device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<T, kP>& s, const Front<T>& F, const LevelDesc& d) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
+__device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<T, kP>& s, const Front<T>& F, const LevelDesc& d,
+                                               const PivotFlag& pf, double* scratch, int tsub, int nsub) {
     const char* lb = t.blob + d.blob_off;
-    const int* dptr = reinterpret_cast<const int*>(lb);
-    const int* tptr = reinterpret_cast<const int*>(lb + d.o_tptr);
-    const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
-    const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
-    const int2* tab = reinterpret_cast<const int2*>(lb + d.o_tab);
+    // block-targets without terms (sorted behind the class ranges): copy J(m,j) / J(j,m)
     {
-        const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
-        const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-        for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
-            const bool valid = base + tl < d.m1;
-            const int m = valid ? base + tl : d.m1 - 1;
-            const bool lead = valid && part == 0;
-            const int t0 = dptr[m - d.m0], t1 = valid ? dptr[m - d.m0 + 1] : t0;
-            Blk<T> D = {T(0), T(0), T(0), T(0)};
-            T y0 = T(0), y1 = T(0);
-            if (lead) {
-                D = s.ldD(m);
-                if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
-            }
-            for (int q = t0 + part; q < t1; q += S) {
-                const int2 ak = dak[q];
-                const Blk<T> L = s.ldL(ak.x);
-                mulsub(D, L, s.ldU(ak.x));
-                if (kSolve) { const double2 x = s.rh(ak.y); y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y); }
-            }
-            for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) {
-                blk_add_shx(D, o);
-                if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
-            }
-            if (lead) {
-                const int r = m - F.f0;
-                F.stM(r, r, D);
-                if (r == 0) F.stI(0, inv(D));
-                if (kSolve) *F.yp(r) = make_double2(double(y0), double(y1));
-            }
+        const int* tord = reinterpret_cast<const int*>(lb + d.o_tord);
+        const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
+        const int nb1 = d.n_tcls ? d.tcls[d.n_tcls - 1].i1 : 0, nbt = 2 * (d.p1 - d.p0);
+        for (int bt = nb1 + tsub; bt < nbt; bt += nsub) {
+            const int pl = tord[bt >> 1], h = bt & 1;
+            const int2 mj = pmj[pl];
+            const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
+            const Blk<T> v = s.ldP(d.p0 + pl, h);
+            if (h) F.stM(c, r, v); else F.stM(r, c, v);
         }
     }
-    {
-        const int ssh = d.sp, tsh = 5 - gsh - ssh, S = 1 << ssh;
-        const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-        for (int base = d.p0 + ((nwarps - 1 - warp) << tsh); base < d.p1; base += nwarps << tsh) {
-            const bool valid = base + tl < d.p1;
-            const int p = valid ? base + tl : d.p1 - 1;
-            const int t0 = tptr[p - d.p0], t1 = valid ? tptr[p - d.p0 + 1] : t0;
-            const bool lead = valid && part == 0;
-            Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
-            if (lead) { U = s.ldU(p); L = s.ldL(p); }
-            for (int q = t0 + part; q < t1; q += S) {
-                const int2 ab = tab[q];
-                mulsub(U, s.ldL(ab.x), s.ldU(ab.y));
-                mulsub(L, s.ldL(ab.y), s.ldU(ab.x));
-            }
-            for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
-            if (lead) {
-                const int2 mj = pmj[p - d.p0];
-                const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
-                F.stM(r, c, U); F.stM(c, r, L);
-            }
-        }
-    }
+    int wrot = 0;
+    const FrontSink<T> sink{F, pf};
+    accumulate_level<T, kP, true, kSolve, false>(s, d, lb, sink, pf, scratch, wrot);
     __syncthreads();
 }
 
 // Right-looking block LU of M with the forward substitution as an extra column.  K barriers.
 template <typename T, bool kSolve>
-__device__ __forceinline__ void front_factor(const Front<T>& F, int tsub, int nsub) {
+__device__ __forceinline__ void front_factor(const Front<T>& F, const PivotFlag& pf, int tsub, int nsub) {
     const int K = F.K;
     for (int r = 0; r + 1 < K; ++r) {
         const int nr = K - 1 - r, ncol = nr + (kSolve ? 1 : 0), n = nr * ncol;
@@ -142,7 +116,7 @@ __device__ __forceinline__ void front_factor(const Front<T>& F, int tsub, int ns
                     Blk<T> X = F.ldM(c, cc);
                     mulsub(X, Lc, F.ldM(r, cc));
                     F.stM(c, cc, X);
-                    if (i == 0) F.stI(r + 1, inv(X));            // pivot of the next step
+                    if (i == 0) { bool bad = false; F.stI(r + 1, inv(X, bad)); if (bad) pf.raise(); }   // pivot of the next step
                 } else {
                     const double2 yr = *F.yp(r);
                     double2 yc = *F.yp(c);
@@ -179,7 +153,7 @@ __device__ __forceinline__ void front_backward(const Slot<T, kP>& s, const Front
     }
 }
 
-// kept factors: the front's D^-1, U and scaled L into the sparse slots (pairs p0 .. p1 of LevelDesc d).  No barrier.
+// kept factors: the front's D^-1, U and L' into the sparse slots (pairs p0 .. p1 of LevelDesc d).  No barrier.
 template <typename T, int kP>
 __device__ __forceinline__ void front_store(const DevTemplate& t, const Slot<T, kP>& s, const Front<T>& F, const LevelDesc& d, int tsub, int nsub) {
     const int2* pmj = reinterpret_cast<const int2*>(t.blob + d.blob_off + d.o_pmj);
@@ -188,7 +162,7 @@ __device__ __forceinline__ void front_store(const DevTemplate& t, const Slot<T, 
         const int2 mj = pmj[i];
         const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
         s.stU(d.p0 + i, F.ldM(r, c));
-        s.stL(d.p0 + i, mul(F.ldM(c, r), F.ldI(r)));
+        s.stL(d.p0 + i, F.ldM(c, r));
     }
 }
 

@@ -15,54 +15,57 @@ struct SolveArgs {
     double *vm, *va, *final_norm;
     int32_t* iterations;
     uint8_t* converged;
+    int32_t* pivot;           // [batch] tiny-pivot flags: bit 0 = seen in some refactorisation of the scenario, bit 1 = in the last one
     char* factors;            // [groups + 1][fac_stride << gsh] bytes, group-interleaved (sable_device.cuh)
     char* work;               // [groups + 1][work_stride << gsh] bytes
     int64_t fac_stride, work_stride;
-    int32_t gsh, dg_cut, pr_cut, st_cut;                   // slots per CTA = 1 << gsh; placement cuts (nodes, pairs, nodes)
+    int32_t gsh;                                           // slots per CTA = 1 << gsh
     int32_t ring_r, ring_slot, first_staged;               // level-blob ring: slots, bytes per slot, first streamed level
     int32_t front_k, front_f0, front_level;                // dense top front (sable_front.cuh): K nodes from f0 = levels >= front_level; 0 = off
-    int64_t front_off;                                     // its byte offset in the CTA's dynamic shared memory
+    int32_t big_off;                                       // byte offset of the big-target scratch in dynamic shared memory
+    int32_t slot_off;                                      // on-chip placement: byte offset of the slots in dynamic shared memory
+    int64_t front_off;                                     // HBM placement: byte offset of the front in dynamic shared memory
     LevelDesc front;                                       // assembly lists of the front
     unsigned long long* tim;  // optional cycle counters (sable_debug_timing), else nullptr
     int32_t* queue;           // persistent-kernel scenario counter
     int32_t* status;          // staged mode: [batch] 0 = active, 1 = converged, 2 = stopped
     int32_t* it;              // staged mode: [batch]
+    int32_t* active;          // staged mode: [max_it + 2] scenarios still active after each mismatch pass
+    int32_t stage_it;         // staged mode: index of this mismatch pass
 };
 
-constexpr int kRedBytes = 16 * 32 * 8;                      // per-slot norm reduction scratch: 16 warps x 32 slots
-constexpr int kSmemHeader = kRedBytes + 128 + 64;           // + slot bookkeeping + ring mbarriers
+constexpr int kRedBytes = 32 * 32 * 8;                      // per-slot norm reduction scratch: 32 warps x 32 slots
+constexpr int kSmemHeader = kRedBytes + 128 + 8 * kMaxRing; // + slot bookkeeping + ring mbarriers
 __host__ __device__ inline int64_t align16(int64_t x) { return (x + 15) & ~int64_t(15); }
 template <typename T> __host__ __device__ inline int64_t fac_bytes(int n_node, int n_pair) { return (int64_t)(n_node + 2 * (int64_t)n_pair) * 4 * sizeof(T); }
 __host__ __device__ inline int64_t work_bytes(int n_node) { return 3 * (int64_t)(n_node + 1) * 16; }
-// dynamic shared memory of a kernel that keeps nodes >= st_cut / dg_cut and pairs >= pr_cut on chip for 2^gsh slots
-__host__ __device__ inline int64_t smem_fixed(int n_level, int ring_bytes) {
-    return kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc)) + align16(ring_bytes);
+__host__ __device__ inline int64_t big_bytes(int threads, int gsh) { return ((int64_t)(threads >> 5) * kBigDoubles * 8) << gsh; }
+// dynamic shared memory: header, level descriptors, blob ring, big-target scratch, then (on-chip placement) the slots
+__host__ __device__ inline int64_t smem_fixed(int n_level, int ring_bytes, int big) {
+    return kSmemHeader + align16((int64_t)n_level * (int64_t)sizeof(LevelDesc)) + align16(ring_bytes) + align16(big);
 }
-template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut) {
-    int64_t b = smem_fixed(n_level, ring_bytes);
-    b += (3 * (int64_t)(n_node + 1 - st_cut) * 16) << gsh;
-    b += ((int64_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh;
-    b += (2 * (int64_t)(n_pair - pr_cut) * 4 * sizeof(T)) << gsh;
+template <typename T> __host__ __device__ inline int64_t smem_need(int n_node, int n_pair, int n_level, int ring_bytes, int big, int gsh, bool on_chip) {
+    int64_t b = smem_fixed(n_level, ring_bytes, big);
+    if (on_chip) b += (work_bytes(n_node) + fac_bytes<T>(n_node, n_pair)) << gsh;
     return b;
 }
 
-// shared-memory part of a slot view (fixed for the lifetime of the CTA)
+// shared-memory part of a slot view (fixed for the lifetime of the CTA) and the CTA-uniform offsets of the HBM arrays
 template <typename T, int kP>
-__device__ __forceinline__ Slot<T, kP> carve(unsigned char* smem, int n_node, int n_pair, int n_level, int ring_bytes, int gsh, int dg_cut, int pr_cut, int st_cut, int g) {
+__device__ __forceinline__ Slot<T, kP> carve(unsigned char* smem, int64_t slot_off, int n_node, int n_pair, int gsh, int g) {
     Slot<T, kP> s;
-    char* p = reinterpret_cast<char*>(smem) + smem_fixed(n_level, ring_bytes) + g * 16;
-    const unsigned ns = (unsigned)(((size_t)(n_node + 1 - st_cut) * 16) << gsh);
-    s.sb = p; s.so_ma = ns; s.so_rh = 2 * ns; s.so_dg = 3 * ns;
-    s.so_pr = s.so_dg + (unsigned)(((size_t)(n_node - dg_cut) * 4 * sizeof(T)) << gsh);
+    const unsigned ns = (unsigned)(((size_t)(n_node + 1) * 16) << gsh), nd = (unsigned)(((size_t)n_node * 4 * sizeof(T)) << gsh);
+    const unsigned np = (unsigned)(((size_t)n_pair * 4 * sizeof(T)) << gsh);
+    s.sb = reinterpret_cast<char*>(smem) + slot_off + g * 16;
+    s.so_ma = ns; s.so_rh = 2 * ns; s.so_dg = 3 * ns; s.so_pu = s.so_dg + nd; s.so_pl = s.so_pu + np;
     s.gf = s.gw = nullptr;
-    s.go_pr = (unsigned)(((size_t)n_node * 4 * sizeof(T)) << gsh);
-    s.go_ma = (unsigned)(((size_t)(n_node + 1) * 16) << gsh); s.go_rh = 2 * s.go_ma;
-    s.dg_cut = dg_cut; s.pr_cut = pr_cut; s.st_cut = st_cut; s.gsh = gsh;
+    s.go_pu = nd; s.go_pl = nd + np; s.go_ma = ns; s.go_rh = 2 * ns;
+    s.gsh = gsh;
     return s;
 }
 // HBM part: the slices of scenario b's group (b >> gsh), offset to lane b & (G - 1); strides are per scenario
 template <typename T, int kP>
-__device__ __forceinline__ void bind(Slot<T, kP>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int n_node, int b) {
+__device__ __forceinline__ void bind(Slot<T, kP>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b) {
     const int gsh = s.gsh;
     const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
     s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
@@ -82,6 +85,7 @@ __device__ __forceinline__ void scen_init(const SolveArgs& A, const Slot<T, kP>&
         s.set_ma(m, make_double2(vm, th));
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
+    if (tsub == 0) A.pivot[b] = 0;
 }
 
 template <typename T, int kP>
@@ -100,16 +104,14 @@ __device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kP
     }
 }
 
-// kept factors (reading 16): the on-chip part of the factors of J1 at the final
-// iterate goes to the scenario's HBM slice, next to the part that already lives there
+// kept factors (reading 16): the on-chip factors of J1 at the final iterate go to the
+// scenario's HBM slice (same order dg | pu | pl, same interleaving)
 template <typename T, int kP>
-__device__ __forceinline__ void store_top_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
+__device__ __forceinline__ void store_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
     constexpr int VPB = Slot<T, kP>::VPB;
-    const int n_dg = (t.n_node - s.dg_cut) * VPB, n_pr = 2 * (t.n_pair - s.pr_cut) * VPB;
-    char* gd = s.g_dg() + (((size_t)s.dg_cut * VPB) << (s.gsh + 4));
-    char* gp = s.g_pr() + (((size_t)2 * s.pr_cut * VPB) << (s.gsh + 4));
-    for (int i = tsub; i < n_dg; i += nsub) *reinterpret_cast<int4*>(gd + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_dg() + ((size_t)i << (s.gsh + 4)));
-    for (int i = tsub; i < n_pr; i += nsub) *reinterpret_cast<int4*>(gp + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.s_pr() + ((size_t)i << (s.gsh + 4)));
+    const int n = (t.n_node + 2 * t.n_pair) * VPB;
+    for (int i = tsub; i < n; i += nsub)
+        *reinterpret_cast<int4*>(s.gf + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.sb + s.so_dg + ((size_t)i << (s.gsh + 4)));
 }
 
 __device__ __forceinline__ int pop_group(const SolveArgs& A) {
@@ -122,10 +124,10 @@ __device__ __forceinline__ int pop_group(const SolveArgs& A) {
 // A CTA takes one GROUP of G consecutive scenarios at a time from the atomic queue (slot g serves scenario
 // group * G + g, whose HBM slices are interleaved with the rest of its group) and advances its slots in lockstep; a slot
 // that has finished stops being evaluated (its lanes run along and write nothing that is read) until the group is done.
-// Register budgets (measured, profiles/r01_v2_sweeps.md): on chip 1 CTA of up to 512 threads (up to 128 registers); HBM
-// placement 2 x 512 threads (64 registers) or, kSmall, 7 x 128 threads (72 registers, no spills).
-template <typename T, int kP, bool kSmall>
-__global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 : 2)) k_nr_fused(const SolveArgs A) {
+// Register budgets: on chip 1 CTA of up to 512 threads (up to 128 registers); HBM placement kCtas CTAs per SM of up to
+// kThreads threads each.
+template <typename T, int kP, int kThreads, int kCtas>
+__global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
@@ -133,7 +135,8 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
     int* s_b = reinterpret_cast<int*>(smem + kRedBytes);
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
     for (int i = threadIdx.x; i < t.n_level; i += blockDim.x) lv[i] = t.level[i];
-    Slot<T, kP> s = carve<T, kP>(smem, t.n_node, t.n_pair, t.n_level, A.ring_r * A.ring_slot, gsh, A.dg_cut, A.pr_cut, A.st_cut, g);
+    double* scratch = reinterpret_cast<double*>(smem + A.big_off);
+    Slot<T, kP> s = carve<T, kP>(smem, A.slot_off, t.n_node, t.n_pair, gsh, g);
     Front<T> F = carve_front<T>(smem, A.front_off, A.front_k, A.front_f0, gsh, g);
     BlobRing ring;
     ring.slots = reinterpret_cast<char*>(smem) + kSmemHeader + align16((int64_t)t.n_level * (int64_t)sizeof(LevelDesc));
@@ -152,6 +155,11 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
     const double kInf = __longlong_as_double(0x7ff0000000000000LL);
     int b = -1, it = 0;
     bool fin = false;
+    PivotFlag pf{nullptr};
+    auto to_trash = [&]() {
+        b = -1; pf.w = nullptr;
+        bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, (A.trash_grp << gsh) + g);
+    };
     auto any_slot = [&](bool mine) {                       // CTA-uniform OR over the slots; two barriers
         __syncthreads();
         if (threadIdx.x < G) s_b[threadIdx.x] = mine ? 1 : 0;
@@ -161,6 +169,7 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
         return any;
     };
     for (;;) {
+        if (b >= 0 && tsub == 0) atomicAnd(pf.w, 1);       // bit 1 = "in the last refactorisation": cleared before each one
         if (!any_slot(b >= 0)) {                           // group done: take the next one
             __syncthreads();
             if (threadIdx.x == 0) s_b[0] = pop_group(A);
@@ -168,17 +177,17 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
             const int grp = s_b[0];
             if (grp < 0) { ring.drain(); return; }
             const int bb = (grp << gsh) + g;
-            bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, bb);
+            bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, bb);
             b = bb < A.batch ? bb : -1;
             it = 0; fin = false;
-            if (b < 0) bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
-            if (b >= 0) scen_init<T, kP>(A, s, b, tsub, nsub);
+            if (b < 0) to_trash();
+            else { pf.w = A.pivot + b; scen_init<T, kP>(A, s, b, tsub, nsub); }
             __syncthreads();
         }
         ring.tick(4 * t.n_level + 2, tk);                  // group bookkeeping + init
         {
             const size_t row = (size_t)(b >= 0 ? b : 0) * t.n_bus;
-            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0, lv[0].m1);
+            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0, lv[0].m1, pf);
             const double r = slot_max_nan(loc, red, gsh);
             ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
             if (b >= 0) {
@@ -188,25 +197,25 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
                 if (done) {
                     scen_output<T, kP>(A, s, b, it, conv, r, tsub, nsub);
                     if (A.keep) fin = true;
-                    else { b = -1; bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g); }
+                    else to_trash();
                 }
             }
         }
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
-        stage_fill_pairs<T, kP, true>(t, s, tsub, nsub, lv[0].p1);
+        stage_fill_pairs<T, kP>(t, s, tsub, nsub);
         if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub, nsub);
         __syncthreads();
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
         if (kP == 2) {
             // HBM placement: the levels below the dense top front level by level (all of them if there is no front:
             // front_level = n_level), the front itself as one dense block in shared memory (sable_front.cuh)
-            stage_factor_forward<T, kP, true, true, false, true, false>(t, s, lv, ring, A.front_level);
+            stage_factor_forward<T, kP, true, true, false, true, false>(t, s, lv, ring, pf, scratch, A.front_level);
             if (A.front_k > 0) {
                 tk = clock64();
-                front_assemble<T, kP, true>(t, s, F, A.front);
+                front_assemble<T, kP, true>(t, s, F, A.front, pf, scratch, tsub, nsub);
                 ring.tick(3, tk);
-                front_factor<T, true>(F, tsub, nsub);
+                front_factor<T, true>(F, pf, tsub, nsub);
                 ring.tick(7, tk);
             }
             if (any_slot(b >= 0 && !fin)) {                // a trip that only refactors for kept factors needs no solve
@@ -216,7 +225,7 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
             }
             if (fin && A.front_k > 0) front_store<T, kP>(t, s, F, A.front, tsub, nsub);
         } else {
-            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring);
+            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, pf, scratch);
             if (any_slot(b >= 0 && !fin)) {
                 stage_backward<T, kP, false>(t, s, lv, ring);
                 stage_update<T, kP>(t, s, tsub, nsub);
@@ -225,9 +234,8 @@ __global__ void __launch_bounds__(kSmall ? 128 : 512, kP == 0 ? 1 : (kSmall ? 7 
         if (ring.tim && threadIdx.x == 0) { ring.tim[4 * t.n_level + 1] += 1; tk = clock64(); }   // trips
         if (b >= 0 && !fin) ++it;
         if (fin) {
-            store_top_factors<T, kP>(t, s, tsub, nsub);
-            b = -1; fin = false;                           // the kept factors stay untouched: run along on the spare group
-            bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, t.n_node, (A.trash_grp << gsh) + g);
+            if (kP == 0) store_factors<T, kP>(t, s, tsub, nsub);
+            fin = false; to_trash();                       // the kept factors stay untouched: run along on the spare group
         }
     }
 }

@@ -1,20 +1,18 @@
 // Staged kernels (one kernel per stage, state in HBM between stages -- the per-stage profiling mode), the adjoint /
-// linear-solve kernel on kept factors, and the debug kernels.  The staged and debug kernels serve one scenario per CTA
-// (gsh = 0); the adjoint kernel serves one group per CTA in the layout the factors were written in.
+// linear-solve kernel on kept factors, and the debug kernels.  The staged kernels run the fused kernel's own stage
+// routines in the fused kernel's workspace layout (one CTA per group of G scenarios, slots in lockstep); the debug
+// kernels serve one scenario per CTA (gsh = 0).
 #pragma once
 #include "sable_kernels.cuh"
 
 namespace sable {
 
-// everything in the scenario's HBM slices
-template <typename T, int kP = 2>
-__device__ __forceinline__ Slot<T, kP> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
-    Slot<T, kP> s;
-    s.sb = nullptr; s.so_ma = s.so_rh = s.so_dg = s.so_pr = 0;
-    s.go_pr = (unsigned)(((size_t)t.n_node * 4 * sizeof(T)) << gsh);
-    s.go_ma = (unsigned)(((size_t)(t.n_node + 1) * 16) << gsh); s.go_rh = 2 * s.go_ma;
-    s.dg_cut = t.n_node; s.pr_cut = t.n_pair; s.st_cut = t.n_node + 1; s.gsh = gsh;
-    bind<T, kP>(s, factors, fac_stride, work, work_stride, t.n_node, b);
+// everything in the HBM slices of scenario b's group
+template <typename T>
+__device__ __forceinline__ Slot<T, 2> hbm_slot(const DevTemplate& t, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b, int gsh = 0) {
+    Slot<T, 2> s = carve<T, 2>(nullptr, 0, t.n_node, t.n_pair, gsh, 0);
+    s.sb = nullptr;
+    bind<T, 2>(s, factors, fac_stride, work, work_stride, b);
     return s;
 }
 
@@ -26,47 +24,72 @@ __device__ __forceinline__ BlobRing no_ring(const DevTemplate& t) {
     return r;
 }
 
+constexpr int kStageScratch = 32 * 8 * kBigDoubles;   // doubles: big-target partials of up to 32 warps x 8 slots
+
 template <typename T>
 __global__ void k_st_init(const SolveArgs A) {
-    const int b = blockIdx.x;
-    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    scen_init<T, 2>(A, s, b, threadIdx.x, blockDim.x);
-    if (threadIdx.x == 0) { A.status[b] = 0; A.it[b] = 0; }
+    const int gsh = A.gsh, g = threadIdx.x & ((1 << gsh) - 1), b = (blockIdx.x << gsh) + g;
+    if (b >= A.batch) return;
+    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b, gsh);
+    scen_init<T, 2>(A, s, b, threadIdx.x >> gsh, blockDim.x >> gsh);
+    if ((threadIdx.x >> gsh) == 0) { A.status[b] = 0; A.it[b] = 0; }
 }
 
 // a1 + a6 + a2: mismatch, norm, convergence decision, Jacobian fill (in place, into the factor value array) for the
-// scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here
+// scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here.
+// Masked slots (finished earlier, or beyond the batch) run along on the spare workspace group.
 template <typename T>
 __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) {
     __shared__ double red[32 * 32];
-    const int b = blockIdx.x;
-    if (A.status[b] != 0) return;                                   // masked: no loads, no stores
-    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    const double r = slot_max_nan(stage_mismatch<T, 2>(A.t, s, A.p_spec + (size_t)b * A.t.n_bus, A.q_spec + (size_t)b * A.t.n_bus, true, A.t.level[0].m1), red, 0);
-    const int it = A.it[b];
+    __shared__ double scratch[kStageScratch];
+    const DevTemplate& t = A.t;
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
+    const int bb = (blockIdx.x << gsh) + g;
+    const bool act = bb < A.batch && A.status[bb] == 0;
+    if (!__syncthreads_or(act)) return;                              // whole group masked: no loads, no stores
+    const int trash = (A.trash_grp << gsh) + g;
+    Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, act ? bb : trash, gsh);
+    PivotFlag pf{act ? A.pivot + bb : nullptr};
+    if (act && tsub == 0) atomicAnd(pf.w, 1);
+    __syncthreads();
+    const size_t row = (size_t)(act ? bb : 0) * t.n_bus;
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec + row, A.q_spec + row, act, t.level[0].m1, pf), red, gsh);
     int st = 0;
-    if (r <= A.tol) st = 1;
-    else if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) st = 2;
-    if (st == 0 || A.keep) stage_fill_pairs<T, 2, true>(A.t, s, threadIdx.x, blockDim.x, A.t.level[0].p1);
-    if (st != 0) {
-        scen_output<T, 2>(A, s, b, it, st == 1, r, threadIdx.x, blockDim.x);
-        __syncthreads();
-        if (threadIdx.x == 0) A.status[b] = st;
-        if (A.keep) { BlobRing ring = no_ring(A.t); stage_factor_forward<T, 2, true, false, false, true>(A.t, s, A.t.level, ring); }
+    if (act) {
+        const int it = A.it[bb];
+        if (r <= A.tol) st = 1;
+        else if (it == A.max_it || !(fabs(r) < __longlong_as_double(0x7ff0000000000000LL))) st = 2;
+        if (st != 0) {
+            scen_output<T, 2>(A, s, bb, it, st == 1, r, tsub, nsub);
+            if (tsub == 0) A.status[bb] = st;
+        } else if (tsub == 0) atomicAdd(A.active + A.stage_it, 1);
     }
+    const bool go_on = act && st == 0, fin = act && st != 0 && A.keep;
+    if (!go_on && !fin) { bind<T, 2>(s, A.factors, A.fac_stride, A.work, A.work_stride, trash); pf.w = nullptr; }
+    __syncthreads();                                                 // scen_output has read the state the fill's trash lanes may overwrite
+    stage_fill_pairs<T, 2>(t, s, tsub, nsub);
+    if (!__syncthreads_or(fin)) return;
+    if (!fin) { bind<T, 2>(s, A.factors, A.fac_stride, A.work, A.work_stride, trash); pf.w = nullptr; }
+    BlobRing ring = no_ring(t);
+    stage_factor_forward<T, 2, true, false, false, true>(t, s, t.level, ring, pf, scratch);
 }
 
 // a4 + a5: refactor, forward/backward substitution, FP64 state update
 template <typename T>
 __global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
-    const int b = blockIdx.x;
-    if (A.status[b] != 0) return;
-    const Slot<T, 2> s = hbm_slot<T>(A.t, A.factors, A.fac_stride, A.work, A.work_stride, b);
-    BlobRing ring = no_ring(A.t);
-    stage_factor_forward<T, 2, true, true, false, true>(A.t, s, A.t.level, ring);
-    stage_backward<T, 2, false>(A.t, s, A.t.level, ring);
-    stage_update<T, 2>(A.t, s, threadIdx.x, blockDim.x);
-    if (threadIdx.x == 0) A.it[b] += 1;
+    __shared__ double scratch[kStageScratch];
+    const DevTemplate& t = A.t;
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
+    const int bb = (blockIdx.x << gsh) + g;
+    const bool act = bb < A.batch && A.status[bb] == 0;
+    if (!__syncthreads_or(act)) return;
+    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, act ? bb : (A.trash_grp << gsh) + g, gsh);
+    const PivotFlag pf{act ? A.pivot + bb : nullptr};
+    BlobRing ring = no_ring(t);
+    stage_factor_forward<T, 2, true, true, false, true>(t, s, t.level, ring, pf, scratch);
+    stage_backward<T, 2, false>(t, s, t.level, ring);
+    stage_update<T, 2>(t, s, tsub, nsub);
+    if (act && tsub == 0) A.it[bb] += 1;
 }
 
 // ---- adjoint / generic linear solve on stored factors ---------------------------------------------------------
@@ -75,12 +98,16 @@ struct LinArgs {
     int32_t batch, transposed, rhs_in_smem, gsh;   // gsh: group size (log2) of the factor layout = that of the kernel that wrote them
     const double *rhs_p, *rhs_q;      // [batch][n_bus]: theta/P component and Vm/Q component per bus
     double *x_p, *x_q;
+    const int32_t* pivot;             // tiny-pivot flags of the kept factors (bit 1), or nullptr
     char* factors; char* work; int64_t fac_stride, work_stride;
+    int32_t big_off;                  // big-target scratch at the start of dynamic shared memory, right-hand sides behind it
 };
 
-// a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, L^T lambda = w descending.
+// a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, (L' D^-1)^T lambda = w descending.
 // One CTA per group of G scenarios in lockstep (lane layout as in the NR kernel): factors stream from the group's
-// interleaved HBM slices (coalesced), the right-hand sides live in shared memory when they fit.
+// interleaved HBM slices (coalesced; U only in the first sweep, L' only in the second), the right-hand sides live in
+// shared memory when they fit.  A scenario whose kept factors carry a tiny-pivot flag gets NaN (its lambda would be
+// garbage that nothing else reveals: the adjoint has no residual test).
 template <typename T>
 __global__ void k_linsolve(const LinArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -88,8 +115,9 @@ __global__ void k_linsolve(const LinArgs A) {
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
     const int bb = (blockIdx.x << gsh) + g;
     const bool act = bb < A.batch;
-    Slot<T, 1> s = hbm_slot<T, 1>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
-    if (A.rhs_in_smem) { s.st_cut = 0; s.sb = reinterpret_cast<char*>(smem) + g * 16; s.so_rh = 0; }   // only rh is touched
+    Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
+    double* scratch = reinterpret_cast<double*>(smem);
+    if (A.rhs_in_smem) { s.gw = reinterpret_cast<char*>(smem) + A.big_off + g * 16; s.go_rh = 0; }   // only rh is touched: generic loads from shared memory
     const size_t o = (size_t)(act ? bb : 0) * t.n_bus;
     for (int m = tsub; m < t.n_node; m += nsub) {
         const int bus = t.node_bus[m];
@@ -97,15 +125,19 @@ __global__ void k_linsolve(const LinArgs A) {
     }
     __syncthreads();
     BlobRing ring = no_ring(t);
-    if (A.transposed) { stage_factor_forward<T, 1, false, true, true, false>(t, s, t.level, ring); stage_backward<T, 1, true>(t, s, t.level, ring); }
-    else              { stage_factor_forward<T, 1, false, true, false, false>(t, s, t.level, ring); stage_backward<T, 1, false>(t, s, t.level, ring); }
-    if (act)
+    const PivotFlag pf{nullptr};
+    if (A.transposed) { stage_factor_forward<T, 2, false, true, true, false>(t, s, t.level, ring, pf, scratch); stage_backward<T, 2, true>(t, s, t.level, ring); }
+    else              { stage_factor_forward<T, 2, false, true, false, false>(t, s, t.level, ring, pf, scratch); stage_backward<T, 2, false>(t, s, t.level, ring); }
+    if (act) {
+        const bool bad = A.pivot && (A.pivot[bb] & 2);
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
         for (int m = tsub; m <= t.n_node; m += nsub) {
             const int bus = t.node_bus[m];
             const double2 x = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
-            A.x_p[o + bus] = x.x;
-            A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? x.y : 0.0;
+            A.x_p[o + bus] = m < t.n_node ? (bad ? nan : x.x) : 0.0;
+            A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? (bad ? nan : x.y) : 0.0;
         }
+    }
 }
 
 // ---- Step-2 explicit recovery (PAPER.md:80 eq. 5, :95-99 eq. 9): with dF2/dz2 = I the block z2 = [p_g at the slack;
@@ -275,14 +307,18 @@ struct DebugArgs {
     double *f_p, *f_q, *norm, *diag, *pairs;
     char* factors; char* work; int64_t fac_stride, work_stride;
     const double* zeros;              // [n_bus] zeros: stands in for absent p_spec / q_spec
+    int32_t* pivot;                   // [batch] tiny-pivot flags (what = 2), or nullptr
 };
 
 template <typename T>
 __global__ void k_debug(const DebugArgs A) {
     __shared__ double red[32 * 32];
+    __shared__ double scratch[32 * kBigDoubles];
     const DevTemplate& t = A.t;
     const int b = blockIdx.x;
     const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b);
+    const PivotFlag pf{A.pivot ? A.pivot + b : nullptr};
+    if (A.pivot && threadIdx.x == 0) A.pivot[b] = 0;
     const size_t o = (size_t)b * t.n_bus;
     for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
         const int bus = t.node_bus[m];
@@ -292,7 +328,7 @@ __global__ void k_debug(const DebugArgs A) {
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0, pf), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];
@@ -303,17 +339,21 @@ __global__ void k_debug(const DebugArgs A) {
         if (threadIdx.x == 0) A.norm[b] = r;
         return;
     }
-    stage_fill_pairs<T, 2, false>(t, s, threadIdx.x, blockDim.x, 0);
+    stage_fill_pairs<T, 2>(t, s, threadIdx.x, blockDim.x);
     __syncthreads();
     if (A.what == 1) {
-        const T* dg = reinterpret_cast<const T*>(s.g_dg());
-        const T* pr = reinterpret_cast<const T*>(s.g_pr());
+        const T* dg = reinterpret_cast<const T*>(s.gf);
+        const T* pu = reinterpret_cast<const T*>(s.gf + s.go_pu);
+        const T* pl = reinterpret_cast<const T*>(s.gf + s.go_pl);
         for (int i = threadIdx.x; i < 4 * t.n_node; i += blockDim.x) A.diag[(size_t)b * 4 * t.n_node + i] = double(dg[i]);
-        for (int i = threadIdx.x; i < 8 * t.n_pair; i += blockDim.x) A.pairs[(size_t)b * 8 * t.n_pair + i] = double(pr[i]);
+        for (int i = threadIdx.x; i < 4 * t.n_pair; i += blockDim.x) {
+            A.pairs[(size_t)b * 8 * t.n_pair + 8 * (i >> 2) + (i & 3)] = double(pu[i]);
+            A.pairs[(size_t)b * 8 * t.n_pair + 8 * (i >> 2) + 4 + (i & 3)] = double(pl[i]);
+        }
         return;
     }
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring);
+    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring, pf, scratch);
 }
 
 }  // namespace sable

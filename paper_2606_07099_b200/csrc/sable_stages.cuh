@@ -1,20 +1,30 @@
 // CTA-wide stage routines of the batched Newton-Raphson power flow (eq. 6-8, eq. 14).  A CTA serves G
 // scenario slots in lockstep: thread tid serves slot g = tid % G.  Targets of one elimination level are spread over
 // the warps; a target whose multiply-subtract list is long is served by S = 2^s consecutive lane groups that each
-// take every S-th term and combine by warp shuffles (lane = (target_in_warp, part, slot), slot fastest).
+// take every S-th item and combine by warp shuffles (lane = (target_in_warp, part, slot), slot fastest).  The targets
+// of a level are sorted by list length and cut into classes with their own S (LevelDesc::dcls / tcls); the few
+// diagonal targets with very long lists ("big": hubs with hundreds of eliminated neighbours) are served by every warp
+// of the CTA in turn, combined through shared memory.
 #pragma once
 #include "sable_device.cuh"
 
 namespace sable {
+
+// Per-thread handle for reporting a tiny pivot: points at the scenario's flag word, or at
+// nothing for lanes that serve no scenario.
+struct PivotFlag {
+    int32_t* w;
+    __device__ __forceinline__ void raise() const { if (w) atomicOr(w, 3); }
+};
 
 // a1 (+ diagonal case of a2): S = V o conj(Ybus V), F1 rows (eq. 6), real form of
 // PAPER.md:201-207; writes rh = -F1 and the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated
 // P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
 template <typename T, int kP>
 __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kP>& s, const double* p_row,
-                                                 const double* q_row, bool act, int leaf_m1) {
+                                                 const double* q_row, bool act, int leaf_m1, const PivotFlag& pf) {
     // leaf_m1: nodes m < leaf_m1 (level 0: no earlier neighbour, so D_m = J(m,m) and y_m = rhs_m) get their pivot inverse
-    // stored right here -- with stage_fill_pairs<kPrescale> and kLeafDone the refactor has nothing left to do at level 0
+    // and z_m = D_m^-1 rhs_m stored right here -- the refactor then has nothing to do at level 0 (kLeafDone)
     // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
     // the evaluation (act = false) takes part in the shuffles and writes nothing
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
@@ -45,7 +55,6 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
                 const bool pq = row.w >> 30;
                 const int bus = row.w & kIdxMask;
                 const double fp = P - p_row[bus], fq = pq ? Q - q_row[bus] : 0.0;
-                s.set_rh(m, make_double2(-fp, -fq));
                 loc = nan_max(loc, nan_max(fabs(fp), fabs(fq)));
                 const double2 yd = t.ydiag_gb[m];
                 const double v2 = vm * vm, iv = 1.0 / vm;
@@ -53,7 +62,17 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
                 d.a = T(-Q - yd.y * v2);
                 if (pq) { d.b = T(P * iv + yd.x * vm); d.c = T(P - yd.x * v2); d.d = T(Q * iv - yd.y * vm); }
                 else    { d.b = T(0); d.c = T(0); d.d = T(1); }
-                s.stD(m, m < leaf_m1 ? inv(d) : d);
+                if (m < leaf_m1) {
+                    bool bad = false;
+                    const Blk<T> di = inv(d, bad);
+                    if (bad) pf.raise();
+                    s.stD(m, di);
+                    const T r0 = T(-fp), r1 = T(-fq);
+                    s.set_rh(m, make_double2(double(di.a * r0 + di.b * r1), double(di.c * r0 + di.d * r1)));
+                } else {
+                    s.stD(m, d);
+                    s.set_rh(m, make_double2(-fp, -fq));
+                }
             }
         }
     }
@@ -77,155 +96,214 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4
     L.a = T(l1);  L.b = T(l2 * ivm);  L.c = jpq ? T(-l2) : T(0);  L.d = jpq ? T(l1 * ivm) : T(0);
 }
 
-// a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  kPrescale: the pairs owned by
-// level-0 nodes (p < leaf_p1; such a node has no earlier neighbour, so D_m = J(m,m) and its pairs have no terms) get
-// their final values here -- U(m,j) = J(m,j), L(j,m) = J(j,m) J(m,m)^-1 (the inverse comes from stage_mismatch) -- and
-// the refactor skips level 0 altogether (kLeafDone).
-template <typename T, int kP, bool kPrescale>
-__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub, int leaf_p1) {
+// a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  The pairs owned by level-0
+// nodes have no terms, so these are already their final U and L' values.
+template <typename T, int kP>
+__device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
     for (int p = tsub; p < t.n_pair; p += nsub) {
         Blk<T> U, L;
-        const int2 mj = t.pair_mj[p];
-        fill_pair<T, kP>(s, mj, t.pair_y[p], U, L);
-        if (kPrescale && p < leaf_p1) L = mul(L, s.ldD(mj.x & kIdxMask));       // D^-1 left there by stage_mismatch
+        fill_pair<T, kP>(s, t.pair_mj[p], t.pair_y[p], U, L);
         s.stU(p, U); s.stL(p, L);
     }
 }
 
-// a4 + forward half of a5: block LU on the static pattern, level by level (unit-lower L, pivot blocks D_m stored
-// inverted), fused with the forward substitution L y = rhs which walks the same lists.  Contains barriers.
-//   diag target m :  D_m = J(m,m) - sum_k L(m,k) U(k,m);   y_m = rhs_m - sum_k L(m,k) y_k      (k: pairs (k,m))
-//   pair target p :  U(m,j) = J(m,j) - sum_k L(m,k) U(k,j);  L(j,m) = (J(j,m) - sum_k L(j,k) U(k,m)) D_m^-1
-// kLeafDone: the pairs of level 0 already hold their final values (stage_fill_pairs<kPrescale>), level 0 then has
-// diagonal targets only and a single barrier.  A pair target without terms is not touched by the accumulate pass.
-// kTransposed runs U^T w = g instead of L y = rhs:  w_m = D_m^-T (g_m - sum_k U(k,m)^T w_k).
-// kAll = false: only the levels [0, nl_) are processed (those below the dense top front: sable_front.cuh).
-template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone, bool kAll = true>
-__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl_ = 0) {
-    const int nl = kAll ? t.n_level : nl_;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
-    long long tk = clock64();
-    for (int l = 0; l < nl; ++l) {
-        const LevelDesc d = lv[l];
-        const char* lb = ring.acquire(l, d);
-        const int* dptr = reinterpret_cast<const int*>(lb);
+// Where the accumulate phase of a level leaves its results: the sparse slots (stage_factor_forward) or the dense top
+// front in shared memory (front_assemble, sable_front.cuh).
+template <typename T, int kP> struct SparseSink {
+    const Slot<T, kP>& s;
+    static constexpr bool kInvert = true;       // the lead lane inverts the pivot block and applies it to y
+    __device__ __forceinline__ void diag(int m, const Blk<T>& Dinv, T z0, T z1, bool factor, bool solve) const {
+        if (factor) s.stD(m, Dinv);
+        if (solve) s.set_rh(m, make_double2(double(z0), double(z1)));
+    }
+    __device__ __forceinline__ void pair(int p, int h, int2, const Blk<T>& v) const { s.stP(p, h, v); }
+};
+
+// Accumulate phase of one level (or of the front's assembly), the heart of a4 + the forward half of a5.  With the
+// factorisation J1 = L' D^-1 U (sable_device.cuh):
+//   diag target m :  D_m = J(m,m) - sum_a L'(a) D_k^-1 U(a);   y_m = rhs_m - sum_a L'(a) z_k;   z_m = D_m^-1 y_m     (a = pair (k,m))
+//   block-target  :  U(m,j) = J(m,j) - sum L'(a) D_k^-1 U(b)   (h = 0);   L'(j,m) = J(j,m) - sum L'(b) D_k^-1 U(a)   (h = 1)
+// kTransposed (solve only) runs U^T w = g instead:  w_m = D_m^-T (g_m - sum_a U(a)^T w_k).
+// No barrier except around the big targets (d.n_big > 0), whose partial sums go through `scratch` (kBigScratch bytes per slot).
+constexpr int kBigDoubles = 6;      // D (4) + y (2) per warp partial
+template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, typename Sink>
+__device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const LevelDesc& d, const char* lb, const Sink& sink,
+                                                 const PivotFlag& pf, double* scratch, int& wrot) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh, G = 1 << gsh;
+    const int* dptr = reinterpret_cast<const int*>(lb);
+    const int* dord = reinterpret_cast<const int*>(lb + d.o_dord);
+    const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
+    auto diag_item = [&](const int2 ak, Blk<T>& D, T& y0, T& y1) {
+        if (kFactor || kTransposed) {
+            const Blk<T> U = s.ldU(ak.x);
+            if (kFactor) { const Blk<T> W = mul(s.ldL(ak.x), s.ldD(ak.y)); mulsub(D, W, U); }
+            if (kSolve && kTransposed) { const double2 x = s.rh(ak.y); y0 -= U.a * T(x.x) + U.c * T(x.y);  y1 -= U.b * T(x.x) + U.d * T(x.y); }
+        }
+        if (kSolve && !kTransposed) {
+            const Blk<T> L = s.ldL(ak.x);
+            const double2 x = s.rh(ak.y);
+            y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y);
+        }
+    };
+    auto diag_finish = [&](int m, Blk<T> D, T y0, T y1) {
+        Blk<T> Di = D;
+        if (Sink::kInvert) {
+            if (kFactor) { bool bad = false; Di = inv(D, bad); if (bad) pf.raise(); }
+            else if (kSolve) Di = s.ldD(m);
+            if (kSolve) {
+                const T z0 = kTransposed ? Di.a * y0 + Di.c * y1 : Di.a * y0 + Di.b * y1;
+                const T z1 = kTransposed ? Di.b * y0 + Di.d * y1 : Di.c * y0 + Di.d * y1;
+                y0 = z0; y1 = z1;
+            }
+        }
+        sink.diag(m, Di, y0, y1, kFactor, kSolve);
+    };
+    // ---- big diagonal targets: one at a time, every lane of the CTA takes every (lanes)-th item ----------------------
+    for (int i = 0; i < d.n_big; ++i) {
+        const int m = d.m0 + dord[i], t0 = dptr[i], t1 = dptr[i + 1];
+        Blk<T> D = {T(0), T(0), T(0), T(0)};
+        T y0 = T(0), y1 = T(0);
+        for (int q = t0 + (threadIdx.x >> gsh); q < t1; q += blockDim.x >> gsh) diag_item(dak[q], D, y0, y1);
+        for (int o = 16; o >= G; o >>= 1) {
+            if (kFactor) blk_add_shx(D, o);
+            if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
+        }
+        __syncthreads();                                   // scratch free (previous big target consumed)
+        if (lane < G) {
+            double* w = scratch + ((size_t)warp * G + lane) * kBigDoubles;
+            w[0] = double(D.a); w[1] = double(D.b); w[2] = double(D.c); w[3] = double(D.d); w[4] = double(y0); w[5] = double(y1);
+        }
+        __syncthreads();
+        if (threadIdx.x < G) {
+            double a[kBigDoubles] = {0, 0, 0, 0, 0, 0};
+            for (int w = 0; w < nwarps; ++w) {
+#pragma unroll
+                for (int e = 0; e < kBigDoubles; ++e) a[e] += scratch[((size_t)w * G + threadIdx.x) * kBigDoubles + e];
+            }
+            Blk<T> Dm = {T(0), T(0), T(0), T(0)};
+            T r0 = T(0), r1 = T(0);
+            if (kFactor) { const Blk<T> J = s.ldD(m); Dm = {J.a + T(a[0]), J.b + T(a[1]), J.c + T(a[2]), J.d + T(a[3])}; }
+            if (kSolve) { const double2 r = s.rh(m); r0 = T(r.x) + T(a[4]); r1 = T(r.y) + T(a[5]); }
+            diag_finish(m, Dm, r0, r1);
+        }
+    }
+    // ---- diagonal targets by class ------------------------------------------------------------------------------------
+    int i0 = d.n_big;
+    for (int c = 0; c < d.n_dcls; ++c) {
+        const int i1 = d.dcls[c].i1, ssh = min(d.dcls[c].ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
+        const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
+        const int w0 = warp - wrot < 0 ? warp - wrot + nwarps : warp - wrot;
+        for (int base = i0 + (w0 << tsh); base < i1; base += nwarps << tsh) {
+            const bool valid = base + tl < i1;
+            const int i = valid ? base + tl : i1 - 1, m = d.m0 + dord[i];
+            const bool lead = valid && part == 0;
+            const int t0 = dptr[i], t1 = valid ? dptr[i + 1] : t0;
+            Blk<T> D = {T(0), T(0), T(0), T(0)};
+            T y0 = T(0), y1 = T(0);
+            if (lead) {
+                if (kFactor) D = s.ldD(m);
+                if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
+            }
+            for (int q = t0 + part; q < t1; q += S) diag_item(dak[q], D, y0, y1);
+            for (int o = (S >> 1) << gsh; o >= G; o >>= 1) {
+                if (kFactor) blk_add_shx(D, o);
+                if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
+            }
+            if (lead) diag_finish(m, D, y0, y1);
+        }
+        const int tasks = ((i1 - i0) + (1 << tsh) - 1) >> tsh;
+        wrot = (wrot + tasks) % nwarps;
+        i0 = i1;
+    }
+    // ---- pair block-targets by class (they only need factors of earlier levels: concurrent with the diagonal targets) ---
+    if (kFactor) {
         const int* tptr = reinterpret_cast<const int*>(lb + d.o_tptr);
-        const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
+        const int* tord = reinterpret_cast<const int*>(lb + d.o_tord);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
-        const int2* tab = reinterpret_cast<const int2*>(lb + d.o_tab);
-        if (!(kLeafDone && l == 0)) {
-            const int ssh = d.sd, tsh = 5 - gsh - ssh, S = 1 << ssh;
+        const int4* tab = reinterpret_cast<const int4*>(lb + d.o_tab);
+        int b0 = 0;
+        for (int c = 0; c < d.n_tcls; ++c) {
+            const int b1 = d.tcls[c].i1, ssh = min(d.tcls[c].ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
             const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-            for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
-                const bool valid = base + tl < d.m1;
-                const int m = valid ? base + tl : d.m1 - 1;
+            const int w0 = warp - wrot < 0 ? warp - wrot + nwarps : warp - wrot;
+            for (int base = b0 + (w0 << tsh); base < b1; base += nwarps << tsh) {
+                const bool valid = base + tl < b1;
+                const int bt = valid ? base + tl : b1 - 1, i = bt >> 1, h = bt & 1;
+                const int t0 = tptr[i], t1 = valid ? tptr[i + 1] : t0;
                 const bool lead = valid && part == 0;
-                const int t0 = dptr[m - d.m0], t1 = valid ? dptr[m - d.m0 + 1] : t0;
-                Blk<T> D = {T(0), T(0), T(0), T(0)};
-                T y0 = T(0), y1 = T(0);
-                if (lead) {
-                    if (kFactor) D = s.ldD(m);
-                    if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
-                }
+                const int pl = tord[i], p = d.p0 + pl;
+                Blk<T> acc = {T(0), T(0), T(0), T(0)};
+                if (lead) acc = s.ldP(p, h);
                 for (int q = t0 + part; q < t1; q += S) {
-                    const int2 ak = dak[q];
-                    if (kFactor || kTransposed) {
-                        const Blk<T> U = s.ldU(ak.x);
-                        if (kFactor) mulsub(D, s.ldL(ak.x), U);
-                        if (kSolve && kTransposed) { const double2 x = s.rh(ak.y); y0 -= U.a * T(x.x) + U.c * T(x.y);  y1 -= U.b * T(x.x) + U.d * T(x.y); }
-                    }
-                    if (kSolve && !kTransposed) {
-                        const Blk<T> L = s.ldL(ak.x);
-                        const double2 x = s.rh(ak.y);
-                        y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y);
-                    }
+                    const int4 ab = tab[q];
+                    const Blk<T> W = mul(s.ldL(h ? ab.y : ab.x), s.ldD(ab.z));
+                    mulsub(acc, W, s.ldU(h ? ab.x : ab.y));
                 }
-                for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) {
-                    if (kFactor) blk_add_shx(D, o);
-                    if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
-                }
-                if (lead) {
-                    if (kFactor) { D = inv(D); s.stD(m, D); }
-                    if (kSolve) {
-                        if (kTransposed) {
-                            if (!kFactor) D = s.ldD(m);
-                            const T z0 = D.a * y0 + D.c * y1, z1 = D.b * y0 + D.d * y1; y0 = z0; y1 = z1;
-                        }
-                        s.set_rh(m, make_double2(double(y0), double(y1)));
-                    }
-                }
+                for (int o = (S >> 1) << gsh; o >= G; o >>= 1) blk_add_shx(acc, o);
+                if (lead) sink.pair(p, h, pmj[pl], acc);
             }
+            const int tasks = ((b1 - b0) + (1 << tsh) - 1) >> tsh;
+            wrot = (wrot + tasks) % nwarps;
+            b0 = b1;
         }
-        if (kFactor && !(kLeafDone && l == 0)) {
-            // pair targets accumulate J - sum(terms) concurrently with the diagonal targets (they only need factors of
-            // earlier levels); warps are taken from the other end so that a narrow level spreads over distinct warps
-            const int ssh = d.sp, tsh = 5 - gsh - ssh, S = 1 << ssh;
-            const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-            for (int base = d.p0 + ((nwarps - 1 - warp) << tsh); base < d.p1; base += nwarps << tsh) {
-                const bool valid = base + tl < d.p1;
-                const int p = valid ? base + tl : d.p1 - 1;
-                const int t0 = tptr[p - d.p0], t1 = valid ? tptr[p - d.p0 + 1] : t0;
-                const bool lead = valid && part == 0 && t1 > t0;
-                Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
-                if (lead) { U = s.ldU(p); L = s.ldL(p); }
-                for (int q = t0 + part; q < t1; q += S) {
-                    const int2 ab = tab[q];
-                    mulsub(U, s.ldL(ab.x), s.ldU(ab.y));
-                    mulsub(L, s.ldL(ab.y), s.ldU(ab.x));
-                }
-                for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
-                if (lead) { s.stU(p, U); s.stL(p, L); }
-            }
-            __syncthreads();
-            ring.tick(4 * l, tk);
-            // scale: L(j,m) = L'(j,m) D_m^-1 with the pivot inverses of this level
-            const int np = d.p1 - d.p0;
-            for (int i = threadIdx.x >> gsh; i < np; i += blockDim.x >> gsh) {
-                const int p = d.p0 + i;
-                s.stL(p, mul(s.ldL(p), s.ldD(pmj[i].x & kIdxMask)));
-            }
-        }
+    }
+}
+
+// a4 + forward half of a5 level by level.  One barrier per level.  kLeafDone: level 0 needs nothing (stage_mismatch left
+// D^-1 and z of its nodes, stage_fill_pairs the final values of its pairs).  kAll = false: only the levels [0, nl_) are
+// processed (those below the dense top front: sable_front.cuh).
+template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone, bool kAll = true>
+__device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring,
+                                                     const PivotFlag& pf, double* scratch, int nl_ = 0) {
+    const int nl = kAll ? t.n_level : nl_;
+    long long tk = clock64();
+    int wrot = 0;
+    const SparseSink<T, kP> sink{s};
+    for (int l = 0; l < nl; ++l) {
+        const LevelDesc& d = lv[l];
+        const char* lb = ring.acquire(l, d);
+        if (!(kLeafDone && l == 0)) accumulate_level<T, kP, kFactor, kSolve, kTransposed>(s, d, lb, sink, pf, scratch, wrot);
         if (kLeafDone && l == 0 && !ring.on) continue;   // nothing was done at level 0: no barrier needed
         __syncthreads();
-        ring.tick(4 * l + 1, tk);
+        ring.tick(4 * l, tk);
         ring.release(l);
     }
 }
 
-// backward half of a5: U x = y, i.e. x_m = D_m^-1 (y_m - sum_j U(m,j) x_j) over the pairs owned by m, levels
-// descending.  kTransposed: L^T lambda = w, lambda_m = w_m - sum_j L(j,m)^T lambda_j.  Contains barriers.
+// backward half of a5: U x = y with rh holding z = D^-1 y, i.e. x_m = z_m - D_m^-1 sum_j U(m,j) x_j over the pairs owned
+// by m, levels descending.  kTransposed: (L' D^-1)^T lambda = w, lambda_m = w_m - D_m^-T sum_j L'(j,m)^T lambda_j.
+// Contains barriers.
 template <typename T, int kP, bool kTransposed, bool kAll = true>
 __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl_ = 0) {
     const int nl = kAll ? t.n_level : nl_;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
     long long tk = clock64();
     for (int l = nl - 1; l >= 0; --l) {
-        const LevelDesc d = lv[l];
+        const LevelDesc& d = lv[l];
         const char* lb = ring.acquire(l, d);
         const int* pptr = reinterpret_cast<const int*>(lb + d.o_pptr);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
-        const int ssh = d.sb, tsh = 5 - gsh - ssh, S = 1 << ssh;
+        const int ssh = min((int)d.sb, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
         const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
         for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
             const bool valid = base + tl < d.m1;
             const int m = valid ? base + tl : d.m1 - 1;
             const bool lead = valid && part == 0;
-            const int p0 = pptr[m - d.m0] & kIdxMask, p1 = valid ? pptr[m - d.m0 + 1] & kIdxMask : p0;
+            const int p0 = pptr[m - d.m0], p1 = valid ? pptr[m - d.m0 + 1] : p0;
             T y0 = T(0), y1 = T(0);
-            if (lead) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
             for (int pi = p0 + part; pi < p1; pi += S) {
                 const int j = pmj[pi].y & kIdxMask, p = d.p0 + pi;
                 const double2 x = s.rh(j);
-                if (!kTransposed) { const Blk<T> U = s.ldU(p); y0 -= U.a * T(x.x) + U.b * T(x.y); y1 -= U.c * T(x.x) + U.d * T(x.y); }
-                else              { const Blk<T> L = s.ldL(p); y0 -= L.a * T(x.x) + L.c * T(x.y); y1 -= L.b * T(x.x) + L.d * T(x.y); }
+                if (!kTransposed) { const Blk<T> U = s.ldU(p); y0 += U.a * T(x.x) + U.b * T(x.y); y1 += U.c * T(x.x) + U.d * T(x.y); }
+                else              { const Blk<T> L = s.ldL(p); y0 += L.a * T(x.x) + L.c * T(x.y); y1 += L.b * T(x.x) + L.d * T(x.y); }
             }
             for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { y0 += shx(y0, o); y1 += shx(y1, o); }
-            if (lead) {
-                if (!kTransposed) {
-                    const Blk<T> D = s.ldD(m);
-                    const T z0 = D.a * y0 + D.b * y1, z1 = D.c * y0 + D.d * y1; y0 = z0; y1 = z1;
-                }
-                s.set_rh(m, make_double2(double(y0), double(y1)));
+            if (lead && p1 > p0) {
+                const Blk<T> D = s.ldD(m);
+                const double2 r = s.rh(m);
+                const T z0 = kTransposed ? D.a * y0 + D.c * y1 : D.a * y0 + D.b * y1;
+                const T z1 = kTransposed ? D.b * y0 + D.d * y1 : D.c * y0 + D.d * y1;
+                s.set_rh(m, make_double2(double(T(r.x) - z0), double(T(r.y) - z1)));
             }
         }
         __syncthreads();

@@ -118,9 +118,15 @@ int build_template(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx
 
     // ---- 4. final order: by level, then by elimination step (any topological order of the elimination tree
     //         gives the same fill); positions, maps, levels --------------------------------------------------
-    std::vector<int32_t> order(N);
-    for (int p = 0; p < N; ++p) order[p] = p;
-    std::sort(order.begin(), order.end(), [&](int a, int b) { return lvl[a] != lvl[b] ? lvl[a] < lvl[b] : elim_pos[a] < elim_pos[b]; });
+    //         Within a level the nodes with the most eliminated neighbours come first (their diagonal targets have the
+    //         longest multiply-subtract lists: the per-level target classes of the kernels are then contiguous ranges).
+    std::vector<int32_t> order(N), n_lower(N, 0);
+    for (int p = 0; p < N; ++p) { order[p] = p; for (int32_t u : upper[p]) n_lower[u]++; }
+    std::sort(order.begin(), order.end(), [&](int a, int b) {
+        if (lvl[a] != lvl[b]) return lvl[a] < lvl[b];
+        if (n_lower[a] != n_lower[b]) return n_lower[a] > n_lower[b];
+        return elim_pos[a] < elim_pos[b];
+    });
     std::vector<int32_t> pos(N);
     for (int q = 0; q < N; ++q) pos[order[q]] = q;
     T.n_bus = n_bus; T.slack = slack; T.n_node = N;

@@ -394,7 +394,7 @@ def test_two_live_contexts():
     shared-memory attribute is per-function state): create cfg 2 (83 KB per CTA), create cfg 1 (7 KB), solve on the first."""
     net2, Y2 = get_net(2)
     net1, Y1 = get_net(1)
-    a = make_ctx(net2, max_batch=256, keep_factors=False)
+    a = make_ctx(net2, max_batch=1024, keep_factors=False)
     b = make_ctx(net1, max_batch=64, keep_factors=False)
     assert a.info["placement"] == 0 and b.info["placement"] == 0 and a.info["smem_bytes"] > 48 * 1024 > b.info["smem_bytes"]
     ps, qs, vs = S.make_scenarios(net2, batch=256)
@@ -485,17 +485,18 @@ def test_host_buffer_calls_match_device_calls():
 
 
 # ---- every placement / slot-group layout of the fused kernel gives the same answers -----------------------------------
-@pytest.mark.parametrize("env", [dict(SABLE_G="1"), dict(SABLE_G="8"), dict(SABLE_G="4", SABLE_CUT="3"),
-                                 dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="64"),
-                                 dict(SABLE_G="32", SABLE_CUT="99", SABLE_THREADS="128"),
-                                 dict(SABLE_G="2", SABLE_CUT="2", SABLE_RING_R="2", SABLE_RING_SLOT="4096"),
+@pytest.mark.parametrize("env", [dict(SABLE_G="1"), dict(SABLE_G="8"), dict(SABLE_G="2", SABLE_ONCHIP="1"),
+                                 dict(SABLE_G="4", SABLE_ONCHIP="0", SABLE_THREADS="64"),
+                                 dict(SABLE_G="32", SABLE_ONCHIP="0", SABLE_THREADS="128"),
+                                 dict(SABLE_G="16", SABLE_ONCHIP="0", SABLE_THREADS="1024"),
+                                 dict(SABLE_G="2", SABLE_ONCHIP="1", SABLE_RING_R="2", SABLE_RING_SLOT="4096"),
                                  dict(SABLE_RING_R="0"),
-                                 dict(SABLE_G="4", SABLE_CUT="99", SABLE_THREADS="128", SABLE_FRONT="13", SABLE_FRONT_KB="64"),
-                                 dict(SABLE_G="1", SABLE_CUT="99", SABLE_THREADS="256", SABLE_FRONT="33", SABLE_FRONT_KB="200"),
-                                 dict(SABLE_G="1", SABLE_CUT="99", SABLE_THREADS="256", SABLE_FRONT="57", SABLE_FRONT_KB="200"),
-                                 dict(SABLE_G="2", SABLE_CUT="99", SABLE_THREADS="64", SABLE_FRONT="0")])
+                                 dict(SABLE_G="4", SABLE_ONCHIP="0", SABLE_THREADS="128", SABLE_FRONT="13", SABLE_FRONT_KB="64"),
+                                 dict(SABLE_G="1", SABLE_ONCHIP="0", SABLE_THREADS="256", SABLE_FRONT="33", SABLE_FRONT_KB="200"),
+                                 dict(SABLE_G="1", SABLE_ONCHIP="0", SABLE_THREADS="256", SABLE_FRONT="57", SABLE_FRONT_KB="200"),
+                                 dict(SABLE_G="2", SABLE_ONCHIP="0", SABLE_THREADS="64", SABLE_FRONT="0")])
 def test_placements_and_group_layouts(env, monkeypatch):
-    for k in ("SABLE_G", "SABLE_CUT", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT", "SABLE_FRONT", "SABLE_FRONT_KB"):
+    for k in ("SABLE_G", "SABLE_ONCHIP", "SABLE_THREADS", "SABLE_CTAS", "SABLE_RING_R", "SABLE_RING_SLOT", "SABLE_FRONT", "SABLE_FRONT_KB"):
         monkeypatch.delenv(k, raising=False)
     for k, v in env.items():
         monkeypatch.setenv(k, v)
@@ -510,8 +511,8 @@ def test_placements_and_group_layouts(env, monkeypatch):
         ctx = make_ctx(net, max_batch=256, keep_factors=keep)
         if "SABLE_G" in env:
             assert ctx.info["slots_per_cta"] == int(env["SABLE_G"])
-        if "SABLE_CUT" in env:      # mixed placement below the last level, plain HBM placement beyond
-            assert ctx.info["placement"] == (1 if int(env["SABLE_CUT"]) < ctx.info["n_level"] else 2)
+        if "SABLE_ONCHIP" in env:
+            assert ctx.info["placement"] == (0 if env["SABLE_ONCHIP"] == "1" else 2)
         if "SABLE_FRONT" in env:    # dense top front: the last levels whose nodes fit the cap (cfg 2: 13 -> levels 4-7, 33 -> 2-7)
             want = {"13": (13, 4), "33": (33, 2), "57": (57, 1), "0": (0, ctx.info["n_level"])}[env["SABLE_FRONT"]]   # 57: all but level 0
             assert (ctx.info["front_k"], ctx.info["front_level"]) == want
@@ -526,6 +527,104 @@ def test_placements_and_group_layouts(env, monkeypatch):
             assert (np.abs(lp - rp).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
             assert (np.abs(lq - rq).max(axis=1)[ok] <= 1e-8 * scale[ok]).all()
         ctx.close()
+
+
+# ---- static pivoting can fail: the library must flag, not return garbage -------------------------------------------------
+def _weak_pivot_network(c2):
+    """4 buses: 0 slack - 1 PQ - {2 PQ leaf, 3 PQ leaf}; the lossless line 1-2 has series susceptance -10 and bus 2 a shunt
+    charging of c2.  With c2 = 5 the 2x2 diagonal Jacobian block of bus 2 at the flat start is [[10, 0], [0, 0]]: singular,
+    although J1 as a whole is not (dQ_2/dVm_1 = -10) -- a partially pivoting solver passes, static block pivots cannot."""
+    nb = 4
+    Yd = np.zeros((nb, nb), complex)
+    for f, t, y in ((0, 1, 1 / (0.01 + 0.05j)), (1, 2, -10j), (1, 3, 1 / (0.02 + 0.1j))):
+        Yd[f, f] += y; Yd[t, t] += y; Yd[f, t] -= y; Yd[t, f] -= y
+    Yd[2, 2] += 1j * c2
+    rp, col, g, b = [0], [], [], []
+    for i in range(nb):
+        for j in range(nb):
+            if Yd[i, j] != 0:
+                col.append(j); g.append(Yd[i, j].real); b.append(Yd[i, j].imag)
+        rp.append(len(col))
+    return (np.array(rp, np.int32), np.array(col, np.int32), np.array(g), np.array(b)), np.array([2, 0, 0, 0], np.uint8)
+
+
+@pytest.mark.parametrize("c2", [5.0, 5.0 + 1e-12])
+@pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
+def test_tiny_pivot_is_flagged(c2, mode):
+    Y, bt = _weak_pivot_network(c2)
+    ps = np.array([[0, -0.3, -0.2, -0.4], [0, -0.3, -0.2, -0.4]])
+    qs = np.array([[0, -0.1, -4.0, -0.1], [0, -0.1, -4.0, -0.1]])
+    vs = np.ones((2, 4))
+    ref = oracle.nr_batch(Y, bt, ps, qs, vs, tol=1e-8, max_it=20, method=1)
+    assert ref["converged"].all()                        # the pivoting oracle solves it
+    ctx = sb.Context(4, *Y, bt, 0, max_batch=2, mode=mode, keep_factors=True)
+    # scenario 1 starts away from the flat start (warm start at the oracle's solution): no weak pivot on its way
+    vm0, va0 = np.ones((2, 4)), np.zeros((2, 4))
+    vm0[1], va0[1] = ref["vm"][1], ref["va"][1]
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), vm0=dev(vm0), va0=dev(va0), tol=1e-8, max_it=20))
+    flags = ctx.pivot_flags(2).cpu().numpy()
+    assert flags[0] & 1, "the singular pivot block of bus 2 at the flat start was not flagged"
+    assert flags[1] == 0 and res["converged"][1] == 1 and res["iterations"][1] == 0
+    # flagged: either the scenario is reported as not converged, or (a tiny but finite pivot) it converged to the oracle's
+    # solution under the FP64 residual test -- never a silently wrong answer
+    if res["converged"][0]:
+        assert res["final_norm"][0] <= 1e-8 and np.abs(res["vm"][0] - ref["vm"][0]).max() <= 1e-7
+    else:
+        assert res["iterations"][0] == 20
+    # the adjoint of a scenario whose kept factors are flagged is NaN, the other one is right
+    g_va = np.array([[0, 1.0, 2.0, 3.0]] * 2); g_vm = np.array([[0, 0.5, -1.0, 0.25]] * 2)
+    lp, lq = ctx.adjoint(dev(g_va), dev(g_vm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    rp, rq, _ = oracle.adjoint_batch(Y, bt, res["vm"][1:], res["va"][1:], g_va[1:], g_vm[1:], method=1)
+    assert np.abs(lp[1] - rp[0]).max() <= 1e-8 * max(1, np.abs(rp).max()) and np.abs(lq[1] - rq[0]).max() <= 1e-8 * max(1, np.abs(rq).max())
+    if flags[0] & 2:
+        assert np.isnan(lp[0][1:]).all()
+    ctx.close()
+
+
+def test_tiny_pivot_linear_solve_flag():
+    """One refactorisation at the flat start of the weak-pivot network: flag raised; the oracle's pivoting solve of the same
+    system is finite (J1 is well conditioned)."""
+    Y, bt = _weak_pivot_network(5.0)
+    ctx = sb.Context(4, *Y, bt, 0, max_batch=1)
+    vm, va = np.ones((1, 4)), np.zeros((1, 4))
+    rp, rq = np.array([[0, 1.0, 2.0, 3.0]]), np.array([[0, 0.5, -1.0, 0.25]])
+    ctx.debug_linear_solve(dev(vm), dev(va), dev(rp), dev(rq))
+    assert ctx.pivot_flags(1).cpu().numpy()[0] == 3
+    n, jr, jc, jv = oracle.jacobian(Y, bt, vm[0], va[0])
+    x = oracle.linear_solve(n, jr, jc, jv, np.arange(1.0, n + 1), method=1)
+    assert np.isfinite(x).all()
+    # a healthy network raises nothing
+    net, _ = get_net(2)
+    c2 = make_ctx(net, max_batch=3)
+    vm, va = random_state(net, 3, 5)
+    z = np.zeros_like(vm)
+    c2.debug_linear_solve(dev(vm), dev(va), dev(z + 1.0), dev(z))
+    assert (c2.pivot_flags(3).cpu().numpy() == 0).all()
+    ctx.close(); c2.close()
+
+
+def test_tuning_through_options():
+    """The launch tuning goes through sable_options.tune (the environment variables are a debug override only)."""
+    net, Y = get_net(2)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=100)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    for tune, want in ((dict(group=8, on_chip=1), dict(slots_per_cta=8, placement=0)),
+                       (dict(group=2, on_chip=0, front_nodes=0), dict(slots_per_cta=2, placement=2, front_k=0)),
+                       (dict(on_chip=0, group=4, front_nodes=13, front_kb=64, threads_lin=64), dict(placement=2, front_k=13, threads_lin=64)),
+                       (dict(group=64, ctas_per_sm=1000), dict(slots_per_cta=32))):        # out-of-range values are clamped
+        ctx = make_ctx(net, max_batch=128, keep_factors=False, threads=128, **tune)
+        for k, v in want.items():
+            assert ctx.info[k] == v, (tune, k, ctx.info[k])
+        res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+        check_solution(res, ref, c.tol, 1e-9)
+        ctx.close()
+    with pytest.raises(TypeError):
+        make_ctx(net, max_batch=8, no_such_knob=1)
+    with pytest.raises(ValueError):          # the binding checks dtype / shape of the boundary arrays
+        c3 = make_ctx(net, max_batch=8)
+        c3.solve(dev(ps[:8]).float(), dev(qs[:8]), dev(vs[:8]))
 
 
 # ---- NEXT row 1: Step-2 explicit recovery (PAPER.md:80, :95-99) ---------------------------------------------------------
@@ -711,7 +810,7 @@ def test_dense_front(cfg, batch, precision, front, monkeypatch):
     slots serve sable_adjoint (1e-8 relative in FP64, FP32-factor accuracy in mixed mode)."""
     monkeypatch.setenv("SABLE_FRONT", front)
     monkeypatch.setenv("SABLE_FRONT_KB", "200")
-    monkeypatch.setenv("SABLE_CUT", "99")          # HBM placement also for these small batches, in the bench's launch shapes
+    monkeypatch.setenv("SABLE_ONCHIP", "0")        # HBM placement also for these small batches, in the bench's launch shapes
     monkeypatch.setenv("SABLE_G", "4" if cfg == 3 else "1")
     monkeypatch.setenv("SABLE_THREADS", {3: "128", 4: "256", 5: "512"}[cfg])
     net, Y = get_net(cfg)
