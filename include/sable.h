@@ -55,6 +55,8 @@ typedef struct {
     int32_t threads_stage;    /* threads per CTA of the staged kernels, 32 ... 512; 0 = automatic       (SABLE_THREADS1) */
     int32_t threads_lin;      /* threads per CTA of the adjoint kernel, 32 ... 1024; 0 = automatic      (SABLE_THREADS_LIN) */
     int32_t timing;           /* 1 = per-phase cycle counters of CTA 0 (sable_debug_timing)            (SABLE_TIMING) */
+    int32_t cluster;          /* HBM placement: CTAs (one thread-block cluster) that serve one group of scenarios together,
+                                 1, 2, 4, 8; 0 = automatic (teams when the batch is too small to fill the SMs)  (SABLE_CLUSTER) */
 } sable_tuning;
 
 typedef struct {
@@ -106,6 +108,7 @@ typedef struct {
     int32_t front_level;    /* first elimination level of that front (n_level if none) */
     int32_t threads_lin;    /* threads per CTA of the adjoint kernel */
     int32_t threads_stage;  /* threads per CTA of the staged kernels */
+    int32_t cluster;        /* CTAs per team (thread-block cluster) of the NR kernel; 1 = every CTA works alone */
 } sable_info;
 
 /* Build the shared fixed-pattern template for one network (host symbolic phase, run once; PAPER.md:185-197:

@@ -31,7 +31,7 @@ class SableError(RuntimeError):
 class Tuning(C.Structure):
     _fields_ = [("group", C.c_int32), ("ctas_per_sm", C.c_int32), ("on_chip", C.c_int32), ("ring_slots", C.c_int32),
                 ("ring_slot_bytes", C.c_int32), ("front_nodes", C.c_int32), ("front_kb", C.c_int32),
-                ("threads_stage", C.c_int32), ("threads_lin", C.c_int32), ("timing", C.c_int32)]
+                ("threads_stage", C.c_int32), ("threads_lin", C.c_int32), ("timing", C.c_int32), ("cluster", C.c_int32)]
 
 
 class Options(C.Structure):
@@ -48,7 +48,8 @@ class Info(C.Structure):
                 ("factor_bytes", C.c_int64), ("bytes_iter_m0", C.c_int64), ("bytes_adjoint_m0", C.c_int64),
                 ("smem_bytes", C.c_int32), ("placement", C.c_int32), ("threads", C.c_int32),
                 ("ctas_per_sm", C.c_int32), ("slots_per_cta", C.c_int32), ("cut_level", C.c_int32),
-                ("front_k", C.c_int32), ("front_level", C.c_int32), ("threads_lin", C.c_int32), ("threads_stage", C.c_int32)]
+                ("front_k", C.c_int32), ("front_level", C.c_int32), ("threads_lin", C.c_int32), ("threads_stage", C.c_int32),
+                ("cluster", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -27,6 +27,7 @@ struct sable_ctx {
     // launch plan of the fused kernel (choose_launch) and of the other kernel families
     int threads = 0, grid = 0, placement = 0, smem = 0, gsh = 0, ctas_per_sm = 1, variant = 0;
     int big_off = 0, slot_off = 0;
+    int csz = 1, csz_lin = 1; double* team_red = nullptr;                 // CTAs per team (cluster size) of the fused kernel; per-team norm scratch
     int threads_stage = 0, threads_lin = 0, threads1 = 0;    // staged kernels (group layout), adjoint kernel, one-scenario debug kernels
     int factor_gsh = 0;                                      // group layout of the factors currently in the workspace
     const LevelDesc* level_fused = nullptr; const LevelDesc* level_stage = nullptr;
@@ -89,7 +90,7 @@ static void fill_info(sable_ctx* c) {
     I.smem_bytes = c->smem; I.placement = c->placement; I.threads = c->threads;
     I.ctas_per_sm = c->ctas_per_sm; I.slots_per_cta = 1 << c->gsh; I.cut_level = c->placement == 0 ? 0 : T.n_level;
     I.front_k = c->front_k; I.front_level = c->front_k > 0 ? c->front_level : T.n_level;
-    I.threads_lin = c->threads_lin; I.threads_stage = c->threads_stage;
+    I.threads_lin = c->threads_lin; I.threads_stage = c->threads_stage; I.cluster = c->csz;
 }
 
 // kernel variants of the fused kernel: (placement, max threads per CTA, CTAs per SM the registers are budgeted for)
@@ -196,8 +197,8 @@ static LevelLists pack_level(const Template& T, LevelDesc& d, int k_limit, std::
 // target: targets are sorted by descending list length `len`; a class is a run of targets that get the same number of
 // lanes 2^ssh.  A target asks for enough lanes to leave at most kSerial items per lane; when the level has more lanes than
 // its targets ask for, every target gets proportionally more (up to its list length), so that a narrow level spreads over
-// the whole CTA.  `unit` = lanes one target position stands for (2 for pair targets: two block-targets each).
-static int cut_classes(const std::vector<int>& len, int first, int count, int unit, int lanes, int wmax, Cls* cls) {
+// the whole CTA.
+static int cut_classes(const std::vector<int>& len, int first, int count, int lanes, int wmax, bool diag, int unit, Cls* cls) {
     constexpr int kSerial = 2;
     auto want = [&](int n, int boost) {
         int s = 0;
@@ -231,7 +232,11 @@ static int cut_classes(const std::vector<int>& len, int first, int count, int un
         runs[best - 1].first = runs[best].first;      // run `best` joins its predecessor (larger or equal split: lists are sorted descending)
         runs.erase(runs.begin() + best);
     }
-    for (size_t r = 0; r < runs.size(); ++r) cls[r] = Cls{(first + runs[r].first) * unit, runs[r].second};
+    int prev = first;
+    for (size_t r = 0; r < runs.size(); ++r) {
+        cls[r] = Cls{prev * unit, (first + runs[r].first) * unit, (uint8_t)runs[r].second, (uint8_t)(diag ? 1 : 0), 0};
+        prev = first + runs[r].first;
+    }
     return (int)runs.size();
 }
 
@@ -248,10 +253,11 @@ static void plan_level(const Template& T, LevelDesc& d, const LevelLists& L, int
     int nbig = 0;
     if (allow_big && lanes >= 2 * wmax) while (nbig < nm && nbig < 4 && L.dlen[nbig] >= 3 * wmax && L.dlen[nbig] >= 64) ++nbig;
     d.n_big = nbig;
-    d.n_dcls = (uint8_t)cut_classes(L.dlen, nbig, nm - nbig, 1, lanes, wmax, d.dcls);
+    int nc = cut_classes(L.dlen, nbig, nm - nbig, lanes, wmax, true, 1, d.cls);
     int with_terms = 0;
     while (with_terms < (int)L.tlen.size() && L.tlen[with_terms] > 0) ++with_terms;
-    d.n_tcls = (uint8_t)cut_classes(L.tlen, 0, with_terms, 2, lanes, wmax, d.tcls);
+    nc += cut_classes(L.tlen, 0, with_terms, lanes, wmax, false, kTargetUnit, d.cls + nc);
+    d.n_cls = (uint8_t)nc;
     int maxb = 0;
     for (int m = d.m0; m < d.m1; ++m) maxb = std::max(maxb, T.pair_ptr[m + 1] - T.pair_ptr[m]);
     d.sb = pick_split(nm, maxb, lanes, wmax);
@@ -348,23 +354,35 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     }
     int th, gsh;
     if (on_chip) {
-        ctx->placement = 0; th = th0; gsh = gsh0;
+        ctx->placement = 0; th = th0; gsh = gsh0; ctx->csz = 1;
     } else {
         // ---- HBM placement (everything in the group-interleaved workspace, blobs read in place, no ring) --------------
-        // Occupancy model: the path is latency-bound, so the SM should hold as many independent elimination chains
-        // (scenarios) as its registers allow, each with enough lanes for the wide levels.  Lanes per scenario
-        // L = 2^floor(log2(n_node / 8)) in [32, 512] (a level-1 target per lane or so); slots per CTA G such that a CTA
-        // has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72 registers) but never so many that
-        // the batch leaves SMs without a CTA.
+        // Occupancy model.  The path is bound by memory latency and by the L1 data pipe: a lane's
+        // 16-byte access is one L1 wavefront unless the lanes beside it read the words beside it, which is what a group of
+        // G interleaved scenarios gives (measured per-SM throughput on the 9 241-bus grid, same 1 024 threads per SM:
+        // G = 2 / 4 / 8 / 16 -> 0.32 / 0.47 / 0.63 / 0.78 scenarios per SM and ms).  So:
+        //  * many scenarios (batch >= 8 per SM): lanes per scenario L = 2^floor(log2(n_node / 8)) in [32, 512], G such that a
+        //    CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72 registers), CTAs work alone;
+        //  * few scenarios: groups of G = 8 (fewer if the batch is smaller) served by a TEAM of csz CTAs (one cluster) of
+        //    1 024 threads each, csz = the largest power of two <= 8 that the teams of the batch still fit the SMs with.
         const int L = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
+        const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
+        int csz = 1;
         int G = std::max(1, 128 / L);
         if (g_given) G = g_want;
         else while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
+        const bool few = !th_given && !g_given && (int64_t)mb * L < (int64_t)n_sm * 1024 * 4 && nn >= 1024;   // the batch cannot fill the SMs' threads four times over
+        if (few) {
+            G = 8; while (G > 1 && G > mb) G /= 2;
+            const int teams = (mb + G - 1) / G;
+            csz = 1; while (csz < 8 && teams * csz * 2 <= n_sm) csz *= 2;
+        }
+        if (c_given) csz = pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8));
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : L << gsh;
-        th = std::min(1024, std::max(32 << 0, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : (few || csz > 1) ? 1024 : L << gsh;
+        th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
-        ctx->placement = 2;
+        ctx->placement = 2; ctx->csz = csz;
         set_ring(RingOpt{0, 0});
         if (need(th, gsh, false) > max_optin) return fail(ctx, SABLE_ERR_INVALID_ARG, "placement does not fit shared memory");
     }
@@ -379,7 +397,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         // dense top front: shared memory that still leaves most of the L1 to the resident CTAs
         const int kcap = tune(tu.front_nodes, -1, "SABLE_FRONT", 64, 0, 96);
         const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : 16, 0, 220) * 1024LL;
-        if (kcap >= 2) build_front(ctx, th, gsh, budget, kcap, true);
+        if (kcap >= 2 && ctx->csz == 1) build_front(ctx, th, gsh, budget, kcap, true);
         if (ctx->front_k > 0) {
             ctx->front_off = align16(ctx->smem);
             ctx->smem = (int)(ctx->front_off + (mixed ? front_bytes<float>(ctx->front_k, gsh) : front_bytes<double>(ctx->front_k, gsh)));
@@ -392,12 +410,13 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, th, (size_t)ctx->smem));
     if (occ < 1) return fail(ctx, SABLE_ERR_CUDA, "NR kernel does not fit on an SM");
     occ = std::min(occ, tune(tu.ctas_per_sm, 0, "SABLE_CTAS", occ, 1, 32));
-    ctx->ctas_per_sm = occ; ctx->grid = occ * n_sm;
+    ctx->ctas_per_sm = occ; ctx->grid = occ * n_sm / ctx->csz * ctx->csz;
     // the other kernel families: staged kernels (same group layout; the fused kernel's own shape when it is an HBM kernel),
     // the adjoint kernel (32 targets in flight per slot measured best in round 1), one-scenario debug kernels
     const int Ls = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
     ctx->threads_stage = (tune(tu.threads_stage, 0, "SABLE_THREADS1", ctx->placement == 2 ? std::min(th, 512) : std::min(512, Ls << gsh), 32, 512) + 31) / 32 * 32;
-    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    ctx->csz_lin = ctx->csz;
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     return SABLE_OK;
 }
@@ -493,9 +512,9 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     sable_status st = choose_launch(c, P);
     if (st != SABLE_OK) return bail(st);
     {
-        std::vector<LevelDesc> lf = build_levels(T, P, c->threads, c->gsh, true, c->first_staged);
+        std::vector<LevelDesc> lf = build_levels(T, P, c->threads * c->csz, c->gsh, c->csz == 1, c->first_staged);
         std::vector<LevelDesc> ls = build_levels(T, P, c->threads_stage, c->gsh, ((c->threads_stage >> 5) << c->gsh) <= 256, T.n_level);
-        std::vector<LevelDesc> ll = build_levels(T, P, c->threads_lin, c->gsh, true, T.n_level);
+        std::vector<LevelDesc> ll = build_levels(T, P, c->threads_lin * c->csz_lin, c->gsh, c->csz_lin == 1, T.n_level);
         std::vector<LevelDesc> l1 = build_levels(T, P, c->threads1, 0, true, T.n_level);
         up(lf, &c->level_fused); up(ls, &c->level_stage); up(ll, &c->level_lin); up(l1, &c->level_one); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
@@ -512,7 +531,8 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     const size_t G = (size_t)1 << c->gsh, mb_alloc = (mb + G - 1) / G * G + G;
     const size_t n_ints = kMaxChunk + 3 * mb + kMaxActive;
     if (!dmalloc((void**)&c->factors, mb_alloc * c->fac_stride) || !dmalloc((void**)&c->work, mb_alloc * c->work_stride) ||
-        !dmalloc((void**)&c->ints, n_ints * 4) || !dmalloc((void**)&c->zeros, nb * 8))
+        !dmalloc((void**)&c->ints, n_ints * 4) || !dmalloc((void**)&c->zeros, nb * 8) ||
+        !dmalloc((void**)&c->team_red, (size_t)kMaxChunk * std::max(1, c->grid) * G * 8))
         return bail(SABLE_ERR_ALLOC);
     if (cudaMemset(c->zeros, 0, nb * 8) != cudaSuccess || cudaMemset(c->work, 0, mb_alloc * c->work_stride) != cudaSuccess ||
         cudaMemset(c->factors, 0, mb_alloc * c->fac_stride) != cudaSuccess || cudaMemset(c->ints, 0, n_ints * 4) != cudaSuccess) {
@@ -532,7 +552,7 @@ extern "C" sable_options sable_default_options(void) {
     sable_options o{};
     o.max_batch = 1; o.precision = SABLE_FP64; o.keep_factors = 1; o.mode = SABLE_MODE_FUSED; o.device = 0; o.threads = 0; o.ir_sweeps = 0;
     o.tune.group = 0; o.tune.ctas_per_sm = 0; o.tune.on_chip = -1; o.tune.ring_slots = -1; o.tune.ring_slot_bytes = -1;
-    o.tune.front_nodes = -1; o.tune.front_kb = -1; o.tune.threads_stage = 0; o.tune.threads_lin = 0; o.tune.timing = 0;
+    o.tune.front_nodes = -1; o.tune.front_kb = -1; o.tune.threads_stage = 0; o.tune.threads_lin = 0; o.tune.timing = 0; o.tune.cluster = 0;
     return o;
 }
 
@@ -560,15 +580,21 @@ static int32_t* ctx_active(sable_ctx* c) { return c->ints + kMaxChunk + 3 * (siz
 
 template <typename T>
 static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s) {
-    const int G = 1 << c->gsh, grid = std::min((A.batch + G - 1) / G, c->grid);
+    const int G = 1 << c->gsh, groups = (A.batch + G - 1) / G;
+    const int grid = std::min(groups, std::max(1, c->grid / c->csz)) * c->csz;     // whole teams
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(c->threads); cfg.dynamicSmemBytes = (size_t)c->smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = c->csz; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = c->csz > 1 ? 1 : 0;
     switch (c->variant) {
-        case 0: k_nr_fused<T, 0, 512, 1><<<grid, c->threads, c->smem, s>>>(A); break;
-        case 1: k_nr_fused<T, 2, 128, 7><<<grid, c->threads, c->smem, s>>>(A); break;
-        case 2: k_nr_fused<T, 2, 256, 4><<<grid, c->threads, c->smem, s>>>(A); break;
-        case 3: k_nr_fused<T, 2, 512, 2><<<grid, c->threads, c->smem, s>>>(A); break;
-        default: k_nr_fused<T, 2, 1024, 1><<<grid, c->threads, c->smem, s>>>(A); break;
+        case 0: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 0, 512, 1>, A);
+        case 1: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 128, 7>, A);
+        case 2: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 256, 4>, A);
+        case 3: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 512, 2>, A);
+        default: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 1024, 1>, A);
     }
-    return cudaGetLastError();
 }
 
 // Scenarios [b0, b0 + nb) of the caller's arrays (b0 a multiple of the group size) on stream s, with queue counter `chunk`.
@@ -589,7 +615,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
         if (e != cudaSuccess) return e;
         A.t.level = c->level_fused;
         A.ring_r = c->ring_r; A.ring_slot = c->ring_slot; A.first_staged = c->first_staged;
-        A.big_off = c->big_off; A.slot_off = c->slot_off;
+        A.big_off = c->big_off; A.slot_off = c->slot_off; A.csz = c->csz; A.team_red = c->team_red + (size_t)chunk * c->grid * G;
         A.front_k = c->front_k; A.front_f0 = c->front_f0; A.front_level = c->front_level; A.front_off = c->front_off; A.front = c->front;
         // the attribute is per-function state shared by every live context: set it for THIS context right before the launch
         e = cudaFuncSetAttribute(fused_fn(sizeof(T) == 4, c->variant), cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem);
@@ -679,23 +705,31 @@ static sable_status launch_lin(sable_ctx* ctx, int b0, int batch, const double* 
     const int gsh = ctx->factor_gsh, G = 1 << gsh, g0 = b0 >> gsh;
     const size_t o = (size_t)b0 * ctx->T.n_bus;
     L.t = ctx->d;
-    L.t.level = gsh == 0 ? ctx->level_one : ctx->level_lin;
+    L.t.level = gsh == 0 && gsh != ctx->gsh ? ctx->level_one : ctx->level_lin;
     L.batch = batch; L.transposed = transposed; L.gsh = gsh; L.rhs_p = rp + o; L.rhs_q = rq + o; L.x_p = xp + o; L.x_q = xq + o;
     L.pivot = use_flags ? ctx_pivot(ctx) + b0 : nullptr;
     L.factors = ctx->factors + (size_t)g0 * G * ctx->fac_stride; L.fac_stride = ctx->fac_stride;
     L.work = ctx->work + (size_t)g0 * G * ctx->work_stride; L.work_stride = ctx->work_stride;
-    const int th = gsh == 0 ? ctx->threads1 : ctx->threads_lin, grid = (batch + G - 1) / G;
+    // the adjoint kernel follows the layout of the kernel that wrote the factors; with teams (cluster) when the NR kernel used them
+    const int csz = gsh == ctx->gsh ? ctx->csz_lin : 1;
+    const int th = gsh == 0 && gsh != ctx->gsh ? ctx->threads1 : ctx->threads_lin, grid = (batch + G - 1) / G * csz;
     L.big_off = (int)align16(big_bytes(th, gsh));
+    L.csz = csz;
     const size_t rhs = ((size_t)ctx->T.n_node * 16) << gsh;
     int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
-    L.rhs_in_smem = L.big_off + rhs <= std::min<size_t>((size_t)max_optin, 64 * 1024);
+    L.rhs_in_smem = csz == 1 && L.big_off + rhs <= std::min<size_t>((size_t)max_optin, 64 * 1024);
     const size_t sm = L.big_off + (L.rhs_in_smem ? rhs : 0);
     const void* lin = ctx->opt.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
     CU(cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(sm, 48 * 1024)));
-    if (ctx->opt.precision == SABLE_MIXED) k_linsolve<float><<<grid, th, sm, s>>>(L);
-    else k_linsolve<double><<<grid, th, sm, s>>>(L);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(th); cfg.dynamicSmemBytes = sm; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = csz; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = csz > 1 ? 1 : 0;
+    if (ctx->opt.precision == SABLE_MIXED) CU(cudaLaunchKernelEx(&cfg, k_linsolve<float>, L));
+    else CU(cudaLaunchKernelEx(&cfg, k_linsolve<double>, L));
     ctx->launches += 1;
-    CU(cudaGetLastError());
     return SABLE_OK;
 }
 

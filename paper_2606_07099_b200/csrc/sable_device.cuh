@@ -26,10 +26,18 @@
 
 namespace sable {
 
-// Targets of one kind (diagonal targets or pair block-targets) of a level, sorted by descending list length, are cut
-// into classes; the targets [i0, i1) of a class are served by 1 << ssh lanes each (per slot).
-struct Cls { int32_t i1; int32_t ssh; };
-constexpr int kMaxCls = 4;
+// Targets of one kind (diagonal targets or pair targets) of a level, sorted by descending list length, are cut into
+// classes; the targets [start, i1) of a class are served by 1 << ssh lanes each (per slot).  A warp-sized group of
+// targets of one class is a TASK; the tasks of a level (diagonal classes first) are dealt to the warps round-robin, so a
+// narrow level costs every warp at most one dependent chain.
+struct Cls { int32_t start, i1; uint8_t ssh, diag; uint16_t pad; };
+constexpr int kMaxCls = 3;      // per kind
+// 1: a pair target is served as two block-targets (U half, L' half: three operand blocks per item and lane);
+// 0: as one target with both accumulators (five operand blocks per item and lane)
+#ifndef SABLE_HALF_TARGETS
+#define SABLE_HALF_TARGETS 0
+#endif
+constexpr int kTargetUnit = SABLE_HALF_TARGETS ? 2 : 1;
 
 // One elimination level: node range [m0, m1), the pairs those nodes own [p0, p1), and the level's slice of the index
 // program ("blob": everything the factor / forward / backward phases of this level read besides values).  Blob layout
@@ -42,16 +50,14 @@ constexpr int kMaxCls = 4;
 //   int2  dak[]        (pair a = (k,m), node k)                                             at o_dak
 //   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                                     at o_pmj
 //   int4  tab[]        (pair a = (k,m), pair b = (k,j), node k, 0)                          at o_tab
-// A pair target is two BLOCK-targets bt = 2 i + h:  h = 0: U(m,j) -= L'(a) D_k^-1 U(b);  h = 1: L'(j,m) -= L'(b) D_k^-1 U(a)
-// -- one uniform item  acc -= A D_k^-1 B  with three operand blocks, served by neighbouring lane groups.
+// Pair target (m,j):  U(m,j) -= L'(a) D_k^-1 U(b);  L'(j,m) -= L'(b) D_k^-1 U(a)   per item.
 struct LevelDesc {
     int32_t m0, m1, p0, p1;
     int32_t blob_off, blob_bytes;     // slice of DevTemplate::blob (16-byte aligned, size a multiple of 16)
     int32_t o_dord, o_tptr, o_tord, o_pptr, o_dak, o_pmj, o_tab;
-    uint8_t sb, n_dcls, n_tcls, staged;   // backward lane split; class counts; staged: streamed through the blob ring
+    uint8_t sb, n_cls, staged, pad;   // backward lane split; classes in use (diagonal classes first); staged: streamed through the blob ring
     int32_t n_big;                    // the first n_big diag targets are "big": served by every warp of the CTA in turn
-    Cls dcls[kMaxCls];                // diag classes over the targets [n_big, nm)
-    Cls tcls[kMaxCls];                // block-target classes over bt in [0, 2 x (pair targets with at least one term))
+    Cls cls[2 * kMaxCls];
 };
 
 struct RowClass { int32_t i0, i1, ssh; };   // rows mm_order[i0 .. i1) of the mismatch pass are served by 1 << ssh lanes each
@@ -238,6 +244,17 @@ struct BlobRing {
             for (unsigned e = use; e < use + (unsigned)R; ++e) mbar_wait(mbar + (e % (unsigned)R), (e / (unsigned)R) & 1u);
     }
 };
+
+// A TEAM of `csz` CTAs (one thread-block cluster) can serve one group of scenarios together: every CTA keeps the same
+// control state, the targets of a level are dealt over the warps of the whole team, the data lives in the group's HBM slices,
+// and the per-level barrier is a cluster barrier with release / acquire semantics (which also drops the L1 lines a peer
+// may have made stale).  csz = 1: the CTA works alone and the barrier is __syncthreads.
+struct Team { int rank, csz; };
+__device__ __forceinline__ int cluster_ctarank() { int r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void team_sync(const Team& tm) {
+    if (tm.csz == 1) { __syncthreads(); return; }
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 
 __device__ __forceinline__ double nan_max(double x, double y) {   // NaN-propagating max of non-negative values
     return (x != x || y != y) ? __longlong_as_double(0x7ff8000000000000LL) : fmax(x, y);

@@ -85,8 +85,10 @@ __device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<
     {
         const int* tord = reinterpret_cast<const int*>(lb + d.o_tord);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
-        const int nb1 = d.n_tcls ? d.tcls[d.n_tcls - 1].i1 : 0, nbt = 2 * (d.p1 - d.p0);
-        for (int bt = nb1 + tsub; bt < nbt; bt += nsub) {
+        int with_terms = 0;                         // pair targets with terms: the end of the last pair class
+        for (int c = 0; c < d.n_cls; ++c) if (!d.cls[c].diag) with_terms = d.cls[c].i1 / kTargetUnit;
+        const int nbt = 2 * (d.p1 - d.p0);
+        for (int bt = 2 * with_terms + tsub; bt < nbt; bt += nsub) {
             const int pl = tord[bt >> 1], h = bt & 1;
             const int2 mj = pmj[pl];
             const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
@@ -94,9 +96,8 @@ __device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<
             if (h) F.stM(c, r, v); else F.stM(r, c, v);
         }
     }
-    int wrot = 0;
     const FrontSink<T> sink{F, pf};
-    accumulate_level<T, kP, true, kSolve, false>(s, d, lb, sink, pf, scratch, wrot);
+    accumulate_level<T, kP, true, kSolve, false>(s, d, lb, sink, pf, scratch, Team{0, 1});
     __syncthreads();
 }
 

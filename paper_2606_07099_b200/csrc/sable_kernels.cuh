@@ -20,6 +20,8 @@ struct SolveArgs {
     char* work;               // [groups + 1][work_stride << gsh] bytes
     int64_t fac_stride, work_stride;
     int32_t gsh;                                           // slots per CTA = 1 << gsh
+    int32_t csz;                                           // CTAs per team (cluster size); 1 = every CTA works alone
+    double* team_red;                                      // [teams][csz][G] per-slot norm partials of the CTAs of a team
     int32_t ring_r, ring_slot, first_staged;               // level-blob ring: slots, bytes per slot, first streamed level
     int32_t front_k, front_f0, front_level;                // dense top front (sable_front.cuh): K nodes from f0 = levels >= front_level; 0 = off
     int32_t big_off;                                       // byte offset of the big-target scratch in dynamic shared memory
@@ -130,7 +132,12 @@ template <typename T, int kP, int kThreads, int kCtas>
 __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
-    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
+    // team of CTAs (cluster) serving one group together: HBM placement only; every CTA of a team runs the same control flow
+    const Team tm{kP == 2 && A.csz > 1 ? cluster_ctarank() : 0, kP == 2 && A.csz > 1 ? A.csz : 1};
+    const int team = blockIdx.x / tm.csz, n_teams = gridDim.x / tm.csz;
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1);
+    const int tsub_c = threadIdx.x >> gsh, nsub_c = blockDim.x >> gsh;               // lanes of this CTA (front, on-chip copies)
+    const int tsub = tm.rank * nsub_c + tsub_c, nsub = nsub_c * tm.csz;              // lanes of the team (wide passes)
     double* red = reinterpret_cast<double*>(smem);
     int* s_b = reinterpret_cast<int*>(smem + kRedBytes);
     LevelDesc* lv = reinterpret_cast<LevelDesc*>(smem + kSmemHeader);
@@ -153,14 +160,14 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A)
     __syncthreads();                                       // lv[] complete before the producer reads it
     ring.start();
     const double kInf = __longlong_as_double(0x7ff0000000000000LL);
-    int b = -1, it = 0;
+    int b = -1, it = 0, next_grp = team;
     bool fin = false;
     PivotFlag pf{nullptr};
     auto to_trash = [&]() {
         b = -1; pf.w = nullptr;
         bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, (A.trash_grp << gsh) + g);
     };
-    auto any_slot = [&](bool mine) {                       // CTA-uniform OR over the slots; two barriers
+    auto any_slot = [&](bool mine) {                       // CTA-uniform OR over the slots (team-uniform: the state is replicated); two barriers
         __syncthreads();
         if (threadIdx.x < G) s_b[threadIdx.x] = mine ? 1 : 0;
         __syncthreads();
@@ -170,25 +177,39 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A)
     };
     for (;;) {
         if (b >= 0 && tsub == 0) atomicAnd(pf.w, 1);       // bit 1 = "in the last refactorisation": cleared before each one
+        if (tm.csz > 1) team_sync(tm);                     // the update of the last trip (all CTAs) before this trip's mismatch
         if (!any_slot(b >= 0)) {                           // group done: take the next one
-            __syncthreads();
-            if (threadIdx.x == 0) s_b[0] = pop_group(A);
-            __syncthreads();
-            const int grp = s_b[0];
-            if (grp < 0) { ring.drain(); return; }
+            int grp;
+            if (tm.csz > 1) {                              // teams: static assignment (team t serves groups t, t + n_teams, ...)
+                grp = next_grp < ((A.batch + G - 1) >> gsh) ? next_grp : -1;
+                next_grp += n_teams;
+            } else {
+                __syncthreads();
+                if (threadIdx.x == 0) s_b[0] = pop_group(A);
+                __syncthreads();
+                grp = s_b[0];
+            }
+            if (grp < 0) { ring.drain(); break; }
             const int bb = (grp << gsh) + g;
             bind<T, kP>(s, A.factors, A.fac_stride, A.work, A.work_stride, bb);
             b = bb < A.batch ? bb : -1;
             it = 0; fin = false;
             if (b < 0) to_trash();
             else { pf.w = A.pivot + b; scen_init<T, kP>(A, s, b, tsub, nsub); }
-            __syncthreads();
+            team_sync(tm);
         }
         ring.tick(4 * t.n_level + 2, tk);                  // group bookkeeping + init
         {
             const size_t row = (size_t)(b >= 0 ? b : 0) * t.n_bus;
-            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0, lv[0].m1, pf);
-            const double r = slot_max_nan(loc, red, gsh);
+            const double loc = stage_mismatch<T, kP>(t, s, A.p_spec + row, A.q_spec + row, b >= 0, lv[0].m1, pf, tm);
+            double r = slot_max_nan(loc, red, gsh);
+            if (tm.csz > 1) {                              // combine the CTAs' per-slot norms through the team's scratch words
+                double* tr = A.team_red + (size_t)team * tm.csz * G;
+                if (threadIdx.x < G) tr[tm.rank * G + g] = r;
+                team_sync(tm);
+                r = tr[g];
+                for (int k = 1; k < tm.csz; ++k) r = nan_max(r, tr[k * G + g]);
+            }
             ring.tick(4 * t.n_level + 3, tk);              // mismatch + norm
             if (b >= 0) {
                 bool done = false, conv = false;
@@ -204,30 +225,31 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A)
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
         // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
         stage_fill_pairs<T, kP>(t, s, tsub, nsub);
-        if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub, nsub);
-        __syncthreads();
+        if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub_c, nsub_c);
+        team_sync(tm);
         ring.tick(4 * t.n_level, tk);                      // decision + output + Jacobian fill
         if (kP == 2) {
             // HBM placement: the levels below the dense top front level by level (all of them if there is no front:
-            // front_level = n_level), the front itself as one dense block in shared memory (sable_front.cuh)
-            stage_factor_forward<T, kP, true, true, false, true, false>(t, s, lv, ring, pf, scratch, A.front_level);
+            // front_level = n_level), the front itself as one dense block in shared memory (sable_front.cuh; a CTA working
+            // alone only)
+            stage_factor_forward<T, kP, true, true, false, true, false>(t, s, lv, ring, pf, scratch, tm, A.front_level);
             if (A.front_k > 0) {
                 tk = clock64();
-                front_assemble<T, kP, true>(t, s, F, A.front, pf, scratch, tsub, nsub);
+                front_assemble<T, kP, true>(t, s, F, A.front, pf, scratch, tsub_c, nsub_c);
                 ring.tick(3, tk);
-                front_factor<T, true>(F, pf, tsub, nsub);
+                front_factor<T, true>(F, pf, tsub_c, nsub_c);
                 ring.tick(7, tk);
             }
             if (any_slot(b >= 0 && !fin)) {                // a trip that only refactors for kept factors needs no solve
-                if (A.front_k > 0) { front_backward<T, kP>(s, F, tsub, nsub); ring.tick(11, tk); }
-                stage_backward<T, kP, false, false>(t, s, lv, ring, A.front_level);
+                if (A.front_k > 0) { front_backward<T, kP>(s, F, tsub_c, nsub_c); ring.tick(11, tk); }
+                stage_backward<T, kP, false, false>(t, s, lv, ring, tm, A.front_level);
                 stage_update<T, kP>(t, s, tsub, nsub);
             }
-            if (fin && A.front_k > 0) front_store<T, kP>(t, s, F, A.front, tsub, nsub);
+            if (fin && A.front_k > 0) front_store<T, kP>(t, s, F, A.front, tsub_c, nsub_c);
         } else {
-            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, pf, scratch);
+            stage_factor_forward<T, kP, true, true, false, true>(t, s, lv, ring, pf, scratch, tm);
             if (any_slot(b >= 0 && !fin)) {
-                stage_backward<T, kP, false>(t, s, lv, ring);
+                stage_backward<T, kP, false>(t, s, lv, ring, tm);
                 stage_update<T, kP>(t, s, tsub, nsub);
             } else ring.skip_sweep();
         }
@@ -238,6 +260,7 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A)
             fin = false; to_trash();                       // the kept factors stay untouched: run along on the spare group
         }
     }
+    if (tm.csz > 1) team_sync(tm);                         // no CTA of a cluster exits while a peer may still wait on it
 }
 
 }  // namespace sable

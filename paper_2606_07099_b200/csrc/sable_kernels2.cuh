@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     if (act && tsub == 0) atomicAnd(pf.w, 1);
     __syncthreads();
     const size_t row = (size_t)(act ? bb : 0) * t.n_bus;
-    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec + row, A.q_spec + row, act, t.level[0].m1, pf), red, gsh);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec + row, A.q_spec + row, act, t.level[0].m1, pf, Team{0, 1}), red, gsh);
     int st = 0;
     if (act) {
         const int it = A.it[bb];
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     if (!__syncthreads_or(fin)) return;
     if (!fin) { bind<T, 2>(s, A.factors, A.fac_stride, A.work, A.work_stride, trash); pf.w = nullptr; }
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, 2, true, false, false, true>(t, s, t.level, ring, pf, scratch);
+    stage_factor_forward<T, 2, true, false, false, true>(t, s, t.level, ring, pf, scratch, Team{0, 1});
 }
 
 // a4 + a5: refactor, forward/backward substitution, FP64 state update
@@ -86,8 +86,8 @@ __global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
     const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, act ? bb : (A.trash_grp << gsh) + g, gsh);
     const PivotFlag pf{act ? A.pivot + bb : nullptr};
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, 2, true, true, false, true>(t, s, t.level, ring, pf, scratch);
-    stage_backward<T, 2, false>(t, s, t.level, ring);
+    stage_factor_forward<T, 2, true, true, false, true>(t, s, t.level, ring, pf, scratch, Team{0, 1});
+    stage_backward<T, 2, false>(t, s, t.level, ring, Team{0, 1});
     stage_update<T, 2>(t, s, tsub, nsub);
     if (act && tsub == 0) A.it[bb] += 1;
 }
@@ -101,6 +101,7 @@ struct LinArgs {
     const int32_t* pivot;             // tiny-pivot flags of the kept factors (bit 1), or nullptr
     char* factors; char* work; int64_t fac_stride, work_stride;
     int32_t big_off;                  // big-target scratch at the start of dynamic shared memory, right-hand sides behind it
+    int32_t csz;                      // CTAs per team (cluster size); the right-hand sides then live in the group's workspace slice
 };
 
 // a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, (L' D^-1)^T lambda = w descending.
@@ -112,8 +113,10 @@ template <typename T>
 __global__ void k_linsolve(const LinArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
-    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
-    const int bb = (blockIdx.x << gsh) + g;
+    const Team tm{A.csz > 1 ? cluster_ctarank() : 0, A.csz > 1 ? A.csz : 1};
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1);
+    const int nsub = (blockDim.x >> gsh) * tm.csz, tsub = tm.rank * (blockDim.x >> gsh) + (threadIdx.x >> gsh);
+    const int bb = ((blockIdx.x / tm.csz) << gsh) + g;
     const bool act = bb < A.batch;
     Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, bb, gsh);
     double* scratch = reinterpret_cast<double*>(smem);
@@ -123,11 +126,11 @@ __global__ void k_linsolve(const LinArgs A) {
         const int bus = t.node_bus[m];
         s.set_rh(m, act ? make_double2(A.rhs_p[o + bus], t.node_pq[m] ? A.rhs_q[o + bus] : 0.0) : make_double2(0.0, 0.0));
     }
-    __syncthreads();
+    team_sync(tm);
     BlobRing ring = no_ring(t);
     const PivotFlag pf{nullptr};
-    if (A.transposed) { stage_factor_forward<T, 2, false, true, true, false>(t, s, t.level, ring, pf, scratch); stage_backward<T, 2, true>(t, s, t.level, ring); }
-    else              { stage_factor_forward<T, 2, false, true, false, false>(t, s, t.level, ring, pf, scratch); stage_backward<T, 2, false>(t, s, t.level, ring); }
+    if (A.transposed) { stage_factor_forward<T, 2, false, true, true, false>(t, s, t.level, ring, pf, scratch, tm); stage_backward<T, 2, true>(t, s, t.level, ring, tm); }
+    else              { stage_factor_forward<T, 2, false, true, false, false>(t, s, t.level, ring, pf, scratch, tm); stage_backward<T, 2, false>(t, s, t.level, ring, tm); }
     if (act) {
         const bool bad = A.pivot && (A.pivot[bb] & 2);
         const double nan = __longlong_as_double(0x7ff8000000000000LL);
@@ -138,6 +141,7 @@ __global__ void k_linsolve(const LinArgs A) {
             A.x_q[o + bus] = (m < t.n_node && t.node_pq[m]) ? (bad ? nan : x.y) : 0.0;
         }
     }
+    if (tm.csz > 1) team_sync(tm);
 }
 
 // ---- Step-2 explicit recovery (PAPER.md:80 eq. 5, :95-99 eq. 9): with dF2/dz2 = I the block z2 = [p_g at the slack;
@@ -328,7 +332,7 @@ __global__ void k_debug(const DebugArgs A) {
         s.set_vv(m, make_double2(vm * cs, vm * sn));
     }
     __syncthreads();
-    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0, pf), red, 0);
+    const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0, pf, Team{0, 1}), red, 0);
     if (A.what == 0) {
         for (int m = threadIdx.x; m <= t.n_node; m += blockDim.x) {
             const int bus = t.node_bus[m];
@@ -353,7 +357,7 @@ __global__ void k_debug(const DebugArgs A) {
         return;
     }
     BlobRing ring = no_ring(t);
-    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring, pf, scratch);
+    stage_factor_forward<T, 2, true, false, false, false>(t, s, t.level, ring, pf, scratch, Team{0, 1});
 }
 
 }  // namespace sable

@@ -22,12 +22,12 @@ struct PivotFlag {
 // P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
 template <typename T, int kP>
 __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kP>& s, const double* p_row,
-                                                 const double* q_row, bool act, int leaf_m1, const PivotFlag& pf) {
+                                                 const double* q_row, bool act, int leaf_m1, const PivotFlag& pf, const Team& tm) {
     // leaf_m1: nodes m < leaf_m1 (level 0: no earlier neighbour, so D_m = J(m,m) and y_m = rhs_m) get their pivot inverse
     // and z_m = D_m^-1 rhs_m stored right here -- the refactor then has nothing to do at level 0 (kLeafDone)
     // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
     // the evaluation (act = false) takes part in the shuffles and writes nothing
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
+    const int lane = threadIdx.x & 31, nwarps = (blockDim.x >> 5) * tm.csz, warp = tm.rank * (blockDim.x >> 5) + (threadIdx.x >> 5), gsh = s.gsh;
     double loc = 0.0;
     for (int c = 0; c < t.n_class; ++c) {
         const RowClass rc = t.mm_class[c];
@@ -40,12 +40,24 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
             const bool lead = valid && part == 0 && act;
             double ire = 0.0, iim = 0.0;
             const int k1 = valid ? row.z : 0;
-            for (int k = row.y + part; k < k1; k += S) {
-                const int col = t.ycol[k];
-                const double2 y = t.ygb[k];
-                const double2 x = s.vv(col);
-                ire += y.x * x.x - y.y * x.y;
-                iim += y.y * x.x + y.x * x.y;
+            // four entries per step: their index / admittance loads are issued together, then the four V gathers -- a lane
+            // that walks a row alone has 2 dependent round trips per step instead of 2 per entry
+            for (int k = row.y + part; k < k1; k += 4 * S) {
+                int col[4]; double2 y[4], x[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int ku = k + u * S;
+                    const bool on = ku < k1;
+                    col[u] = on ? t.ycol[ku] : m;
+                    y[u] = on ? t.ygb[ku] : make_double2(0.0, 0.0);
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) x[u] = s.vv(col[u]);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    ire += y[u].x * x[u].x - y[u].y * x[u].y;
+                    iim += y[u].y * x[u].x + y[u].x * x[u].y;
+                }
             }
             for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { ire += shx(ire, o); iim += shx(iim, o); }
             if (lead) {
@@ -100,10 +112,17 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4
 // nodes have no terms, so these are already their final U and L' values.
 template <typename T, int kP>
 __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
-    for (int p = tsub; p < t.n_pair; p += nsub) {
-        Blk<T> U, L;
-        fill_pair<T, kP>(s, t.pair_mj[p], t.pair_y[p], U, L);
-        s.stU(p, U); s.stL(p, L);
+    // two pairs per step and lane: the index / admittance loads of both are issued before the state gathers of either
+    for (int p = tsub; p < t.n_pair; p += 2 * nsub) {
+        const int p2 = p + nsub;
+        const bool on2 = p2 < t.n_pair;
+        const int2 mj0 = t.pair_mj[p], mj1 = t.pair_mj[on2 ? p2 : p];
+        const double4 y0 = t.pair_y[p], y1 = t.pair_y[on2 ? p2 : p];
+        Blk<T> U0, L0, U1, L1;
+        fill_pair<T, kP>(s, mj0, y0, U0, L0);
+        fill_pair<T, kP>(s, mj1, y1, U1, L1);
+        s.stU(p, U0); s.stL(p, L0);
+        if (on2) { s.stU(p2, U1); s.stL(p2, L1); }
     }
 }
 
@@ -128,8 +147,9 @@ template <typename T, int kP> struct SparseSink {
 constexpr int kBigDoubles = 6;      // D (4) + y (2) per warp partial
 template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, typename Sink>
 __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const LevelDesc& d, const char* lb, const Sink& sink,
-                                                 const PivotFlag& pf, double* scratch, int& wrot) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh, G = 1 << gsh;
+                                                 const PivotFlag& pf, double* scratch, const Team& tm) {
+    // warps of the whole team; the big targets (CTA-wide through this CTA's shared memory) only when the CTA works alone
+    const int lane = threadIdx.x & 31, nwarps = (blockDim.x >> 5) * tm.csz, warp = tm.rank * (blockDim.x >> 5) + (threadIdx.x >> 5), gsh = s.gsh, G = 1 << gsh;
     const int* dptr = reinterpret_cast<const int*>(lb);
     const int* dord = reinterpret_cast<const int*>(lb + d.o_dord);
     const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
@@ -159,7 +179,7 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
         sink.diag(m, Di, y0, y1, kFactor, kSolve);
     };
     // ---- big diagonal targets: one at a time, every lane of the CTA takes every (lanes)-th item ----------------------
-    for (int i = 0; i < d.n_big; ++i) {
+    for (int i = 0; i < (tm.csz == 1 ? d.n_big : 0); ++i) {
         const int m = d.m0 + dord[i], t0 = dptr[i], t1 = dptr[i + 1];
         Blk<T> D = {T(0), T(0), T(0), T(0)};
         T y0 = T(0), y1 = T(0);
@@ -170,13 +190,13 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
         }
         __syncthreads();                                   // scratch free (previous big target consumed)
         if (lane < G) {
-            double* w = scratch + ((size_t)warp * G + lane) * kBigDoubles;
+            double* w = scratch + ((size_t)(threadIdx.x >> 5) * G + lane) * kBigDoubles;
             w[0] = double(D.a); w[1] = double(D.b); w[2] = double(D.c); w[3] = double(D.d); w[4] = double(y0); w[5] = double(y1);
         }
         __syncthreads();
         if (threadIdx.x < G) {
             double a[kBigDoubles] = {0, 0, 0, 0, 0, 0};
-            for (int w = 0; w < nwarps; ++w) {
+            for (int w = 0; w < (int)(blockDim.x >> 5); ++w) {
 #pragma unroll
                 for (int e = 0; e < kBigDoubles; ++e) a[e] += scratch[((size_t)w * G + threadIdx.x) * kBigDoubles + e];
             }
@@ -187,16 +207,27 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             diag_finish(m, Dm, r0, r1);
         }
     }
-    // ---- diagonal targets by class ------------------------------------------------------------------------------------
-    int i0 = d.n_big;
-    for (int c = 0; c < d.n_dcls; ++c) {
-        const int i1 = d.dcls[c].i1, ssh = min(d.dcls[c].ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
+    // ---- tasks: a warp-sized group of targets of one class; dealt to the warps round-robin ---------------------------
+    const int* tptr = reinterpret_cast<const int*>(lb + d.o_tptr);
+    const int* tord = reinterpret_cast<const int*>(lb + d.o_tord);
+    const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
+    const int4* tab = reinterpret_cast<const int4*>(lb + d.o_tab);
+    const int ncls = d.n_cls;
+    int c = 0, tc0 = 0, tc1 = 0;                           // class of the current task and its task range [tc0, tc1)
+    auto class_tasks = [&](int cc) { const Cls k = d.cls[cc]; const int tsh = 5 - gsh - min((int)k.ssh, 5 - gsh); return ((k.i1 - k.start) + (1 << tsh) - 1) >> tsh; };
+    if (ncls > 0) tc1 = class_tasks(0);
+    for (int t = warp; ; t += nwarps) {
+        while (c < ncls && t >= tc1) { ++c; tc0 = tc1; if (c < ncls) tc1 += class_tasks(c); }
+        if (c >= ncls) break;
+        const Cls k = d.cls[c];
+        if (!kFactor && !k.diag) break;                    // solve-only sweeps have no pair targets (diagonal classes come first)
+        const int ssh = min((int)k.ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
         const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-        const int w0 = warp - wrot < 0 ? warp - wrot + nwarps : warp - wrot;
-        for (int base = i0 + (w0 << tsh); base < i1; base += nwarps << tsh) {
-            const bool valid = base + tl < i1;
-            const int i = valid ? base + tl : i1 - 1, m = d.m0 + dord[i];
-            const bool lead = valid && part == 0;
+        const int idx = k.start + ((t - tc0) << tsh) + tl;
+        const bool valid = idx < k.i1, lead = valid && part == 0;
+        const int i = valid ? idx : k.i1 - 1;
+        if (k.diag) {
+            const int m = d.m0 + dord[i];
             const int t0 = dptr[i], t1 = valid ? dptr[i + 1] : t0;
             Blk<T> D = {T(0), T(0), T(0), T(0)};
             T y0 = T(0), y1 = T(0);
@@ -210,41 +241,37 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
                 if (kSolve) { y0 += shx(y0, o); y1 += shx(y1, o); }
             }
             if (lead) diag_finish(m, D, y0, y1);
-        }
-        const int tasks = ((i1 - i0) + (1 << tsh) - 1) >> tsh;
-        wrot = (wrot + tasks) % nwarps;
-        i0 = i1;
-    }
-    // ---- pair block-targets by class (they only need factors of earlier levels: concurrent with the diagonal targets) ---
-    if (kFactor) {
-        const int* tptr = reinterpret_cast<const int*>(lb + d.o_tptr);
-        const int* tord = reinterpret_cast<const int*>(lb + d.o_tord);
-        const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
-        const int4* tab = reinterpret_cast<const int4*>(lb + d.o_tab);
-        int b0 = 0;
-        for (int c = 0; c < d.n_tcls; ++c) {
-            const int b1 = d.tcls[c].i1, ssh = min(d.tcls[c].ssh, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
-            const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
-            const int w0 = warp - wrot < 0 ? warp - wrot + nwarps : warp - wrot;
-            for (int base = b0 + (w0 << tsh); base < b1; base += nwarps << tsh) {
-                const bool valid = base + tl < b1;
-                const int bt = valid ? base + tl : b1 - 1, i = bt >> 1, h = bt & 1;
-                const int t0 = tptr[i], t1 = valid ? tptr[i + 1] : t0;
-                const bool lead = valid && part == 0;
-                const int pl = tord[i], p = d.p0 + pl;
-                Blk<T> acc = {T(0), T(0), T(0), T(0)};
-                if (lead) acc = s.ldP(p, h);
-                for (int q = t0 + part; q < t1; q += S) {
-                    const int4 ab = tab[q];
-                    const Blk<T> W = mul(s.ldL(h ? ab.y : ab.x), s.ldD(ab.z));
-                    mulsub(acc, W, s.ldU(h ? ab.x : ab.y));
-                }
-                for (int o = (S >> 1) << gsh; o >= G; o >>= 1) blk_add_shx(acc, o);
-                if (lead) sink.pair(p, h, pmj[pl], acc);
+        } else if (kFactor) {
+#if SABLE_HALF_TARGETS
+            // block-targets bt = 2 i + h (h = 0: U(m,j), h = 1: L'(j,m)): one uniform item acc -= A D_k^-1 B, three operand blocks
+            const int ip = i >> 1, h = i & 1;
+            const int t0 = tptr[ip], t1 = valid ? tptr[ip + 1] : t0;
+            const int pl = tord[ip], p = d.p0 + pl;
+            Blk<T> acc = {T(0), T(0), T(0), T(0)};
+            if (lead) acc = s.ldP(p, h);
+            for (int q = t0 + part; q < t1; q += S) {
+                const int4 ab = tab[q];
+                const Blk<T> W = mul(s.ldL(h ? ab.y : ab.x), s.ldD(ab.z));
+                mulsub(acc, W, s.ldU(h ? ab.x : ab.y));
             }
-            const int tasks = ((b1 - b0) + (1 << tsh) - 1) >> tsh;
-            wrot = (wrot + tasks) % nwarps;
-            b0 = b1;
+            for (int o = (S >> 1) << gsh; o >= G; o >>= 1) blk_add_shx(acc, o);
+            if (lead) sink.pair(p, h, pmj[pl], acc);
+#else
+            // whole pair targets: five operand blocks in flight per item, both accumulators in one lane
+            const int t0 = tptr[i], t1 = valid ? tptr[i + 1] : t0;
+            const int pl = tord[i], p = d.p0 + pl;
+            Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
+            if (lead) { U = s.ldU(p); L = s.ldL(p); }
+            for (int q = t0 + part; q < t1; q += S) {
+                const int4 ab = tab[q];
+                const Blk<T> Dk = s.ldD(ab.z);
+                const Blk<T> La = s.ldL(ab.x), Ub = s.ldU(ab.y), Lb = s.ldL(ab.y), Ua = s.ldU(ab.x);
+                mulsub(U, mul(La, Dk), Ub);
+                mulsub(L, mul(Lb, Dk), Ua);
+            }
+            for (int o = (S >> 1) << gsh; o >= G; o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
+            if (lead) { const int2 mj = pmj[pl]; sink.pair(p, 0, mj, U); sink.pair(p, 1, mj, L); }
+#endif
         }
     }
 }
@@ -254,17 +281,16 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
 // processed (those below the dense top front: sable_front.cuh).
 template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone, bool kAll = true>
 __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring,
-                                                     const PivotFlag& pf, double* scratch, int nl_ = 0) {
+                                                     const PivotFlag& pf, double* scratch, const Team& tm, int nl_ = 0) {
     const int nl = kAll ? t.n_level : nl_;
     long long tk = clock64();
-    int wrot = 0;
     const SparseSink<T, kP> sink{s};
     for (int l = 0; l < nl; ++l) {
         const LevelDesc& d = lv[l];
         const char* lb = ring.acquire(l, d);
-        if (!(kLeafDone && l == 0)) accumulate_level<T, kP, kFactor, kSolve, kTransposed>(s, d, lb, sink, pf, scratch, wrot);
+        if (!(kLeafDone && l == 0)) accumulate_level<T, kP, kFactor, kSolve, kTransposed>(s, d, lb, sink, pf, scratch, tm);
         if (kLeafDone && l == 0 && !ring.on) continue;   // nothing was done at level 0: no barrier needed
-        __syncthreads();
+        team_sync(tm);
         ring.tick(4 * l, tk);
         ring.release(l);
     }
@@ -274,9 +300,9 @@ __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const
 // by m, levels descending.  kTransposed: (L' D^-1)^T lambda = w, lambda_m = w_m - D_m^-T sum_j L'(j,m)^T lambda_j.
 // Contains barriers.
 template <typename T, int kP, bool kTransposed, bool kAll = true>
-__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, int nl_ = 0) {
+__device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring, const Team& tm, int nl_ = 0) {
     const int nl = kAll ? t.n_level : nl_;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, gsh = s.gsh;
+    const int lane = threadIdx.x & 31, nwarps = (blockDim.x >> 5) * tm.csz, warp = tm.rank * (blockDim.x >> 5) + (threadIdx.x >> 5), gsh = s.gsh;
     long long tk = clock64();
     for (int l = nl - 1; l >= 0; --l) {
         const LevelDesc& d = lv[l];
@@ -306,7 +332,7 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
                 s.set_rh(m, make_double2(double(T(r.x) - z0), double(T(r.y) - z1)));
             }
         }
-        __syncthreads();
+        team_sync(tm);
         ring.tick(4 * l + 2, tk);
         ring.release(l);
     }
@@ -316,13 +342,19 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
 // off the level-by-level critical path of the backward sweep).  No barrier.
 template <typename T, int kP>
 __device__ __forceinline__ void stage_update(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
-    for (int m = tsub; m < t.n_node; m += nsub) {
-        const double2 a = s.ma(m), x = s.rh(m);
-        const double th = a.y + x.x;
-        const double vm = t.node_pq[m] ? a.x + x.y : a.x;
-        double sn, cs; sincos(th, &sn, &cs);
-        s.set_ma(m, make_double2(vm, th));
-        s.set_vv(m, make_double2(vm * cs, vm * sn));
+    for (int m = tsub; m < t.n_node; m += 2 * nsub) {
+        const int m2 = m + nsub < t.n_node ? m + nsub : m;
+        const double2 a0 = s.ma(m), x0 = s.rh(m), a1 = s.ma(m2), x1 = s.rh(m2);
+        const bool q0 = t.node_pq[m], q1 = t.node_pq[m2];
+        const double th0 = a0.y + x0.x, th1 = a1.y + x1.x;
+        const double vm0 = q0 ? a0.x + x0.y : a0.x, vm1 = q1 ? a1.x + x1.y : a1.x;
+        double sn0, cs0, sn1, cs1; sincos(th0, &sn0, &cs0); sincos(th1, &sn1, &cs1);
+        s.set_ma(m, make_double2(vm0, th0));
+        s.set_vv(m, make_double2(vm0 * cs0, vm0 * sn0));
+        if (m2 != m) {
+            s.set_ma(m2, make_double2(vm1, th1));
+            s.set_vv(m2, make_double2(vm1 * cs1, vm1 * sn1));
+        }
     }
 }
 
