@@ -357,29 +357,29 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         ctx->placement = 0; th = th0; gsh = gsh0; ctx->csz = 1;
     } else {
         // ---- HBM placement (everything in the group-interleaved workspace, blobs read in place, no ring) --------------
-        // Occupancy model.  The path is bound by memory latency and by the L1 data pipe: a lane's
-        // 16-byte access is one L1 wavefront unless the lanes beside it read the words beside it, which is what a group of
-        // G interleaved scenarios gives (measured per-SM throughput on the 9 241-bus grid, same 1 024 threads per SM:
-        // G = 2 / 4 / 8 / 16 -> 0.32 / 0.47 / 0.63 / 0.78 scenarios per SM and ms).  So:
-        //  * many scenarios (batch >= 8 per SM): lanes per scenario L = 2^floor(log2(n_node / 8)) in [32, 512], G such that a
-        //    CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72 registers), CTAs work alone;
-        //  * few scenarios: groups of G = 8 (fewer if the batch is smaller) served by a TEAM of csz CTAs (one cluster) of
-        //    1 024 threads each, csz = the largest power of two <= 8 that the teams of the batch still fit the SMs with.
-        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
+        // Occupancy model.  The path is bound by memory latency: the SM should hold as many
+        // independent elimination chains (scenarios) as its registers allow, each with enough lanes for its levels.
+        //  * lanes per scenario L: 0.6 x the mean number of work items of an elimination level (diagonal and pair targets
+        //    plus their multiply-subtract items), as a power of two in [32, 512] -- a tree-like 300-bus grid gets 32, a
+        //    2 000-bus grid 256, a 900-bus mesh with 3x fill 256, the 9 241-bus grid 512;
+        //  * slots per CTA G such that a CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72
+        //    registers), never so many that the batch leaves SMs without a CTA;
+        //  * single-wave batches (at most two scenarios per SM, e.g. 256 scenarios of 9 241 buses): two CTAs would share an
+        //    SM anyway, so they are merged into one CTA of twice the threads whose two scenarios interleave their slices --
+        //    neighbouring lanes then read neighbouring 16-byte words (half the L1 wavefronts: 6.2 vs 6.6 ms measured);
+        //  * teams (a cluster of CTAs per group, tune.cluster) only on request.
+        const double items = (double)T.term_a.size() + (double)T.dterm.size() + (double)np + (double)nn;
+        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, (int)(0.6 * items / std::max(1, nl))))));
         const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
-        int csz = 1;
+        const int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
         int G = std::max(1, 128 / L);
         if (g_given) G = g_want;
-        else while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
-        const bool few = !th_given && !g_given && (int64_t)mb * L < (int64_t)n_sm * 1024 * 4 && nn >= 1024;   // the batch cannot fill the SMs' threads four times over
-        if (few) {
-            G = 8; while (G > 1 && G > mb) G /= 2;
-            const int teams = (mb + G - 1) / G;
-            csz = 1; while (csz < 8 && teams * csz * 2 <= n_sm) csz *= 2;
+        else {
+            while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
+            if (G == 1 && 2 * L <= 1024 && mb <= 2 * n_sm && 20 * ((mb + 1) / 2) >= 17 * n_sm) G = 2;
         }
-        if (c_given) csz = pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8));
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : (few || csz > 1) ? 1024 : L << gsh;
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : std::min(1024, L << gsh);
         th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
         ctx->placement = 2; ctx->csz = csz;
@@ -416,7 +416,9 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     const int Ls = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
     ctx->threads_stage = (tune(tu.threads_stage, 0, "SABLE_THREADS1", ctx->placement == 2 ? std::min(th, 512) : std::min(512, Ls << gsh), 32, 512) + 31) / 32 * 32;
     ctx->csz_lin = ctx->csz;
-    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    // adjoint kernel: 32 lanes per slot (measured best in round 1: a pure latency chain wants many small CTAs); the merged
+    // single-wave layout (two slots of a large grid per CTA) wants the whole SM
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh == 1 && th == 1024) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     return SABLE_OK;
 }
