@@ -126,6 +126,18 @@ __device__ __forceinline__ void st_blk(double* p, int vs, const Blk<double>& v) 
 __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
     *reinterpret_cast<float4*>(p) = make_float4(v.a, v.b, v.c, v.d);
 }
+// whole block in one access (HBM workspace: blocks are interleaved over the slots as units of 4 sizeof(T) bytes): one
+// 256-bit load / store per FP64 block (sm_100: LDG.256 / STG.256) -- half the L1 wavefronts of two 128-bit accesses
+__device__ __forceinline__ Blk<double> ldg_blk(const double* p) {
+    Blk<double> v;
+    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.a), "=d"(v.b), "=d"(v.c), "=d"(v.d) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ Blk<float> ldg_blk(const float* p) { return ld_blk(p, 0); }
+__device__ __forceinline__ void stg_blk(double* p, const Blk<double>& v) {
+    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.a), "d"(v.b), "d"(v.c), "d"(v.d) : "memory");
+}
+__device__ __forceinline__ void stg_blk(float* p, const Blk<float>& v) { st_blk(p, 0, v); }
 
 // One thread's view of the slot it serves.  kP = 0: everything in shared memory; 2: everything in the HBM workspace
 // (two kernel families without placement branches).
@@ -137,21 +149,26 @@ template <typename T, int kP> struct Slot {
     char *sb, *gf, *gw;
     unsigned so_ma, so_rh, so_dg, so_pu, so_pl, go_pu, go_pl, go_ma, go_rh;
     int gsh;
-    // byte offsets are 32-bit: a group's slice (and shared memory) is far below 4 GB
-    __device__ __forceinline__ T* blk_ptr(unsigned so, unsigned go, int idx, int& vs) const {
-        vs = 16 << gsh;
-        if (kP == 0) return reinterpret_cast<T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4))));
-        return reinterpret_cast<T*>(gf + (go + ((unsigned)(idx * VPB) << (gsh + 4))));
+    // byte offsets are 32-bit: a group's slice (and shared memory) is far below 4 GB.  Shared memory: blocks interleaved
+    // over the slots in 16-byte vectors (sb carries g * 16); HBM: interleaved as whole blocks (gf carries g * kBlk).
+    static constexpr int kBlk = (int)(4 * sizeof(T));
+    __device__ __forceinline__ Blk<T> ldB(unsigned so, unsigned go, int idx) const {
+        if (kP == 0) return ld_blk(reinterpret_cast<const T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4)))), 16 << gsh);
+        return ldg_blk(reinterpret_cast<const T*>(gf + (go + (((unsigned)idx << gsh) * kBlk))));
     }
-    __device__ __forceinline__ Blk<T> ldD(int m) const { int vs; const T* p = blk_ptr(so_dg, 0u, m, vs); return ld_blk(p, vs); }
-    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { int vs; T* p = blk_ptr(so_dg, 0u, m, vs); st_blk(p, vs, v); }
-    __device__ __forceinline__ Blk<T> ldU(int p) const { int vs; const T* q = blk_ptr(so_pu, go_pu, p, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ Blk<T> ldL(int p) const { int vs; const T* q = blk_ptr(so_pl, go_pl, p, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(so_pu, go_pu, p, vs); st_blk(q, vs, v); }
-    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { int vs; T* q = blk_ptr(so_pl, go_pl, p, vs); st_blk(q, vs, v); }
-    // h = 0: the U block of pair p, h = 1: the L' block (block-targets, sable_stages.cuh)
-    __device__ __forceinline__ Blk<T> ldP(int p, int h) const { int vs; const T* q = blk_ptr(h ? so_pl : so_pu, h ? go_pl : go_pu, p, vs); return ld_blk(q, vs); }
-    __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { int vs; T* q = blk_ptr(h ? so_pl : so_pu, h ? go_pl : go_pu, p, vs); st_blk(q, vs, v); }
+    __device__ __forceinline__ void stB(unsigned so, unsigned go, int idx, const Blk<T>& v) const {
+        if (kP == 0) st_blk(reinterpret_cast<T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4)))), 16 << gsh, v);
+        else stg_blk(reinterpret_cast<T*>(gf + (go + (((unsigned)idx << gsh) * kBlk))), v);
+    }
+    __device__ __forceinline__ Blk<T> ldD(int m) const { return ldB(so_dg, 0u, m); }
+    __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { stB(so_dg, 0u, m, v); }
+    __device__ __forceinline__ Blk<T> ldU(int p) const { return ldB(so_pu, go_pu, p); }
+    __device__ __forceinline__ Blk<T> ldL(int p) const { return ldB(so_pl, go_pl, p); }
+    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { stB(so_pu, go_pu, p, v); }
+    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { stB(so_pl, go_pl, p, v); }
+    // h = 0: the U block of pair p, h = 1: the L' block
+    __device__ __forceinline__ Blk<T> ldP(int p, int h) const { return ldB(h ? so_pl : so_pu, h ? go_pl : go_pu, p); }
+    __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { stB(h ? so_pl : so_pu, h ? go_pl : go_pu, p, v); }
 
     __device__ __forceinline__ double2* st_ptr(unsigned so, unsigned go, int m) const {
         if (kP == 0) return reinterpret_cast<double2*>(sb + (so + ((unsigned)m << (gsh + 4))));

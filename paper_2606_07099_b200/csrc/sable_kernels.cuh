@@ -70,7 +70,7 @@ template <typename T, int kP>
 __device__ __forceinline__ void bind(Slot<T, kP>& s, char* factors, int64_t fac_stride, char* work, int64_t work_stride, int b) {
     const int gsh = s.gsh;
     const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
-    s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + lane16;
+    s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + (size_t)(b & ((1 << gsh) - 1)) * (4 * sizeof(T));   // whole blocks interleave
     s.gw = work + ((grp * (size_t)work_stride) << gsh) + lane16;
 }
 
@@ -110,10 +110,10 @@ __device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kP
 // scenario's HBM slice (same order dg | pu | pl, same interleaving)
 template <typename T, int kP>
 __device__ __forceinline__ void store_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
-    constexpr int VPB = Slot<T, kP>::VPB;
-    const int n = (t.n_node + 2 * t.n_pair) * VPB;
+    // dg | pu | pl are contiguous block arrays in both memories: block i of the shared copy goes to block i of the HBM slice
+    const int n = t.n_node + 2 * t.n_pair;
     for (int i = tsub; i < n; i += nsub)
-        *reinterpret_cast<int4*>(s.gf + ((size_t)i << (s.gsh + 4))) = *reinterpret_cast<const int4*>(s.sb + s.so_dg + ((size_t)i << (s.gsh + 4)));
+        stg_blk(reinterpret_cast<T*>(s.gf + (((size_t)i << s.gsh) * (4 * sizeof(T)))), s.ldB(s.so_dg, 0u, i));
 }
 
 __device__ __forceinline__ int pop_group(const SolveArgs& A) {
