@@ -359,17 +359,17 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         // ---- HBM placement (everything in the group-interleaved workspace, blobs read in place, no ring) --------------
         // Occupancy model.  The path is bound by memory latency: the SM should hold as many
         // independent elimination chains (scenarios) as its registers allow, each with enough lanes for its levels.
-        //  * lanes per scenario L: 0.6 x the mean number of work items of an elimination level (diagonal and pair targets
-        //    plus their multiply-subtract items), as a power of two in [32, 512] -- a tree-like 300-bus grid gets 32, a
-        //    2 000-bus grid 256, a 900-bus mesh with 3x fill 256, the 9 241-bus grid 512;
+        //  * lanes per scenario L: 0.75 x the mean number of multiply-subtract items of an elimination level, as a power of
+        //    two in [32, 512] -- a tree-like 300-bus grid gets 32, a 2 000-bus grid 128, a 900-bus mesh with 3x fill 256, the
+        //    9 241-bus grid 512 (each measured best: 3.83 vs 4.03 ms at 256 on the 2 000-bus grid, 4.1 vs 5.2 ms at 128 on the mesh);
         //  * slots per CTA G such that a CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72
         //    registers), never so many that the batch leaves SMs without a CTA;
         //  * single-wave batches (at most two scenarios per SM, e.g. 256 scenarios of 9 241 buses): two CTAs would share an
         //    SM anyway, so they are merged into one CTA of twice the threads whose two scenarios interleave their slices --
         //    neighbouring lanes then read neighbouring 16-byte words (half the L1 wavefronts: 6.2 vs 6.6 ms measured);
         //  * teams (a cluster of CTAs per group, tune.cluster) only on request.
-        const double items = (double)T.term_a.size() + (double)T.dterm.size() + (double)np + (double)nn;
-        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, (int)(0.6 * items / std::max(1, nl))))));
+        const double items = (double)T.term_a.size() + (double)T.dterm.size();
+        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, (int)(0.75 * items / std::max(1, nl))))));
         const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
         const int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
         int G = std::max(1, 128 / L);
@@ -396,7 +396,9 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     if (ctx->placement == 2) {
         // dense top front: shared memory that still leaves most of the L1 to the resident CTAs
         const int kcap = tune(tu.front_nodes, -1, "SABLE_FRONT", 64, 0, 96);
-        const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : 16, 0, 220) * 1024LL;
+        // (a CTA that has the SM to itself -- the merged single-wave layout -- can afford a large front: 5.69 ms with 32 nodes
+        // against 5.98 with 15 and 6.17 without on the 9 241-bus grid; small CTAs that share the SM keep the L1)
+        const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : th <= 512 ? 16 : 72, 0, 220) * 1024LL;
         if (kcap >= 2 && ctx->csz == 1) build_front(ctx, th, gsh, budget, kcap, true);
         if (ctx->front_k > 0) {
             ctx->front_off = align16(ctx->smem);

@@ -152,11 +152,26 @@ template <typename T, int kP> struct Slot {
     // byte offsets are 32-bit: a group's slice (and shared memory) is far below 4 GB.  Shared memory: blocks interleaved
     // over the slots in 16-byte vectors (sb carries g * 16); HBM: interleaved as whole blocks (gf carries g * kBlk).
     static constexpr int kBlk = (int)(4 * sizeof(T));
+#ifdef SABLE_BOUNDS
+    // debug build (-DSABLE_BOUNDS): every block / state access is checked against the array it addresses; a violation traps
+    // (compute-sanitizer is closed on the measurement pool: profiles/r02_sanitizer.md)
+    int nn_, np_;
+    __device__ __forceinline__ void chk_blk(unsigned go, int idx) const {
+        const int n = go == 0u ? nn_ : np_;
+        if (idx < 0 || idx >= n || (go != 0u && go != go_pu && go != go_pl)) __trap();
+    }
+    __device__ __forceinline__ void chk_st(int m) const { if (m < 0 || m > nn_) __trap(); }
+#else
+    __device__ __forceinline__ void chk_blk(unsigned, int) const {}
+    __device__ __forceinline__ void chk_st(int) const {}
+#endif
     __device__ __forceinline__ Blk<T> ldB(unsigned so, unsigned go, int idx) const {
+        chk_blk(kP == 0 ? (so == so_dg ? 0u : so == so_pu ? go_pu : go_pl) : go, idx);
         if (kP == 0) return ld_blk(reinterpret_cast<const T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4)))), 16 << gsh);
         return ldg_blk(reinterpret_cast<const T*>(gf + (go + (((unsigned)idx << gsh) * kBlk))));
     }
     __device__ __forceinline__ void stB(unsigned so, unsigned go, int idx, const Blk<T>& v) const {
+        chk_blk(kP == 0 ? (so == so_dg ? 0u : so == so_pu ? go_pu : go_pl) : go, idx);
         if (kP == 0) st_blk(reinterpret_cast<T*>(sb + (so + ((unsigned)(idx * VPB) << (gsh + 4)))), 16 << gsh, v);
         else stg_blk(reinterpret_cast<T*>(gf + (go + (((unsigned)idx << gsh) * kBlk))), v);
     }
@@ -171,6 +186,7 @@ template <typename T, int kP> struct Slot {
     __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { stB(h ? so_pl : so_pu, h ? go_pl : go_pu, p, v); }
 
     __device__ __forceinline__ double2* st_ptr(unsigned so, unsigned go, int m) const {
+        chk_st(m);
         if (kP == 0) return reinterpret_cast<double2*>(sb + (so + ((unsigned)m << (gsh + 4))));
         return reinterpret_cast<double2*>(gw + (go + ((unsigned)m << (gsh + 4))));
     }

@@ -63,6 +63,9 @@ __device__ __forceinline__ Slot<T, kP> carve(unsigned char* smem, int64_t slot_o
     s.gf = s.gw = nullptr;
     s.go_pu = nd; s.go_pl = nd + np; s.go_ma = ns; s.go_rh = 2 * ns;
     s.gsh = gsh;
+#ifdef SABLE_BOUNDS
+    s.nn_ = n_node; s.np_ = n_pair;
+#endif
     return s;
 }
 // HBM part: the slices of scenario b's group (b >> gsh), offset to lane b & (G - 1); strides are per scenario
@@ -112,8 +115,10 @@ template <typename T, int kP>
 __device__ __forceinline__ void store_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
     // dg | pu | pl are contiguous block arrays in both memories: block i of the shared copy goes to block i of the HBM slice
     const int n = t.n_node + 2 * t.n_pair;
-    for (int i = tsub; i < n; i += nsub)
-        stg_blk(reinterpret_cast<T*>(s.gf + (((size_t)i << s.gsh) * (4 * sizeof(T)))), s.ldB(s.so_dg, 0u, i));
+    for (int i = tsub; i < n; i += nsub) {
+        const Blk<T> v = i < t.n_node ? s.ldD(i) : i < t.n_node + t.n_pair ? s.ldU(i - t.n_node) : s.ldL(i - t.n_node - t.n_pair);
+        stg_blk(reinterpret_cast<T*>(s.gf + (((size_t)i << s.gsh) * (4 * sizeof(T)))), v);
+    }
 }
 
 __device__ __forceinline__ int pop_group(const SolveArgs& A) {
