@@ -118,15 +118,32 @@ int build_template(int32_t n_bus, const int32_t* row_ptr, const int32_t* col_idx
 
     // ---- 4. final order: by level, then by elimination step (any topological order of the elimination tree
     //         gives the same fill); positions, maps, levels --------------------------------------------------
-    //         Within a level the nodes with the most eliminated neighbours come first (their diagonal targets have the
-    //         longest multiply-subtract lists: the per-level target classes of the kernels are then contiguous ranges).
-    std::vector<int32_t> order(N), n_lower(N, 0);
-    for (int p = 0; p < N; ++p) { order[p] = p; for (int32_t u : upper[p]) n_lower[u]++; }
-    std::sort(order.begin(), order.end(), [&](int a, int b) {
-        if (lvl[a] != lvl[b]) return lvl[a] < lvl[b];
-        if (n_lower[a] != n_lower[b]) return n_lower[a] > n_lower[b];
-        return elim_pos[a] < elim_pos[b];
-    });
+    //         Within a level the order is free: nodes are placed next to the nodes that share their first later
+    //         neighbour (levels are placed from the top down; key = position of the earliest-placed later neighbour), so
+    //         that the leaves of one hub are contiguous -- the hub's Y row, its diagonal target's item list and the pairs
+    //         those leaves own are then contiguous in memory and the lanes that walk them read neighbouring words.
+    std::vector<int32_t> order(N);
+    {
+        int nlev = 0;
+        for (int p = 0; p < N; ++p) nlev = std::max(nlev, lvl[p] + 1);
+        std::vector<std::vector<int32_t>> by_level(nlev);
+        for (int p = 0; p < N; ++p) by_level[lvl[p]].push_back(p);
+        std::vector<int32_t> level_start(nlev + 1, 0), rank(N, 0);          // rank: position within the level
+        for (int l = 0; l < nlev; ++l) level_start[l + 1] = level_start[l] + (int32_t)by_level[l].size();
+        for (int l = nlev - 1; l >= 0; --l) {
+            std::vector<int32_t>& v = by_level[l];
+            std::vector<int64_t> key(N, 0);
+            for (int32_t p : v) {
+                int64_t k = (int64_t)N;                                    // nodes of the top level: elimination order
+                for (int32_t u : upper[p]) k = std::min<int64_t>(k, (int64_t)level_start[lvl[u]] + rank[u]);
+                key[p] = k;
+            }
+            std::stable_sort(v.begin(), v.end(), [&](int a, int b) { return key[a] != key[b] ? key[a] < key[b] : elim_pos[a] < elim_pos[b]; });
+            for (size_t i = 0; i < v.size(); ++i) rank[v[i]] = (int32_t)i;
+        }
+        int q = 0;
+        for (int l = 0; l < nlev; ++l) for (int32_t p : by_level[l]) order[q++] = p;
+    }
     std::vector<int32_t> pos(N);
     for (int q = 0; q < N; ++q) pos[order[q]] = q;
     T.n_bus = n_bus; T.slack = slack; T.n_node = N;
