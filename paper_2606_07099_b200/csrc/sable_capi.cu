@@ -95,7 +95,12 @@ static void fill_info(sable_ctx* c) {
 
 // kernel variants of the fused kernel: (placement, max threads per CTA, CTAs per SM the registers are budgeted for)
 struct Variant { int place, threads, ctas; };
-static const Variant kVariants[] = {{0, 512, 1}, {2, 128, 7}, {2, 256, 4}, {2, 512, 2}, {2, 1024, 1}};
+// CTAs per SM the 128-thread variant is budgeted for: 7 (72 registers) with FP64 factors, kSmallCtasF32 with FP32 factors
+template <typename T> struct SmallCtas { static constexpr int v = 7; };
+#ifndef SABLE_SMALL_CTAS_F32
+#define SABLE_SMALL_CTAS_F32 8
+#endif
+template <> struct SmallCtas<float> { static constexpr int v = SABLE_SMALL_CTAS_F32; };
 static int pick_variant(int place, int th) {
     if (place == 0) return 0;
     return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : 4;
@@ -103,7 +108,7 @@ static int pick_variant(int place, int th) {
 template <typename T> static const void* fused_fn_t(int v) {
     switch (v) {
         case 0: return (const void*)k_nr_fused<T, 0, 512, 1>;
-        case 1: return (const void*)k_nr_fused<T, 2, 128, 7>;
+        case 1: return (const void*)k_nr_fused<T, 2, 128, SmallCtas<T>::v>;
         case 2: return (const void*)k_nr_fused<T, 2, 256, 4>;
         case 3: return (const void*)k_nr_fused<T, 2, 512, 2>;
         default: return (const void*)k_nr_fused<T, 2, 1024, 1>;
@@ -594,7 +599,7 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
     cfg.attrs = at; cfg.numAttrs = c->csz > 1 ? 1 : 0;
     switch (c->variant) {
         case 0: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 0, 512, 1>, A);
-        case 1: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 128, 7>, A);
+        case 1: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 128, SmallCtas<T>::v>, A);
         case 2: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 256, 4>, A);
         case 3: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 512, 2>, A);
         default: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 1024, 1>, A);
