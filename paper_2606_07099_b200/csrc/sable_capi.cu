@@ -98,7 +98,7 @@ struct Variant { int place, threads, ctas; };
 // CTAs per SM the 128-thread variant is budgeted for: 7 (72 registers) with FP64 factors, kSmallCtasF32 with FP32 factors
 template <typename T> struct SmallCtas { static constexpr int v = 7; };
 #ifndef SABLE_SMALL_CTAS_F32
-#define SABLE_SMALL_CTAS_F32 8
+#define SABLE_SMALL_CTAS_F32 7
 #endif
 template <> struct SmallCtas<float> { static constexpr int v = SABLE_SMALL_CTAS_F32; };
 static int pick_variant(int place, int th) {
