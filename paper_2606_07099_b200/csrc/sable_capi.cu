@@ -103,7 +103,7 @@ template <typename T> struct SmallCtas { static constexpr int v = 7; };
 template <> struct SmallCtas<float> { static constexpr int v = SABLE_SMALL_CTAS_F32; };
 static int pick_variant(int place, int th) {
     if (place == 0) return 0;
-    return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : 4;
+    return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : th <= 768 ? 5 : 4;
 }
 template <typename T> static const void* fused_fn_t(int v) {
     switch (v) {
@@ -111,6 +111,7 @@ template <typename T> static const void* fused_fn_t(int v) {
         case 1: return (const void*)k_nr_fused<T, 2, 128, SmallCtas<T>::v>;
         case 2: return (const void*)k_nr_fused<T, 2, 256, 4>;
         case 3: return (const void*)k_nr_fused<T, 2, 512, 2>;
+        case 5: return (const void*)k_nr_fused<T, 2, 768, 1>;
         default: return (const void*)k_nr_fused<T, 2, 1024, 1>;
     }
 }
@@ -384,7 +385,8 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
             if (G == 1 && 2 * L <= 1024 && mb <= 2 * n_sm && 20 * ((mb + 1) / 2) >= 17 * n_sm) G = 2;
         }
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : std::min(1024, L << gsh);
+        // (the merged layout runs 768 threads, 80 registers each: 5.35 ms against 5.63 at 1 024 threads / 64 registers)
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : (L << gsh) >= 1024 ? 768 : (L << gsh);
         th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
         ctx->placement = 2; ctx->csz = csz;
@@ -403,7 +405,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         const int kcap = tune(tu.front_nodes, -1, "SABLE_FRONT", 64, 0, 96);
         // (a CTA that has the SM to itself -- the merged single-wave layout -- can afford a large front: 5.69 ms with 32 nodes
         // against 5.98 with 15 and 6.17 without on the 9 241-bus grid; small CTAs that share the SM keep the L1)
-        const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : th <= 512 ? 16 : 72, 0, 220) * 1024LL;
+        const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : th <= 512 ? 16 : 96, 0, 220) * 1024LL;
         if (kcap >= 2 && ctx->csz == 1) build_front(ctx, th, gsh, budget, kcap, true);
         if (ctx->front_k > 0) {
             ctx->front_off = align16(ctx->smem);
@@ -425,7 +427,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     ctx->csz_lin = ctx->csz;
     // adjoint kernel: 32 lanes per slot (measured best in round 1: a pure latency chain wants many small CTAs); the merged
     // single-wave layout (two slots of a large grid per CTA) wants the whole SM
-    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh == 1 && th == 1024) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh == 1 && th >= 768) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     return SABLE_OK;
 }
@@ -602,6 +604,7 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
         case 1: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 128, SmallCtas<T>::v>, A);
         case 2: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 256, 4>, A);
         case 3: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 512, 2>, A);
+        case 5: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 768, 1>, A);
         default: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 1024, 1>, A);
     }
 }
