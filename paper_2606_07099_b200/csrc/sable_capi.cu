@@ -373,20 +373,31 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         //  * single-wave batches (at most two scenarios per SM, e.g. 256 scenarios of 9 241 buses): two CTAs would share an
         //    SM anyway, so they are merged into one CTA of twice the threads whose two scenarios interleave their slices --
         //    neighbouring lanes then read neighbouring 16-byte words (half the L1 wavefronts: 6.2 vs 6.6 ms measured);
-        //  * teams (a cluster of CTAs per group, tune.cluster) only on request.
+        //  * teams (a cluster of CTAs per group): for tiny batches of large grids (below), or on request (tune.cluster).
         const double items = (double)T.term_a.size() + (double)T.dterm.size();
         const int L = std::min(512, std::max(32, pow2_floor(std::max(1, (int)(0.75 * items / std::max(1, nl))))));
         const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
-        const int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
+        int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
         int G = std::max(1, 128 / L);
         if (g_given) G = g_want;
         else {
             while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
             if (G == 1 && 2 * L <= 1024 && mb <= 2 * n_sm && 20 * ((mb + 1) / 2) >= 17 * n_sm) G = 2;
         }
+        // tiny batches of large grids (the paper's own shapes: 4 ... 32 scenarios of 9 241 buses): the scenarios cannot fill
+        // the SMs, and one scenario's wide levels want more lanes than a CTA has -- a team of 2 / 4 / 8 CTAs (one cluster) per
+        // scenario, as large as keeps all teams within half of the SMs (clusters are placed GPC by GPC).  Measured on the
+        // only the very large grids gain: see below.
+        if (!c_given && !g_given && !th_given && ctx->opt.threads <= 0 && G == 1 && L >= 512 && nn >= 16384)
+            while (csz < 8 && (int64_t)mb * csz * 2 * 2 <= n_sm) csz *= 2;
+        // batches that leave every CTA an SM of its own: the CTA takes 768 threads (and the large front budget below) whatever
+        // the grid -- 9 241-bus stand-in, 64 scenarios: 4.14 ms at 256 threads, 2.46 at 768; 3 120 buses x 8: 2.05 -> 1.29;
+        // 1 354 buses x 8: 0.79 -> 0.60 (a team of CTAs per scenario is slower there: 2.40 ms for 4 scenarios of 9 241 buses
+        // against 2.28; it wins on the 25 000-bus stand-in, 27 vs 33 ms for 8 scenarios x 30 iterations)
+        const bool alone = (int64_t)(mb + G - 1) / G <= n_sm && G == 1;
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
         // (the merged layout runs 768 threads, 80 registers each: 5.35 ms against 5.63 at 1 024 threads / 64 registers)
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : (L << gsh) >= 1024 ? 768 : (L << gsh);
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : (alone || (L << gsh) >= 1024) ? 768 : (L << gsh);
         th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
         ctx->placement = 2; ctx->csz = csz;
