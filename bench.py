@@ -364,10 +364,12 @@ def paper_sweep(reps=7):
         seed, net, Yh, ps, qs, vs = chosen
         row = {"network_seed": seed, "n_branch": int(net.f.shape[0])}
         for prec, pname in ((sb.FP64, "fp64"), (sb.MIXED, "mixed")):
-            ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=256, precision=prec, keep_factors=False, device=dev.index)
-            row.setdefault("info", {k: ctx.info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level")})
             res = {}
             for B in (4, 8, 16, 32, 64, 128, 256):
+                # one context per batch size: the launch plan is made for max_batch (the paper, too, sets up once per topology
+                # AND batch size)
+                ctx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=B, precision=prec, keep_factors=False, device=dev.index)
+                row.setdefault("info", {k: ctx.info[k] for k in ("n", "nnz_j", "nnz_lu", "n_level")})
                 a = (d(ps[:B]), d(qs[:B]), d(vs[:B]))
                 for _ in range(3):
                     o = ctx.solve(*a, tol=1e-8, max_it=30)
@@ -377,9 +379,10 @@ def paper_sweep(reps=7):
                     e0.record(); o = ctx.solve(*a, tol=1e-8, max_it=30); e1.record(); torch.cuda.synchronize()
                     ts.append(e0.elapsed_time(e1))
                 its = o["iterations"].cpu().numpy()
-                res[str(B)] = {"ms": float(np.median(ts)), "iterations_max": int(its.max()), "converged": int(o["converged"].sum().item())}
+                res[str(B)] = {"ms": float(np.median(ts)), "iterations_max": int(its.max()), "converged": int(o["converged"].sum().item()),
+                               "plan": {k: ctx.info[k] for k in ("threads", "slots_per_cta", "cluster", "front_k")}}
+                ctx.close()
             row[pname] = res
-            ctx.close()
         out[str(nb)] = row
     return out
 
