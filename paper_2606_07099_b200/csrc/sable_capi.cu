@@ -11,6 +11,7 @@
 
 using namespace sable;
 
+struct FrontPlan_ { int k = 0, f0 = 0, level = 0; LevelDesc d{}; };
 struct sable_ctx {
     Template T;
     sable_options opt{};
@@ -36,6 +37,7 @@ struct sable_ctx {
     std::vector<char> blob_host;
     int ring_r = 0, ring_slot = 0, first_staged = 0;
     int front_k = 0, front_f0 = 0, front_level = 0; int64_t front_off = 0; LevelDesc front{};   // dense top front (sable_front.cuh)
+    FrontPlan_ lin_front;                                    // the adjoint kernel's own (larger) front
     int last_batch = -1;  bool have_factors = false;
     int64_t launches = 0;
     std::string err;
@@ -281,21 +283,23 @@ static std::vector<LevelDesc> build_levels(const Template& T, const LevelPack& P
 // Dense top front (sable_front.cuh): the nodes of the last elimination levels, as many levels as keep the K x K block
 // matrix within `budget` bytes of shared memory per CTA (K <= kcap).  Appends the assembly lists (the front targets'
 // items whose eliminated node k lies below the front) to the blob and fills ctx->front*.
-static void build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap, bool allow_big) {
+struct FrontPlan { int k = 0, f0 = 0, level = 0; LevelDesc d{}; };
+static FrontPlan build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap, bool allow_big) {
     const Template& T = c->T;
     const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
     const bool mixed = c->opt.precision == SABLE_MIXED;
-    c->front_k = 0; c->front_f0 = nn; c->front_level = nl; c->front = LevelDesc{};
+    FrontPlan fp; fp.k = 0; fp.f0 = nn; fp.level = nl;
     auto bytes = [&](int K) { return mixed ? front_bytes<float>(K, gsh) : front_bytes<double>(K, gsh); };
     int lc = nl;
     while (lc > 1 && nn - T.level_ptr[lc - 1] <= kcap && bytes(nn - T.level_ptr[lc - 1]) <= budget) --lc;
-    if (nl - lc < 2) return;                                 // merging fewer than two levels saves nothing
+    if (nl - lc < 2) return fp;                              // merging fewer than two levels saves nothing
     const int f0 = T.level_ptr[lc];
     LevelDesc d{};
     d.m0 = f0; d.m1 = nn; d.p0 = T.pair_ptr[f0]; d.p1 = np;
     const LevelLists L = pack_level(T, d, f0, c->blob_host);
     plan_level(T, d, L, threads, gsh, allow_big, false);
-    c->front = d; c->front_k = nn - f0; c->front_f0 = f0; c->front_level = lc;
+    fp.d = d; fp.k = nn - f0; fp.f0 = f0; fp.level = lc;
+    return fp;
 }
 
 // Launch plan of the fused kernel (DESIGN.md "Placement" and "Launch policy").
@@ -417,7 +421,10 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         // (a CTA that has the SM to itself -- the merged single-wave layout -- can afford a large front: 5.69 ms with 32 nodes
         // against 5.98 with 15 and 6.17 without on the 9 241-bus grid; small CTAs that share the SM keep the L1)
         const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : th <= 512 ? 16 : 96, 0, 220) * 1024LL;
-        if (kcap >= 2 && ctx->csz == 1) build_front(ctx, th, gsh, budget, kcap, true);
+        if (kcap >= 2 && ctx->csz == 1) {
+            const FrontPlan fp = build_front(ctx, th, gsh, budget, kcap, true);
+            ctx->front = fp.d; ctx->front_k = fp.k; ctx->front_f0 = fp.f0; ctx->front_level = fp.level;
+        }
         if (ctx->front_k > 0) {
             ctx->front_off = align16(ctx->smem);
             ctx->smem = (int)(ctx->front_off + (mixed ? front_bytes<float>(ctx->front_k, gsh) : front_bytes<double>(ctx->front_k, gsh)));
@@ -440,6 +447,14 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     // single-wave layout (two slots of a large grid per CTA) wants the whole SM
     ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh == 1 && th >= 768) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
+    // the adjoint kernel's dense front: its shared memory holds nothing else of size, so when every CTA has an SM of its own
+    // the front takes up to 180 KB (9 241-bus grid: 54 nodes instead of the NR kernel's 38); otherwise the NR kernel's front
+    ctx->lin_front = FrontPlan_{ctx->front_k, ctx->front_f0, ctx->front_level, ctx->front};
+    if (ctx->placement == 2 && ctx->csz == 1 && ctx->front_k > 0 && (int64_t)((mb + (1 << gsh) - 1) >> gsh) <= n_sm &&
+        !tune_given(tu.front_kb, -1, "SABLE_FRONT_KB") && !tune_given(tu.front_nodes, -1, "SABLE_FRONT")) {
+        const FrontPlan fp = build_front(ctx, ctx->threads_lin, gsh, 180 * 1024LL, 96, true);
+        if (fp.k > ctx->front_k) ctx->lin_front = FrontPlan_{fp.k, fp.f0, fp.level, fp.d};
+    }
     return SABLE_OK;
 }
 
@@ -741,7 +756,17 @@ static sable_status launch_lin(sable_ctx* ctx, int b0, int batch, const double* 
     const size_t rhs = ((size_t)ctx->T.n_node * 16) << gsh;
     int max_optin = 0; CU(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->opt.device));
     L.rhs_in_smem = csz == 1 && L.big_off + rhs <= std::min<size_t>((size_t)max_optin, 64 * 1024);
-    const size_t sm = L.big_off + (L.rhs_in_smem ? rhs : 0);
+    size_t sm = L.big_off + (L.rhs_in_smem ? rhs : 0);
+    // dense top front of the transposed sweeps: the NR kernel's front (same nodes, same assembly lists), when the factors were
+    // written in this context's layout by a CTA working alone and the front still fits beside the right-hand sides
+    if (transposed && csz == 1 && gsh == ctx->gsh && ctx->lin_front.k > 0) {
+        const FrontPlan_& fp = ctx->lin_front;
+        const size_t fb = (size_t)(ctx->opt.precision == SABLE_MIXED ? front_bytes<float>(fp.k, gsh) : front_bytes<double>(fp.k, gsh));
+        if (align16(sm) + fb <= (size_t)max_optin) {
+            L.front_k = fp.k; L.front_f0 = fp.f0; L.front_level = fp.level; L.front = fp.d;
+            L.front_off = align16(sm); sm = L.front_off + fb;
+        }
+    }
     const void* lin = ctx->opt.precision == SABLE_MIXED ? (const void*)k_linsolve<float> : (const void*)k_linsolve<double>;
     CU(cudaFuncSetAttribute(lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)std::max<size_t>(sm, 48 * 1024)));
     cudaLaunchConfig_t cfg{};

@@ -20,9 +20,9 @@
 
 namespace sable {
 
-// bytes of shared memory per CTA: M (K*K blocks), the pivot inverses (K blocks), y (K double2), for 2^gsh slots
+// bytes of shared memory per CTA: M (K*K blocks), the pivot inverses (K blocks), y and w (K double2 each), for 2^gsh slots
 template <typename T> __host__ __device__ inline int64_t front_bytes(int K, int gsh) {
-    return (((int64_t)K * K + K) * 4 * (int64_t)sizeof(T) + (int64_t)K * 16) << gsh;
+    return (((int64_t)K * K + K) * 4 * (int64_t)sizeof(T) + (int64_t)2 * K * 16) << gsh;
 }
 
 template <typename T> struct Front {
@@ -38,6 +38,7 @@ template <typename T> struct Front {
     __device__ __forceinline__ Blk<T> ldI(int r) const { int vs; const T* p = bp(o_dinv, r, vs); return ld_blk(p, vs); }
     __device__ __forceinline__ void stI(int r, const Blk<T>& v) const { int vs; T* p = bp(o_dinv, r, vs); st_blk(p, vs, v); }
     __device__ __forceinline__ double2* yp(int r) const { return reinterpret_cast<double2*>(base + (o_y + ((unsigned)r << (gsh + 4)))); }
+    __device__ __forceinline__ double2* wp(int r) const { return reinterpret_cast<double2*>(base + (o_y + ((unsigned)(K + r) << (gsh + 4)))); }
 };
 
 template <typename T>
@@ -63,10 +64,12 @@ template <typename T> struct FrontSink {
     const Front<T>& F;
     const PivotFlag& pf;
     static constexpr bool kInvert = false;      // pivots are inverted by front_factor, in elimination order
-    __device__ __forceinline__ void diag(int m, const Blk<T>& D, T y0, T y1, bool, bool solve) const {
+    __device__ __forceinline__ void diag(int m, const Blk<T>& D, T y0, T y1, bool factor, bool solve) const {
         const int r = m - F.f0;
-        F.stM(r, r, D);
-        if (r == 0) { bool bad = false; F.stI(0, inv(D, bad)); if (bad) pf.raise(); }
+        if (factor) {
+            F.stM(r, r, D);
+            if (r == 0) { bool bad = false; F.stI(0, inv(D, bad)); if (bad) pf.raise(); }
+        }
         if (solve) *F.yp(r) = make_double2(double(y0), double(y1));
     }
     __device__ __forceinline__ void pair(int, int h, int2 mj, const Blk<T>& v) const {
@@ -164,6 +167,69 @@ __device__ __forceinline__ void front_store(const DevTemplate& t, const Slot<T, 
         const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
         s.stU(d.p0 + i, F.ldM(r, c));
         s.stL(d.p0 + i, F.ldM(c, r));
+    }
+}
+
+// ---- the front in the adjoint kernel (transposed sweeps on kept factors) ---------------------------------------------
+// Load: M[r][c] = U(m,j), M[c][r] = L'(j,m) of the front's pairs and the pivot inverses from the sparse slots (entries
+// outside the pattern stay zero: call front_zero and a barrier first).  No barrier.
+template <typename T, int kP>
+__device__ __forceinline__ void front_load(const DevTemplate& t, const Slot<T, kP>& s, const Front<T>& F, const LevelDesc& d, int tsub, int nsub) {
+    const int2* pmj = reinterpret_cast<const int2*>(t.blob + d.blob_off + d.o_pmj);
+    for (int r = tsub; r < F.K; r += nsub) F.stI(r, s.ldD(F.f0 + r));
+    for (int i = tsub; i < d.p1 - d.p0; i += nsub) {
+        const int2 mj = pmj[i];
+        const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
+        F.stM(r, c, s.ldU(d.p0 + i));
+        F.stM(c, r, s.ldL(d.p0 + i));
+    }
+}
+
+// U^T w = y on the front (y = g - contributions of the sparse nodes, assembled by accumulate_level): ascending,
+// w_c = D_c^-T y_c, then y_c' -= U(c,c')^T w_c for c' > c; w goes to F.wp.  K barriers.
+template <typename T>
+__device__ __forceinline__ void front_forward_t(const Front<T>& F, int tsub, int nsub) {
+    for (int c = 0; c < F.K; ++c) {
+        if (tsub < F.K - c) {
+            const Blk<T> Di = F.ldI(c);
+            const double2 yc = *F.yp(c);
+            const T w0 = Di.a * T(yc.x) + Di.c * T(yc.y), w1 = Di.b * T(yc.x) + Di.d * T(yc.y);
+            for (int e = tsub; e < F.K - c; e += nsub) {
+                if (e == 0) *F.wp(c) = make_double2(double(w0), double(w1));
+                else {
+                    const Blk<T> U = F.ldM(c, c + e);
+                    double2 y = *F.yp(c + e);
+                    y.x = double(T(y.x) - (U.a * w0 + U.c * w1));  y.y = double(T(y.y) - (U.b * w0 + U.d * w1));
+                    *F.yp(c + e) = y;
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// (L' D^-1)^T lambda = w on the front: descending, lambda_j = w_j - D_j^-T acc_j, then acc_c += L'(j,c)^T lambda_j for c < j;
+// lambda goes to rh(f0 + j) of the slot.  acc lives in F.yp (zeroed here).  K + 1 barriers.
+template <typename T, int kP>
+__device__ __forceinline__ void front_backward_t(const Slot<T, kP>& s, const Front<T>& F, int tsub, int nsub) {
+    for (int r = tsub; r < F.K; r += nsub) *F.yp(r) = make_double2(0.0, 0.0);
+    __syncthreads();
+    for (int j = F.K - 1; j >= 0; --j) {
+        if (tsub <= j) {
+            const Blk<T> Di = F.ldI(j);
+            const double2 a = *F.yp(j), w = *F.wp(j);
+            const T l0 = T(w.x) - (Di.a * T(a.x) + Di.c * T(a.y)), l1 = T(w.y) - (Di.b * T(a.x) + Di.d * T(a.y));
+            for (int c = tsub; c <= j; c += nsub) {
+                if (c == j) s.set_rh(F.f0 + j, make_double2(double(l0), double(l1)));
+                else {
+                    const Blk<T> L = F.ldM(j, c);
+                    double2 y = *F.yp(c);
+                    y.x = double(T(y.x) + (L.a * l0 + L.c * l1));  y.y = double(T(y.y) + (L.b * l0 + L.d * l1));
+                    *F.yp(c) = y;
+                }
+            }
+        }
+        __syncthreads();
     }
 }
 

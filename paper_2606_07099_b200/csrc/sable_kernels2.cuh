@@ -102,6 +102,9 @@ struct LinArgs {
     char* factors; char* work; int64_t fac_stride, work_stride;
     int32_t big_off;                  // big-target scratch at the start of dynamic shared memory, right-hand sides behind it
     int32_t csz;                      // CTAs per team (cluster size); the right-hand sides then live in the group's workspace slice
+    int32_t front_k, front_f0, front_level;   // dense top front of the transposed sweeps (0 = none): the last levels in shared memory
+    int64_t front_off;
+    LevelDesc front;
 };
 
 // a7: J1^T lambda = g with the kept factors (eq. 14): U^T w = g ascending, (L' D^-1)^T lambda = w descending.
@@ -129,7 +132,22 @@ __global__ void k_linsolve(const LinArgs A) {
     team_sync(tm);
     BlobRing ring = no_ring(t);
     const PivotFlag pf{nullptr};
-    if (A.transposed) { stage_factor_forward<T, 2, false, true, true, false>(t, s, t.level, ring, pf, scratch, tm); stage_backward<T, 2, true>(t, s, t.level, ring, tm); }
+    if (A.transposed && A.front_k > 0) {
+        // the last elimination levels as one dense block matrix in shared memory (sable_front.cuh): two short loops of
+        // shared-memory steps instead of two barrier-separated, memory-latency-bound phases per level
+        const int tsub_c = threadIdx.x >> gsh, nsub_c = blockDim.x >> gsh;
+        const Front<T> F = carve_front<T>(smem, A.front_off, A.front_k, A.front_f0, gsh, g);
+        front_zero<T>(F, tsub_c, nsub_c);
+        stage_factor_forward<T, 2, false, true, true, false, false>(t, s, t.level, ring, pf, scratch, tm, A.front_level);
+        front_load<T, 2>(t, s, F, A.front, tsub_c, nsub_c);
+        const FrontSink<T> sink{F, pf};
+        accumulate_level<T, 2, false, true, true>(s, A.front, t.blob + A.front.blob_off, sink, pf, scratch, tm);
+        __syncthreads();
+        front_forward_t<T>(F, tsub_c, nsub_c);
+        front_backward_t<T, 2>(s, F, tsub_c, nsub_c);
+        stage_backward<T, 2, true, false>(t, s, t.level, ring, tm, A.front_level);
+    }
+    else if (A.transposed) { stage_factor_forward<T, 2, false, true, true, false>(t, s, t.level, ring, pf, scratch, tm); stage_backward<T, 2, true>(t, s, t.level, ring, tm); }
     else              { stage_factor_forward<T, 2, false, true, false, false>(t, s, t.level, ring, pf, scratch, tm); stage_backward<T, 2, false>(t, s, t.level, ring, tm); }
     if (act) {
         const bool bad = A.pivot && (A.pivot[bb] & 2);
