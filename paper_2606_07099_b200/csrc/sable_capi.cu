@@ -358,7 +358,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     // all on chip only while the SMs can hold a good part of the batch at once; a batch of many waves runs faster from
     // the group-interleaved HBM workspace with many small CTAs (round 1: cfg 3 3.5 ms vs 4.4 ms)
     bool on_chip = gsh0 >= 0;
-    if (on_chip && want_chip < 0 && !g_given && !th_given) {
+    if (on_chip && want_chip < 0) {
         const int64_t slots_sm = (int64_t)std::max<int64_t>(1, smem_sm / (need(th0, gsh0, true) + 1024)) << gsh0;
         if (slots_sm * n_sm * 2 < (int64_t)mb) on_chip = false;
     }
