@@ -557,7 +557,7 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         if (!ok) return bail(SABLE_ERR_ALLOC);
     }
     const bool mixed = o.precision == SABLE_MIXED;
-    c->fac_stride = align16(mixed ? fac_bytes<float>(nn, np) : fac_bytes<double>(nn, np));
+    c->fac_stride = ((mixed ? fac_bytes<float>(nn, np) + 16 : fac_bytes<double>(nn, np)) + 31) & ~int64_t(31);   // whole 32-byte units (FP32: room for the alignment of the pair records)
     c->work_stride = work_bytes(nn);
     auto dmalloc = [&](void** p, size_t bytes) {
         if (cudaMalloc(p, bytes) != cudaSuccess) { c->err = "device allocation failed (" + std::to_string(bytes) + " bytes)"; return false; }

@@ -177,13 +177,49 @@ template <typename T, int kP> struct Slot {
     }
     __device__ __forceinline__ Blk<T> ldD(int m) const { return ldB(so_dg, 0u, m); }
     __device__ __forceinline__ void stD(int m, const Blk<T>& v) const { stB(so_dg, 0u, m, v); }
-    __device__ __forceinline__ Blk<T> ldU(int p) const { return ldB(so_pu, go_pu, p); }
-    __device__ __forceinline__ Blk<T> ldL(int p) const { return ldB(so_pl, go_pl, p); }
-    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const { stB(so_pu, go_pu, p, v); }
-    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const { stB(so_pl, go_pl, p, v); }
+    // Pairs.  HBM workspace with FP32 factors: U and L' of a pair sit side by side in one 32-byte RECORD (one 256-bit access
+    // moves both: an item of the refactor needs both blocks of each of its pairs -- 3 loads per pair item instead of 5); with
+    // FP64 factors (a block is 32 bytes already) and in shared memory they are two arrays.  gpx: extra lane offset of the
+    // record interleave (records are twice as wide as the blocks gf is offset for).
+    static constexpr bool kPairRec = kP == 2 && sizeof(T) == 4;
+    unsigned gpx;
+    __device__ __forceinline__ char* rec_ptr(int p) const { return gf + (go_pu + gpx + (((unsigned)p << gsh) * 32u)); }
+    __device__ __forceinline__ Blk<T> ldU(int p) const {
+        if (kPairRec) { chk_blk(go_pu, p); return ldg_blk(reinterpret_cast<const T*>(rec_ptr(p))); }
+        return ldB(so_pu, go_pu, p);
+    }
+    __device__ __forceinline__ Blk<T> ldL(int p) const {
+        if (kPairRec) { chk_blk(go_pu, p); return ldg_blk(reinterpret_cast<const T*>(rec_ptr(p) + 16)); }
+        return ldB(so_pl, go_pl, p);
+    }
+    __device__ __forceinline__ void stU(int p, const Blk<T>& v) const {
+        if (kPairRec) { chk_blk(go_pu, p); stg_blk(reinterpret_cast<T*>(rec_ptr(p)), v); }
+        else stB(so_pu, go_pu, p, v);
+    }
+    __device__ __forceinline__ void stL(int p, const Blk<T>& v) const {
+        if (kPairRec) { chk_blk(go_pu, p); stg_blk(reinterpret_cast<T*>(rec_ptr(p) + 16), v); }
+        else stB(so_pl, go_pl, p, v);
+    }
+    // both blocks of a pair
+    __device__ __forceinline__ void ldUL(int p, Blk<T>& U, Blk<T>& L) const {
+        if (kPairRec) {
+            chk_blk(go_pu, p);
+            float a, b, c, d, e, f, g, h;
+            asm volatile("ld.global.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(a), "=f"(b), "=f"(c), "=f"(d), "=f"(e), "=f"(f), "=f"(g), "=f"(h) : "l"(rec_ptr(p)) : "memory");
+            U = {T(a), T(b), T(c), T(d)}; L = {T(e), T(f), T(g), T(h)};
+        } else { U = ldU(p); L = ldL(p); }
+    }
+    __device__ __forceinline__ void stUL(int p, const Blk<T>& U, const Blk<T>& L) const {
+        if (kPairRec) {
+            chk_blk(go_pu, p);
+            asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(rec_ptr(p)), "f"(float(U.a)), "f"(float(U.b)), "f"(float(U.c)),
+                         "f"(float(U.d)), "f"(float(L.a)), "f"(float(L.b)), "f"(float(L.c)), "f"(float(L.d)) : "memory");
+        } else { stU(p, U); stL(p, L); }
+    }
     // h = 0: the U block of pair p, h = 1: the L' block
-    __device__ __forceinline__ Blk<T> ldP(int p, int h) const { return ldB(h ? so_pl : so_pu, h ? go_pl : go_pu, p); }
-    __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { stB(h ? so_pl : so_pu, h ? go_pl : go_pu, p, v); }
+    __device__ __forceinline__ Blk<T> ldP(int p, int h) const { return h ? ldL(p) : ldU(p); }
+    __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { if (h) stL(p, v); else stU(p, v); }
 
     __device__ __forceinline__ double2* st_ptr(unsigned so, unsigned go, int m) const {
         chk_st(m);

@@ -76,6 +76,10 @@ template <typename T> struct FrontSink {
         const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
         if (h) F.stM(c, r, v); else F.stM(r, c, v);
     }
+    __device__ __forceinline__ void pair2(int, int2 mj, const Blk<T>& U, const Blk<T>& L) const {
+        const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
+        F.stM(r, c, U); F.stM(c, r, L);
+    }
 };
 
 // Fills M and y of the front: entries with terms through accumulate_level, the others straight from the sparse slots

@@ -61,8 +61,9 @@ __device__ __forceinline__ Slot<T, kP> carve(unsigned char* smem, int64_t slot_o
     s.sb = reinterpret_cast<char*>(smem) + slot_off + g * 16;
     s.so_ma = ns; s.so_rh = 2 * ns; s.so_dg = 3 * ns; s.so_pu = s.so_dg + nd; s.so_pl = s.so_pu + np;
     s.gf = s.gw = nullptr;
-    s.go_pu = nd; s.go_pl = nd + np; s.go_ma = ns; s.go_rh = 2 * ns;
-    s.gsh = gsh;
+    s.go_pu = Slot<T, kP>::kPairRec ? ((nd + 31u) & ~31u) : nd;      // pair records (FP32 factors in HBM) are 32-byte aligned
+    s.go_pl = s.go_pu + np; s.go_ma = ns; s.go_rh = 2 * ns;
+    s.gsh = gsh; s.gpx = 0;
 #ifdef SABLE_BOUNDS
     s.nn_ = n_node; s.np_ = n_pair;
 #endif
@@ -75,6 +76,7 @@ __device__ __forceinline__ void bind(Slot<T, kP>& s, char* factors, int64_t fac_
     const size_t grp = (size_t)(b >> gsh), lane16 = (size_t)(b & ((1 << gsh) - 1)) * 16;
     s.gf = factors + ((grp * (size_t)fac_stride) << gsh) + (size_t)(b & ((1 << gsh) - 1)) * (4 * sizeof(T));   // whole blocks interleave
     s.gw = work + ((grp * (size_t)work_stride) << gsh) + lane16;
+    s.gpx = Slot<T, kP>::kPairRec ? (unsigned)lane16 : 0u;     // pair records are 32 bytes wide: 16 more per lane than the blocks
 }
 
 template <typename T, int kP>
@@ -114,11 +116,11 @@ __device__ __forceinline__ void scen_output(const SolveArgs& A, const Slot<T, kP
 template <typename T, int kP>
 __device__ __forceinline__ void store_factors(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
     // dg | pu | pl are contiguous block arrays in both memories: block i of the shared copy goes to block i of the HBM slice
-    const int n = t.n_node + 2 * t.n_pair;
-    for (int i = tsub; i < n; i += nsub) {
-        const Blk<T> v = i < t.n_node ? s.ldD(i) : i < t.n_node + t.n_pair ? s.ldU(i - t.n_node) : s.ldL(i - t.n_node - t.n_pair);
-        stg_blk(reinterpret_cast<T*>(s.gf + (((size_t)i << s.gsh) * (4 * sizeof(T)))), v);
-    }
+    Slot<T, 2> h = carve<T, 2>(nullptr, 0, t.n_node, t.n_pair, s.gsh, 0);    // the HBM view of the same slot
+    h.sb = nullptr; h.gf = s.gf; h.gw = s.gw;
+    h.gpx = Slot<T, 2>::kPairRec ? (unsigned)((threadIdx.x & ((1 << s.gsh) - 1)) * 16) : 0u;
+    for (int i = tsub; i < t.n_node; i += nsub) h.stD(i, s.ldD(i));
+    for (int p = tsub; p < t.n_pair; p += nsub) h.stUL(p, s.ldU(p), s.ldL(p));
 }
 
 __device__ __forceinline__ int pop_group(const SolveArgs& A) {

@@ -364,13 +364,17 @@ __global__ void k_debug(const DebugArgs A) {
     stage_fill_pairs<T, 2>(t, s, threadIdx.x, blockDim.x);
     __syncthreads();
     if (A.what == 1) {
-        const T* dg = reinterpret_cast<const T*>(s.gf);
-        const T* pu = reinterpret_cast<const T*>(s.gf + s.go_pu);
-        const T* pl = reinterpret_cast<const T*>(s.gf + s.go_pl);
-        for (int i = threadIdx.x; i < 4 * t.n_node; i += blockDim.x) A.diag[(size_t)b * 4 * t.n_node + i] = double(dg[i]);
-        for (int i = threadIdx.x; i < 4 * t.n_pair; i += blockDim.x) {
-            A.pairs[(size_t)b * 8 * t.n_pair + 8 * (i >> 2) + (i & 3)] = double(pu[i]);
-            A.pairs[(size_t)b * 8 * t.n_pair + 8 * (i >> 2) + 4 + (i & 3)] = double(pl[i]);
+        for (int m = threadIdx.x; m < t.n_node; m += blockDim.x) {
+            const Blk<T> d = s.ldD(m);
+            double* o4 = A.diag + ((size_t)b * t.n_node + m) * 4;
+            o4[0] = double(d.a); o4[1] = double(d.b); o4[2] = double(d.c); o4[3] = double(d.d);
+        }
+        for (int p = threadIdx.x; p < t.n_pair; p += blockDim.x) {
+            Blk<T> U, L;
+            s.ldUL(p, U, L);
+            double* o8 = A.pairs + ((size_t)b * t.n_pair + p) * 8;
+            o8[0] = double(U.a); o8[1] = double(U.b); o8[2] = double(U.c); o8[3] = double(U.d);
+            o8[4] = double(L.a); o8[5] = double(L.b); o8[6] = double(L.c); o8[7] = double(L.d);
         }
         return;
     }

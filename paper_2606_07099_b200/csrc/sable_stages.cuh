@@ -121,8 +121,8 @@ __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slo
         Blk<T> U0, L0, U1, L1;
         fill_pair<T, kP>(s, mj0, y0, U0, L0);
         fill_pair<T, kP>(s, mj1, y1, U1, L1);
-        s.stU(p, U0); s.stL(p, L0);
-        if (on2) { s.stU(p2, U1); s.stL(p2, L1); }
+        s.stUL(p, U0, L0);
+        if (on2) s.stUL(p2, U1, L1);
     }
 }
 
@@ -136,6 +136,7 @@ template <typename T, int kP> struct SparseSink {
         if (solve) s.set_rh(m, make_double2(double(z0), double(z1)));
     }
     __device__ __forceinline__ void pair(int p, int h, int2, const Blk<T>& v) const { s.stP(p, h, v); }
+    __device__ __forceinline__ void pair2(int p, int2, const Blk<T>& U, const Blk<T>& L) const { s.stUL(p, U, L); }
 };
 
 // Accumulate phase of one level (or of the front's assembly), the heart of a4 + the forward half of a5.  With the
@@ -154,13 +155,13 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
     const int* dord = reinterpret_cast<const int*>(lb + d.o_dord);
     const int2* dak = reinterpret_cast<const int2*>(lb + d.o_dak);
     auto diag_item = [&](const int2 ak, Blk<T>& D, T& y0, T& y1) {
-        if (kFactor || kTransposed) {
-            const Blk<T> U = s.ldU(ak.x);
-            if (kFactor) { const Blk<T> W = mul(s.ldL(ak.x), s.ldD(ak.y)); mulsub(D, W, U); }
-            if (kSolve && kTransposed) { const double2 x = s.rh(ak.y); y0 -= U.a * T(x.x) + U.c * T(x.y);  y1 -= U.b * T(x.x) + U.d * T(x.y); }
-        }
+        Blk<T> U, L;
+        if (kFactor) s.ldUL(ak.x, U, L);                    // both blocks of the pair (one access with FP32 factors)
+        else if (kTransposed) U = s.ldU(ak.x);
+        else L = s.ldL(ak.x);
+        if (kFactor) mulsub(D, mul(L, s.ldD(ak.y)), U);
+        if (kSolve && kTransposed) { const double2 x = s.rh(ak.y); y0 -= U.a * T(x.x) + U.c * T(x.y);  y1 -= U.b * T(x.x) + U.d * T(x.y); }
         if (kSolve && !kTransposed) {
-            const Blk<T> L = s.ldL(ak.x);
             const double2 x = s.rh(ak.y);
             y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y);
         }
@@ -261,16 +262,17 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             const int t0 = tptr[i], t1 = valid ? tptr[i + 1] : t0;
             const int pl = tord[i], p = d.p0 + pl;
             Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
-            if (lead) { U = s.ldU(p); L = s.ldL(p); }
+            if (lead) s.ldUL(p, U, L);
             for (int q = t0 + part; q < t1; q += S) {
                 const int4 ab = tab[q];
                 const Blk<T> Dk = s.ldD(ab.z);
-                const Blk<T> La = s.ldL(ab.x), Ub = s.ldU(ab.y), Lb = s.ldL(ab.y), Ua = s.ldU(ab.x);
+                Blk<T> La, Ua, Lb, Ub;
+                s.ldUL(ab.x, Ua, La); s.ldUL(ab.y, Ub, Lb);
                 mulsub(U, mul(La, Dk), Ub);
                 mulsub(L, mul(Lb, Dk), Ua);
             }
             for (int o = (S >> 1) << gsh; o >= G; o >>= 1) { blk_add_shx(U, o); blk_add_shx(L, o); }
-            if (lead) { const int2 mj = pmj[pl]; sink.pair(p, 0, mj, U); sink.pair(p, 1, mj, L); }
+            if (lead) sink.pair2(p, pmj[pl], U, L);
 #endif
         }
     }
