@@ -241,17 +241,16 @@ class Context:
 
     def stage_times(self, p_spec, q_spec, v_set, reps=1):
         """sable_debug_stage_times: mean ms of the mismatch + fill launch and of the refactor + solve launch over three Newton
-        iterations of the whole batch in the default workspace layout (averaged over `reps` calls)."""
+        iterations of the whole batch in the default workspace layout (median over `reps` calls)."""
         batch = self._begin(p_spec)
         a, b = C.c_double(0), C.c_double(0)
-        ta = tb = 0.0
+        ta, tb = [], []
         for _ in range(max(1, int(reps))):
             self._check(lib().sable_debug_stage_times(self._h, C.c_int32(batch), self._bn(p_spec), self._bn(q_spec), self._bn(v_set),
                                                       C.byref(a), C.byref(b), _stream()))
-            ta += a.value
-            tb += b.value
-        n = max(1, int(reps))
-        return {"mismatch_fill_ms": ta / n, "factor_solve_ms": tb / n}
+            ta.append(a.value)
+            tb.append(b.value)
+        return {"mismatch_fill_ms": float(np.median(ta)), "factor_solve_ms": float(np.median(tb))}
 
     # -- host-buffer calls (numpy) ----------------------------------------------------------------------
     def solve_host(self, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, max_it=20, out=None):
