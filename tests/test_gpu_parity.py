@@ -484,6 +484,60 @@ def test_host_buffer_calls_match_device_calls():
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,batch", [(2, 1024), (3, 3001)])
+def test_host_wrappers_chunk_pipeline(cfg, batch):
+    """Batches large enough for the host wrappers to cut them into several chunks on their own streams (each chunk with its
+    own queue counter and workspace part, kernels of different chunks running concurrently): bitwise the results of the
+    device-pointer calls, forward and adjoint, including a ragged last chunk."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, keep_factors=True)
+    a = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    la = [t.cpu().numpy() for t in ctx.adjoint(dev(gva), dev(gvm))]
+    b = ctx.solve_host(ps, qs, vs, tol=c.tol, max_it=c.max_it)
+    lb = ctx.adjoint_host(gva, gvm)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(la[0], lb[0]) and np.array_equal(la[1], lb[1])
+    assert a["converged"].all()
+    # and once more in the other order (the device call after the host call sees no stale state)
+    a2 = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    for k in a:
+        assert np.array_equal(a[k], a2[k]), k
+    ctx.close()
+
+
+def test_masking_with_wide_iteration_spread():
+    """Groups whose slots finish at very different times (half of the scenarios warm-started at the solution: zero updates;
+    one scenario that never converges): every scenario's result is that of the scenario alone, whatever shares its group."""
+    net, Y = get_net(3)
+    c = net.cfg
+    batch = 96
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ps[11] *= 25.0
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    vm0, va0 = vs.copy(), np.zeros_like(vs)
+    pq = net.bus_type == S.PQ
+    vm0[:, pq] = 1.0
+    warm = np.arange(batch) % 2 == 0
+    warm[11] = False
+    vm0[warm], va0[warm] = ref["vm"][warm], ref["va"][warm]
+    for tune in (dict(group=4, on_chip=0), dict(group=8, on_chip=0, threads=256), dict(group=1, on_chip=0)):
+        ctx = make_ctx(net, max_batch=batch, keep_factors=False, **tune)
+        res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), vm0=dev(vm0), va0=dev(va0), tol=c.tol, max_it=c.max_it))
+        assert res["converged"][11] == 0 and res["iterations"][11] == c.max_it
+        ok = np.arange(batch) != 11
+        assert (res["converged"][ok] == 1).all()
+        assert (res["iterations"][warm] == 0).all() and np.array_equal(res["vm"][warm], ref["vm"][warm])
+        cold = ok & ~warm
+        assert (np.abs(res["iterations"][cold].astype(int) - ref["iterations"][cold]) <= 1).all()
+        same = cold & (res["iterations"] == ref["iterations"])
+        assert np.abs(res["vm"][same] - ref["vm"][same]).max() <= 1e-9 and np.abs(res["va"][same] - ref["va"][same]).max() <= 1e-9
+        ctx.close()
+
+
 # ---- every placement / slot-group layout of the fused kernel gives the same answers -----------------------------------
 @pytest.mark.parametrize("env", [dict(SABLE_G="1"), dict(SABLE_G="8"), dict(SABLE_G="2", SABLE_ONCHIP="1"),
                                  dict(SABLE_G="4", SABLE_ONCHIP="0", SABLE_THREADS="64"),
