@@ -188,7 +188,7 @@ static LevelLists pack_level(const Template& T, LevelDesc& d, int k_limit, std::
     }
     dptr[nm] = q; q = 0;
     for (int i = 0; i < np; ++i) {
-        tptr[i] = q; tor[i] = tord[i];
+        tptr[i] = q; tor[i] = tord[i] | (T.pair_yu[d.p0 + tord[i]] < 0 ? kFromZero : 0);
         for (const int4& e : tl[tord[i]]) tab[q++] = e;
         L.tlen.push_back((int)tl[tord[i]].size());
     }
@@ -488,13 +488,21 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     std::vector<double2> ygb(T.ycol.size()), ydg(nn);
     for (size_t k = 0; k < T.ycol.size(); ++k) ygb[k] = make_double2(T.yg[k], T.yb[k]);
     for (int m = 0; m < nn; ++m) ydg[m] = make_double2(T.yg[T.ydiag[m]], T.yb[T.ydiag[m]]);
-    std::vector<double4> py(np);
-    std::vector<int2> pmj(np);
+    // Jacobian destinations of the Y entries (stage_mismatch): entry (m,j) of row m feeds the U half of pair (m,j) when j is
+    // eliminated later, the L' half of pair (j,m) otherwise; diagonal entries and the slack column feed nothing
+    std::vector<int2> ycd(T.ycol.size());
+    std::vector<int4> jmj;
+    std::vector<double4> jy;
+    for (size_t k = 0; k < T.ycol.size(); ++k) ycd[k] = make_int2(T.ycol[k], -1);
     for (int p = 0; p < np; ++p) {
         const int su = T.pair_yu[p], sl = T.pair_yl[p];
-        py[p] = make_double4(su >= 0 ? T.yg[su] : 0.0, su >= 0 ? T.yb[su] : 0.0, sl >= 0 ? T.yg[sl] : 0.0, sl >= 0 ? T.yb[sl] : 0.0);
+        if ((su >= 0) != (sl >= 0)) { c->err = "internal: Y pattern not symmetric"; return bail(SABLE_ERR_STRUCTURE); }
+        if (su < 0) continue;
+        ycd[su].y = p | (T.node_pq[T.pair_col[p]] ? 1 << 30 : 0);
         const int m = T.pair_row[p], j = T.pair_col[p];
-        pmj[p] = make_int2(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0));
+        jmj.push_back(make_int4(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0), p, 0));
+        jy.push_back(make_double4(T.yg[su], T.yb[su], T.yg[sl], T.yb[sl]));
+        ycd[sl].y = p | 1 << 29 | (T.node_pq[T.pair_row[p]] ? 1 << 30 : 0);
     }
     DevTemplate& d = c->d;
     d.n_bus = T.n_bus; d.n_node = nn; d.n_pair = np; d.n_level = T.n_level; d.slack = T.slack;
@@ -535,7 +543,8 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         up(tpos, &c->ftpos); up(bt, &c->d_bus_type);
     }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
-    up(T.ycol, &d.ycol); up(ygb, &d.ygb); up(ydg, &d.ydiag_gb); up(pmj, &d.pair_mj); up(py, &d.pair_y);
+    up(T.ycol, &d.ycol); up(ycd, &d.ycd); up(ygb, &d.ygb); up(jmj, &d.jp_mj); up(jy, &d.jp_y);
+    d.n_jpair = (int)jmj.size(); up(ydg, &d.ydiag_gb);
     if (!ok) return bail(SABLE_ERR_ALLOC);
     ctx = c;
     LevelPack P;

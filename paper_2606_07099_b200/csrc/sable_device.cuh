@@ -45,7 +45,8 @@ constexpr int kTargetUnit = SABLE_HALF_TARGETS ? 2 : 1;
 //   int32 dptr[nm+1]   the diag target at SORTED position i (descending list length) subtracts dak[dptr[i] .. dptr[i+1])
 //   int32 dord[nm]     local node index (m - m0) of sorted position i                       at o_dord
 //   int32 tptr[np+1]   the pair target at SORTED position i (descending list length) subtracts tab[tptr[i] .. tptr[i+1])
-//   int32 tord[np]     local pair index (p - p0) of sorted position i                       at o_tord
+//   int32 tord[np]     local pair index (p - p0) of sorted position i, | kFromZero for a fill-in   at o_tord
+//                      pair (no Y entry: J(m,j) = J(j,m) = 0, nothing is stored for it before the refactor)
 //   int32 pptr[nm+1]   node i owns the pairs p0 + [pptr[i], pptr[i+1])                        at o_pptr
 //   int2  dak[]        (pair a = (k,m), node k)                                             at o_dak
 //   int2  pmj[np]      (m | pq_m << 30, j | pq_j << 30)                                     at o_pmj
@@ -72,13 +73,18 @@ struct DevTemplate {
     const int32_t* node_bus;    // [n_node+1]  (entry n_node = slack bus)
     const uint8_t* node_pq;     // [n_node]
     const int32_t* yptr;        // [n_node+1]  Y rows of the non-slack buses in node order
-    const int32_t* ycol;        // node positions (slack = n_node)
+    const int32_t* ycol;        // per stored Y entry: column node position (slack = n_node)
+    const int2*    ycd;         // the same with the walk's destination: (column node position (slack = n_node), destination of the Jacobian
+                                // block J(row, column): pair p | half << 29 (0: U, 1: L') | column is PQ << 30; -1: none)
     const double2* ygb;         // (G, B) per stored Y entry
+    int32_t n_jpair;            // pairs with a Y entry (the others are fill-in), for the pair-pass form of a2:
+    const int4*    jp_mj;       // [n_jpair] (m | pq_m << 30, j | pq_j << 30, pair p, 0)
+    const double4* jp_y;        // [n_jpair] (G_mj, B_mj, G_jm, B_jm)
     const double2* ydiag_gb;    // [n_node] (G_mm, B_mm)
-    const int2*    pair_mj;     // [n_pair] (m | pq_m << 30, j | pq_j << 30)   (fill pass)
-    const double4* pair_y;      // [n_pair]                                     (fill pass)
 };
 constexpr int kIdxMask = 0x3fffffff;
+constexpr int kPairMask = 0x1fffffff;   // pair index of a ycd destination
+constexpr int kFromZero = 1 << 30;      // tord flag
 
 template <typename T> struct Blk { T a, b, c, d; };   // [[a b][c d]]
 

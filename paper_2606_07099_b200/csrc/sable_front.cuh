@@ -83,7 +83,7 @@ template <typename T> struct FrontSink {
 };
 
 // Fills M and y of the front: entries with terms through accumulate_level, the others straight from the sparse slots
-// (where stage_fill_pairs / stage_mismatch left J).  Ends with a barrier.
+// (where stage_mismatch left J; a fill-in pair without terms below the front stays zero).  Ends with a barrier.
 template <typename T, int kP, bool kSolve>
 __device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<T, kP>& s, const Front<T>& F, const LevelDesc& d,
                                                const PivotFlag& pf, double* scratch, int tsub, int nsub) {
@@ -96,7 +96,8 @@ __device__ __forceinline__ void front_assemble(const DevTemplate& t, const Slot<
         for (int c = 0; c < d.n_cls; ++c) if (!d.cls[c].diag) with_terms = d.cls[c].i1 / kTargetUnit;
         const int nbt = 2 * (d.p1 - d.p0);
         for (int bt = 2 * with_terms + tsub; bt < nbt; bt += nsub) {
-            const int pl = tord[bt >> 1], h = bt & 1;
+            const int to = tord[bt >> 1], pl = to & kIdxMask, h = bt & 1;
+            if (to & kFromZero) continue;
             const int2 mj = pmj[pl];
             const int r = (mj.x & kIdxMask) - F.f0, c = (mj.y & kIdxMask) - F.f0;
             const Blk<T> v = s.ldP(d.p0 + pl, h);

@@ -230,7 +230,8 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_nr_fused(const SolveArgs A)
             }
         }
         if (!any_slot(b >= 0)) continue;                   // every slot finished (and no factors to keep)
-        // a2 as one wide pass over all pairs (keeps the divisions of the fill off the level-by-level critical path)
+        // a2 happened inside the mismatch walk (stage_mismatch), or happens here as a pass over the pairs (FP32 pair records);
+        // either way the pairs with a Y entry hold J afterwards and the fill-in pairs nothing yet
         stage_fill_pairs<T, kP>(t, s, tsub, nsub);
         if (kP == 2 && A.front_k > 0) front_zero<T>(F, tsub_c, nsub_c);
         team_sync(tm);

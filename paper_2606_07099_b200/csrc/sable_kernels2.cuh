@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
     if (!go_on && !fin) { bind<T, 2>(s, A.factors, A.fac_stride, A.work, A.work_stride, trash); pf.w = nullptr; }
     __syncthreads();                                                 // scen_output has read the state the fill's trash lanes may overwrite
     stage_fill_pairs<T, 2>(t, s, tsub, nsub);
-    if (!__syncthreads_or(fin)) return;
+    if (!__syncthreads_or(fin)) return;                              // (the barrier also orders the J stores before the refactor)
     if (!fin) { bind<T, 2>(s, A.factors, A.fac_stride, A.work, A.work_stride, trash); pf.w = nullptr; }
     BlobRing ring = no_ring(t);
     stage_factor_forward<T, 2, true, false, false, true>(t, s, t.level, ring, pf, scratch, Team{0, 1});
@@ -348,6 +348,10 @@ __global__ void k_debug(const DebugArgs A) {
         double sn, cs; sincos(th, &sn, &cs);
         s.set_ma(m, make_double2(vm, th));
         s.set_vv(m, make_double2(vm * cs, vm * sn));
+    }
+    if (A.what == 1) {                                               // export of J: the fill-in pairs (never written by the walk) read as zero
+        const Blk<T> z = {T(0), T(0), T(0), T(0)};
+        for (int p = threadIdx.x; p < t.n_pair; p += blockDim.x) s.stUL(p, z, z);
     }
     __syncthreads();
     const double r = slot_max_nan(stage_mismatch<T, 2>(t, s, A.p_spec ? A.p_spec + o : A.zeros, A.q_spec ? A.q_spec + o : A.zeros, true, 0, pf, Team{0, 1}), red, 0);

@@ -10,6 +10,19 @@
 
 namespace sable {
 
+#ifndef SABLE_MM_UNROLL
+#define SABLE_MM_UNROLL 3
+#endif
+// Where the off-diagonal Jacobian blocks are evaluated: inside the mismatch walk (one block per Y entry, no second pass over
+// the state), or -- FP32 pair records, where a lane must write both blocks of a pair at once -- in a pass over the pairs
+#ifndef SABLE_WALK_FILL
+#define SABLE_WALK_FILL 1
+#endif
+template <typename T, int kP> struct FillMode {
+    static constexpr bool kWalk = SABLE_WALK_FILL && kP == 2 && !Slot<T, kP>::kPairRec;   // measured: the walk form pays in the HBM workspace with FP64 blocks only
+    static constexpr int kUnroll = kWalk ? SABLE_MM_UNROLL : 4;                            // Y entries per step and lane
+};
+
 // Per-thread handle for reporting a tiny pivot: points at the scenario's flag word, or at
 // nothing for lanes that serve no scenario.
 struct PivotFlag {
@@ -17,16 +30,25 @@ struct PivotFlag {
     __device__ __forceinline__ void raise() const { if (w) atomicOr(w, 3); }
 };
 
-// a1 (+ diagonal case of a2): S = V o conj(Ybus V), F1 rows (eq. 6), real form of
-// PAPER.md:201-207; writes rh = -F1 and the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated
-// P_i, Q_i -- PAPER.md:193, :215); returns this thread's max |F1| (NaN-propagating).  No barrier, no shuffle.
+// a1 + a2 in one walk over the Y rows: S = V o conj(Ybus V), F1 rows (eq. 6), real form of
+// PAPER.md:201-207; writes rh = -F1, the diagonal Jacobian blocks (Alg. 1 diagonal case: uses the calculated P_i, Q_i --
+// PAPER.md:193, :215) and, entry by entry, the off-diagonal blocks (Alg. 1 off-diagonal case; body
+// reconstructed, reading 4): with t = Y_mj V_j (the term the row sum needs anyway) and V_m conj(t) = u2 + i u1,
+//   u2 = Vm_m Vm_j (G cos th_mj + B sin th_mj),   u1 = Vm_m Vm_j (G sin th_mj - B cos th_mj)
+//   dP_m/dth_j = u1     dP_m/dVm_j = u2 / Vm_j     dQ_m/dth_j = -u2     dQ_m/dVm_j = u1 / Vm_j
+// evaluated in FP64 and rounded to T (Table I: value update DP, solver copy SP); rows / columns of the identity
+// padding of PV nodes are zero.  The block goes to the U half (j later than m in the elimination order) or the L' half of
+// its pair; fill-in pairs have no entry and are not written (their targets start from zero: kFromZero).  Returns this
+// thread's max |F1| (NaN-propagating).  No barrier, no shuffle beyond the row split.
 template <typename T, int kP>
 __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slot<T, kP>& s, const double* p_row,
                                                  const double* q_row, bool act, int leaf_m1, const PivotFlag& pf, const Team& tm) {
     // leaf_m1: nodes m < leaf_m1 (level 0: no earlier neighbour, so D_m = J(m,m) and y_m = rhs_m) get their pivot inverse
     // and z_m = D_m^-1 rhs_m stored right here -- the refactor then has nothing to do at level 0 (kLeafDone)
     // every lane of a warp runs the pass (the row split combines lanes by shuffles); a lane whose slot does not need
-    // the evaluation (act = false) takes part in the shuffles and writes nothing
+    // the evaluation (act = false) takes part in the shuffles; its slot is bound to the spare workspace group
+    constexpr bool kWalk = FillMode<T, kP>::kWalk;
+    constexpr int kU = FillMode<T, kP>::kUnroll;
     const int lane = threadIdx.x & 31, nwarps = (blockDim.x >> 5) * tm.csz, warp = tm.rank * (blockDim.x >> 5) + (threadIdx.x >> 5), gsh = s.gsh;
     double loc = 0.0;
     for (int c = 0; c < t.n_class; ++c) {
@@ -38,33 +60,48 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
             const int4 row = t.mm_row[valid ? base + tl : rc.i1 - 1];
             const int m = row.x;
             const bool lead = valid && part == 0 && act;
+            const bool pq = row.w >> 30;
+            double2 v = make_double2(0.0, 0.0);
+            if (kWalk) v = s.vv(m);
             double ire = 0.0, iim = 0.0;
             const int k1 = valid ? row.z : 0;
-            // four entries per step: their index / admittance loads are issued together, then the four V gathers -- a lane
+            // kU entries per step: their index / admittance loads are issued together, then the V gathers -- a lane
             // that walks a row alone has 2 dependent round trips per step instead of 2 per entry
-            for (int k = row.y + part; k < k1; k += 4 * S) {
-                int col[4]; double2 y[4], x[4];
+            for (int k = row.y + part; k < k1; k += kU * S) {
+                int2 cd[kU]; double2 y[kU], x[kU];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < kU; ++u) {
                     const int ku = k + u * S;
                     const bool on = ku < k1;
-                    col[u] = on ? t.ycol[ku] : m;
+                    if (kWalk) cd[u] = on ? t.ycd[ku] : make_int2(m, -1);
+                    else cd[u] = make_int2(on ? t.ycol[ku] : m, -1);
                     y[u] = on ? t.ygb[ku] : make_double2(0.0, 0.0);
                 }
 #pragma unroll
-                for (int u = 0; u < 4; ++u) x[u] = s.vv(col[u]);
+                for (int u = 0; u < kU; ++u) x[u] = s.vv(cd[u].x);
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    ire += y[u].x * x[u].x - y[u].y * x[u].y;
-                    iim += y[u].y * x[u].x + y[u].x * x[u].y;
+                for (int u = 0; u < kU; ++u) {
+                    if (!kWalk) {
+                        ire += y[u].x * x[u].x - y[u].y * x[u].y;
+                        iim += y[u].y * x[u].x + y[u].x * x[u].y;
+                        continue;
+                    }
+                    const double tr = y[u].x * x[u].x - y[u].y * x[u].y, ti = y[u].y * x[u].x + y[u].x * x[u].y;
+                    ire += tr; iim += ti;
+                    if (cd[u].y >= 0) {
+                        const double u2 = v.x * tr + v.y * ti, u1 = v.y * tr - v.x * ti;
+                        const double iv = (cd[u].y >> 30) ? rsqrt(x[u].x * x[u].x + x[u].y * x[u].y) : 0.0;
+                        Blk<T> J;
+                        J.a = T(u1);  J.b = T(u2 * iv);  J.c = pq ? T(-u2) : T(0);  J.d = pq ? T(u1 * iv) : T(0);
+                        s.stP(cd[u].y & kPairMask, (cd[u].y >> 29) & 1, J);
+                    }
                 }
             }
             for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { ire += shx(ire, o); iim += shx(iim, o); }
             if (lead) {
-                const double2 v = s.vv(m);
+                if (!kWalk) v = s.vv(m);
                 const double vm = s.ma(m).x;
                 const double P = v.x * ire + v.y * iim, Q = v.y * ire - v.x * iim;
-                const bool pq = row.w >> 30;
                 const int bus = row.w & kIdxMask;
                 const double fp = P - p_row[bus], fq = pq ? Q - q_row[bus] : 0.0;
                 loc = nan_max(loc, nan_max(fabs(fp), fabs(fq)));
@@ -91,12 +128,10 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
     return loc;
 }
 
-// a2, off-diagonal case of Alg. 1 (body reconstructed, reading 4) with
-// theta_mj = theta_m - theta_j:  a = Vm_m Vm_j cos theta_mj,  b = Vm_m Vm_j sin theta_mj
-//   dP_m/dth_j = G b - B a     dP_m/dVm_j = (G a + B b)/Vm_j     dQ_m/dth_j = -(G a + B b)     dQ_m/dVm_j = (G b - B a)/Vm_j
-// evaluated in FP64 and rounded to T (Table I: value update DP, solver copy SP).  Fill pairs get zeros.
+// a2 as a pass over the pairs that have a Y entry (FillMode::kWalk = false), same blocks as the walk above:
+// a = Vm_m Vm_j cos theta_mj, b = Vm_m Vm_j sin theta_mj; both blocks of a pair leave in one store.
 template <typename T, int kP>
-__device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4 y, Blk<T>& U, Blk<T>& L) {
+__device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int4 mj, double4 y, Blk<T>& U, Blk<T>& L) {
     const int m = mj.x & kIdxMask, j = mj.y & kIdxMask;
     const bool mpq = mj.x >> 30, jpq = mj.y >> 30;
     const double2 vm_ = s.vv(m), vj = s.vv(j);
@@ -107,22 +142,20 @@ __device__ __forceinline__ void fill_pair(const Slot<T, kP>& s, int2 mj, double4
     U.a = T(u1);  U.b = T(u2 * ivj);  U.c = mpq ? T(-u2) : T(0);  U.d = mpq ? T(u1 * ivj) : T(0);
     L.a = T(l1);  L.b = T(l2 * ivm);  L.c = jpq ? T(-l2) : T(0);  L.d = jpq ? T(l1 * ivm) : T(0);
 }
-
-// a2 as one wide pass over all pairs: every pair slot of the filled pattern is written.  The pairs owned by level-0
-// nodes have no terms, so these are already their final U and L' values.
 template <typename T, int kP>
 __device__ __forceinline__ void stage_fill_pairs(const DevTemplate& t, const Slot<T, kP>& s, int tsub, int nsub) {
+    if (FillMode<T, kP>::kWalk) return;
     // two pairs per step and lane: the index / admittance loads of both are issued before the state gathers of either
-    for (int p = tsub; p < t.n_pair; p += 2 * nsub) {
-        const int p2 = p + nsub;
-        const bool on2 = p2 < t.n_pair;
-        const int2 mj0 = t.pair_mj[p], mj1 = t.pair_mj[on2 ? p2 : p];
-        const double4 y0 = t.pair_y[p], y1 = t.pair_y[on2 ? p2 : p];
+    for (int i = tsub; i < t.n_jpair; i += 2 * nsub) {
+        const int i2 = i + nsub;
+        const bool on2 = i2 < t.n_jpair;
+        const int4 mj0 = t.jp_mj[i], mj1 = t.jp_mj[on2 ? i2 : i];
+        const double4 y0 = t.jp_y[i], y1 = t.jp_y[on2 ? i2 : i];
         Blk<T> U0, L0, U1, L1;
         fill_pair<T, kP>(s, mj0, y0, U0, L0);
         fill_pair<T, kP>(s, mj1, y1, U1, L1);
-        s.stUL(p, U0, L0);
-        if (on2) s.stUL(p2, U1, L1);
+        s.stUL(mj0.z, U0, L0);
+        if (on2) s.stUL(mj1.z, U1, L1);
     }
 }
 
@@ -247,9 +280,9 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             // block-targets bt = 2 i + h (h = 0: U(m,j), h = 1: L'(j,m)): one uniform item acc -= A D_k^-1 B, three operand blocks
             const int ip = i >> 1, h = i & 1;
             const int t0 = tptr[ip], t1 = valid ? tptr[ip + 1] : t0;
-            const int pl = tord[ip], p = d.p0 + pl;
+            const int to = tord[ip], pl = to & kIdxMask, p = d.p0 + pl;
             Blk<T> acc = {T(0), T(0), T(0), T(0)};
-            if (lead) acc = s.ldP(p, h);
+            if (lead && !(to & kFromZero)) acc = s.ldP(p, h);
             for (int q = t0 + part; q < t1; q += S) {
                 const int4 ab = tab[q];
                 const Blk<T> W = mul(s.ldL(h ? ab.y : ab.x), s.ldD(ab.z));
@@ -260,9 +293,9 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
 #else
             // whole pair targets: five operand blocks in flight per item, both accumulators in one lane
             const int t0 = tptr[i], t1 = valid ? tptr[i + 1] : t0;
-            const int pl = tord[i], p = d.p0 + pl;
+            const int to = tord[i], pl = to & kIdxMask, p = d.p0 + pl;
             Blk<T> U = {T(0), T(0), T(0), T(0)}, L = {T(0), T(0), T(0), T(0)};
-            if (lead) s.ldUL(p, U, L);
+            if (lead && !(to & kFromZero)) s.ldUL(p, U, L);
             for (int q = t0 + part; q < t1; q += S) {
                 const int4 ab = tab[q];
                 const Blk<T> Dk = s.ldD(ab.z);
@@ -279,7 +312,7 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
 }
 
 // a4 + forward half of a5 level by level.  One barrier per level.  kLeafDone: level 0 needs nothing (stage_mismatch left
-// D^-1 and z of its nodes, stage_fill_pairs the final values of its pairs).  kAll = false: only the levels [0, nl_) are
+// D^-1 and z of its nodes and the final values of its pairs).  kAll = false: only the levels [0, nl_) are
 // processed (those below the dense top front: sable_front.cuh).
 template <typename T, int kP, bool kFactor, bool kSolve, bool kTransposed, bool kLeafDone, bool kAll = true>
 __device__ __forceinline__ void stage_factor_forward(const DevTemplate& t, const Slot<T, kP>& s, const LevelDesc* lv, BlobRing& ring,
