@@ -370,7 +370,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         // Occupancy model.  The path is bound by memory latency: the SM should hold as many
         // independent elimination chains (scenarios) as its registers allow, each with enough lanes for its levels.
         //  * lanes per scenario L: 0.75 x the mean number of multiply-subtract items of an elimination level, as a power of
-        //    two in [32, 512] -- a tree-like 300-bus grid gets 32, a 2 000-bus grid 128, a 900-bus mesh with 3x fill 256, the
+        //    two in [16, 512] -- a tree-like 300-bus grid gets 16 (2.05 ms against 2.15 at 32), a 2 000-bus grid 128, a 900-bus mesh with 3x fill 256, the
         //    9 241-bus grid 512 (each measured best: 3.83 vs 4.03 ms at 256 on the 2 000-bus grid, 4.1 vs 5.2 ms at 128 on the mesh);
         //  * slots per CTA G such that a CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72
         //    registers), never so many that the batch leaves SMs without a CTA;
@@ -379,7 +379,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         //    neighbouring lanes then read neighbouring 16-byte words (half the L1 wavefronts: 6.2 vs 6.6 ms measured);
         //  * teams (a cluster of CTAs per group): for tiny batches of large grids (below), or on request (tune.cluster).
         const double items = (double)T.term_a.size() + (double)T.dterm.size();
-        const int L = std::min(512, std::max(32, pow2_floor(std::max(1, (int)(0.75 * items / std::max(1, nl))))));
+        const int L = std::min(512, std::max(16, pow2_floor(std::max(1, (int)(0.75 * items / std::max(1, nl))))));
         const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
         int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
         int G = std::max(1, 128 / L);
