@@ -223,6 +223,16 @@ template <typename T, int kP> struct Slot {
                          "f"(float(U.d)), "f"(float(L.a)), "f"(float(L.b)), "f"(float(L.c)), "f"(float(L.d)) : "memory");
         } else { stU(p, U); stL(p, L); }
     }
+    // ask the L2 for the U (h = 0) or L' (h = 1) blocks of the pairs [p0, p1) of this thread's GROUP (HBM workspace; the
+    // blocks of a pair range are contiguous across the slots): every lane `tsub` of `nsub` takes every nsub-th 128-byte line
+    __device__ __forceinline__ void prefetch_pairs_l2(int p0, int p1, int h, int tsub, int nsub) const {
+        if (kP != 2) return;
+        const unsigned rec = kPairRec ? 32u : (unsigned)kBlk;
+        const char* base = gf - (size_t)(threadIdx.x & ((1 << gsh) - 1)) * kBlk + ((kPairRec || !h) ? go_pu : go_pl);
+        const unsigned b0 = (((unsigned)p0 << gsh) * rec) & ~127u, b1 = ((unsigned)p1 << gsh) * rec;
+        for (unsigned o = b0 + (unsigned)tsub * 128u; o < b1; o += (unsigned)nsub * 128u)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
+    }
     // h = 0: the U block of pair p, h = 1: the L' block
     __device__ __forceinline__ Blk<T> ldP(int p, int h) const { return h ? ldL(p) : ldU(p); }
     __device__ __forceinline__ void stP(int p, int h, const Blk<T>& v) const { if (h) stL(p, v); else stU(p, v); }

@@ -113,7 +113,7 @@ struct LinArgs {
 // shared memory when they fit.  A scenario whose kept factors carry a tiny-pivot flag gets NaN (its lambda would be
 // garbage that nothing else reveals: the adjoint has no residual test).
 template <typename T>
-__global__ void k_linsolve(const LinArgs A) {
+__global__ void __launch_bounds__(1024, 1) k_linsolve(const LinArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const DevTemplate& t = A.t;
     const Team tm{A.csz > 1 ? cluster_ctarank() : 0, A.csz > 1 ? A.csz : 1};

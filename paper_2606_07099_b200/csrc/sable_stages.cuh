@@ -23,6 +23,15 @@ template <typename T, int kP> struct FillMode {
     static constexpr int kUnroll = kWalk ? SABLE_MM_UNROLL : 4;                            // Y entries per step and lane
 };
 
+#ifndef SABLE_BWD_PREFETCH
+#define SABLE_BWD_PREFETCH 1
+#endif
+#ifndef SABLE_BWD_AHEAD
+#define SABLE_BWD_AHEAD 2
+#endif
+constexpr int kBwdAhead = SABLE_BWD_AHEAD;
+constexpr int kBwdPrefetchPairs = 512;      // levels with more pairs than this are throughput-bound: no prefetch
+
 // Per-thread handle for reporting a tiny pivot: points at the scenario's flag word, or at
 // nothing for lanes that serve no scenario.
 struct PivotFlag {
@@ -199,11 +208,11 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             y0 -= L.a * T(x.x) + L.b * T(x.y);  y1 -= L.c * T(x.x) + L.d * T(x.y);
         }
     };
+    // (solve-only sweeps: D holds the kept pivot inverse, loaded by the caller before the item loop)
     auto diag_finish = [&](int m, Blk<T> D, T y0, T y1) {
         Blk<T> Di = D;
         if (Sink::kInvert) {
             if (kFactor) { bool bad = false; Di = inv(D, bad); if (bad) pf.raise(); }
-            else if (kSolve) Di = s.ldD(m);
             if (kSolve) {
                 const T z0 = kTransposed ? Di.a * y0 + Di.c * y1 : Di.a * y0 + Di.b * y1;
                 const T z1 = kTransposed ? Di.b * y0 + Di.d * y1 : Di.c * y0 + Di.d * y1;
@@ -237,6 +246,7 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             Blk<T> Dm = {T(0), T(0), T(0), T(0)};
             T r0 = T(0), r1 = T(0);
             if (kFactor) { const Blk<T> J = s.ldD(m); Dm = {J.a + T(a[0]), J.b + T(a[1]), J.c + T(a[2]), J.d + T(a[3])}; }
+            else if (Sink::kInvert) Dm = s.ldD(m);
             if (kSolve) { const double2 r = s.rh(m); r0 = T(r.x) + T(a[4]); r1 = T(r.y) + T(a[5]); }
             diag_finish(m, Dm, r0, r1);
         }
@@ -266,7 +276,7 @@ __device__ __forceinline__ void accumulate_level(const Slot<T, kP>& s, const Lev
             Blk<T> D = {T(0), T(0), T(0), T(0)};
             T y0 = T(0), y1 = T(0);
             if (lead) {
-                if (kFactor) D = s.ldD(m);
+                if (kFactor || Sink::kInvert) D = s.ldD(m);   // J(m,m), or (solve-only) the kept pivot inverse
                 if (kSolve) { const double2 r = s.rh(m); y0 = T(r.x); y1 = T(r.y); }
             }
             for (int q = t0 + part; q < t1; q += S) diag_item(dak[q], D, y0, y1);
@@ -344,6 +354,12 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
         const char* lb = ring.acquire(l, d);
         const int* pptr = reinterpret_cast<const int*>(lb + d.o_pptr);
         const int2* pmj = reinterpret_cast<const int2*>(lb + d.o_pmj);
+#if SABLE_BWD_PREFETCH
+        // the next level's blocks (one contiguous pair range) on their way into the L2 while this level's chain runs
+        for (int a = (l == nl - 1 ? 1 : kBwdAhead); a <= kBwdAhead; ++a)
+            if (l - a >= 0 && lv[l - a].p1 - lv[l - a].p0 <= kBwdPrefetchPairs)
+                s.prefetch_pairs_l2(lv[l - a].p0, lv[l - a].p1, kTransposed ? 1 : 0, threadIdx.x >> gsh, blockDim.x >> gsh);
+#endif
         const int ssh = min((int)d.sb, 5 - gsh), tsh = 5 - gsh - ssh, S = 1 << ssh;
         const int tl = lane >> (gsh + ssh), part = (lane >> gsh) & (S - 1);
         for (int base = d.m0 + (warp << tsh); base < d.m1; base += nwarps << tsh) {
@@ -352,6 +368,12 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
             const bool lead = valid && part == 0;
             const int p0 = pptr[m - d.m0], p1 = valid ? pptr[m - d.m0 + 1] : p0;
             T y0 = T(0), y1 = T(0);
+            // the lead lane's own pivot inverse and right-hand side: asked for before the pair loop, not after the reduction
+            // (one dependent memory round trip less per level)
+            const bool fin = lead && p1 > p0;
+            Blk<T> D = {T(0), T(0), T(0), T(0)};
+            double2 r = make_double2(0.0, 0.0);
+            if (fin) { D = s.ldD(m); r = s.rh(m); }
             for (int pi = p0 + part; pi < p1; pi += S) {
                 const int j = pmj[pi].y & kIdxMask, p = d.p0 + pi;
                 const double2 x = s.rh(j);
@@ -359,9 +381,7 @@ __device__ __forceinline__ void stage_backward(const DevTemplate& t, const Slot<
                 else              { const Blk<T> L = s.ldL(p); y0 += L.a * T(x.x) + L.c * T(x.y); y1 += L.b * T(x.x) + L.d * T(x.y); }
             }
             for (int o = (S >> 1) << gsh; o >= (1 << gsh); o >>= 1) { y0 += shx(y0, o); y1 += shx(y1, o); }
-            if (lead && p1 > p0) {
-                const Blk<T> D = s.ldD(m);
-                const double2 r = s.rh(m);
+            if (fin) {
                 const T z0 = kTransposed ? D.a * y0 + D.c * y1 : D.a * y0 + D.b * y1;
                 const T z1 = kTransposed ? D.b * y0 + D.d * y1 : D.c * y0 + D.d * y1;
                 s.set_rh(m, make_double2(double(T(r.x) - z0), double(T(r.y) - z1)));
