@@ -485,70 +485,46 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     if (guard.err != cudaSuccess) { c->err = std::string("cudaSetDevice: ") + cudaGetErrorString(guard.err); return bail(SABLE_ERR_CUDA); }
     // packed device arrays
     std::vector<int32_t> node_bus(T.node_bus); node_bus.push_back(T.slack);
-    std::vector<double2> ydg(nn);
+    std::vector<double2> ygb(T.ycol.size()), ydg(nn);
+    for (size_t k = 0; k < T.ycol.size(); ++k) ygb[k] = make_double2(T.yg[k], T.yb[k]);
     for (int m = 0; m < nn; ++m) ydg[m] = make_double2(T.yg[T.ydiag[m]], T.yb[T.ydiag[m]]);
+    // Jacobian destinations of the Y entries (stage_mismatch): entry (m,j) of row m feeds the U half of pair (m,j) when j is
+    // eliminated later, the L' half of pair (j,m) otherwise; diagonal entries and the slack column feed nothing
+    std::vector<int2> ycd(T.ycol.size());
+    std::vector<int4> jmj;
+    std::vector<double4> jy;
+    for (size_t k = 0; k < T.ycol.size(); ++k) ycd[k] = make_int2(T.ycol[k], -1);
+    for (int p = 0; p < np; ++p) {
+        const int su = T.pair_yu[p], sl = T.pair_yl[p];
+        if ((su >= 0) != (sl >= 0)) { c->err = "internal: Y pattern not symmetric"; return bail(SABLE_ERR_STRUCTURE); }
+        if (su < 0) continue;
+        ycd[su].y = p | (T.node_pq[T.pair_col[p]] ? 1 << 30 : 0);
+        const int m = T.pair_row[p], j = T.pair_col[p];
+        jmj.push_back(make_int4(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0), p, 0));
+        jy.push_back(make_double4(T.yg[su], T.yb[su], T.yg[sl], T.yb[sl]));
+        ycd[sl].y = p | 1 << 29 | (T.node_pq[T.pair_row[p]] ? 1 << 30 : 0);
+    }
     DevTemplate& d = c->d;
     d.n_bus = T.n_bus; d.n_node = nn; d.n_pair = np; d.n_level = T.n_level; d.slack = T.slack;
-    // mismatch pass: nodes by descending Y-row length; a row of up to 12 << s entries is served by 1 << s lanes.  The entries
-    // are stored in WALK ORDER: contiguous per row for the split classes; for the rows served by one lane each (the bulk) in
-    // slices of 32 rows, entry-major (entry i of the slice's row r at slice base + 32 i + r: the lanes of a warp read
-    // neighbouring words; rows are sorted by length, so a slice is as wide as its first row and the padding is small)
+    // mismatch pass: nodes by descending Y-row length; a row of up to 12 << s entries is served by 1 << s lanes
     std::vector<int32_t> mm_order(nn);
     std::vector<int4> mm_row(nn);
-    std::vector<int32_t> newpos(T.ycol.size(), -1);
-    std::vector<int2> ycd;
-    std::vector<double2> ygb;
     {
         for (int m = 0; m < nn; ++m) mm_order[m] = m;
         auto deg = [&](int m) { return T.yptr[m + 1] - T.yptr[m]; };
         std::stable_sort(mm_order.begin(), mm_order.end(), [&](int a, int b) { return deg(a) > deg(b); });
         auto cls = [&](int m) { int sft = 0; while (sft < 5 && deg(m) > (12 << sft)) ++sft; return sft; };
-        auto grow = [&](size_t n) { if (ycd.size() < n) { ycd.resize(n, make_int2(0, -1)); ygb.resize(n, make_double2(0.0, 0.0)); } };
-        auto put = [&](size_t pos, int k) {
-            grow(pos + 1);
-            ycd[pos] = make_int2(T.ycol[k], -1); ygb[pos] = make_double2(T.yg[k], T.yb[k]); newpos[k] = (int32_t)pos;
-        };
         d.n_class = 0;
         for (int i = 0; i < nn;) {
             int j = i; const int sft = cls(mm_order[i]);
             while (j < nn && cls(mm_order[j]) == sft) ++j;
-            d.mm_class[d.n_class++] = RowClass{i, j, sft, sft == 0 ? 32 : 1};
-            size_t base = (ycd.size() + 31) / 32 * 32;                       // 256-byte aligned class start
-            if (sft == 0) {
-                for (int s0 = i; s0 < j; s0 += 32) {
-                    const int w = deg(mm_order[s0]);
-                    for (int r = 0; r < 32 && s0 + r < j; ++r) {
-                        const int m = mm_order[s0 + r];
-                        mm_row[s0 + r] = make_int4(m, (int)(base + r), deg(m), T.node_bus[m] | (T.node_pq[m] ? 1 << 30 : 0));
-                        for (int e = 0; e < deg(m); ++e) put(base + (size_t)32 * e + r, T.yptr[m] + e);
-                    }
-                    base += (size_t)32 * w;
-                    grow(base);
-                }
-            } else {
-                for (int r = i; r < j; ++r) {
-                    const int m = mm_order[r];
-                    mm_row[r] = make_int4(m, (int)base, deg(m), T.node_bus[m] | (T.node_pq[m] ? 1 << 30 : 0));
-                    for (int e = 0; e < deg(m); ++e) put(base + e, T.yptr[m] + e);
-                    base += deg(m);
-                }
-            }
+            d.mm_class[d.n_class++] = RowClass{i, j, sft};
             i = j;
         }
-    }
-    // Jacobian destinations of the Y entries (stage_mismatch): entry (m,j) of row m feeds the U half of pair (m,j) when j is
-    // eliminated later, the L' half of pair (j,m) otherwise; diagonal entries and the slack column feed nothing
-    std::vector<int4> jmj;
-    std::vector<double4> jy;
-    for (int p = 0; p < np; ++p) {
-        const int su = T.pair_yu[p], sl = T.pair_yl[p];
-        if ((su >= 0) != (sl >= 0)) { c->err = "internal: Y pattern not symmetric"; return bail(SABLE_ERR_STRUCTURE); }
-        if (su < 0) continue;
-        ycd[newpos[su]].y = p | (T.node_pq[T.pair_col[p]] ? 1 << 30 : 0);
-        ycd[newpos[sl]].y = p | 1 << 29 | (T.node_pq[T.pair_row[p]] ? 1 << 30 : 0);
-        const int m = T.pair_row[p], j = T.pair_col[p];
-        jmj.push_back(make_int4(m | (T.node_pq[m] ? 1 << 30 : 0), j | (T.node_pq[j] ? 1 << 30 : 0), p, 0));
-        jy.push_back(make_double4(T.yg[su], T.yb[su], T.yg[sl], T.yb[sl]));
+        for (int i = 0; i < nn; ++i) {
+            const int m = mm_order[i];
+            mm_row[i] = make_int4(m, T.yptr[m], T.yptr[m + 1], T.node_bus[m] | (T.node_pq[m] ? 1 << 30 : 0));
+        }
     }
     bool ok = true;
     auto up = [&](auto& vec, auto** dst) { if (ok && upload(c, vec, dst) != cudaSuccess) { ok = false; c->err = "template upload failed"; } };
@@ -567,7 +543,7 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         up(tpos, &c->ftpos); up(bt, &c->d_bus_type);
     }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
-    up(ycd, &d.ycd); up(ygb, &d.ygb); up(jmj, &d.jp_mj); up(jy, &d.jp_y);
+    up(T.ycol, &d.ycol); up(ycd, &d.ycd); up(ygb, &d.ygb); up(jmj, &d.jp_mj); up(jy, &d.jp_y);
     d.n_jpair = (int)jmj.size(); up(ydg, &d.ydiag_gb);
     if (!ok) return bail(SABLE_ERR_ALLOC);
     ctx = c;

@@ -61,24 +61,22 @@ struct LevelDesc {
     Cls cls[2 * kMaxCls];
 };
 
-// rows mm_order[i0 .. i1) of the mismatch pass are served by 1 << ssh lanes each; entry i of a row sits at first + i * es
-// in the walk-order entry arrays (es = 1: the row's entries are contiguous; es = 32: rows served by one lane each are stored
-// in slices of 32 rows, entry-major, so that the lanes of a warp read neighbouring words)
-struct RowClass { int32_t i0, i1, ssh, es; };
+struct RowClass { int32_t i0, i1, ssh; };   // rows mm_order[i0 .. i1) of the mismatch pass are served by 1 << ssh lanes each
 
 struct DevTemplate {
     int32_t n_bus, n_node, n_pair, n_level, slack;
     int32_t n_class;            // mismatch pass: nodes sorted by Y-row length, long rows split over lanes
     RowClass mm_class[6];
-    const int4* mm_row;         // [n_node] (node m, first entry, number of entries, bus | pq << 30), longest rows first
+    const int4* mm_row;         // [n_node] (node m, first Y slot, end Y slot, bus | pq << 30), longest rows first
     const LevelDesc* level;     // [n_level]
     const char* blob;           // level slices of the index program
     const int32_t* node_bus;    // [n_node+1]  (entry n_node = slack bus)
     const uint8_t* node_pq;     // [n_node]
     const int32_t* yptr;        // [n_node+1]  Y rows of the non-slack buses in node order
-    const int2*    ycd;         // per Y entry, in WALK ORDER (RowClass): (column node position (slack = n_node), destination of the
-                                // Jacobian block J(row, column): pair p | half << 29 (0: U, 1: L') | column is PQ << 30; -1: none)
-    const double2* ygb;         // (G, B) per Y entry, walk order
+    const int32_t* ycol;        // per stored Y entry: column node position (slack = n_node)
+    const int2*    ycd;         // the same with the walk's destination: (column node position (slack = n_node), destination of the Jacobian
+                                // block J(row, column): pair p | half << 29 (0: U, 1: L') | column is PQ << 30; -1: none)
+    const double2* ygb;         // (G, B) per stored Y entry
     int32_t n_jpair;            // pairs with a Y entry (the others are fill-in), for the pair-pass form of a2:
     const int4*    jp_mj;       // [n_jpair] (m | pq_m << 30, j | pq_j << 30, pair p, 0)
     const double4* jp_y;        // [n_jpair] (G_mj, B_mj, G_jm, B_jm)

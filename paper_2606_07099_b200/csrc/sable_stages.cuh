@@ -73,17 +73,17 @@ __device__ __forceinline__ double stage_mismatch(const DevTemplate& t, const Slo
             double2 v = make_double2(0.0, 0.0);
             if (kWalk) v = s.vv(m);
             double ire = 0.0, iim = 0.0;
-            const int cnt = valid ? row.z : 0, es = rc.es;
+            const int k1 = valid ? row.z : 0;
             // kU entries per step: their index / admittance loads are issued together, then the V gathers -- a lane
             // that walks a row alone has 2 dependent round trips per step instead of 2 per entry
-            for (int i = part; i < cnt; i += kU * S) {
+            for (int k = row.y + part; k < k1; k += kU * S) {
                 int2 cd[kU]; double2 y[kU], x[kU];
 #pragma unroll
                 for (int u = 0; u < kU; ++u) {
-                    const int iu = i + u * S;
-                    const bool on = iu < cnt;
-                    const int ku = row.y + iu * es;
-                    cd[u] = on ? t.ycd[ku] : make_int2(m, -1);
+                    const int ku = k + u * S;
+                    const bool on = ku < k1;
+                    if (kWalk) cd[u] = on ? t.ycd[ku] : make_int2(m, -1);
+                    else cd[u] = make_int2(on ? t.ycol[ku] : m, -1);
                     y[u] = on ? t.ygb[ku] : make_double2(0.0, 0.0);
                 }
 #pragma unroll
