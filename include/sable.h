@@ -273,6 +273,28 @@ sable_status sable_debug_stage_times(sable_ctx* ctx, int32_t batch, const double
  * n = entries wanted, at most 4 L + 4 (HOST out). */
 sable_status sable_debug_timing(sable_ctx* ctx, uint64_t* out, int32_t n);
 
+/* ---- the allocation-free entry point -------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * the Step-2 recovery of sable_recover (PAPER.md:80 eq. 5, :95-99 eq. 9; S = V o conj(Y_bus V)) WITHOUT a context.
+ * It calls no cudaMalloc, cudaFree or allocating library routine: the kernel's scratch (the voltages in rectangular form,
+ * 16 bytes per bus and scenario) lives in one file-scope __device__ array of SABLE_STATIC_SCRATCH_BYTES that every GPU
+ * loading the library holds until exit (csrc/sable_static.cu).
+ *   n_bus, batch          batch * n_bus * 16 must not exceed SABLE_STATIC_SCRATCH_BYTES (524 288 voltages: e.g. 56 scenarios of
+ *                         9 241 buses), else INVALID_ARG with a message that names the limit; batch = 0 only does the one-time
+ *                         set-up for the current device (look-up of the array's address) -- do that before a graph capture
+ *   row_ptr [n_bus+1], col_idx, y_re, y_im   Y_bus in CSR form, DEVICE pointers, read as given: any column order, duplicates
+ *                         add up, indices must be valid (they cannot be checked without a copy)
+ *   vm, va [batch][n_bus] DEVICE in;   p_inj, q_inj [batch][n_bus] DEVICE out: calculated net injections at every bus
+ *   cuda_stream           cudaStream_t of the CURRENT device; the call only enqueues one kernel
+ *   errbuf, errbuf_len    optional HOST buffer for the message of a failed call (may be NULL / 0)
+ * Every call shares the one array: calls that overlap on the GPU (different streams, or different host threads) RACE on it and
+ * must be serialised by the caller.  The array keeps the last call's contents; nothing in it has to start at zero (each
+ * CTA writes its slice before reading it).  Errors: INVALID_ARG, CUDA. */
+#define SABLE_STATIC_SCRATCH_BYTES (8u << 20)
+sable_status sable_injections_static(int32_t n_bus, int32_t batch, const int32_t* row_ptr, const int32_t* col_idx,
+                                     const double* y_re, const double* y_im, const double* vm, const double* va,
+                                     double* p_inj, double* q_inj, void* cuda_stream, char* errbuf, int32_t errbuf_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -59,7 +59,9 @@ EXPORTS = ["sable_create", "sable_default_options", "sable_solve", "sable_adjoin
            "sable_layer_backward", "sable_adjoint_refined", "sable_solve_host", "sable_adjoint_host",
            "sable_get_info", "sable_last_error", "sable_destroy", "sable_launch_count", "sable_debug_pattern",
            "sable_debug_mismatch", "sable_debug_jacobian", "sable_debug_linear_solve", "sable_debug_timing",
-           "sable_debug_stage_times"]
+           "sable_debug_stage_times", "sable_injections_static"]
+
+STATIC_SCRATCH_BYTES = 8 << 20      # SABLE_STATIC_SCRATCH_BYTES of include/sable.h
 
 
 def lib():
@@ -332,3 +334,25 @@ class Context:
 
 def sable_create(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt) -> Context:
     return Context(n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, **opt)
+
+
+def injections_static(row_ptr, col_idx, y_re, y_im, vm, va, out=None):
+    """sable_injections_static: the Step-2 recovery without a context and without any allocation inside the library (its
+    scratch is a static device array of STATIC_SCRATCH_BYTES shared by all calls -- calls that overlap on the GPU race).
+    Everything is a CUDA tensor on the current device: Y_bus CSR (int32 row_ptr [n_bus+1], int32 col_idx, float64 y_re, y_im),
+    vm, va [batch][n_bus] float64.  Returns (p_inj, q_inj); pass `out` to keep the call free of torch allocations too."""
+    import torch
+    n_bus, batch = int(row_ptr.shape[0]) - 1, int(vm.shape[0])
+    dv = torch.cuda.current_device()
+    if out is None:
+        out = (torch.empty_like(vm), torch.empty_like(vm))
+    nnz = tuple(col_idx.shape)
+    err = C.create_string_buffer(512)
+    st = lib().sable_injections_static(
+        C.c_int32(n_bus), C.c_int32(batch), _dp(row_ptr, (n_bus + 1,), torch.int32, dv), _dp(col_idx, nnz, torch.int32, dv),
+        _dp(y_re, nnz, torch.float64, dv), _dp(y_im, nnz, torch.float64, dv), _dp(vm, (batch, n_bus), torch.float64, dv),
+        _dp(va, (batch, n_bus), torch.float64, dv), _dp(out[0], (batch, n_bus), torch.float64, dv),
+        _dp(out[1], (batch, n_bus), torch.float64, dv), _stream(), err, C.c_int32(len(err)))
+    if st != 0:
+        raise SableError(st, err.value.decode())
+    return out

@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SRC = [os.path.join(CSRC, f) for f in ("sable_capi.cu", "sable_symbolic.cpp")]
+SRC = [os.path.join(CSRC, f) for f in ("sable_capi.cu", "sable_symbolic.cpp", "sable_static.cu")]
 OUT = os.path.join(HERE, "libsable.so")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "--extended-lambda",
          "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "550"]
