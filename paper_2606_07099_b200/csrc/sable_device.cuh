@@ -134,14 +134,37 @@ __device__ __forceinline__ void st_blk(float* p, int, const Blk<float>& v) {
 }
 // whole block in one access (HBM workspace: blocks are interleaved over the slots as units of 4 sizeof(T) bytes): one
 // 256-bit load / store per FP64 block (sm_100: LDG.256 / STG.256) -- half the L1 wavefronts of two 128-bit accesses
+// Cache hints of the factor blocks in the HBM workspace (SABLE_FAC_HINT = 0 switches them off): a scenario's factors are a
+// stream several times its SM's share of the L2 and far beyond the L1 -- loads do not allocate in the L1 (which stays with
+// the state gathers and the index program), stores are first in line for eviction from the L2.  Measured on the B200: cfg 3
+// 2.07 -> 2.03 ms, cfg 5 5.00 -> 4.85, mesh 3.66 -> 3.56, adjoint on the mesh 0.445 -> 0.40; other combinations
+// (L2::evict_first on the loads, L1 / L2 evict_last on the state gathers) were neutral or slower.
+#ifndef SABLE_FAC_HINT
+#define SABLE_FAC_HINT 1
+#endif
+#if SABLE_FAC_HINT
+#define SABLE_FAC_LD ".L1::no_allocate"
+#define SABLE_FAC_ST ".L2::evict_first"
+#else
+#define SABLE_FAC_LD ""
+#define SABLE_FAC_ST ""
+#endif
 __device__ __forceinline__ Blk<double> ldg_blk(const double* p) {
     Blk<double> v;
-    asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.a), "=d"(v.b), "=d"(v.c), "=d"(v.d) : "l"(p) : "memory");
+    asm volatile("ld.global" SABLE_FAC_LD ".v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.a), "=d"(v.b), "=d"(v.c), "=d"(v.d) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ Blk<float> ldg_blk(const float* p) { return ld_blk(p, 0); }
+__device__ __forceinline__ Blk<float> ldg_blk(const float* p) {
+#if SABLE_FAC_HINT
+    Blk<float> v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.a), "=f"(v.b), "=f"(v.c), "=f"(v.d) : "l"(p) : "memory");
+    return v;
+#else
+    return ld_blk(p, 0);
+#endif
+}
 __device__ __forceinline__ void stg_blk(double* p, const Blk<double>& v) {
-    asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.a), "d"(v.b), "d"(v.c), "d"(v.d) : "memory");
+    asm volatile("st.global" SABLE_FAC_ST ".v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(v.a), "d"(v.b), "d"(v.c), "d"(v.d) : "memory");
 }
 __device__ __forceinline__ void stg_blk(float* p, const Blk<float>& v) { st_blk(p, 0, v); }
 
@@ -211,7 +234,7 @@ template <typename T, int kP> struct Slot {
         if (kPairRec) {
             chk_blk(go_pu, p);
             float a, b, c, d, e, f, g, h;
-            asm volatile("ld.global.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            asm volatile("ld.global" SABLE_FAC_LD ".v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                          : "=f"(a), "=f"(b), "=f"(c), "=f"(d), "=f"(e), "=f"(f), "=f"(g), "=f"(h) : "l"(rec_ptr(p)) : "memory");
             U = {T(a), T(b), T(c), T(d)}; L = {T(e), T(f), T(g), T(h)};
         } else { U = ldU(p); L = ldL(p); }
@@ -219,7 +242,7 @@ template <typename T, int kP> struct Slot {
     __device__ __forceinline__ void stUL(int p, const Blk<T>& U, const Blk<T>& L) const {
         if (kPairRec) {
             chk_blk(go_pu, p);
-            asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(rec_ptr(p)), "f"(float(U.a)), "f"(float(U.b)), "f"(float(U.c)),
+            asm volatile("st.global" SABLE_FAC_ST ".v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(rec_ptr(p)), "f"(float(U.a)), "f"(float(U.b)), "f"(float(U.c)),
                          "f"(float(U.d)), "f"(float(L.a)), "f"(float(L.b)), "f"(float(L.c)), "f"(float(L.d)) : "memory");
         } else { stU(p, U); stL(p, L); }
     }
