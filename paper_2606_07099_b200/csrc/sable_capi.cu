@@ -374,19 +374,27 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         //    9 241-bus grid 512 (each measured best: 3.83 vs 4.03 ms at 256 on the 2 000-bus grid, 4.1 vs 5.2 ms at 128 on the mesh);
         //  * slots per CTA G such that a CTA has about 128 threads (small CTAs pack the register file best: 7 x 128 at 72
         //    registers), never so many that the batch leaves SMs without a CTA;
-        //  * single-wave batches (at most two scenarios per SM, e.g. 256 scenarios of 9 241 buses): two CTAs would share an
-        //    SM anyway, so they are merged into one CTA of twice the threads whose two scenarios interleave their slices --
-        //    neighbouring lanes then read neighbouring 16-byte words (half the L1 wavefronts: 6.2 vs 6.6 ms measured);
+        //  * single-wave batches (2 / 4 / 8 / 16 scenarios per SM fill the SMs in one wave: 256 scenarios of 9 241 buses, 512 of
+        //    the 900-bus mesh, 2 048 of 2 000 buses): the CTAs that would share an SM anyway are merged into ONE CTA of 768
+        //    (1 024) threads whose scenarios interleave their slices -- neighbouring lanes then read neighbouring words (a
+        //    fraction of the L1 wavefronts: 6.2 vs 6.6 ms on the 9 241-bus grid, 2.63 vs 3.56 on the mesh, 3.63 vs 3.93 on
+        //    the 2 000-bus grid with FP32 factors);
         //  * teams (a cluster of CTAs per group): for tiny batches of large grids (below), or on request (tune.cluster).
         const double items = (double)T.term_a.size() + (double)T.dterm.size();
         const int L = std::min(512, std::max(16, pow2_floor(std::max(1, (int)(0.75 * items / std::max(1, nl))))));
         const int c_given = tune_given(tu.cluster, 0, "SABLE_CLUSTER");
         int csz = c_given ? pow2_floor(tune(tu.cluster, 0, "SABLE_CLUSTER", 1, 1, 8)) : 1;
         int G = std::max(1, 128 / L);
+        bool merged = false;
         if (g_given) G = g_want;
         else {
             while (G > 1 && (int64_t)n_sm * G > (int64_t)std::max(mb, 1)) G /= 2;
-            if (G == 1 && 2 * L <= 1024 && mb <= 2 * n_sm && 20 * ((mb + 1) / 2) >= 17 * n_sm) G = 2;
+            // merged single-wave layout: when g = 2 / 4 / 8 / 16 scenarios per SM make one wave that still fills the SMs (at
+            // least 85 % of them get a group), the g CTAs that would share an SM become ONE CTA whose g scenarios interleave
+            for (int g = 2 * G; g <= 16 && !merged; g *= 2) {
+                const int64_t groups = ((int64_t)mb + g - 1) / g;
+                if (groups <= n_sm && 20 * groups >= 17 * (int64_t)n_sm) { G = g; merged = true; }
+            }
         }
         // tiny batches of large grids (the paper's own shapes: 4 ... 32 scenarios of 9 241 buses): the scenarios cannot fill
         // the SMs, and one scenario's wide levels want more lanes than a CTA has -- a team of 2 / 4 / 8 CTAs (one cluster) per
@@ -401,7 +409,9 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         const bool alone = (int64_t)(mb + G - 1) / G <= n_sm && G == 1;
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
         // (the merged layout runs 768 threads, 80 registers each: 5.35 ms against 5.63 at 1 024 threads / 64 registers)
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : (alone || (L << gsh) >= 1024) ? 768 : (L << gsh);
+        // (a merged CTA wants at least 64 lanes per scenario: 1 024 threads for 16 scenarios, 768 otherwise)
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : merged ? (768 >> gsh >= 64 ? 768 : 1024)
+                                                                              : (alone || (L << gsh) >= 1024) ? 768 : (L << gsh);
         th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
         ctx->placement = 2; ctx->csz = csz;
@@ -445,7 +455,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     ctx->csz_lin = ctx->csz;
     // adjoint kernel: 32 lanes per slot (measured best in round 1: a pure latency chain wants many small CTAs); the merged
     // single-wave layout (two slots of a large grid per CTA) wants the whole SM
-    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh == 1 && th >= 768) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh >= 1 && th >= 768) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     // the adjoint kernel's dense front: its shared memory holds nothing else of size, so when every CTA has an SM of its own
     // the front takes up to 180 KB (9 241-bus grid: 54 nodes instead of the NR kernel's 38); otherwise the NR kernel's front
