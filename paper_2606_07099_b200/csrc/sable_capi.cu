@@ -207,7 +207,7 @@ static LevelLists pack_level(const Template& T, LevelDesc& d, int k_limit, std::
 // its targets ask for, every target gets proportionally more (up to its list length), so that a narrow level spreads over
 // the whole CTA.
 static int cut_classes(const std::vector<int>& len, int first, int count, int lanes, int wmax, bool diag, int unit, Cls* cls) {
-    constexpr int kSerial = 2;
+    constexpr int kSerial = 3;      // measured on the B200 (cfg 3 / 4 / 5 / mesh, ms): 1: 2.10 / 3.70 / 5.45 / 2.74; 2: 2.04 / 3.60 / 4.90 / 2.64; 3: 2.02 / 3.63 / 4.74 / 2.55; 4: 2.05 / 3.61 / 4.78 / 2.52
     auto want = [&](int n, int boost) {
         int s = 0;
         while ((1 << s) < wmax && (n + (1 << s) - 1) / (1 << s) > kSerial) ++s;
