@@ -64,6 +64,10 @@ def main():
     run(3, 37, group=1, on_chip=0, threads=256, front_nodes=9, front_kb=64, keep=False)
     run(3, 19, group=8, on_chip=0, threads=256, precision=sb.MIXED)
     run(3, 19, group=4, on_chip=0, cluster=2, threads=256)
+    # merged single-wave layouts: 4 / 16 scenarios per CTA of 768 / 1 024 threads, FP64 and FP32 pair records
+    run(2, 43, group=4, on_chip=0, threads=768)
+    run(3, 37, group=16, on_chip=0, threads=1024, precision=sb.MIXED)
+    run(3, 37, group=16, on_chip=0, threads=1024, keep=False)
     print("sanitizer cases done")
 
 

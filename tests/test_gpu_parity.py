@@ -389,6 +389,43 @@ def test_full_batch_parity(cfg):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,batch,precision,slots", [(3, 2300, "fp64", 16), (4, 1100, "mixed", 8),
+                                                        ("mesh", 512, "fp64", 4)])
+def test_merged_single_wave_layouts(cfg, batch, precision, slots):
+    """Batches for which the launch policy merges 4 / 8 / 16 scenarios into one CTA per SM: the plan is
+    what the policy is documented to pick, ragged last groups included (2 300 = 143 groups of 16 + 12, 1 100 = 137 groups of 8 + 4), and the whole batch
+    agrees with the oracle, forward and adjoint."""
+    if cfg == "mesh":
+        net = S.mesh_network(30, 30, kappa=0.3)
+        Y = oracle_Y(net)
+    else:
+        net, Y = get_net(cfg)
+    c = net.cfg
+    prec = sb.FP64 if precision == "fp64" else sb.MIXED
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ctx = make_ctx(net, max_batch=batch, precision=prec, keep_factors=True)
+    assert ctx.info["placement"] == 2 and ctx.info["slots_per_cta"] == slots and ctx.info["ctas_per_sm"] == 1, ctx.info
+    assert ctx.info["threads"] == (1024 if slots == 16 else 768)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    if prec == sb.FP64:
+        check_solution(res, ref, c.tol, 1e-9, max_edge_frac=0.01, label=f"merged cfg{cfg} x {batch}")
+    else:
+        assert np.array_equal(res["converged"], ref["converged"])
+        assert (np.abs(res["iterations"].astype(int) - ref["iterations"]) <= 1).all()
+        assert np.abs(res["vm"] - ref["vm"]).max() <= 1e-7 and np.abs(res["va"] - ref["va"]).max() <= 1e-7
+    assert (res["final_norm"][res["converged"] == 1] <= c.tol).all() and res["converged"].mean() >= 0.99
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    lp, lq = ctx.adjoint(dev(gva), dev(gvm))
+    lp, lq = lp.cpu().numpy(), lq.cpu().numpy()
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res["vm"], res["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    tol_adj = 1e-8 if prec == sb.FP64 else 5e-4      # FP32 factors: the tolerance of test_adjoint_mixed_precision
+    assert (np.abs(lp - rp).max(axis=1) <= tol_adj * scale).all()
+    assert (np.abs(lq - rq).max(axis=1) <= tol_adj * scale).all()
+    ctx.close()
+
+
 def test_two_live_contexts():
     """Two contexts that map to the same kernel instantiation with different shared-memory sizes (the dynamic
     shared-memory attribute is per-function state): create cfg 2 (83 KB per CTA), create cfg 1 (7 KB), solve on the first."""
