@@ -654,6 +654,14 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
     }
 }
 
+// staged kernels: the instantiation whose register budget fits the thread count
+template <typename T> static void launch_st_mismatch_fill(const SolveArgs& A, int grid, int th, cudaStream_t s) {
+    if (th <= 128) k_st_mismatch_fill<T, 128, 7><<<grid, th, 0, s>>>(A); else k_st_mismatch_fill<T, 512, 2><<<grid, th, 0, s>>>(A);
+}
+template <typename T> static void launch_st_factor_solve(const SolveArgs& A, int grid, int th, cudaStream_t s) {
+    if (th <= 128) k_st_factor_solve<T, 128, 7><<<grid, th, 0, s>>>(A); else k_st_factor_solve<T, 512, 2><<<grid, th, 0, s>>>(A);
+}
+
 // Scenarios [b0, b0 + nb) of the caller's arrays (b0 a multiple of the group size) on stream s, with queue counter `chunk`.
 template <typename T>
 static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int chunk, cudaStream_t s) {
@@ -692,7 +700,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
     for (int i = 0; i <= A.max_it; ++i) {
         A.stage_it = std::min(i, kMaxActive - 1);
         if (i >= kMaxActive - 1) cudaMemsetAsync(A.active + A.stage_it, 0, 4, s);
-        k_st_mismatch_fill<T><<<grid, th, 0, s>>>(A);
+        launch_st_mismatch_fill<T>(A, grid, th, s);
         c->launches += 1;
         if (i >= 3 || i == A.max_it) {
             int32_t left = 0;
@@ -701,7 +709,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
             if (e != cudaSuccess) return e;
             if (left == 0) break;
         }
-        if (i < A.max_it) { k_st_factor_solve<T><<<grid, th, 0, s>>>(A); c->launches += 1; }
+        if (i < A.max_it) { launch_st_factor_solve<T>(A, grid, th, s); c->launches += 1; }
     }
     return cudaGetLastError();
 }
@@ -1033,9 +1041,9 @@ extern "C" sable_status sable_debug_stage_times(sable_ctx* ctx, int32_t batch, c
     if (mixed) k_st_init<float><<<grid, th, 0, s>>>(A); else k_st_init<double><<<grid, th, 0, s>>>(A);
     for (int i = 0; i < 3; ++i) {
         CU(cudaEventRecord(ev[2 * i], s));
-        if (mixed) k_st_mismatch_fill<float><<<grid, th, 0, s>>>(A); else k_st_mismatch_fill<double><<<grid, th, 0, s>>>(A);
+        if (mixed) launch_st_mismatch_fill<float>(A, grid, th, s); else launch_st_mismatch_fill<double>(A, grid, th, s);
         CU(cudaEventRecord(ev[2 * i + 1], s));
-        if (mixed) k_st_factor_solve<float><<<grid, th, 0, s>>>(A); else k_st_factor_solve<double><<<grid, th, 0, s>>>(A);
+        if (mixed) launch_st_factor_solve<float>(A, grid, th, s); else launch_st_factor_solve<double>(A, grid, th, s);
     }
     CU(cudaEventRecord(ev[6], s));
     CU(cudaStreamSynchronize(s));

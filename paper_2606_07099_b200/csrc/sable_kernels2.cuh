@@ -38,8 +38,10 @@ __global__ void k_st_init(const SolveArgs A) {
 // a1 + a6 + a2: mismatch, norm, convergence decision, Jacobian fill (in place, into the factor value array) for the
 // scenarios that go on; a scenario that finishes with keep_factors gets its factors of J1 at the final iterate here.
 // Masked slots (finished earlier, or beyond the batch) run along on the spare workspace group.
-template <typename T>
-__global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) {
+// (kThreads, kCtas: the register budget -- up to 128 threads x 7 CTAs per SM (72 registers), as the fused kernel's small
+// variant, or up to 512 x 2 (64))
+template <typename T, int kThreads, int kCtas>
+__global__ void __launch_bounds__(kThreads, kCtas) k_st_mismatch_fill(const SolveArgs A) {
     __shared__ double red[32 * 32];
     __shared__ double scratch[kStageScratch];
     const DevTemplate& t = A.t;
@@ -75,8 +77,8 @@ __global__ void __launch_bounds__(512, 2) k_st_mismatch_fill(const SolveArgs A) 
 }
 
 // a4 + a5: refactor, forward/backward substitution, FP64 state update
-template <typename T>
-__global__ void __launch_bounds__(512, 2) k_st_factor_solve(const SolveArgs A) {
+template <typename T, int kThreads, int kCtas>
+__global__ void __launch_bounds__(kThreads, kCtas) k_st_factor_solve(const SolveArgs A) {
     __shared__ double scratch[kStageScratch];
     const DevTemplate& t = A.t;
     const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), tsub = threadIdx.x >> gsh, nsub = blockDim.x >> gsh;
