@@ -204,9 +204,10 @@ static LevelLists pack_level(const Template& T, LevelDesc& d, int k_limit, std::
 // Class cuts of one target kind for a kernel family with `lanes` lanes per slot and at most `wmax` lanes of one warp per
 // target: targets are sorted by descending list length `len`; a class is a run of targets that get the same number of
 // lanes 2^ssh.  A target asks for enough lanes to leave at most kSerial items per lane; when the level has more lanes than
-// its targets ask for, every target gets proportionally more (up to its list length), so that a narrow level spreads over
-// the whole CTA.
-static int cut_classes(const std::vector<int>& len, int first, int count, int lanes, int wmax, bool diag, int unit, Cls* cls) {
+// its targets ask for, every target gets proportionally more (up to its list length, `boost_max` doublings), so that a narrow
+// level spreads over the whole CTA -- in the solve-only sweeps (adjoint kernel); the refactor's levels take no boost (fewer
+// lanes per target, shorter shuffle reductions: cfg 5 4.78 -> 4.67 ms, mesh 2.55 -> 2.49, adjoint unchanged).
+static int cut_classes(const std::vector<int>& len, int first, int count, int lanes, int wmax, bool diag, int unit, int boost_max, Cls* cls) {
     constexpr int kSerial = 3;      // measured on the B200 (cfg 3 / 4 / 5 / mesh, ms): 1: 2.10 / 3.70 / 5.45 / 2.74; 2: 2.04 / 3.60 / 4.90 / 2.64; 3: 2.02 / 3.63 / 4.74 / 2.55; 4: 2.05 / 3.61 / 4.78 / 2.52
     auto want = [&](int n, int boost) {
         int s = 0;
@@ -221,7 +222,7 @@ static int cut_classes(const std::vector<int>& len, int first, int count, int la
         for (int i = first; i < first + count; ++i) need += (int64_t)unit << want(len[i], boost + 1);
         bool grew = false;
         for (int i = first; i < first + count && !grew; ++i) grew = want(len[i], boost + 1) > want(len[i], boost);
-        if (need > lanes || !grew || boost >= 5) break;
+        if (need > lanes || !grew || boost >= boost_max) break;
     }
     std::vector<int> ssh(count);
     for (int i = 0; i < count; ++i) ssh[i] = want(len[first + i], boost);
@@ -248,6 +249,8 @@ static int cut_classes(const std::vector<int>& len, int first, int count, int la
     return (int)runs.size();
 }
 
+constexpr int kBoostFactor = 0, kBoostSolve = 5;      // lane boost of narrow levels: refactor levels / solve-only sweeps
+
 // lanes per target (log2) for the backward sweep of a level with n targets whose longest list has max_len entries
 static uint8_t pick_split(int n, int max_len, int lanes, int wmax) {
     int s = 0;
@@ -256,15 +259,15 @@ static uint8_t pick_split(int n, int max_len, int lanes, int wmax) {
 }
 
 // splits / classes of one level descriptor for a kernel family (threads per CTA, slots per CTA)
-static void plan_level(const Template& T, LevelDesc& d, const LevelLists& L, int threads, int gsh, bool allow_big, bool staged) {
+static void plan_level(const Template& T, LevelDesc& d, const LevelLists& L, int threads, int gsh, bool allow_big, bool staged, int boost_max) {
     const int lanes = std::max(1, threads >> gsh), wmax = std::max(1, 32 >> gsh), nm = d.m1 - d.m0;
     int nbig = 0;
     if (allow_big && lanes >= 2 * wmax) while (nbig < nm && nbig < 4 && L.dlen[nbig] >= 3 * wmax && L.dlen[nbig] >= 64) ++nbig;
     d.n_big = nbig;
-    int nc = cut_classes(L.dlen, nbig, nm - nbig, lanes, wmax, true, 1, d.cls);
+    int nc = cut_classes(L.dlen, nbig, nm - nbig, lanes, wmax, true, 1, boost_max, d.cls);
     int with_terms = 0;
     while (with_terms < (int)L.tlen.size() && L.tlen[with_terms] > 0) ++with_terms;
-    nc += cut_classes(L.tlen, 0, with_terms, lanes, wmax, false, kTargetUnit, d.cls + nc);
+    nc += cut_classes(L.tlen, 0, with_terms, lanes, wmax, false, kTargetUnit, boost_max, d.cls + nc);
     d.n_cls = (uint8_t)nc;
     int maxb = 0;
     for (int m = d.m0; m < d.m1; ++m) maxb = std::max(maxb, T.pair_ptr[m + 1] - T.pair_ptr[m]);
@@ -274,9 +277,9 @@ static void plan_level(const Template& T, LevelDesc& d, const LevelLists& L, int
 
 struct LevelPack { std::vector<LevelDesc> lv; std::vector<LevelLists> lists; };
 
-static std::vector<LevelDesc> build_levels(const Template& T, const LevelPack& P, int threads, int gsh, bool allow_big, int first_staged) {
+static std::vector<LevelDesc> build_levels(const Template& T, const LevelPack& P, int threads, int gsh, bool allow_big, int first_staged, int boost_max) {
     std::vector<LevelDesc> lv(P.lv);
-    for (int l = 0; l < T.n_level; ++l) plan_level(T, lv[l], P.lists[l], threads, gsh, allow_big, l >= first_staged);
+    for (int l = 0; l < T.n_level; ++l) plan_level(T, lv[l], P.lists[l], threads, gsh, allow_big, l >= first_staged, boost_max);
     return lv;
 }
 
@@ -284,7 +287,7 @@ static std::vector<LevelDesc> build_levels(const Template& T, const LevelPack& P
 // matrix within `budget` bytes of shared memory per CTA (K <= kcap).  Appends the assembly lists (the front targets'
 // items whose eliminated node k lies below the front) to the blob and fills ctx->front*.
 struct FrontPlan { int k = 0, f0 = 0, level = 0; LevelDesc d{}; };
-static FrontPlan build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap, bool allow_big) {
+static FrontPlan build_front(sable_ctx* c, int threads, int gsh, int64_t budget, int kcap, bool allow_big, int boost_max) {
     const Template& T = c->T;
     const int nn = T.n_node, np = (int)T.pair_col.size(), nl = T.n_level;
     const bool mixed = c->opt.precision == SABLE_MIXED;
@@ -297,7 +300,7 @@ static FrontPlan build_front(sable_ctx* c, int threads, int gsh, int64_t budget,
     LevelDesc d{};
     d.m0 = f0; d.m1 = nn; d.p0 = T.pair_ptr[f0]; d.p1 = np;
     const LevelLists L = pack_level(T, d, f0, c->blob_host);
-    plan_level(T, d, L, threads, gsh, allow_big, false);
+    plan_level(T, d, L, threads, gsh, allow_big, false, boost_max);
     fp.d = d; fp.k = nn - f0; fp.f0 = f0; fp.level = lc;
     return fp;
 }
@@ -432,7 +435,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         // against 5.98 with 15 and 6.17 without on the 9 241-bus grid; small CTAs that share the SM keep the L1)
         const int64_t budget = tune(tu.front_kb, -1, "SABLE_FRONT_KB", th <= 128 ? 8 : th <= 256 ? 6 : th <= 512 ? 16 : 96, 0, 220) * 1024LL;
         if (kcap >= 2 && ctx->csz == 1) {
-            const FrontPlan fp = build_front(ctx, th, gsh, budget, kcap, true);
+            const FrontPlan fp = build_front(ctx, th, gsh, budget, kcap, true, kBoostFactor);
             ctx->front = fp.d; ctx->front_k = fp.k; ctx->front_f0 = fp.f0; ctx->front_level = fp.level;
         }
         if (ctx->front_k > 0) {
@@ -462,7 +465,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     ctx->lin_front = FrontPlan_{ctx->front_k, ctx->front_f0, ctx->front_level, ctx->front};
     if (ctx->placement == 2 && ctx->csz == 1 && ctx->front_k > 0 && (int64_t)((mb + (1 << gsh) - 1) >> gsh) <= n_sm &&
         !tune_given(tu.front_kb, -1, "SABLE_FRONT_KB") && !tune_given(tu.front_nodes, -1, "SABLE_FRONT")) {
-        const FrontPlan fp = build_front(ctx, ctx->threads_lin, gsh, 180 * 1024LL, 96, true);
+        const FrontPlan fp = build_front(ctx, ctx->threads_lin, gsh, 180 * 1024LL, 96, true, kBoostSolve);
         if (fp.k > ctx->front_k) ctx->lin_front = FrontPlan_{fp.k, fp.f0, fp.level, fp.d};
     }
     return SABLE_OK;
@@ -568,10 +571,10 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     sable_status st = choose_launch(c, P);
     if (st != SABLE_OK) return bail(st);
     {
-        std::vector<LevelDesc> lf = build_levels(T, P, c->threads * c->csz, c->gsh, c->csz == 1, c->first_staged);
-        std::vector<LevelDesc> ls = build_levels(T, P, c->threads_stage, c->gsh, ((c->threads_stage >> 5) << c->gsh) <= 256, T.n_level);
-        std::vector<LevelDesc> ll = build_levels(T, P, c->threads_lin * c->csz_lin, c->gsh, c->csz_lin == 1, T.n_level);
-        std::vector<LevelDesc> l1 = build_levels(T, P, c->threads1, 0, true, T.n_level);
+        std::vector<LevelDesc> lf = build_levels(T, P, c->threads * c->csz, c->gsh, c->csz == 1, c->first_staged, c->placement == 2 ? kBoostFactor : kBoostSolve);
+        std::vector<LevelDesc> ls = build_levels(T, P, c->threads_stage, c->gsh, ((c->threads_stage >> 5) << c->gsh) <= 256, T.n_level, kBoostFactor);
+        std::vector<LevelDesc> ll = build_levels(T, P, c->threads_lin * c->csz_lin, c->gsh, c->csz_lin == 1, T.n_level, kBoostSolve);
+        std::vector<LevelDesc> l1 = build_levels(T, P, c->threads1, 0, true, T.n_level, kBoostSolve);
         up(lf, &c->level_fused); up(ls, &c->level_stage); up(ll, &c->level_lin); up(l1, &c->level_one); up(c->blob_host, &d.blob);
         if (!ok) return bail(SABLE_ERR_ALLOC);
     }
