@@ -426,6 +426,26 @@ def test_merged_single_wave_layouts(cfg, batch, precision, slots):
     ctx.close()
 
 
+def test_merged_layout_staged_mode():
+    """The staged kernels in a merged layout (sixteen scenarios per group, 512-thread CTAs, host early stop): the same
+    results as the fused kernel of the same context layout, bit for bit in the iteration counts and flags, within 1e-12 in the state."""
+    net, Y = get_net(3)
+    c = net.cfg
+    batch = 2300
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    outs = []
+    for mode in (sb.FUSED, sb.STAGED):
+        ctx = make_ctx(net, max_batch=batch, keep_factors=False, mode=mode)
+        assert ctx.info["slots_per_cta"] == 16
+        outs.append(to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it)))
+        ctx.close()
+    a, b = outs
+    assert np.array_equal(a["converged"], b["converged"]) and np.array_equal(a["iterations"], b["iterations"])
+    assert np.abs(a["vm"] - b["vm"]).max() <= 1e-12 and np.abs(a["va"] - b["va"]).max() <= 1e-12
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    check_solution(b, ref, c.tol, 1e-9, max_edge_frac=0.01, label="merged staged")
+
+
 def test_two_live_contexts():
     """Two contexts that map to the same kernel instantiation with different shared-memory sizes (the dynamic
     shared-memory attribute is per-function state): create cfg 2 (83 KB per CTA), create cfg 1 (7 KB), solve on the first."""
