@@ -60,7 +60,10 @@ typedef struct {
 } sable_tuning;
 
 typedef struct {
-    int32_t max_batch;      /* scenarios per sable_solve call; all device buffers are sized for it at create time */
+    int32_t max_batch;      /* scenarios per sable_solve call; all device buffers are sized for it at create time, and the launch
+                               plan (scenarios interleaved per CTA, threads) is made for a batch of THIS size: a context planned for a
+                               large batch serves a much smaller one at about the large batch's latency -- create one context per
+                               batch size in use, or fix the layout through tune.group / threads */
     int32_t precision;      /* SABLE_FP64 or SABLE_MIXED */
     int32_t keep_factors;   /* 1: after the NR loop, J1 is re-factored at the final iterate and the factors are kept
                                for sable_adjoint (reading 16) */
