@@ -52,7 +52,7 @@ typedef struct {
     int32_t ring_slot_bytes;  /* bytes per ring slot, 256 ... 65536; -1 = automatic                     (SABLE_RING_SLOT) */
     int32_t front_nodes;      /* HBM placement: cap on the nodes of the dense top front, 0 ... 96 (0 = off); -1 = automatic  (SABLE_FRONT) */
     int32_t front_kb;         /* shared-memory budget of the front per CTA in KB, 0 ... 220; -1 = automatic  (SABLE_FRONT_KB) */
-    int32_t threads_stage;    /* threads per CTA of the staged kernels, 32 ... 512; 0 = automatic       (SABLE_THREADS1) */
+    int32_t threads_stage;    /* threads per CTA of the staged kernels, 32 ... 1024; 0 = automatic       (SABLE_THREADS1) */
     int32_t threads_lin;      /* threads per CTA of the adjoint kernel, 32 ... 1024; 0 = automatic      (SABLE_THREADS_LIN) */
     int32_t timing;           /* 1 = per-phase cycle counters of CTA 0 (sable_debug_timing)            (SABLE_TIMING) */
     int32_t cluster;          /* HBM placement: CTAs (one thread-block cluster) that serve one group of scenarios together,

@@ -454,7 +454,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     // the other kernel families: staged kernels (same group layout; the fused kernel's own shape when it is an HBM kernel),
     // the adjoint kernel (32 targets in flight per slot measured best in round 1), one-scenario debug kernels
     const int Ls = std::min(512, std::max(32, pow2_floor(std::max(1, nn / 8))));
-    ctx->threads_stage = (tune(tu.threads_stage, 0, "SABLE_THREADS1", ctx->placement == 2 ? std::min(th, 512) : std::min(512, Ls << gsh), 32, 512) + 31) / 32 * 32;
+    ctx->threads_stage = (tune(tu.threads_stage, 0, "SABLE_THREADS1", ctx->placement == 2 ? th : std::min(512, Ls << gsh), 32, 1024) + 31) / 32 * 32;
     ctx->csz_lin = ctx->csz;
     // adjoint kernel: 32 lanes per slot (measured best in round 1: a pure latency chain wants many small CTAs); the merged
     // single-wave layout (two slots of a large grid per CTA) wants the whole SM
@@ -659,10 +659,16 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
 
 // staged kernels: the instantiation whose register budget fits the thread count
 template <typename T> static void launch_st_mismatch_fill(const SolveArgs& A, int grid, int th, cudaStream_t s) {
-    if (th <= 128) k_st_mismatch_fill<T, 128, 7><<<grid, th, 0, s>>>(A); else k_st_mismatch_fill<T, 512, 2><<<grid, th, 0, s>>>(A);
+    if (th <= 128) k_st_mismatch_fill<T, 128, 7><<<grid, th, 0, s>>>(A);
+    else if (th <= 512) k_st_mismatch_fill<T, 512, 2><<<grid, th, 0, s>>>(A);
+    else if (th <= 768) k_st_mismatch_fill<T, 768, 1><<<grid, th, 0, s>>>(A);
+    else k_st_mismatch_fill<T, 1024, 1><<<grid, th, 0, s>>>(A);
 }
 template <typename T> static void launch_st_factor_solve(const SolveArgs& A, int grid, int th, cudaStream_t s) {
-    if (th <= 128) k_st_factor_solve<T, 128, 7><<<grid, th, 0, s>>>(A); else k_st_factor_solve<T, 512, 2><<<grid, th, 0, s>>>(A);
+    if (th <= 128) k_st_factor_solve<T, 128, 7><<<grid, th, 0, s>>>(A);
+    else if (th <= 512) k_st_factor_solve<T, 512, 2><<<grid, th, 0, s>>>(A);
+    else if (th <= 768) k_st_factor_solve<T, 768, 1><<<grid, th, 0, s>>>(A);
+    else k_st_factor_solve<T, 1024, 1><<<grid, th, 0, s>>>(A);
 }
 
 // Scenarios [b0, b0 + nb) of the caller's arrays (b0 a multiple of the group size) on stream s, with queue counter `chunk`.
