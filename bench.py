@@ -252,6 +252,15 @@ def run_ours(cfg_key, steps, warmup, rank, world, e2e=True, clocks=True, mode=0,
     if adjoint:
         res["next_rows_ms"]["layer_backward"] = timed(lambda: ctx.layer_backward(out["vm"], out["va"], dga, dgm, dgm, dga, out=pq))
         res["next_rows_ms"]["adjoint_refined_2_sweeps"] = timed(lambda: ctx.adjoint_refined(out["vm"], out["va"], dga, dgm, sweeps=2, out=lam))
+    if c.precision == 1:
+        # NEXT 3: inner refinement of the forward solve (staged pipeline, FP32 factors), beside the plain staged mixed solve
+        for key, kw in (("staged_mixed_solve", {}), ("staged_mixed_solve_ir2", {"ir_sweeps": 2})):
+            cx = sb.Context(net.n_bus, *Yh, net.bus_type, net.slack, max_batch=B, precision=c.precision, keep_factors=False, mode=1,
+                            device=torch.cuda.current_device(), **kw)
+            o2 = {k: torch.empty_like(v) for k, v in out.items()}
+            res["next_rows_ms"][key] = timed(lambda: cx.solve(dps, dqs, dvs, tol=c.tol, max_it=c.max_it, out=o2), reps=3)
+            res["next_rows_ms"][key + "_iterations_hist"] = np.bincount(o2["iterations"].cpu().numpy()).tolist()
+            cx.close()
     if e2e:
         pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory().numpy()
         hps, hqs, hvs, hga, hgm = pin(ps), pin(qs), pin(vs), pin(gva), pin(gvm)

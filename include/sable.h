@@ -73,10 +73,15 @@ typedef struct {
     int32_t device;         /* CUDA device ordinal; -1 = host-only context (symbolic phase only: sable_get_info and the
                                sable_debug_* pattern queries work, solve / adjoint return SABLE_ERR_STATE) */
     int32_t threads;        /* threads per CTA for the NR kernel; 0 = library default for the grid size  (SABLE_THREADS) */
-    int32_t ir_sweeps;      /* inner iterative-refinement sweeps of the forward linear solve in SABLE_MIXED mode.  Must be 0:
-                               the paper's scheme has none (Table I) -- the Newton loop with its FP64
-                               residual and FP64 state accumulation is the refinement (reading 15).  FP64
-                               refinement of the ADJOINT solve on FP32 factors: sable_adjoint_refined. */
+    int32_t ir_sweeps;      /* inner iterative-refinement sweeps of the forward linear solve, 0 ... 8 (default 0).  The paper's scheme
+                               has none (Table I): the Newton loop with its FP64 residual and FP64 state
+                               accumulation is the refinement (reading 15).  k > 0 (needs precision = SABLE_MIXED and
+                               mode = SABLE_MODE_STAGED, else sable_create returns INVALID_ARG): after the FP32 solve of
+                               J1 dz = -F1, k times r = -F1 - J1 dz with F1 and J1 evaluated in FP64 from Y_bus and the state
+                               (nothing stored), J1 c = r on the same FP32 factors, dz += c in FP64; the step
+                               then has FP64 accuracy and the iteration counts are those of an FP64 Newton loop.  Costs
+                               2 + 3 k extra launches per iteration and nine [max_batch][n_bus] FP64 arrays (allocated at create).
+                               FP64 refinement of the ADJOINT solve on FP32 factors: sable_adjoint_refined. */
     sable_tuning tune;
 } sable_options;
 

@@ -173,6 +173,39 @@ def nr_batch(Y, bus_type, p_spec, q_spec, v_set, vm0=None, va0=None, tol=1e-8, m
     return out
 
 
+def nr_mixed_ir(Y, bus_type, p_spec, q_spec, v_set, tol=1e-8, max_it=20, ir_sweeps=0, method=1):
+    """One scenario: Newton-Raphson whose linear solves run in FP32 (Table I: "solver copy SP") and are
+    then refined by `ir_sweeps` inner sweeps (SURVEY.md section 8(c) reading 15): r = -F1 - J1 dz with J1, F1 in FP64,
+    J1 c = r solved in FP32, dz += c in FP64.  Loop convention and update as oracle_nr_batch (eq. 7-8).
+    Plain Python over the oracle's own mismatch / Jacobian / linear-solve steps; the FP64 product J1 dz is a numpy
+    scatter-add over the COO entries.  Returns dict(vm, va, iterations, converged, final_norm, hist)."""
+    bus_type = _u8(bus_type)
+    p_spec, q_spec, v_set = _f64(p_spec), _f64(q_spec), _f64(v_set)
+    n, th, vmx = index_maps(bus_type)
+    vm = np.where(bus_type == 0, 1.0, v_set).astype(np.float64)        # PAPER.md:287 flat start; PV / slack at setpoint
+    va = np.zeros_like(vm)
+    hist = np.full(max_it + 1, np.nan)
+    it, conv = 0, 0
+    while True:
+        F, r, _, _ = mismatch(Y, bus_type, p_spec, q_spec, vm, va)
+        hist[it] = r
+        if r <= tol:
+            conv = 1
+            break
+        if it == max_it or not np.isfinite(r):
+            break
+        _, jr, jc, jv = jacobian(Y, bus_type, vm, va)
+        dz = linear_solve(n, jr, jc, jv, -F, method=method, mixed=True)
+        for _ in range(int(ir_sweeps)):
+            res = -F.copy()
+            np.subtract.at(res, jr, jv * dz[jc])                       # r = -F1 - J1 dz, FP64
+            dz = dz + linear_solve(n, jr, jc, jv, res, method=method, mixed=True)
+        va = va + np.where(th >= 0, dz[np.maximum(th, 0)], 0.0)
+        vm = vm + np.where(vmx >= 0, dz[np.maximum(vmx, 0)], 0.0)
+        it += 1
+    return dict(vm=vm, va=va, iterations=it if conv else max_it, converged=conv, final_norm=r, hist=hist)
+
+
 def adjoint_batch(Y, bus_type, vm, va, g_va, g_vm, method=1, mixed=False, n_threads=0):
     """J1(V)^T lambda = g per scenario.  Returns (lam_p, lam_q, threads)."""
     row_ptr, col, g, bb = Y

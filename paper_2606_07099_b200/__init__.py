@@ -114,7 +114,7 @@ class Context:
     """Owns one `sable_ctx*`.  Method names follow the C calls (sable_solve -> .solve, ...)."""
 
     def __init__(self, n_bus, row_ptr, col_idx, y_re, y_im, bus_type, slack, max_batch=1, precision=FP64,
-                 keep_factors=True, mode=FUSED, device=0, threads=0, **tune):
+                 keep_factors=True, mode=FUSED, device=0, threads=0, ir_sweeps=0, **tune):
         """`tune`: fields of sable_tuning (group, ctas_per_sm, on_chip, ring_slots, ring_slot_bytes, front_nodes, front_kb,
         threads_stage, threads_lin, timing); anything not given stays automatic."""
         L = lib()
@@ -128,6 +128,7 @@ class Context:
         opt = L.sable_default_options()
         opt.max_batch, opt.precision, opt.keep_factors = int(max_batch), int(precision), int(bool(keep_factors))
         opt.mode, opt.device, opt.threads = int(mode), int(device), int(threads)
+        opt.ir_sweeps = int(ir_sweeps)
         for k, v in tune.items():
             if not hasattr(opt.tune, k):
                 raise TypeError(f"unknown tuning field {k!r}")

@@ -23,6 +23,7 @@ struct sable_ctx {
     double* zeros = nullptr;
     const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
     const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward (lbuf: lazily allocated)
+    double* irbuf = nullptr;       // ir_sweeps > 0: nine [max_batch][n_bus] arrays (V re/im, |V|, step, residual, correction), allocated at create
     unsigned long long* tim = nullptr;                       // tuning.timing: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
     // launch plan of the fused kernel (choose_launch) and of the other kernel families
@@ -480,9 +481,11 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
     sable_options o = sable_default_options();
     if (opt) o = *opt;
     if (o.max_batch < 1 || (o.precision != SABLE_FP64 && o.precision != SABLE_MIXED) ||
-        (o.mode != SABLE_MODE_FUSED && o.mode != SABLE_MODE_STAGED) || o.device < -1 || o.threads < 0 || o.ir_sweeps != 0)
-        return fail(nullptr, SABLE_ERR_INVALID_ARG, o.ir_sweeps != 0 ? "ir_sweeps must be 0: the forward Newton loop (FP64 residual, FP32 correction) is the "
-                    "refinement (DESIGN.md reading 15); inner sweeps exist for the adjoint only (sable_adjoint_refined)" : "bad option value");
+        (o.mode != SABLE_MODE_FUSED && o.mode != SABLE_MODE_STAGED) || o.device < -1 || o.threads < 0 || o.ir_sweeps < 0 || o.ir_sweeps > 8)
+        return fail(nullptr, SABLE_ERR_INVALID_ARG, "bad option value");
+    if (o.ir_sweeps > 0 && (o.precision != SABLE_MIXED || o.mode != SABLE_MODE_STAGED))
+        return fail(nullptr, SABLE_ERR_INVALID_ARG, "ir_sweeps > 0 needs precision = SABLE_MIXED (FP32 factors to refine) and mode = SABLE_MODE_STAGED "
+                    "(the sweeps run as kernels of their own between the solve stage and the update)");
     sable_ctx* c = new (std::nothrow) sable_ctx;
     if (!c) return fail(nullptr, SABLE_ERR_ALLOC, "host allocation failed");
     c->opt = o;
@@ -602,6 +605,11 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         if (!dmalloc((void**)&c->tim, tb)) return bail(SABLE_ERR_ALLOC);
         cudaMemset(c->tim, 0, tb);
     }
+    if (o.ir_sweeps > 0) {                                   // sable_solve itself allocates nothing
+        const size_t ib = 9 * (size_t)o.max_batch * nb * 8;
+        if (!dmalloc((void**)&c->irbuf, ib)) return bail(SABLE_ERR_ALLOC);
+        if (cudaMemset(c->irbuf, 0, ib) != cudaSuccess) { c->err = "cudaMemset failed"; return bail(SABLE_ERR_CUDA); }
+    }
     fill_info(c);
     *out = c;
     return SABLE_OK;
@@ -671,6 +679,9 @@ template <typename T> static void launch_st_factor_solve(const SolveArgs& A, int
     else k_st_factor_solve<T, 1024, 1><<<grid, th, 0, s>>>(A);
 }
 
+static sable_status launch_lin(sable_ctx* ctx, int b0, int batch, const double* rp, const double* rq, int transposed, double* xp,
+                               double* xq, bool use_flags, cudaStream_t s);
+
 // Scenarios [b0, b0 + nb) of the caller's arrays (b0 a multiple of the group size) on stream s, with queue counter `chunk`.
 template <typename T>
 static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int chunk, cudaStream_t s) {
@@ -702,6 +713,11 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
     // every mismatch pass and stops launching when it is zero (this mode synchronises; it exists for per-stage profiling)
     A.t.level = c->level_stage;
     const int grid = (nb + G - 1) / G, th = c->threads_stage;
+    if (c->opt.ir_sweeps > 0) {
+        const size_t n = (size_t)c->opt.max_batch * c->T.n_bus;
+        A.ir = 1; A.ir_v = reinterpret_cast<double2*>(c->irbuf) + o; A.ir_vm = c->irbuf + 2 * n + o;
+        A.ir_dzp = c->irbuf + 3 * n + o; A.ir_dzq = c->irbuf + 4 * n + o;
+    }
     cudaError_t e = cudaMemsetAsync(A.active, 0, kMaxActive * 4, s);
     if (e != cudaSuccess) return e;
     k_st_init<T><<<grid, th, 0, s>>>(A);
@@ -718,7 +734,28 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
             if (e != cudaSuccess) return e;
             if (left == 0) break;
         }
-        if (i < A.max_it) { launch_st_factor_solve<T>(A, grid, th, s); c->launches += 1; }
+        if (i == A.max_it) break;
+        launch_st_factor_solve<T>(A, grid, th, s);
+        c->launches += 1;
+        if (!A.ir) continue;
+        // inner refinement (ir_sweeps): dz from the FP32 factors, then `ir_sweeps` times r = -F1 - J1 dz in FP64, J1 c = r on the
+        // same factors, dz += c in FP64; then the update.  Arrays of irbuf: 0-1 V, 2 |V|, 3-4 dz, 5-6 r, 7-8 c
+        const size_t n = (size_t)c->opt.max_batch * c->T.n_bus, tot = (size_t)nb * c->T.n_bus;
+        const int fb = (int)std::min<size_t>((tot + 255) / 256, 8192);
+        k_st_ir_export<T><<<grid, th, 0, s>>>(A);
+        IrArgs R{};
+        R.n_bus = c->T.n_bus; R.batch = nb; R.fptr = c->fptr; R.fcol = c->fcol; R.fgb = c->fgb; R.bus_type = c->d_bus_type;
+        R.status = A.status; R.p_spec = A.p_spec; R.q_spec = A.q_spec; R.v = A.ir_v; R.vm = A.ir_vm; R.dzp = A.ir_dzp; R.dzq = A.ir_dzq;
+        R.rp = c->irbuf + 5 * n + o; R.rq = c->irbuf + 6 * n + o;
+        for (int sw = 0; sw < c->opt.ir_sweeps; ++sw) {
+            k_ir_residual<<<fb, 256, 0, s>>>(R);
+            if (launch_lin(c, b0, nb, c->irbuf + 5 * n, c->irbuf + 6 * n, 0, c->irbuf + 7 * n, c->irbuf + 8 * n, false, s) != SABLE_OK)
+                return cudaErrorLaunchFailure;
+            k_add2<<<fb, 256, 0, s>>>(A.ir_dzp, A.ir_dzq, c->irbuf + 7 * n + o, c->irbuf + 8 * n + o, tot);
+            c->launches += 2;
+        }
+        k_st_ir_update<T><<<grid, th, 0, s>>>(A);
+        c->launches += 2;
     }
     return cudaGetLastError();
 }

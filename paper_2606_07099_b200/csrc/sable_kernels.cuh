@@ -34,6 +34,11 @@ struct SolveArgs {
     int32_t* it;              // staged mode: [batch]
     int32_t* active;          // staged mode: [max_it + 2] scenarios still active after each mismatch pass
     int32_t stage_it;         // staged mode: index of this mismatch pass
+    // inner refinement of the forward linear solve (sable_options.ir_sweeps > 0; staged mode, FP32 factors): the solve stage
+    // leaves the step in rh instead of applying it, and the refinement works on bus-order arrays [batch][n_bus]
+    int32_t ir;
+    double2* ir_v;            // rectangular voltages of the current iterate
+    double *ir_vm, *ir_dzp, *ir_dzq;   // |V|; the step: theta part (non-slack buses), Vm part (PQ buses), zero elsewhere
 };
 
 constexpr int kRedBytes = 32 * 32 * 8;                      // per-slot norm reduction scratch: 32 warps x 32 slots

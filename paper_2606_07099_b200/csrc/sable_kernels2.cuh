@@ -90,8 +90,96 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_st_factor_solve(const Solve
     BlobRing ring = no_ring(t);
     stage_factor_forward<T, 2, true, true, false, true>(t, s, t.level, ring, pf, scratch, Team{0, 1});
     stage_backward<T, 2, false>(t, s, t.level, ring, Team{0, 1});
+    if (A.ir) return;                                                // the step stays in rh: refined, then applied by k_st_ir_update
     stage_update<T, 2>(t, s, tsub, nsub);
     if (act && tsub == 0) A.it[bb] += 1;
+}
+
+// ---- inner iterative refinement of the forward linear solve (sable_options.ir_sweeps; SURVEY.md section 8(c) reading 15:
+// r = -F1 - J1 dz with J1 and F1 in FP64, correction solved on the FP32 factors, added in FP64; PAPER.md:255-271 is the
+// mixed-precision scheme this refines -- the paper itself has no inner sweeps).  Three small kernels around k_linsolve:
+// export of the state and the FP32-solved step to bus-order arrays, the FP64 residual evaluated from Y_bus and V with the
+// Alg. 1 formulas (no stored FP64 Jacobian), and the update z1 += dz (eq. 8).
+template <typename T>
+__global__ void k_st_ir_export(const SolveArgs A) {
+    const int gsh = A.gsh, g = threadIdx.x & ((1 << gsh) - 1), b = (blockIdx.x << gsh) + g;
+    if (b >= A.batch || A.status[b] != 0) return;
+    const DevTemplate& t = A.t;
+    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b, gsh);
+    const size_t o = (size_t)b * t.n_bus;
+    for (int m = threadIdx.x >> gsh; m <= t.n_node; m += blockDim.x >> gsh) {      // node n_node is the slack bus
+        const int bus = t.node_bus[m];
+        const double2 dz = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
+        A.ir_v[o + bus] = s.vv(m);
+        A.ir_vm[o + bus] = s.ma(m).x;
+        A.ir_dzp[o + bus] = dz.x;
+        A.ir_dzq[o + bus] = (m < t.n_node && t.node_pq[m]) ? dz.y : 0.0;
+    }
+}
+
+template <typename T>
+__global__ void k_st_ir_update(const SolveArgs A) {
+    const int gsh = A.gsh, g = threadIdx.x & ((1 << gsh) - 1), b = (blockIdx.x << gsh) + g;
+    if (b >= A.batch || A.status[b] != 0) return;
+    const DevTemplate& t = A.t;
+    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b, gsh);
+    const size_t o = (size_t)b * t.n_bus;
+    for (int m = threadIdx.x >> gsh; m < t.n_node; m += blockDim.x >> gsh) {
+        const int bus = t.node_bus[m];
+        const double2 a = s.ma(m);
+        const double th = a.y + A.ir_dzp[o + bus], vm = t.node_pq[m] ? a.x + A.ir_dzq[o + bus] : a.x;
+        double sn, cs; sincos(th, &sn, &cs);
+        s.set_ma(m, make_double2(vm, th));
+        s.set_vv(m, make_double2(vm * cs, vm * sn));
+    }
+    if ((threadIdx.x >> gsh) == 0) A.it[b] += 1;
+}
+
+struct IrArgs {
+    int32_t n_bus, batch;
+    const int32_t *fptr, *fcol;       // full Y_bus CSR, bus order
+    const double2* fgb;
+    const uint8_t* bus_type;          // 0 PQ, 1 PV, 2 slack
+    const int32_t* status;            // [batch] 0 = scenario still iterating
+    const double *p_spec, *q_spec;    // [batch][n_bus]
+    const double2* v;
+    const double *vm, *dzp, *dzq;
+    double *rp, *rq;                  // out: r = -F1 - J1 dz, rows P (non-slack) and Q (PQ); zero elsewhere and for finished scenarios
+};
+
+// one row of Y_bus per thread: the row sum gives the calculated injection (F1 row, eq. 6) and, entry by entry, the
+// off-diagonal blocks of J1 applied to the neighbour's step; the diagonal block uses the calculated P_i, Q_i
+__global__ void k_ir_residual(const IrArgs A) {
+    const size_t total = (size_t)A.batch * A.n_bus;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int b = (int)(idx / A.n_bus), i = (int)(idx - (size_t)b * A.n_bus);
+        const size_t o = (size_t)b * A.n_bus;
+        const int ti = A.bus_type[i];
+        double rp = 0.0, rq = 0.0;
+        if (ti != 2 && A.status[b] == 0) {
+            const double2 vi = A.v[o + i];
+            double ire = 0.0, iim = 0.0, ap = 0.0, aq = 0.0;
+            double2 yd = make_double2(0.0, 0.0);
+            for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
+                const int j = A.fcol[k];
+                const double2 y = A.fgb[k], x = A.v[o + j];
+                const double tr = y.x * x.x - y.y * x.y, tim = y.y * x.x + y.x * x.y;
+                ire += tr; iim += tim;
+                if (j == i) { yd = y; continue; }
+                const double u2 = vi.x * tr + vi.y * tim, u1 = vi.y * tr - vi.x * tim;
+                const double dth = A.dzp[o + j], dvm = A.dzq[o + j] / A.vm[o + j];            // zero where the column is not in z1
+                ap += u1 * dth + u2 * dvm;
+                aq += -u2 * dth + u1 * dvm;
+            }
+            const double P = vi.x * ire + vi.y * iim, Q = vi.y * ire - vi.x * iim;
+            const double vm = A.vm[o + i], v2 = vm * vm, dth = A.dzp[o + i], dvm = A.dzq[o + i];
+            ap += (-Q - yd.y * v2) * dth + (P / vm + yd.x * vm) * dvm;
+            aq += (P - yd.x * v2) * dth + (Q / vm - yd.y * vm) * dvm;
+            rp = (A.p_spec[o + i] - P) - ap;
+            if (ti == 0) rq = (A.q_spec[o + i] - Q) - aq;
+        }
+        A.rp[idx] = rp; A.rq[idx] = rq;
+    }
 }
 
 // ---- adjoint / generic linear solve on stored factors ---------------------------------------------------------

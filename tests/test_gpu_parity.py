@@ -253,6 +253,62 @@ def test_nr_parity_mixed_precision(cfg, batch, mode):
     ctx.close()
 
 
+@pytest.mark.parametrize("cfg,batch", [(2, 96), (3, 70), (4, 24), (5, 5)])
+def test_forward_inner_refinement(cfg, batch):
+    """NEXT 3 (SURVEY.md section 8(f), 8(c) reading 15): `ir_sweeps` inner sweeps of the forward linear solve on FP32
+    factors -- r = -F1 - J1 dz in FP64, correction on the same factors, added in FP64.  With two sweeps every step has FP64
+    accuracy, so the run is compared with the FP64 oracle at the FP64 tolerances: identical iteration counts, state
+    within 1e-9 (the plain mixed mode is held to 1e-7 and +-1 iteration), and the accepting norm -- which in the plain
+    mixed mode sits ~5e-3 (relative) away from the FP64 loop's -- within 1e-4 of it.  One sweep is compared with the
+    oracle's own mixed + one-sweep loop on a few scenarios.  Batches are ragged against the group size; config 3 mixes
+    iteration counts, so finished scenarios sit masked inside groups that still refine."""
+    net, Y = get_net(cfg)
+    c = net.cfg
+    ps, qs, vs = S.make_scenarios(net, batch=batch)
+    ref = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, tol=c.tol, max_it=c.max_it, method=1)
+    ctx = make_ctx(net, max_batch=batch, mode=sb.STAGED, precision=sb.MIXED, keep_factors=False, ir_sweeps=2)
+    res = to_np(ctx.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    ctx.close()
+    assert np.array_equal(res["converged"], ref["converged"]) and ref["converged"].all()
+    assert np.array_equal(res["iterations"].astype(int), ref["iterations"].astype(int))
+    assert np.abs(res["vm"] - ref["vm"]).max() <= 1e-9 and np.abs(res["va"] - ref["va"]).max() <= 1e-9
+    # (absolute floor: the FP64 evaluation noise of the mismatch itself -- a row of S = V conj(Y V) sums terms of size
+    # |Y_ik| that cancel: a few ulps of the largest absolute row sum of Y_bus)
+    floor = max(1e-12, 16 * np.finfo(float).eps * np.add.reduceat(np.hypot(Y[2], Y[3]), Y[0][:-1]).max())
+    big = ref["final_norm"] >= 100 * floor
+    rel = np.abs(res["final_norm"] - ref["final_norm"]) / ref["final_norm"]
+    assert (np.abs(res["final_norm"] - ref["final_norm"]) <= 1e-4 * ref["final_norm"] + floor).all(), (rel.max(), ref["final_norm"][rel.argmax()])
+    # the same batch without sweeps: the accepting norms leave the FP64 loop's (what the sweeps repair)
+    ctx0 = make_ctx(net, max_batch=batch, mode=sb.STAGED, precision=sb.MIXED, keep_factors=False)
+    res0 = to_np(ctx0.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    ctx0.close()
+    same = (res0["iterations"].astype(int) == ref["iterations"].astype(int)) & big
+    if same.any():                                   # (config 5 accepts at ~1e-11: below the floor, nothing to compare)
+        rel0 = (np.abs(res0["final_norm"] - ref["final_norm"]) / ref["final_norm"])[same]
+        print("accepting norm vs the FP64 loop, relative (median / max): 2 sweeps", np.median(rel[big]), rel[big].max(), " no sweeps", np.median(rel0), rel0.max())
+        assert np.median(rel0) > 10 * max(np.median(rel[big]), 1e-9)
+    else:
+        assert cfg >= 4
+    # one sweep against the oracle's mixed loop with one sweep
+    ctx1 = make_ctx(net, max_batch=batch, mode=sb.STAGED, precision=sb.MIXED, keep_factors=True, ir_sweeps=1)
+    res1 = to_np(ctx1.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    ctx1.close()
+    for b in (0, batch // 2, batch - 1):
+        o1 = oracle.nr_mixed_ir(Y, net.bus_type, ps[b], qs[b], vs[b], tol=c.tol, max_it=c.max_it, ir_sweeps=1)
+        assert o1["converged"] == res1["converged"][b] == 1 and o1["iterations"] == int(res1["iterations"][b])
+        assert np.abs(res1["vm"][b] - o1["vm"]).max() <= 1e-9 and np.abs(res1["va"][b] - o1["va"]).max() <= 1e-9
+        assert abs(res1["final_norm"][b] - o1["final_norm"]) <= 1e-3 * o1["final_norm"] + floor
+
+
+def test_inner_refinement_options():
+    """ir_sweeps needs FP32 factors and the staged pipeline; out-of-range values are rejected at create."""
+    net, _ = get_net(1)
+    for kw in (dict(precision=sb.FP64, mode=sb.STAGED, ir_sweeps=1), dict(precision=sb.MIXED, mode=sb.FUSED, ir_sweeps=1),
+               dict(precision=sb.MIXED, mode=sb.STAGED, ir_sweeps=9), dict(precision=sb.MIXED, mode=sb.STAGED, ir_sweeps=-1)):
+        with pytest.raises(sb.SableError):
+            make_ctx(net, max_batch=4, **kw)
+
+
 @pytest.mark.parametrize("cfg,batch", [(1, 64), (3, 512), (5, 6)])
 @pytest.mark.parametrize("mode", [sb.FUSED, sb.STAGED])
 def test_adjoint_parity(cfg, batch, mode):

@@ -464,6 +464,37 @@ def test_mixed_precision_reference_mode():
             np.testing.assert_allclose(mp["vm"], dp["vm"], atol=1e-8)
 
 
+def test_mixed_precision_inner_refinement():
+    """oracle.nr_mixed_ir (SURVEY.md section 8(c) reading 15) pinned to things other than itself: with 0 sweeps it is the C
+    oracle's mixed mode (same FP32-rounded solves, so the same iterates); with enough sweeps every linear solve reaches
+    FP64 accuracy, so its norm history is that of the FP64 Newton loop (which contains no FP32 arithmetic at all) -- a wrong
+    sign, a dropped term or a transposed index in the residual r = -F1 - J1 dz makes the refined step worse than the FP32
+    one and fails this; one sweep must already shrink the distance to the FP64 history by orders of magnitude."""
+    for cfg in (1, 2):
+        net = S.make_network(cfg)
+        Y = net_Y(net)
+        ps, qs, vs = S.make_scenarios(net, batch=3)
+        dp = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, method=1, want_hist=True)
+        mp = oracle.nr_batch(Y, net.bus_type, ps, qs, vs, method=1, mixed=True, want_hist=True)
+        for b in range(3):
+            r0 = oracle.nr_mixed_ir(Y, net.bus_type, ps[b], qs[b], vs[b], ir_sweeps=0)
+            assert r0["iterations"] == mp["iterations"][b] and r0["converged"] == mp["converged"][b]
+            np.testing.assert_allclose(r0["vm"], mp["vm"][b], rtol=0, atol=1e-14)
+            np.testing.assert_allclose(r0["va"], mp["va"][b], rtol=0, atol=1e-14)
+            r3 = oracle.nr_mixed_ir(Y, net.bus_type, ps[b], qs[b], vs[b], ir_sweeps=3)
+            k = dp["iterations"][b]
+            assert r3["converged"] == 1 and r3["iterations"] == k
+            h64, h3, h0 = dp["hist"][b][:k + 1], r3["hist"][:k + 1], r0["hist"][:k + 1]
+            assert np.all(np.abs(h3 - h64) <= 1e-6 * h64 + 1e-12)
+            np.testing.assert_allclose(r3["vm"], dp["vm"][b], rtol=0, atol=1e-12)
+            np.testing.assert_allclose(r3["va"], dp["va"][b], rtol=0, atol=1e-12)
+            # the unrefined FP32 loop leaves the FP64 history once the norm is small; one sweep brings it back
+            r1 = oracle.nr_mixed_ir(Y, net.bus_type, ps[b], qs[b], vs[b], ir_sweeps=1)
+            d0 = np.nanmax(np.abs(h0[:min(k, r0["iterations"]) + 1] - h64[:min(k, r0["iterations"]) + 1]))
+            d1 = np.nanmax(np.abs(r1["hist"][:k + 1] - h64))
+            assert d1 <= 1e-3 * d0 + 1e-12
+
+
 def test_recorded_configs_are_feasible():
     """sable_synth.CONFIGS carries the (s_net, kappa) accepted by oracle/feasibility_scan.py."""
     for cfg in (1, 2, 3, 4):
