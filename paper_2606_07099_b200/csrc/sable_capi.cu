@@ -23,6 +23,7 @@ struct sable_ctx {
     double* zeros = nullptr;
     const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
     const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward (lbuf: lazily allocated)
+    const int32_t* d_bus_node = nullptr;   // ir_sweeps > 0: node of each bus
     double* irbuf = nullptr;       // ir_sweeps > 0: nine [max_batch][n_bus] arrays (V re/im, |V|, step, residual, correction), allocated at create
     unsigned long long* tim = nullptr;                       // tuning.timing: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
@@ -557,6 +558,7 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
             }
         std::vector<uint8_t> bt(bus_type, bus_type + n_bus);
         up(tpos, &c->ftpos); up(bt, &c->d_bus_type);
+        if (o.ir_sweeps > 0) up(T.bus_node, &c->d_bus_node);
     }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
     up(T.ycol, &d.ycol); up(ycd, &d.ycd); up(ygb, &d.ygb); up(jmj, &d.jp_mj); up(jy, &d.jp_y);
@@ -716,7 +718,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
     if (c->opt.ir_sweeps > 0) {
         const size_t n = (size_t)c->opt.max_batch * c->T.n_bus;
         A.ir = 1; A.ir_v = reinterpret_cast<double2*>(c->irbuf) + o; A.ir_vm = c->irbuf + 2 * n + o;
-        A.ir_dzp = c->irbuf + 3 * n + o; A.ir_dzq = c->irbuf + 4 * n + o;
+        A.ir_dzp = c->irbuf + 3 * n + o; A.ir_dzq = c->irbuf + 4 * n + o; A.ir_bus_node = c->d_bus_node;
     }
     cudaError_t e = cudaMemsetAsync(A.active, 0, kMaxActive * 4, s);
     if (e != cudaSuccess) return e;

@@ -39,6 +39,7 @@ struct SolveArgs {
     int32_t ir;
     double2* ir_v;            // rectangular voltages of the current iterate
     double *ir_vm, *ir_dzp, *ir_dzq;   // |V|; the step: theta part (non-slack buses), Vm part (PQ buses), zero elsewhere
+    const int32_t* ir_bus_node;        // [n_bus] node of each bus (slack -> n_node)
 };
 
 constexpr int kRedBytes = 32 * 32 * 8;                      // per-slot norm reduction scratch: 32 warps x 32 slots

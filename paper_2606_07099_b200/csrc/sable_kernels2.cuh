@@ -100,20 +100,41 @@ __global__ void __launch_bounds__(kThreads, kCtas) k_st_factor_solve(const Solve
 // mixed-precision scheme this refines -- the paper itself has no inner sweeps).  Three small kernels around k_linsolve:
 // export of the state and the FP32-solved step to bus-order arrays, the FP64 residual evaluated from Y_bus and V with the
 // Alg. 1 formulas (no stored FP64 Jacobian), and the update z1 += dz (eq. 8).
+// (tiles of 1024 / G buses go through shared memory: the slots interleave the G scenarios of a group node by node, the
+// bus-order arrays are scenario-major -- reads are coalesced over the scenarios of a node, writes over the buses of a scenario)
+constexpr int kIrTile = 1024;
 template <typename T>
 __global__ void k_st_ir_export(const SolveArgs A) {
-    const int gsh = A.gsh, g = threadIdx.x & ((1 << gsh) - 1), b = (blockIdx.x << gsh) + g;
-    if (b >= A.batch || A.status[b] != 0) return;
+    __shared__ double2 tv[kIrTile + kIrTile / 8];
+    __shared__ double tvm[kIrTile + kIrTile / 8], tdp[kIrTile + kIrTile / 8], tdq[kIrTile + kIrTile / 8];
     const DevTemplate& t = A.t;
-    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, b, gsh);
-    const size_t o = (size_t)b * t.n_bus;
-    for (int m = threadIdx.x >> gsh; m <= t.n_node; m += blockDim.x >> gsh) {      // node n_node is the slack bus
-        const int bus = t.node_bus[m];
-        const double2 dz = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
-        A.ir_v[o + bus] = s.vv(m);
-        A.ir_vm[o + bus] = s.ma(m).x;
-        A.ir_dzp[o + bus] = dz.x;
-        A.ir_dzq[o + bus] = (m < t.n_node && t.node_pq[m]) ? dz.y : 0.0;
+    const int gsh = A.gsh, G = 1 << gsh, g = threadIdx.x & (G - 1), b = (blockIdx.x << gsh) + g;
+    const bool act = b < A.batch && A.status[b] == 0;
+    if (!__syncthreads_or(act)) return;
+    const Slot<T, 2> s = hbm_slot<T>(t, A.factors, A.fac_stride, A.work, A.work_stride, act ? b : (blockIdx.x << gsh), gsh);
+    const int tb = kIrTile >> gsh;                                   // buses per tile; entry (bus bi, slot g) at bi * G + g (+ padding)
+    for (int i0 = 0; i0 < t.n_bus; i0 += tb) {
+        for (int idx = threadIdx.x; idx < kIrTile; idx += blockDim.x) {      // blockDim is a multiple of G: idx & (G - 1) == g
+            const int i = i0 + (idx >> gsh);
+            if (act && i < t.n_bus) {
+                const int m = A.ir_bus_node[i], e = idx + (idx >> 3);
+                const double2 dz = m < t.n_node ? s.rh(m) : make_double2(0.0, 0.0);
+                tv[e] = s.vv(m);
+                tvm[e] = s.ma(m).x;
+                tdp[e] = dz.x;
+                tdq[e] = (m < t.n_node && t.node_pq[m]) ? dz.y : 0.0;
+            }
+        }
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < kIrTile; idx += blockDim.x) {      // bus fastest
+            const int bi = idx & (tb - 1), gg = idx >> (10 - gsh), i = i0 + bi, bb = (blockIdx.x << gsh) + gg;
+            if (i < t.n_bus && bb < A.batch && A.status[bb] == 0) {
+                const int q = (bi << gsh) + gg, e = q + (q >> 3);
+                const size_t o = (size_t)bb * t.n_bus + i;
+                A.ir_v[o] = tv[e]; A.ir_vm[o] = tvm[e]; A.ir_dzp[o] = tdp[e]; A.ir_dzq[o] = tdq[e];
+            }
+        }
+        __syncthreads();
     }
 }
 
