@@ -99,6 +99,11 @@ static void fill_info(sable_ctx* c) {
 
 // kernel variants of the fused kernel: (placement, max threads per CTA, CTAs per SM the registers are budgeted for)
 struct Variant { int place, threads, ctas; };
+// threads of the CTA that has an SM to itself (register budget 65 536 / kWide, in steps of 8)
+#ifndef SABLE_WIDE
+#define SABLE_WIDE 768
+#endif
+constexpr int kWide = SABLE_WIDE;
 // CTAs per SM the 128-thread variant is budgeted for: 7 (72 registers) with FP64 factors, kSmallCtasF32 with FP32 factors
 template <typename T> struct SmallCtas { static constexpr int v = 7; };
 #ifndef SABLE_SMALL_CTAS_F32
@@ -107,7 +112,7 @@ template <typename T> struct SmallCtas { static constexpr int v = 7; };
 template <> struct SmallCtas<float> { static constexpr int v = SABLE_SMALL_CTAS_F32; };
 static int pick_variant(int place, int th) {
     if (place == 0) return 0;
-    return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : th <= 768 ? 5 : 4;
+    return th <= 128 ? 1 : th <= 256 ? 2 : th <= 512 ? 3 : th <= kWide ? 5 : 4;
 }
 template <typename T> static const void* fused_fn_t(int v) {
     switch (v) {
@@ -115,7 +120,7 @@ template <typename T> static const void* fused_fn_t(int v) {
         case 1: return (const void*)k_nr_fused<T, 2, 128, SmallCtas<T>::v>;
         case 2: return (const void*)k_nr_fused<T, 2, 256, 4>;
         case 3: return (const void*)k_nr_fused<T, 2, 512, 2>;
-        case 5: return (const void*)k_nr_fused<T, 2, 768, 1>;
+        case 5: return (const void*)k_nr_fused<T, 2, kWide, 1>;
         default: return (const void*)k_nr_fused<T, 2, 1024, 1>;
     }
 }
@@ -415,8 +420,8 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
         gsh = 0; while ((2 << gsh) <= G) ++gsh;
         // (the merged layout runs 768 threads, 80 registers each: 5.35 ms against 5.63 at 1 024 threads / 64 registers)
         // (a merged CTA wants at least 64 lanes per scenario: 1 024 threads for 16 scenarios, 768 otherwise)
-        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : merged ? (768 >> gsh >= 64 ? 768 : 1024)
-                                                                              : (alone || (L << gsh) >= 1024) ? 768 : (L << gsh);
+        th = ctx->opt.threads > 0 ? ctx->opt.threads : csz > 1 ? 1024 : merged ? (kWide >> gsh >= 64 ? kWide : 1024)
+                                                                              : (alone || (L << gsh) >= 1024) ? kWide : (L << gsh);
         th = std::min(1024, std::max(32, (tune(0, 0, "SABLE_THREADS", th, 32, 1024) + 31) / 32 * 32));
         if ((th >> gsh) < 1) gsh = 0;
         ctx->placement = 2; ctx->csz = csz;
@@ -460,7 +465,7 @@ static sable_status choose_launch(sable_ctx* ctx, const LevelPack& P) {
     ctx->csz_lin = ctx->csz;
     // adjoint kernel: 32 lanes per slot (measured best in round 1: a pure latency chain wants many small CTAs); the merged
     // single-wave layout (two slots of a large grid per CTA) wants the whole SM
-    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh >= 1 && th >= 768) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
+    ctx->threads_lin = (tune(tu.threads_lin, 0, "SABLE_THREADS_LIN", ctx->csz > 1 ? 512 : (gsh >= 1 && th >= kWide) ? 1024 : std::min(512, std::max(32 << gsh, 64)), 32, 1024) + 31) / 32 * 32;
     ctx->threads1 = nn <= 64 ? 32 : nn <= 1200 ? 64 : nn <= 4000 ? 256 : 512;
     // the adjoint kernel's dense front: its shared memory holds nothing else of size, so when every CTA has an SM of its own
     // the front takes up to 180 KB (9 241-bus grid: 54 nodes instead of the NR kernel's 38); otherwise the NR kernel's front
@@ -662,7 +667,7 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
         case 1: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 128, SmallCtas<T>::v>, A);
         case 2: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 256, 4>, A);
         case 3: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 512, 2>, A);
-        case 5: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 768, 1>, A);
+        case 5: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, kWide, 1>, A);
         default: return cudaLaunchKernelEx(&cfg, k_nr_fused<T, 2, 1024, 1>, A);
     }
 }
@@ -671,13 +676,13 @@ static cudaError_t launch_fused(sable_ctx* c, const SolveArgs& A, cudaStream_t s
 template <typename T> static void launch_st_mismatch_fill(const SolveArgs& A, int grid, int th, cudaStream_t s) {
     if (th <= 128) k_st_mismatch_fill<T, 128, 7><<<grid, th, 0, s>>>(A);
     else if (th <= 512) k_st_mismatch_fill<T, 512, 2><<<grid, th, 0, s>>>(A);
-    else if (th <= 768) k_st_mismatch_fill<T, 768, 1><<<grid, th, 0, s>>>(A);
+    else if (th <= kWide) k_st_mismatch_fill<T, kWide, 1><<<grid, th, 0, s>>>(A);
     else k_st_mismatch_fill<T, 1024, 1><<<grid, th, 0, s>>>(A);
 }
 template <typename T> static void launch_st_factor_solve(const SolveArgs& A, int grid, int th, cudaStream_t s) {
     if (th <= 128) k_st_factor_solve<T, 128, 7><<<grid, th, 0, s>>>(A);
     else if (th <= 512) k_st_factor_solve<T, 512, 2><<<grid, th, 0, s>>>(A);
-    else if (th <= 768) k_st_factor_solve<T, 768, 1><<<grid, th, 0, s>>>(A);
+    else if (th <= kWide) k_st_factor_solve<T, kWide, 1><<<grid, th, 0, s>>>(A);
     else k_st_factor_solve<T, 1024, 1><<<grid, th, 0, s>>>(A);
 }
 
