@@ -292,6 +292,17 @@ def test_forward_inner_refinement(cfg, batch):
     # one sweep against the oracle's mixed loop with one sweep
     ctx1 = make_ctx(net, max_batch=batch, mode=sb.STAGED, precision=sb.MIXED, keep_factors=True, ir_sweeps=1)
     res1 = to_np(ctx1.solve(dev(ps), dev(qs), dev(vs), tol=c.tol, max_it=c.max_it))
+    # the factors kept after a refined solve serve the adjoint as after a plain one (the sweeps' triangular solves leave them
+    # alone): refined adjoint at the FP64 tolerance of test_adjoint_refined
+    gva, gvm = S.make_adjoint_rhs(net, batch=batch)
+    lp, lq = ctx1.adjoint_refined(dev(res1["vm"]), dev(res1["va"]), dev(gva), dev(gvm), sweeps=2)
+    rp, rq, _ = oracle.adjoint_batch(Y, net.bus_type, res1["vm"], res1["va"], gva, gvm, method=1)
+    scale = np.maximum(1.0, np.maximum(np.abs(rp).max(axis=1), np.abs(rq).max(axis=1)))
+    assert (np.abs(lp.cpu().numpy() - rp).max(axis=1) <= 1e-8 * scale).all() and (np.abs(lq.cpu().numpy() - rq).max(axis=1) <= 1e-8 * scale).all()
+    # host-buffer call (one chunk in staged mode): the device call bit for bit
+    hres = ctx1.solve_host(ps, qs, vs, tol=c.tol, max_it=c.max_it)
+    for k in ("vm", "va", "iterations", "converged", "final_norm"):
+        assert np.array_equal(np.asarray(hres[k]), res1[k]), k
     ctx1.close()
     for b in (0, batch // 2, batch - 1):
         o1 = oracle.nr_mixed_ir(Y, net.bus_type, ps[b], qs[b], vs[b], tol=c.tol, max_it=c.max_it, ir_sweeps=1)
