@@ -320,19 +320,20 @@ def run_oracle(cfg_key, inputs=None, budget_s=12.0):
     c = net.cfg
     adjoint = net_adjoint(net, cfg_key)
     Y = oracle.ybus(net.n_bus, net.f, net.t, net.r, net.x, net.b)
-    cores = os.cpu_count() or 1
+    # all host cores of this process, whatever OMP_NUM_THREADS says (torchrun sets it to 1)
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
     probe = min(c.batch, cores)
     t0 = time.perf_counter()
-    oracle.nr_batch(Y, net.bus_type, ps[:probe], qs[:probe], vs[:probe], tol=c.tol, max_it=c.max_it, method=1)
+    oracle.nr_batch(Y, net.bus_type, ps[:probe], qs[:probe], vs[:probe], tol=c.tol, max_it=c.max_it, method=1, n_threads=cores)
     per_wave = max(time.perf_counter() - t0, 1e-5)
     m = int(min(c.batch, max(probe, cores * int(budget_s / per_wave))))
     reps = int(max(1, min(10_000, budget_s / (per_wave * max(1.0, m / cores)))))
     conv, threads = 0, 1
     t0 = time.perf_counter()
     for _ in range(reps):
-        r = oracle.nr_batch(Y, net.bus_type, ps[:m], qs[:m], vs[:m], tol=c.tol, max_it=c.max_it, method=1)
+        r = oracle.nr_batch(Y, net.bus_type, ps[:m], qs[:m], vs[:m], tol=c.tol, max_it=c.max_it, method=1, n_threads=cores)
         if adjoint:
-            oracle.adjoint_batch(Y, net.bus_type, r["vm"], r["va"], gva[:m], gvm[:m], method=1)
+            oracle.adjoint_batch(Y, net.bus_type, r["vm"], r["va"], gva[:m], gvm[:m], method=1, n_threads=cores)
         conv += int(r["converged"].sum())
         threads = int(r["threads"])
     dt = time.perf_counter() - t0
