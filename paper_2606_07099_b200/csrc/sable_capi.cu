@@ -887,6 +887,15 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     R.vm = vm; R.va = va; R.p_inj = p_inj; R.q_inj = q_inj; R.work = ctx->work; R.work_stride = ctx->work_stride;
     const size_t sm = (size_t)ctx->T.n_bus * 16;
     R.v_in_smem = sm <= 160 * 1024;            // else the scenario's workspace slice (>= 3 (n_bus) 16 bytes) holds V
+    if (ctx->placement == 2 && sm > 64 * 1024 && (size_t)batch * ctx->T.n_bus >= ((size_t)1 << 18)) {
+        // large grids (V would take most of an SM's shared memory) with an HBM workspace: two launches over all (scenario, bus) pairs
+        const int grid = (int)std::min<size_t>(((size_t)batch * ctx->T.n_bus + 255) / 256, 148 * 32);
+        k_recover_flat<0><<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(R);
+        k_recover_flat<1><<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(R);
+        ctx->launches += 2;
+        CU(cudaGetLastError());
+        return SABLE_OK;
+    }
     if (R.v_in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_recover, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     const int th = bus_threads(ctx->T.n_bus);
     k_recover<<<batch, th, R.v_in_smem ? sm : 0, (cudaStream_t)cuda_stream>>>(R);
@@ -902,6 +911,16 @@ static sable_status need_lbuf(sable_ctx* ctx) {
     CU(cudaMalloc(&p, 4 * (size_t)ctx->opt.max_batch * ctx->T.n_bus * 8));
     ctx->dev_allocs.push_back(p); ctx->lbuf = (double*)p;
     return SABLE_OK;
+}
+
+// k_layer: a CTA per scenario, scratch in shared memory or (grids too large for that) in the scenario's workspace slice
+static cudaError_t launch_layer(sable_ctx* ctx, LayerArgs& L, int batch, cudaStream_t s) {
+    const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
+    L.in_smem = sm <= 160 * 1024;
+    if (L.in_smem && sm > 48 * 1024) { cudaError_t e = cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); if (e != cudaSuccess) return e; }
+    k_layer<<<batch, bus_threads(ctx->T.n_bus), L.in_smem ? sm : 0, s>>>(L);
+    ctx->launches += 1;
+    return cudaGetLastError();
 }
 
 // ---- implicit-layer backward ----------------------------------------------------------------------------------------
@@ -923,19 +942,12 @@ extern "C" sable_status sable_layer_backward(sable_ctx* ctx, int32_t batch, cons
     L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_pg = gl_pg; L.gl_qg = gl_qg; L.gl_vm = gl_vm; L.gl_va = gl_va;
     L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.lam_p = ctx->lbuf + 2 * n; L.lam_q = ctx->lbuf + 3 * n;
     L.dx_pg = dx_pg; L.dx_vm = dx_vm; L.work = ctx->work; L.work_stride = ctx->work_stride;
-    const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
-    L.in_smem = sm <= 160 * 1024;          // else the scenario's workspace slice (48 n_bus bytes) holds them
-    if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const int th = bus_threads(ctx->T.n_bus);
     L.post = 0;
-    k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
-    CU(cudaGetLastError());
+    CU(launch_layer(ctx, L, batch, s));
     st = launch_lin(ctx, 0, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, true, s);
     if (st != SABLE_OK) return st;
     L.post = 1;
-    k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);
-    ctx->launches += 2;
-    CU(cudaGetLastError());
+    CU(launch_layer(ctx, L, batch, s));
     return SABLE_OK;
 }
 
@@ -960,18 +972,13 @@ extern "C" sable_status sable_adjoint_refined(sable_ctx* ctx, int32_t batch, con
     L.n_bus = ctx->T.n_bus; L.batch = batch; L.fptr = ctx->fptr; L.fcol = ctx->fcol; L.ftpos = ctx->ftpos; L.fgb = ctx->fgb;
     L.bus_type = ctx->d_bus_type; L.vm = vm; L.va = va; L.gl_va = g_va; L.gl_vm = g_vm; L.lam_p = lam_p; L.lam_q = lam_q;
     L.g_va = ctx->lbuf; L.g_vm = ctx->lbuf + n; L.work = ctx->work; L.work_stride = ctx->work_stride; L.post = 2;
-    const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
-    L.in_smem = sm <= 160 * 1024;
-    if (L.in_smem && sm > 48 * 1024) CU(cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
-    const int th = bus_threads(ctx->T.n_bus);
     for (int it = 0; it < sweeps; ++it) {
-        k_layer<<<batch, th, L.in_smem ? sm : 0, s>>>(L);                                   // r = g - J1^T lambda   (FP64)
-        CU(cudaGetLastError());
+        CU(launch_layer(ctx, L, batch, s));                                                 // r = g - J1^T lambda   (FP64)
         st = launch_lin(ctx, 0, batch, L.g_va, L.g_vm, 1, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, false, s);   // J1^T d = r  (kept factors)
         if (st != SABLE_OK) return st;
         k_add2<<<(int)std::min<size_t>((nb + 255) / 256, 4096), 256, 0, s>>>(lam_p, lam_q, ctx->lbuf + 2 * n, ctx->lbuf + 3 * n, nb);
         CU(cudaGetLastError());
-        ctx->launches += 2;
+        ctx->launches += 1;
     }
     return SABLE_OK;
 }

@@ -312,6 +312,34 @@ __global__ void k_recover(const RecoverArgs A) {
     }
 }
 
+// the same as two launches over all (scenario, bus) pairs with V in the scenarios' workspace slices: for grids whose V takes
+// most of an SM's shared memory (one CTA per SM, a batch of a few hundred scenarios in two waves: config 5 0.27 -> 0.15 ms;
+// smaller grids are faster with the CTA per scenario: config 4 0.14 against 0.17, config 3 0.08 against 0.09)
+template <int kPass>
+__global__ void k_recover_flat(const RecoverArgs A) {
+    const size_t total = (size_t)A.batch * A.n_bus;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int b = (int)(idx / A.n_bus), i = (int)(idx - (size_t)b * A.n_bus);
+        double2* v = reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
+        if (kPass == 0) {
+            double sn, cs; sincos(A.va[idx], &sn, &cs);
+            const double m = A.vm[idx];
+            v[i] = make_double2(m * cs, m * sn);
+        } else {
+            double ire = 0.0, iim = 0.0;
+            const int k1 = A.fptr[i + 1];
+            for (int k = A.fptr[i]; k < k1; ++k) {
+                const double2 y = A.fgb[k], x = v[A.fcol[k]];
+                ire += y.x * x.x - y.y * x.y;
+                iim += y.y * x.x + y.x * x.y;
+            }
+            const double2 vi = v[i];
+            A.p_inj[idx] = vi.x * ire + vi.y * iim;
+            A.q_inj[idx] = vi.y * ire - vi.x * iim;
+        }
+    }
+}
+
 // ---- implicit-layer backward (eqs. 10-16) around the adjoint solve ---------------------------------
 // Layer: x = [p_g at PV; Vm at PV and slack] -> y = [p_g, q_g at PV and slack; Vm; theta] through Step 1 (F1 = 0) and
 // Step 2 (recovery).  With F = S_calc - S_spec (this repository's sign):
@@ -341,6 +369,83 @@ __device__ __forceinline__ void jac_entry(double2 y, double2 vi, double2 vj, dou
     dP_dth = u1; dP_dvm = u2 * iv; dQ_dth = -u2; dQ_dvm = u1 * iv;
 }
 
+// The three passes of k_layer for one bus of scenario b (o = b * n_bus; v, pq, w: the scenario's scratch arrays)
+__device__ __forceinline__ void layer_pass_state(const LayerArgs& A, size_t o, int i, double2* v, double2* w) {
+    double sn, cs; sincos(A.va[o + i], &sn, &cs);
+    const double vm = A.vm[o + i];
+    v[i] = make_double2(vm * cs, vm * sn);
+    const int ti = A.bus_type[i];
+    if (!A.post) w[i] = make_double2(ti == 2 ? A.gl_pg[o + i] : 0.0, ti != 0 ? A.gl_qg[o + i] : 0.0);   // rows of z2: P at the slack, Q at PV / slack
+    else         w[i] = make_double2(ti != 2 ? A.lam_p[o + i] : 0.0, ti == 0 ? A.lam_q[o + i] : 0.0);   // rows of J1: P non-slack, Q at PQ
+}
+__device__ __forceinline__ void layer_pass_injections(const LayerArgs& A, int i, const double2* v, double2* pq) {
+    double ire = 0.0, iim = 0.0;
+    for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
+        const double2 y = A.fgb[k], x = v[A.fcol[k]];
+        ire += y.x * x.x - y.y * x.y;  iim += y.y * x.x + y.x * x.y;
+    }
+    pq[i] = make_double2(v[i].x * ire + v[i].y * iim, v[i].y * ire - v[i].x * iim);
+}
+__device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o, int j, const double2* v, const double2* pq, const double2* w) {
+    const int tj = A.bus_type[j];
+    const double vmj = A.vm[o + j];
+    if (!A.post) {
+        double vth = 0.0, vvm = 0.0;
+        for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+            const int i = A.fcol[k], ti = A.bus_type[i];
+            if (ti == 0) continue;                                   // rows of z2 sit at PV and slack buses only
+            const double ai = w[i].x, ci = w[i].y;
+            double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+            if (i == j) {
+                const double2 y = A.fgb[k], s = pq[i];
+                dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
+                dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
+            } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+            vth += ai * dP_dth + ci * dQ_dth;
+            vvm += ai * dP_dvm + ci * dQ_dvm;
+        }
+        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + vth : 0.0;
+        A.g_vm[o + j] = A.gl_vm[o + j] + vvm;
+    } else if (A.post == 2) {
+        // residual of eq. 14 in FP64, r = g - J1^T lambda (here gl_va / gl_vm = g, output g_va / g_vm = r): column
+        // theta_j of every non-slack bus, column Vm_j of every PQ bus; rows P_i (non-slack), Q_i (PQ)
+        double sth = 0.0, svm = 0.0;
+        if (tj != 2)
+            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+                const int i = A.fcol[k], ti = A.bus_type[i];
+                if (ti == 2) continue;
+                const double lp = w[i].x, lq = w[i].y;
+                double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+                if (i == j) {
+                    const double2 y = A.fgb[k], s = pq[i];
+                    dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
+                    dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
+                } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+                sth += lp * dP_dth + lq * dQ_dth;
+                svm += lp * dP_dvm + lq * dQ_dvm;
+            }
+        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] - sth : 0.0;
+        A.g_vm[o + j] = tj == 0 ? A.gl_vm[o + j] - svm : 0.0;
+    } else {
+        double sacc = 0.0;
+        if (tj != 0)
+            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+                const int i = A.fcol[k];
+                const double lp = w[i].x, lq = w[i].y;
+                double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
+                if (i == j) {
+                    const double2 y = A.fgb[k], s = pq[i];
+                    dP_dvm = s.x / vmj + y.x * vmj;  dQ_dvm = s.y / vmj - y.y * vmj;
+                } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
+                sacc += lp * dP_dvm + lq * dQ_dvm;
+            }
+        A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - sacc : 0.0;
+        A.dx_pg[o + j] = tj == 1 ? A.gl_pg[o + j] + A.lam_p[o + j] : 0.0;
+    }
+}
+
+// one CTA per scenario; scratch in shared memory, or (grids whose 48 n_bus bytes do not fit) in the scenario's workspace slice.
+// (The three passes as three launches over all (scenario, bus) pairs were measured on config 5: 0.42 ms against 0.40.)
 __global__ void k_layer(const LayerArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int b = blockIdx.x, nb = A.n_bus;
@@ -348,81 +453,11 @@ __global__ void k_layer(const LayerArgs A) {
     double2* v = A.in_smem ? reinterpret_cast<double2*>(smem) : reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
     double2* pq = v + nb;
     double2* w = pq + nb;                  // per bus i: the two row weights the transposed products gather (coalesced here)
-    const double* vm = A.vm + o;
-    for (int i = threadIdx.x; i < nb; i += blockDim.x) {
-        double sn, cs; sincos(A.va[o + i], &sn, &cs);
-        v[i] = make_double2(vm[i] * cs, vm[i] * sn);
-        const int ti = A.bus_type[i];
-        if (!A.post) w[i] = make_double2(ti == 2 ? A.gl_pg[o + i] : 0.0, ti != 0 ? A.gl_qg[o + i] : 0.0);   // rows of z2: P at the slack, Q at PV / slack
-        else         w[i] = make_double2(ti != 2 ? A.lam_p[o + i] : 0.0, ti == 0 ? A.lam_q[o + i] : 0.0);   // rows of J1: P non-slack, Q at PQ
-    }
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) layer_pass_state(A, o, i, v, w);
     __syncthreads();
-    for (int i = threadIdx.x; i < nb; i += blockDim.x) {
-        double ire = 0.0, iim = 0.0;
-        for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
-            const double2 y = A.fgb[k], x = v[A.fcol[k]];
-            ire += y.x * x.x - y.y * x.y;  iim += y.y * x.x + y.x * x.y;
-        }
-        pq[i] = make_double2(v[i].x * ire + v[i].y * iim, v[i].y * ire - v[i].x * iim);
-    }
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) layer_pass_injections(A, i, v, pq);
     __syncthreads();
-    for (int j = threadIdx.x; j < nb; j += blockDim.x) {
-        const int tj = A.bus_type[j];
-        const double vmj = vm[j];
-        if (!A.post) {
-            double vth = 0.0, vvm = 0.0;
-            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
-                const int i = A.fcol[k], ti = A.bus_type[i];
-                if (ti == 0) continue;                                   // rows of z2 sit at PV and slack buses only
-                const double ai = w[i].x, ci = w[i].y;
-                double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
-                if (i == j) {
-                    const double2 y = A.fgb[k], s = pq[i];
-                    dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
-                    dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
-                } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-                vth += ai * dP_dth + ci * dQ_dth;
-                vvm += ai * dP_dvm + ci * dQ_dvm;
-            }
-            A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + vth : 0.0;
-            A.g_vm[o + j] = A.gl_vm[o + j] + vvm;
-        } else if (A.post == 2) {
-            // residual of eq. 14 in FP64, r = g - J1^T lambda (here gl_va / gl_vm = g, output g_va / g_vm = r): column
-            // theta_j of every non-slack bus, column Vm_j of every PQ bus; rows P_i (non-slack), Q_i (PQ)
-            double sth = 0.0, svm = 0.0;
-            if (tj != 2)
-                for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
-                    const int i = A.fcol[k], ti = A.bus_type[i];
-                    if (ti == 2) continue;
-                    const double lp = w[i].x, lq = w[i].y;
-                    double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
-                    if (i == j) {
-                        const double2 y = A.fgb[k], s = pq[i];
-                        dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
-                        dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
-                    } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-                    sth += lp * dP_dth + lq * dQ_dth;
-                    svm += lp * dP_dvm + lq * dQ_dvm;
-                }
-            A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] - sth : 0.0;
-            A.g_vm[o + j] = tj == 0 ? A.gl_vm[o + j] - svm : 0.0;
-        } else {
-            double sacc = 0.0;
-            if (tj != 0)
-                for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
-                    const int i = A.fcol[k];
-                    const double lp = w[i].x, lq = w[i].y;
-                    double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
-                    if (i == j) {
-                        const double2 y = A.fgb[k], s = pq[i];
-                        dP_dvm = s.x / vmj + y.x * vmj;  dQ_dvm = s.y / vmj - y.y * vmj;
-                    } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-                    sacc += lp * dP_dvm + lq * dQ_dvm;
-                }
-            A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - sacc : 0.0;
-            A.dx_pg[o + j] = tj == 1 ? A.gl_pg[o + j] + A.lam_p[o + j] : 0.0;
-        }
-    }
+    for (int j = threadIdx.x; j < nb; j += blockDim.x) layer_pass_columns(A, o, j, v, pq, w);
 }
 
 // lambda += correction (iterative refinement of the adjoint, sable_adjoint_refined)

@@ -858,6 +858,30 @@ def test_step2_recovery_large_grid():
     ctx.close()
 
 
+def test_step2_recovery_two_launch_form():
+    """Large grids with a batch of some size (batch x n_bus >= 2^18, V above 64 KB) take the form with two launches over all
+    (scenario, bus) pairs and V in the workspace slices: config 5's grid with a ragged batch against the oracle, and
+    against the CTA-per-scenario form (a small batch of the same states)."""
+    net, Y = get_net(5)
+    batch = 33
+    vm, va = random_state(net, batch, 77)
+    ctx = make_ctx(net, max_batch=batch, keep_factors=False)
+    l0 = ctx.launch_count()
+    p_inj, q_inj = ctx.recover(dev(vm), dev(va))
+    assert ctx.launch_count() - l0 == 2
+    l0 = ctx.launch_count()
+    p3, q3 = ctx.recover(dev(vm[:3]), dev(va[:3]))
+    assert ctx.launch_count() - l0 == 1
+    p_inj, q_inj, p3, q3 = (a.cpu().numpy() for a in (p_inj, q_inj, p3, q3))
+    sc = row_scale(Y, vm)
+    for b in range(0, batch, 4):
+        P, Q = oracle.injections(Y, vm[b], va[b])
+        assert (np.abs(p_inj[b] - P) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+        assert (np.abs(q_inj[b] - Q) <= 1e-13 * np.maximum(sc[b], 1.0)).all()
+    assert (np.abs(p_inj[:3] - p3) <= 1e-14 * np.maximum(sc[:3], 1.0)).all() and (np.abs(q_inj[:3] - q3) <= 1e-14 * np.maximum(sc[:3], 1.0)).all()
+    ctx.close()
+
+
 # ---- NEXT row 2: implicit-layer backward (PAPER.md eqs. 10-16) ------------------------------------------------------------
 @pytest.mark.parametrize("cfg,batch", [(1, 16), (2, 12), (3, 6)])
 def test_layer_backward(cfg, batch):
