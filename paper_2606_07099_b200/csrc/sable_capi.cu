@@ -24,6 +24,7 @@ struct sable_ctx {
     const int32_t* fptr = nullptr; const int32_t* fcol = nullptr; const double2* fgb = nullptr;   // full Y_bus, bus order
     const int32_t* ftpos = nullptr; const uint8_t* d_bus_type = nullptr; double* lbuf = nullptr;   // layer backward (lbuf: lazily allocated)
     const int32_t* d_bus_node = nullptr;   // ir_sweeps > 0: node of each bus
+    const int32_t* d_long = nullptr; int n_long = 0;   // buses whose Y_bus row has more than 32 entries (warp-served in the bus-order kernels)
     double* irbuf = nullptr;       // ir_sweeps > 0: nine [max_batch][n_bus] arrays (V re/im, |V|, step, residual, correction), allocated at create
     unsigned long long* tim = nullptr;                       // tuning.timing: per-phase cycle counters of CTA 0
     int64_t fac_stride = 0, work_stride = 0;                 // bytes per scenario
@@ -564,6 +565,10 @@ extern "C" sable_status sable_create(int32_t n_bus, const int32_t* row_ptr, cons
         std::vector<uint8_t> bt(bus_type, bus_type + n_bus);
         up(tpos, &c->ftpos); up(bt, &c->d_bus_type);
         if (o.ir_sweeps > 0) up(T.bus_node, &c->d_bus_node);
+        std::vector<int32_t> longr;
+        for (int i = 0; i < T.n_bus; ++i) if (T.fptr[i + 1] - T.fptr[i] > 32) longr.push_back(i);
+        c->n_long = (int)longr.size();
+        if (c->n_long) up(longr, &c->d_long);
     }
     up(mm_row, &d.mm_row); up(node_bus, &d.node_bus); up(T.node_pq, &d.node_pq); up(T.yptr, &d.yptr);
     up(T.ycol, &d.ycol); up(ycd, &d.ycd); up(ygb, &d.ygb); up(jmj, &d.jp_mj); up(jy, &d.jp_y);
@@ -753,7 +758,7 @@ static cudaError_t launch_solve(sable_ctx* c, SolveArgs A, int b0, int nb, int c
         IrArgs R{};
         R.n_bus = c->T.n_bus; R.batch = nb; R.fptr = c->fptr; R.fcol = c->fcol; R.fgb = c->fgb; R.bus_type = c->d_bus_type;
         R.status = A.status; R.p_spec = A.p_spec; R.q_spec = A.q_spec; R.v = A.ir_v; R.vm = A.ir_vm; R.dzp = A.ir_dzp; R.dzq = A.ir_dzq;
-        R.rp = c->irbuf + 5 * n + o; R.rq = c->irbuf + 6 * n + o;
+        R.rp = c->irbuf + 5 * n + o; R.rq = c->irbuf + 6 * n + o; R.long_rows = c->d_long; R.n_long = c->n_long;
         for (int sw = 0; sw < c->opt.ir_sweeps; ++sw) {
             k_ir_residual<<<fb, 256, 0, s>>>(R);
             if (launch_lin(c, b0, nb, c->irbuf + 5 * n, c->irbuf + 6 * n, 0, c->irbuf + 7 * n, c->irbuf + 8 * n, false, s) != SABLE_OK)
@@ -885,6 +890,7 @@ extern "C" sable_status sable_recover(sable_ctx* ctx, int32_t batch, const doubl
     RecoverArgs R{};
     R.n_bus = ctx->T.n_bus; R.batch = batch; R.fptr = ctx->fptr; R.fcol = ctx->fcol; R.fgb = ctx->fgb;
     R.vm = vm; R.va = va; R.p_inj = p_inj; R.q_inj = q_inj; R.work = ctx->work; R.work_stride = ctx->work_stride;
+    R.long_rows = ctx->d_long; R.n_long = ctx->n_long;
     const size_t sm = (size_t)ctx->T.n_bus * 16;
     R.v_in_smem = sm <= 160 * 1024;            // else the scenario's workspace slice (>= 3 (n_bus) 16 bytes) holds V
     if (ctx->placement == 2 && sm > 64 * 1024 && (size_t)batch * ctx->T.n_bus >= ((size_t)1 << 18)) {
@@ -917,6 +923,7 @@ static sable_status need_lbuf(sable_ctx* ctx) {
 static cudaError_t launch_layer(sable_ctx* ctx, LayerArgs& L, int batch, cudaStream_t s) {
     const size_t sm = (size_t)ctx->T.n_bus * 48;       // V, (P, Q), row weights
     L.in_smem = sm <= 160 * 1024;
+    L.long_rows = ctx->d_long; L.n_long = ctx->n_long;
     if (L.in_smem && sm > 48 * 1024) { cudaError_t e = cudaFuncSetAttribute((const void*)k_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); if (e != cudaSuccess) return e; }
     k_layer<<<batch, bus_threads(ctx->T.n_bus), L.in_smem ? sm : 0, s>>>(L);
     ctx->launches += 1;

@@ -166,41 +166,55 @@ struct IrArgs {
     const double2* v;
     const double *vm, *dzp, *dzq;
     double *rp, *rq;                  // out: r = -F1 - J1 dz, rows P (non-slack) and Q (PQ); zero elsewhere and for finished scenarios
+    const int32_t* long_rows; int32_t n_long;   // buses whose Y_bus row has more than kLongRowIr entries
 };
 
-// one row of Y_bus per thread: the row sum gives the calculated injection (F1 row, eq. 6) and, entry by entry, the
-// off-diagonal blocks of J1 applied to the neighbour's step; the diagonal block uses the calculated P_i, Q_i
+// one row of Y_bus per thread (a whole warp for rows above kLongRowIr entries): the row sum gives the calculated injection
+// (F1 row, eq. 6) and, entry by entry, the off-diagonal blocks of J1 applied to the neighbour's step; the diagonal block uses
+// the calculated P_i, Q_i
+constexpr int kLongRowIr = 32;
+__device__ __forceinline__ double warp_sum_ir(double x) {
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+__device__ __forceinline__ void ir_row(const IrArgs& A, int b, int i, bool warp) {
+    const size_t o = (size_t)b * A.n_bus;
+    const int ti = A.bus_type[i], lane = threadIdx.x & 31;
+    double rp = 0.0, rq = 0.0;
+    if (ti != 2 && A.status[b] == 0) {
+        const double2 vi = A.v[o + i];
+        double ire = 0.0, iim = 0.0, ap = 0.0, aq = 0.0, ydx = 0.0, ydy = 0.0;
+        for (int k = A.fptr[i] + (warp ? lane : 0); k < A.fptr[i + 1]; k += warp ? 32 : 1) {
+            const int j = A.fcol[k];
+            const double2 y = A.fgb[k], x = A.v[o + j];
+            const double tr = y.x * x.x - y.y * x.y, tim = y.y * x.x + y.x * x.y;
+            ire += tr; iim += tim;
+            if (j == i) { ydx = y.x; ydy = y.y; continue; }
+            const double u2 = vi.x * tr + vi.y * tim, u1 = vi.y * tr - vi.x * tim;
+            const double dth = A.dzp[o + j], dvm = A.dzq[o + j] / A.vm[o + j];            // zero where the column is not in z1
+            ap += u1 * dth + u2 * dvm;
+            aq += -u2 * dth + u1 * dvm;
+        }
+        if (warp) { ire = warp_sum_ir(ire); iim = warp_sum_ir(iim); ap = warp_sum_ir(ap); aq = warp_sum_ir(aq); ydx = warp_sum_ir(ydx); ydy = warp_sum_ir(ydy); }
+        const double P = vi.x * ire + vi.y * iim, Q = vi.y * ire - vi.x * iim;
+        const double vm = A.vm[o + i], v2 = vm * vm, dth = A.dzp[o + i], dvm = A.dzq[o + i];
+        ap += (-Q - ydy * v2) * dth + (P / vm + ydx * vm) * dvm;
+        aq += (P - ydx * v2) * dth + (Q / vm - ydy * vm) * dvm;
+        rp = (A.p_spec[o + i] - P) - ap;
+        if (ti == 0) rq = (A.q_spec[o + i] - Q) - aq;
+    }
+    if (warp && lane) return;
+    A.rp[o + i] = rp; A.rq[o + i] = rq;
+}
 __global__ void k_ir_residual(const IrArgs A) {
     const size_t total = (size_t)A.batch * A.n_bus;
     for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
         const int b = (int)(idx / A.n_bus), i = (int)(idx - (size_t)b * A.n_bus);
-        const size_t o = (size_t)b * A.n_bus;
-        const int ti = A.bus_type[i];
-        double rp = 0.0, rq = 0.0;
-        if (ti != 2 && A.status[b] == 0) {
-            const double2 vi = A.v[o + i];
-            double ire = 0.0, iim = 0.0, ap = 0.0, aq = 0.0;
-            double2 yd = make_double2(0.0, 0.0);
-            for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
-                const int j = A.fcol[k];
-                const double2 y = A.fgb[k], x = A.v[o + j];
-                const double tr = y.x * x.x - y.y * x.y, tim = y.y * x.x + y.x * x.y;
-                ire += tr; iim += tim;
-                if (j == i) { yd = y; continue; }
-                const double u2 = vi.x * tr + vi.y * tim, u1 = vi.y * tr - vi.x * tim;
-                const double dth = A.dzp[o + j], dvm = A.dzq[o + j] / A.vm[o + j];            // zero where the column is not in z1
-                ap += u1 * dth + u2 * dvm;
-                aq += -u2 * dth + u1 * dvm;
-            }
-            const double P = vi.x * ire + vi.y * iim, Q = vi.y * ire - vi.x * iim;
-            const double vm = A.vm[o + i], v2 = vm * vm, dth = A.dzp[o + i], dvm = A.dzq[o + i];
-            ap += (-Q - yd.y * v2) * dth + (P / vm + yd.x * vm) * dvm;
-            aq += (P - yd.x * v2) * dth + (Q / vm - yd.y * vm) * dvm;
-            rp = (A.p_spec[o + i] - P) - ap;
-            if (ti == 0) rq = (A.q_spec[o + i] - Q) - aq;
-        }
-        A.rp[idx] = rp; A.rq[idx] = rq;
+        if (A.fptr[i + 1] - A.fptr[i] <= kLongRowIr) ir_row(A, b, i, false);
     }
+    const size_t nw = ((size_t)gridDim.x * blockDim.x) >> 5, tot = (size_t)A.batch * A.n_long;
+    for (size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < tot; w += nw)
+        ir_row(A, (int)(w / A.n_long), A.long_rows[w % A.n_long], true);
 }
 
 // ---- adjoint / generic linear solve on stored factors ---------------------------------------------------------
@@ -285,7 +299,34 @@ struct RecoverArgs {
     const double *vm, *va;             // [batch][n_bus]
     double *p_inj, *q_inj;             // [batch][n_bus]
     char* work; int64_t work_stride;   // used when V does not fit shared memory
+    const int32_t* long_rows; int32_t n_long;   // buses whose Y_bus row has more than kLongRow entries (served by a whole warp)
 };
+
+// A row of Y_bus with hundreds of entries (a hub bus) walked by one thread is a chain of dependent gathers that alone takes
+// longer than everything else in these kernels (config 5: longest row 322 entries, ~0.1 ms): rows above kLongRow entries are
+// left out of the thread-per-row passes and served by a whole warp each (lanes take every 32nd entry, shuffle reduction).
+constexpr int kLongRow = 32;
+__device__ __forceinline__ double warp_sum(double x) {
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+// I_i = sum_k Y_ik V_k over the entries k0, k0 + ks, ... of row i
+__device__ __forceinline__ void row_current(const int32_t* fcol, const double2* fgb, const double2* v, int k0, int k1, int ks, double& ire, double& iim) {
+    for (int k = k0; k < k1; k += ks) {
+        const double2 y = fgb[k], x = v[fcol[k]];
+        ire += y.x * x.x - y.y * x.y;
+        iim += y.y * x.x + y.x * x.y;
+    }
+}
+__device__ __forceinline__ void recover_row(const RecoverArgs& A, size_t o, int i, const double2* v, bool warp) {
+    const int k0 = A.fptr[i], k1 = A.fptr[i + 1], lane = threadIdx.x & 31;
+    double ire = 0.0, iim = 0.0;
+    row_current(A.fcol, A.fgb, v, warp ? k0 + lane : k0, k1, warp ? 32 : 1, ire, iim);
+    if (warp) { ire = warp_sum(ire); iim = warp_sum(iim); if (lane) return; }
+    const double2 vi = v[i];
+    A.p_inj[o + i] = vi.x * ire + vi.y * iim;
+    A.q_inj[o + i] = vi.y * ire - vi.x * iim;
+}
 
 __global__ void k_recover(const RecoverArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -298,23 +339,13 @@ __global__ void k_recover(const RecoverArgs A) {
         v[i] = make_double2(m * cs, m * sn);
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < A.n_bus; i += blockDim.x) {
-        double ire = 0.0, iim = 0.0;
-        const int k1 = A.fptr[i + 1];
-        for (int k = A.fptr[i]; k < k1; ++k) {
-            const double2 y = A.fgb[k], x = v[A.fcol[k]];
-            ire += y.x * x.x - y.y * x.y;
-            iim += y.y * x.x + y.x * x.y;
-        }
-        const double2 vi = v[i];
-        A.p_inj[o + i] = vi.x * ire + vi.y * iim;
-        A.q_inj[o + i] = vi.y * ire - vi.x * iim;
-    }
+    for (int i = threadIdx.x; i < A.n_bus; i += blockDim.x)
+        if (A.fptr[i + 1] - A.fptr[i] <= kLongRow) recover_row(A, o, i, v, false);
+    for (int r = threadIdx.x >> 5; r < A.n_long; r += blockDim.x >> 5) recover_row(A, o, A.long_rows[r], v, true);
 }
 
 // the same as two launches over all (scenario, bus) pairs with V in the scenarios' workspace slices: for grids whose V takes
-// most of an SM's shared memory (one CTA per SM, a batch of a few hundred scenarios in two waves: config 5 0.27 -> 0.15 ms;
-// smaller grids are faster with the CTA per scenario: config 4 0.14 against 0.17, config 3 0.08 against 0.09)
+// most of an SM's shared memory (one CTA per SM, a batch of a few hundred scenarios in two waves)
 template <int kPass>
 __global__ void k_recover_flat(const RecoverArgs A) {
     const size_t total = (size_t)A.batch * A.n_bus;
@@ -325,17 +356,13 @@ __global__ void k_recover_flat(const RecoverArgs A) {
             double sn, cs; sincos(A.va[idx], &sn, &cs);
             const double m = A.vm[idx];
             v[i] = make_double2(m * cs, m * sn);
-        } else {
-            double ire = 0.0, iim = 0.0;
-            const int k1 = A.fptr[i + 1];
-            for (int k = A.fptr[i]; k < k1; ++k) {
-                const double2 y = A.fgb[k], x = v[A.fcol[k]];
-                ire += y.x * x.x - y.y * x.y;
-                iim += y.y * x.x + y.x * x.y;
-            }
-            const double2 vi = v[i];
-            A.p_inj[idx] = vi.x * ire + vi.y * iim;
-            A.q_inj[idx] = vi.y * ire - vi.x * iim;
+        } else if (A.fptr[i + 1] - A.fptr[i] <= kLongRow) recover_row(A, (size_t)b * A.n_bus, i, v, false);
+    }
+    if (kPass == 1) {
+        const size_t nw = ((size_t)gridDim.x * blockDim.x) >> 5, tot = (size_t)A.batch * A.n_long;
+        for (size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < tot; w += nw) {
+            const int b = (int)(w / A.n_long), r = (int)(w - (size_t)b * A.n_long);
+            recover_row(A, (size_t)b * A.n_bus, A.long_rows[r], reinterpret_cast<const double2*>(A.work + (size_t)b * A.work_stride), true);
         }
     }
 }
@@ -360,6 +387,7 @@ struct LayerArgs {
     const double *lam_p, *lam_q;             // post: in
     double *dx_pg, *dx_vm;                   // post: out
     char* work; int64_t work_stride;
+    const int32_t* long_rows; int32_t n_long;   // buses whose Y_bus row has more than kLongRow entries (served by a whole warp)
 };
 
 __device__ __forceinline__ void jac_entry(double2 y, double2 vi, double2 vj, double vmj, double& dP_dth, double& dP_dvm,
@@ -378,20 +406,21 @@ __device__ __forceinline__ void layer_pass_state(const LayerArgs& A, size_t o, i
     if (!A.post) w[i] = make_double2(ti == 2 ? A.gl_pg[o + i] : 0.0, ti != 0 ? A.gl_qg[o + i] : 0.0);   // rows of z2: P at the slack, Q at PV / slack
     else         w[i] = make_double2(ti != 2 ? A.lam_p[o + i] : 0.0, ti == 0 ? A.lam_q[o + i] : 0.0);   // rows of J1: P non-slack, Q at PQ
 }
-__device__ __forceinline__ void layer_pass_injections(const LayerArgs& A, int i, const double2* v, double2* pq) {
+// (warp = true: the row is served by a whole warp, see kLongRow)
+__device__ __forceinline__ void layer_pass_injections(const LayerArgs& A, int i, const double2* v, double2* pq, bool warp) {
+    const int k0 = A.fptr[i], k1 = A.fptr[i + 1], lane = threadIdx.x & 31;
     double ire = 0.0, iim = 0.0;
-    for (int k = A.fptr[i]; k < A.fptr[i + 1]; ++k) {
-        const double2 y = A.fgb[k], x = v[A.fcol[k]];
-        ire += y.x * x.x - y.y * x.y;  iim += y.y * x.x + y.x * x.y;
-    }
+    row_current(A.fcol, A.fgb, v, warp ? k0 + lane : k0, k1, warp ? 32 : 1, ire, iim);
+    if (warp) { ire = warp_sum(ire); iim = warp_sum(iim); if (lane) return; }
     pq[i] = make_double2(v[i].x * ire + v[i].y * iim, v[i].y * ire - v[i].x * iim);
 }
-__device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o, int j, const double2* v, const double2* pq, const double2* w) {
-    const int tj = A.bus_type[j];
+__device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o, int j, const double2* v, const double2* pq, const double2* w, bool warp) {
+    const int tj = A.bus_type[j], lane = threadIdx.x & 31;
     const double vmj = A.vm[o + j];
+    const int k0 = warp ? A.fptr[j] + lane : A.fptr[j], k1 = A.fptr[j + 1], ks = warp ? 32 : 1;
+    double a1 = 0.0, a2 = 0.0;             // the two column sums (theta_j / Vm_j), rows weighted by w
     if (!A.post) {
-        double vth = 0.0, vvm = 0.0;
-        for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+        for (int k = k0; k < k1; k += ks) {
             const int i = A.fcol[k], ti = A.bus_type[i];
             if (ti == 0) continue;                                   // rows of z2 sit at PV and slack buses only
             const double ai = w[i].x, ci = w[i].y;
@@ -401,17 +430,14 @@ __device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o,
                 dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
                 dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
             } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-            vth += ai * dP_dth + ci * dQ_dth;
-            vvm += ai * dP_dvm + ci * dQ_dvm;
+            a1 += ai * dP_dth + ci * dQ_dth;
+            a2 += ai * dP_dvm + ci * dQ_dvm;
         }
-        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + vth : 0.0;
-        A.g_vm[o + j] = A.gl_vm[o + j] + vvm;
     } else if (A.post == 2) {
         // residual of eq. 14 in FP64, r = g - J1^T lambda (here gl_va / gl_vm = g, output g_va / g_vm = r): column
         // theta_j of every non-slack bus, column Vm_j of every PQ bus; rows P_i (non-slack), Q_i (PQ)
-        double sth = 0.0, svm = 0.0;
         if (tj != 2)
-            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+            for (int k = k0; k < k1; k += ks) {
                 const int i = A.fcol[k], ti = A.bus_type[i];
                 if (ti == 2) continue;
                 const double lp = w[i].x, lq = w[i].y;
@@ -421,15 +447,12 @@ __device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o,
                     dP_dth = -s.y - y.y * vmj * vmj;  dP_dvm = s.x / vmj + y.x * vmj;
                     dQ_dth = s.x - y.x * vmj * vmj;   dQ_dvm = s.y / vmj - y.y * vmj;
                 } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-                sth += lp * dP_dth + lq * dQ_dth;
-                svm += lp * dP_dvm + lq * dQ_dvm;
+                a1 += lp * dP_dth + lq * dQ_dth;
+                a2 += lp * dP_dvm + lq * dQ_dvm;
             }
-        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] - sth : 0.0;
-        A.g_vm[o + j] = tj == 0 ? A.gl_vm[o + j] - svm : 0.0;
     } else {
-        double sacc = 0.0;
         if (tj != 0)
-            for (int k = A.fptr[j]; k < A.fptr[j + 1]; ++k) {
+            for (int k = k0; k < k1; k += ks) {
                 const int i = A.fcol[k];
                 const double lp = w[i].x, lq = w[i].y;
                 double dP_dth, dP_dvm, dQ_dth, dQ_dvm;
@@ -437,27 +460,41 @@ __device__ __forceinline__ void layer_pass_columns(const LayerArgs& A, size_t o,
                     const double2 y = A.fgb[k], s = pq[i];
                     dP_dvm = s.x / vmj + y.x * vmj;  dQ_dvm = s.y / vmj - y.y * vmj;
                 } else jac_entry(A.fgb[A.ftpos[k]], v[i], v[j], vmj, dP_dth, dP_dvm, dQ_dth, dQ_dvm);
-                sacc += lp * dP_dvm + lq * dQ_dvm;
+                a2 += lp * dP_dvm + lq * dQ_dvm;
             }
-        A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - sacc : 0.0;
+    }
+    if (warp) { a1 = warp_sum(a1); a2 = warp_sum(a2); if (lane) return; }
+    if (!A.post) {
+        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] + a1 : 0.0;
+        A.g_vm[o + j] = A.gl_vm[o + j] + a2;
+    } else if (A.post == 2) {
+        A.g_va[o + j] = tj != 2 ? A.gl_va[o + j] - a1 : 0.0;
+        A.g_vm[o + j] = tj == 0 ? A.gl_vm[o + j] - a2 : 0.0;
+    } else {
+        A.dx_vm[o + j] = tj != 0 ? A.g_vm[o + j] - a2 : 0.0;
         A.dx_pg[o + j] = tj == 1 ? A.gl_pg[o + j] + A.lam_p[o + j] : 0.0;
     }
 }
 
 // one CTA per scenario; scratch in shared memory, or (grids whose 48 n_bus bytes do not fit) in the scenario's workspace slice.
-// (The three passes as three launches over all (scenario, bus) pairs were measured on config 5: 0.42 ms against 0.40.)
+// (The three passes as launches over all (scenario, bus) pairs, in one piece or in L2-sized chunks of scenarios, were measured on
+// config 5: 0.34 ms per call and more against 0.27 -- the row passes re-read the Y entries for every scenario either way.)
 __global__ void k_layer(const LayerArgs A) {
     extern __shared__ __align__(16) unsigned char smem[];
-    const int b = blockIdx.x, nb = A.n_bus;
+    const int b = blockIdx.x, nb = A.n_bus, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const size_t o = (size_t)b * nb;
     double2* v = A.in_smem ? reinterpret_cast<double2*>(smem) : reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
     double2* pq = v + nb;
     double2* w = pq + nb;                  // per bus i: the two row weights the transposed products gather (coalesced here)
     for (int i = threadIdx.x; i < nb; i += blockDim.x) layer_pass_state(A, o, i, v, w);
     __syncthreads();
-    for (int i = threadIdx.x; i < nb; i += blockDim.x) layer_pass_injections(A, i, v, pq);
+    for (int i = threadIdx.x; i < nb; i += blockDim.x)
+        if (A.fptr[i + 1] - A.fptr[i] <= kLongRow) layer_pass_injections(A, i, v, pq, false);
+    for (int r = warp; r < A.n_long; r += nwarp) layer_pass_injections(A, A.long_rows[r], v, pq, true);
     __syncthreads();
-    for (int j = threadIdx.x; j < nb; j += blockDim.x) layer_pass_columns(A, o, j, v, pq, w);
+    for (int j = threadIdx.x; j < nb; j += blockDim.x)
+        if (A.fptr[j + 1] - A.fptr[j] <= kLongRow) layer_pass_columns(A, o, j, v, pq, w, false);
+    for (int r = warp; r < A.n_long; r += nwarp) layer_pass_columns(A, o, A.long_rows[r], v, pq, w, true);
 }
 
 // lambda += correction (iterative refinement of the adjoint, sable_adjoint_refined)
