@@ -178,8 +178,9 @@ sable_status sable_get_pivot_flags(sable_ctx* ctx, int32_t batch, int32_t* flags
  * P_i(V), Q_i(V) of S = V o conj(Y_bus V) for EVERY bus at the given voltages (normally the vm, va of sable_solve):
  * p_inj at the slack is the recovered slack injection, q_inj at PV / slack buses the recovered reactive injections
  * (generation = injection + load); at the other rows they equal the specified values up to the final
- * mismatch.  All DEVICE pointers, [batch][n_bus]; asynchronous on the stream; uses the workspace only for grids above
- * 10 240 buses (then it overwrites the state of the last solve, not the kept factors).
+ * mismatch.  All DEVICE pointers, [batch][n_bus]; asynchronous on the stream; allocates nothing.  Grids above
+ * 4 096 buses with batch x n_bus >= 2^18, and all grids above 10 240 buses, keep V in the context's workspace (that overwrites
+ * the iterate of the last solve there, not the kept factors and not the caller's arrays).
  * Errors: INVALID_ARG, STATE, CUDA. */
 sable_status sable_recover(sable_ctx* ctx, int32_t batch, const double* vm, const double* va, double* p_inj,
                            double* q_inj, void* cuda_stream);
