@@ -346,24 +346,60 @@ __global__ void k_recover(const RecoverArgs A) {
 
 // the same as two launches over all (scenario, bus) pairs with V in the scenarios' workspace slices: for grids whose V takes
 // most of an SM's shared memory (one CTA per SM, a batch of a few hundred scenarios in two waves)
+// (the row pass serves kRecS scenarios per thread: the Y entries of a row are loaded once for all of them, and their gathers
+// are independent loads in flight together)
+constexpr int kRecS = 4;
 template <int kPass>
 __global__ void k_recover_flat(const RecoverArgs A) {
-    const size_t total = (size_t)A.batch * A.n_bus;
-    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
-        const int b = (int)(idx / A.n_bus), i = (int)(idx - (size_t)b * A.n_bus);
-        double2* v = reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
-        if (kPass == 0) {
+    if (kPass == 0) {
+        const size_t total = (size_t)A.batch * A.n_bus;
+        for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+            const int b = (int)(idx / A.n_bus), i = (int)(idx - (size_t)b * A.n_bus);
+            double2* v = reinterpret_cast<double2*>(A.work + (size_t)b * A.work_stride);
             double sn, cs; sincos(A.va[idx], &sn, &cs);
             const double m = A.vm[idx];
             v[i] = make_double2(m * cs, m * sn);
-        } else if (A.fptr[i + 1] - A.fptr[i] <= kLongRow) recover_row(A, (size_t)b * A.n_bus, i, v, false);
-    }
-    if (kPass == 1) {
-        const size_t nw = ((size_t)gridDim.x * blockDim.x) >> 5, tot = (size_t)A.batch * A.n_long;
-        for (size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < tot; w += nw) {
-            const int b = (int)(w / A.n_long), r = (int)(w - (size_t)b * A.n_long);
-            recover_row(A, (size_t)b * A.n_bus, A.long_rows[r], reinterpret_cast<const double2*>(A.work + (size_t)b * A.work_stride), true);
         }
+        return;
+    }
+    const int nbg = (A.batch + kRecS - 1) / kRecS;                       // groups of kRecS scenarios
+    const size_t total = (size_t)nbg * A.n_bus;
+    for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (size_t)gridDim.x * blockDim.x) {
+        const int bg = (int)(idx / A.n_bus), i = (int)(idx - (size_t)bg * A.n_bus);
+        const int k0 = A.fptr[i], k1 = A.fptr[i + 1];
+        if (k1 - k0 > kLongRow) continue;
+        const double2* v[kRecS];
+        double ire[kRecS], iim[kRecS];
+#pragma unroll
+        for (int q = 0; q < kRecS; ++q) {
+            const int b = min(bg * kRecS + q, A.batch - 1);
+            v[q] = reinterpret_cast<const double2*>(A.work + (size_t)b * A.work_stride);
+            ire[q] = 0.0; iim[q] = 0.0;
+        }
+        for (int k = k0; k < k1; ++k) {
+            const double2 y = A.fgb[k];
+            const int j = A.fcol[k];
+#pragma unroll
+            for (int q = 0; q < kRecS; ++q) {
+                const double2 x = v[q][j];
+                ire[q] += y.x * x.x - y.y * x.y;
+                iim[q] += y.y * x.x + y.x * x.y;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < kRecS; ++q) {
+            const int b = bg * kRecS + q;
+            if (b < A.batch) {
+                const double2 vi = v[q][i];
+                A.p_inj[(size_t)b * A.n_bus + i] = vi.x * ire[q] + vi.y * iim[q];
+                A.q_inj[(size_t)b * A.n_bus + i] = vi.y * ire[q] - vi.x * iim[q];
+            }
+        }
+    }
+    const size_t nw = ((size_t)gridDim.x * blockDim.x) >> 5, tot = (size_t)A.batch * A.n_long;
+    for (size_t w = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < tot; w += nw) {
+        const int b = (int)(w / A.n_long), r = (int)(w - (size_t)b * A.n_long);
+        recover_row(A, (size_t)b * A.n_bus, A.long_rows[r], reinterpret_cast<const double2*>(A.work + (size_t)b * A.work_stride), true);
     }
 }
 
