@@ -9,7 +9,9 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`): 2-bus closed form, hand-derived 3
 (tests/golden/), Jacobian vs central finite differences and vs the complex-matrix identities,
 power balance vs branch losses, adjoint vs finite-difference sensitivities, dense vs sparse vs scipy
 solves, permutation / batch-composition invariance; the implicit-layer backward (numpy, below) is pinned by finite
-differences of the whole layer (tests/test_oracle_layer.py).  No function of this oracle is "parity unpinned".
+differences of the whole layer (tests/test_oracle_layer.py); the mixed-precision loop with inner refinement sweeps
+(`nr_mixed_ir`, a Python loop over the C steps) is pinned to the C oracle's mixed mode at 0 sweeps and to the FP64 Newton
+history at 3 (tests/test_oracle_pins.py).  No function of this oracle is "parity unpinned".
 """
 from __future__ import annotations
 
